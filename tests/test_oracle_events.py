@@ -1,0 +1,181 @@
+"""Event-level pins of the oracle: conservation laws, order independence (R-R4),
+counter-keyed determinism, the closed-form classical deflection of a transparent
+traversal, degenerate cases, and a regression digest written by tests/golden/make_golden.py."""
+import ctypes as C
+import json
+import os
+
+import numpy as np
+import pytest
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "oracle_config1_first64.json")
+
+
+def _run(orc, otables, A, Z, E, n, seed, **kw):
+    return orc.simulate(otables, [(A, Z)], np.full(n, float(E)), np.zeros(n, dtype=np.int32), seed, **kw)
+
+
+def _check_conservation(orc, otables, r, A, Z, E_in, rel=1e-9):
+    L = orc.lib()
+    t = C.byref(otables.c)
+    n = len(r["counts"])
+    code = r["species"] & 0x7F
+    mass = orc.SPECIES_M[code]
+    pmag = np.sqrt(r["T"] * (r["T"] + 2 * mass))
+    seg = np.repeat(np.arange(n), r["counts"])
+    sumA = np.bincount(seg, weights=orc.SPECIES_A[code], minlength=n)
+    sumZ = np.bincount(seg, weights=orc.SPECIES_Z[code], minlength=n)
+    ok = (r["status"] & orc.ST_FAILED) == 0
+    # (1) exact baryon number and charge
+    assert np.all((sumA + r["A"])[ok] == A + 1)
+    assert np.all((sumZ + r["Z"])[ok] == Z + 1)
+    # 4-momentum
+    sumE = np.bincount(seg, weights=r["T"] + mass, minlength=n)
+    sp = [np.bincount(seg, weights=pmag * r[k], minlength=n) for k in ("ux", "uy", "uz")]
+    Mres = np.array([L.orc_mass(int(a), int(z), t) for a, z in zip(r["A"], r["Z"])])
+    Pres2 = r["px"] ** 2 + r["py"] ** 2 + r["pz"] ** 2
+    Eres = np.sqrt((Mres + r["Estar"]) ** 2 + Pres2)
+    E_tot = E_in + orc.M_P + L.orc_mass(A, Z, t)
+    p_in = np.sqrt(E_in * (E_in + 2 * orc.M_P))
+    assert np.allclose((sumE + Eres)[ok], E_tot[ok] if np.ndim(E_tot) else E_tot, rtol=rel, atol=0)
+    assert np.allclose((sp[0] + r["px"])[ok], 0.0, atol=rel * np.max(p_in))
+    assert np.allclose((sp[1] + r["py"])[ok], 0.0, atol=rel * np.max(p_in))
+    assert np.allclose((sp[2] + r["pz"])[ok], p_in[ok] if np.ndim(p_in) else p_in, rtol=0, atol=rel * np.max(p_in))
+    # unit directions, non-negative energies
+    assert np.allclose(r["ux"] ** 2 + r["uy"] ** 2 + r["uz"] ** 2, 1.0, atol=1e-12)
+    assert np.all(r["T"] > 0) and np.all(r["Estar"][ok] >= 0)
+
+
+@pytest.mark.parametrize("A,Z,E,seed", [(16, 8, 200.0, 1), (40, 20, 70.0, 3), (48, 22, 250.0, 5), (12, 6, 20.0, 9)])
+def test_conservation_laws(orc, otables, A, Z, E, seed):
+    r = _run(orc, otables, A, Z, E, 3000, seed)
+    assert not np.any(r["status"] & orc.ST_FAILED)
+    _check_conservation(orc, otables, r, A, Z, np.float64(E))
+    # canonical order: cascade nucleons (bit 7 clear, species n/p) then evaporation products
+    for e in range(200):
+        s = r["species"][r["offsets"][e]:r["offsets"][e + 1]]
+        ev = (s & 0x80) != 0
+        assert np.all(np.diff(ev.astype(int)) >= 0)
+        assert np.all((s[~ev]) <= 1) and np.all((s[ev] & 0x7F) <= 5)
+        assert r["casc_count"][e] == np.sum(~ev)
+    # attempts used are recorded in bits 0-7
+    assert np.sum(r["status"] & 0xFF) == r["stats"]["attempts"]
+
+
+def test_cascade_residual_energy_balance(orc, otables):
+    """Post-cascade residual (A,Z,E*,P) closes the 4-momentum balance of the cascade stage."""
+    r = _run(orc, otables, 16, 8, 200.0, 2000, 11, flags=orc.F_CASCADE_ONLY)
+    assert np.all((r["species"] & 0x80) == 0)
+    assert np.array_equal(r["A"], r["casc_A"]) and np.allclose(r["Estar"], r["casc_Estar"])
+    _check_conservation(orc, otables, r, 16, 8, np.float64(200.0))
+
+
+def test_order_independence_lifo_equals_fifo(orc, otables):
+    """R-R4: per-track counters make the pending-track order immaterial, bit for bit."""
+    a = _run(orc, otables, 40, 20, 180.0, 1500, 21)
+    b = _run(orc, otables, 40, 20, 180.0, 1500, 21, flags=orc.F_FIFO)
+    for k in ("species", "T", "ux", "uy", "uz", "counts", "A", "Z", "Estar", "px", "py", "pz", "status"):
+        assert np.array_equal(a[k], b[k]), k
+
+
+def test_event_index_keys_the_rng(orc, otables):
+    """Results depend on the global event index only: shards reproduce the full run."""
+    full = _run(orc, otables, 16, 8, 150.0, 600, 5)
+    lo = _run(orc, otables, 16, 8, 150.0, 250, 5)
+    hi = orc.simulate(otables, [(16, 8)], np.full(350, 150.0), np.zeros(350, dtype=np.int32), 5, e0=250)
+    for k in ("counts", "A", "Z", "Estar", "pz", "status"):
+        assert np.array_equal(full[k], np.concatenate([lo[k], hi[k]])), k
+    assert np.array_equal(full["T"], np.concatenate([lo["T"], hi["T"]]))
+    other = _run(orc, otables, 16, 8, 150.0, 600, 6)
+    assert not np.array_equal(full["counts"], other["counts"])
+    # event index above 2^32 uses the high counter word
+    far = orc.simulate(otables, [(16, 8)], np.full(50, 150.0), np.zeros(50, dtype=np.int32), 5, e0=2**32)
+    assert not np.array_equal(far["counts"], full["counts"][:50])
+
+
+def test_no_cross_section_means_failed(orc):
+    """sigma = 0: every attempt is transparent, so after 256 attempts the event is FAILED."""
+    t0 = orc.Tables(sigma_scale=0.0)
+    r = _run(orc, t0, 16, 8, 200.0, 6, 3)
+    assert np.all(r["status"] & orc.ST_FAILED) and np.all(r["counts"] == 0)
+    assert np.all(r["A"] == 16) and np.all(r["Z"] == 8) and np.all(r["Estar"] == 0) and np.all(r["pz"] == 0)
+    assert r["stats"]["attempts"] == 6 * 256 and r["stats"]["collisions"] == 0
+
+
+@pytest.mark.parametrize("A,Z,E", [(16, 8, 200.0), (40, 20, 60.0)])
+def test_transparent_traversal_closed_form_deflection(orc, A, Z, E):
+    """With sigma = 0 and transparent attempts kept, the proton crosses the 15-step
+    potential: it must leave with T = E_in and the classical deflection of a stepped
+    central potential, Theta = 2 sum_k [asin(L/(p_out,k r_k)) - asin(L/(p_in,k r_k))]
+    over the spheres it crosses inward (angular momentum L = b p_0 conserved), in the
+    plane of incidence, bent towards the axis.  Pins C0, C2 geometry, C4 and shell indexing."""
+    L = orc.lib()
+    t0 = orc.Tables(sigma_scale=0.0)
+    n = 400
+    seed = 17
+    r = orc.simulate(t0, [(A, Z)], np.full(n, E), np.zeros(n, dtype=np.int32), seed,
+                     flags=orc.F_KEEP_TRANSPARENT | orc.F_CASCADE_ONLY)
+    nu = orc.nucleus_arrays(orc.setup_nucleus(A, Z, t0))
+    assert np.all(r["counts"] == 1) and np.all(r["species"] == 1)
+    assert np.allclose(r["T"], E, rtol=1e-12)
+    m = orc.M_P
+    p0 = np.sqrt(E * (E + 2 * m))
+    ns = nu["n_shells"]
+    pk = np.sqrt((E + nu["V_p"]) * (E + nu["V_p"] + 2 * m))    # momentum in region k (k = ns: outside)
+    for e in range(n):
+        ctr = (C.c_uint32 * 4)(0, 1, e, 0)
+        key = (C.c_uint32 * 2)(seed, 0)
+        o = (C.c_uint32 * 4)()
+        L.orc_philox4x32_10(ctr, key, o)
+        b = nu["R"] * np.sqrt(L.orc_u01(o[0]))
+        phi = 2 * np.pi * L.orc_u01(o[1])
+        Lz = b * p0
+        theta = 0.0
+        k = ns
+        while k >= 1 and Lz / pk[k] < nu["r"][k]:      # ray in region k reaches sphere r_k
+            theta += 2 * (np.arcsin(Lz / (pk[k] * nu["r"][k])) - np.arcsin(Lz / (pk[k - 1] * nu["r"][k])))
+            k -= 1
+        ref = np.array([-np.sin(theta) * np.cos(phi), -np.sin(theta) * np.sin(phi), np.cos(theta)])
+        got = np.array([r["ux"][e], r["uy"][e], r["uz"][e]])
+        assert np.allclose(got, ref, atol=1e-9), (e, b, got, ref)
+    # number of boundary crossings of a central ray: 2 * 15 (in and out)
+    assert r["stats"]["reflections"] == 0
+
+
+def test_reaction_cross_section_is_plausible(orc, otables):
+    """sigma_R = pi R^2 n / attempts: a few hundred mb for 16O (sanity, not parity)."""
+    r = _run(orc, otables, 16, 8, 200.0, 4000, 2)
+    R = orc.setup_nucleus(16, 8, otables).R
+    sig = np.pi * R * R * 10.0 * 4000 / r["stats"]["attempts"]
+    assert 200.0 < sig < 400.0
+    # E* < 0 retries are a few percent of accepted events, not tens of percent
+    assert r["stats"]["retry_estar"] / 4000 < 0.2
+
+
+def test_mixed_targets_and_energy_range(orc, otables):
+    import paper_1309_7963_b200.workloads as W
+    E, tid, targets, seed, _ = W.make_inputs(4, 3000)
+    r = orc.simulate(otables, targets, E, tid, seed)
+    assert not np.any(r["status"] & orc.ST_FAILED)
+    L = orc.lib()
+    code = r["species"] & 0x7F
+    seg = np.repeat(np.arange(len(E)), r["counts"])
+    sumA = np.bincount(seg, weights=orc.SPECIES_A[code], minlength=len(E))
+    At = np.array([a for a, z in targets])[tid]
+    assert np.all(sumA + r["A"] == At + 1)
+    assert E.min() >= 70 and E.max() < 250
+
+
+def test_golden_digest(orc, otables):
+    """Regression: the first 64 events of config 1 (written by tests/golden/make_golden.py,
+    which calls only oracle/).  Guards the oracle against unintended edits."""
+    with open(GOLD) as f:
+        g = json.load(f)
+    import paper_1309_7963_b200.workloads as W
+    E, tid, targets, seed, _ = W.make_inputs(1, 64)
+    r = orc.simulate(otables, targets, E, tid, seed)
+    assert r["counts"].tolist() == g["counts"]
+    assert r["A"].tolist() == g["A"] and r["Z"].tolist() == g["Z"]
+    assert r["species"].tolist() == g["species"]
+    assert np.allclose(r["T"], g["T"], rtol=1e-9)
+    assert np.allclose(r["Estar"], g["Estar"], rtol=1e-9, atol=1e-9)

@@ -1,0 +1,137 @@
+"""Pins for the N-steps (nuclear setup), the mass model and table lookup."""
+import ctypes as C
+import os
+
+import numpy as np
+import pytest
+from scipy import integrate
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "paper_constants.txt")
+
+
+def _paper_constants():
+    out = {}
+    with open(GOLDEN) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if line:
+                k, v = line.split("=")
+                out[k.strip()] = float(v)
+    return out
+
+
+@pytest.mark.parametrize("A,Z", [(12, 6), (16, 8), (40, 20), (48, 22), (31, 15)])
+def test_geometry_closed_forms(orc, otables, A, Z):
+    """c = 1.07 A^(1/3), R = c + 2.5 fm, 15 shells of equal thickness."""
+    k = _paper_constants()
+    nu = orc.nucleus_arrays(orc.setup_nucleus(A, Z, otables))
+    c = k["ws_c0"] * A ** (1.0 / 3.0)
+    assert nu["c"] == pytest.approx(c, rel=1e-14)
+    assert nu["R"] == pytest.approx(c + k["ws_rpad"], rel=1e-14)
+    assert nu["n_shells"] == int(k["n_shells"])
+    assert np.allclose(np.diff(nu["r"]), (c + k["ws_rpad"]) / k["n_shells"], rtol=1e-13)
+    assert nu["r"][0] == 0.0 and nu["r"][-1] == pytest.approx(nu["R"], rel=1e-14)
+
+
+@pytest.mark.parametrize("A,Z", [(12, 6), (16, 8), (40, 20), (48, 22)])
+def test_shell_densities(orc, otables, A, Z):
+    """sum rho_i V_i = A exactly; each rho_i is the volume average of Eq. (1) by an
+    independent adaptive quadrature; strictly decreasing; species split Z/A, N/A."""
+    k = _paper_constants()
+    nu = orc.nucleus_arrays(orc.setup_nucleus(A, Z, otables))
+    r = nu["r"]
+    vol = 4.0 * np.pi / 3.0 * (r[1:] ** 3 - r[:-1] ** 3)
+    assert np.sum(nu["rho"] * vol) == pytest.approx(A, rel=1e-12)
+    assert np.sum(nu["rho_p"] * vol) == pytest.approx(Z, rel=1e-12)
+    assert np.sum(nu["rho_n"] * vol) == pytest.approx(A - Z, rel=1e-12)
+    f = lambda x: x * x / (1.0 + np.exp((x - nu["c"]) / k["ws_delta"]))
+    w = np.array([integrate.quad(f, r[i], r[i + 1], epsabs=0, epsrel=1e-13)[0] for i in range(len(vol))])
+    rho_ref = A * w / (vol * w.sum())   # the 4 pi of the shell integral cancels in the ratio
+    assert np.allclose(nu["rho"], rho_ref, rtol=1e-10, atol=0)
+    assert np.all(np.diff(nu["rho"]) < 0)
+    # central density is nuclear-matter-like
+    assert 0.12 < nu["rho"][0] < 0.18
+
+
+def test_fermi_quantities(orc, otables):
+    """p_F = hbar c (3 pi^2 rho)^(1/3): a free Fermi gas filled to p_F holds
+    rho = 2 * (4 pi/3) p_F^3 / (2 pi hbar c)^3 nucleons per fm^3 — checked by inverting."""
+    nu = orc.nucleus_arrays(orc.setup_nucleus(16, 8, otables))
+    hbarc = 197.3269804
+    for sp, m in (("p", orc.M_P), ("n", orc.M_N)):
+        pF = nu["pF_" + sp]
+        rho_back = 2.0 * (4.0 * np.pi / 3.0) * pF ** 3 / (2.0 * np.pi * hbarc) ** 3
+        assert np.allclose(rho_back, nu["rho_" + sp], rtol=1e-13)
+        EF = nu["EF_" + sp]
+        # relativistic: (EF + m)^2 - pF^2 = m^2
+        assert np.allclose((EF + m) ** 2 - pF ** 2, m * m, rtol=1e-13)
+        V = nu["V_" + sp]
+        assert np.allclose(V[:-1], EF + nu["EB_" + sp], rtol=1e-14)
+        assert V[-1] == 0.0
+    assert nu["EC"] == pytest.approx(1.43996448 * 8 / nu["R"], rel=1e-14)
+
+
+def test_semf_against_known_nuclei(orc, otables):
+    """Sanity of the SEMF reading (R-Q4) against well-known measured values: 16O total
+    binding 127.6 MeV (2 %), separation energies S_p = 12.13, S_n = 15.66 MeV (0.6 MeV),
+    40Ca binding 342.1 MeV (2 %), and the light-ion table."""
+    L = orc.lib()
+    t = C.byref(otables.c)
+    assert L.orc_binding(16, 8, t) == pytest.approx(127.62, rel=0.02)
+    assert L.orc_binding(40, 20, t) == pytest.approx(342.05, rel=0.02)
+    nu = orc.nucleus_arrays(orc.setup_nucleus(16, 8, otables))
+    assert nu["EB_p"] == pytest.approx(12.13, abs=0.6)
+    assert nu["EB_n"] == pytest.approx(15.66, abs=0.6)
+    assert L.orc_binding(4, 2, t) == pytest.approx(28.296, abs=1e-3)
+    assert L.orc_binding(2, 1, t) == pytest.approx(2.2246, abs=1e-3)
+    # mass = Z mp + N mn - B
+    assert L.orc_mass(16, 8, t) == pytest.approx(8 * orc.M_P + 8 * orc.M_N - L.orc_binding(16, 8, t), rel=1e-15)
+    # pairing: even-even > odd-A > odd-odd at equal A (sign of delta_p)
+    # removing the pairing term: B(ee) - pairing == B(oo) + pairing at the same smooth part
+    saved = otables.semf
+    otables.semf = saved[:4] + (0.0,)
+    otables.refresh()
+    smooth_16_8, smooth_14_7 = L.orc_binding(16, 8, C.byref(otables.c)), L.orc_binding(14, 7, C.byref(otables.c))
+    otables.semf = saved
+    otables.refresh()
+    t = C.byref(otables.c)
+    assert L.orc_binding(16, 8, t) - smooth_16_8 == pytest.approx(+saved[4] / 4.0, rel=1e-12)   # even-even
+    assert L.orc_binding(14, 7, t) - smooth_14_7 == pytest.approx(-saved[4] / np.sqrt(14.0), rel=1e-12)  # odd-odd
+    assert L.orc_binding(15, 8, t) == pytest.approx(
+        saved[0] * 15 - saved[1] * 15 ** (2 / 3) - saved[2] * 8 * 7 / 15 ** (1 / 3) - saved[3] * 1.0 / 15, rel=1e-13)
+
+
+def test_valid_nuclei(orc):
+    L = orc.lib()
+    valid = {(1, 0), (1, 1), (2, 1), (3, 1), (3, 2), (4, 2)}
+    for A in range(0, 5):
+        for Z in range(-1, 6):
+            assert bool(L.orc_valid_nucleus(A, Z)) == ((A, Z) in valid)
+    assert L.orc_valid_nucleus(5, 0) and L.orc_valid_nucleus(5, 5) and not L.orc_valid_nucleus(5, 6)
+    assert np.isnan(L.orc_binding(4, 1, None))
+
+
+def test_table_lookup_is_numpy_interp(orc, otables):
+    L = orc.lib()
+    dp = C.POINTER(C.c_double)
+    rng = np.random.default_rng(0)
+    p = np.concatenate([rng.uniform(0, otables.plab_max, 500), [0.0, otables.plab_max, 5.0, 0.8, 2.0]])
+    for name in ("sig_pp", "sig_np", "B_pp", "B_np", "a_np"):
+        y = getattr(otables, name)
+        got = np.array([L.orc_lerp_table(y.ctypes.data_as(dp), otables.n_xs, otables.plab_max, float(x)) for x in p])
+        ref = np.interp(p, otables.plab, y)  # clamps outside the grid
+        assert np.allclose(got, ref, rtol=1e-12, atol=1e-12)
+
+
+def test_cugnon_branch_continuity(orc):
+    """The parameterisations join within 3 % at their break points (R-Q10)."""
+    e = 1e-9
+    for f, brk in ((orc.cugnon_sigma_pp, (0.8, 2.0)), (orc.cugnon_sigma_np, (0.8, 2.0)),
+                   (orc.cugnon_B_np, (0.225, 0.6, 1.6)), (orc.cugnon_B_pp, (2.0,)), (orc.cugnon_a_np, (0.8,))):
+        for b in brk:
+            lo, hi = float(f(b - e)), float(f(b + e))
+            assert abs(lo - hi) <= 0.03 * max(abs(lo), abs(hi), 1.0), (f.__name__, b, lo, hi)
+    # mean free path at the centre of 16O for a 240 MeV nucleon ~ 2-3 fm (plausibility)
+    p = np.sqrt(240.0 * (240.0 + 2 * 938.27)) / 1000.0
+    sig = 0.5 * (orc.cugnon_sigma_pp(p) + orc.cugnon_sigma_np(p)) * 0.1
+    assert 1.5 < 1.0 / (0.14 * sig) < 3.5
