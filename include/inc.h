@@ -1,0 +1,197 @@
+/* inc.h — C ABI of the B200-native intranuclear-cascade + evaporation Monte Carlo
+ * (hot path of arXiv:1309.7963; citations "P:NN" are /root/reference/PAPER.md lines,
+ * "R-xx" are the readings frozen in DESIGN.md section 3).
+ *
+ * One source, two shared libraries with identical symbol names:
+ *     libinc_f32.so   INC_REAL = float    production build ("floating point precision")
+ *     libinc_f64.so   INC_REAL = double   parity build, compiled with -fmad=false
+ * Define INC_REAL_IS_DOUBLE before including this header to describe libinc_f64.so.
+ *
+ * Conventions
+ *  - Every function returns 0 (or a non-negative value where stated) on success and a
+ *    negative INC_E_* code on failure.  Nothing throws or aborts; inc_last_error() gives
+ *    a human-readable message for the last failure on the calling thread's library state.
+ *  - "DEVICE" pointers are CUDA device pointers owned by the caller (e.g. torch tensors);
+ *    the library never frees or reallocates them.  "HOST" pointers are ordinary host
+ *    memory.  The library owns only its internal workspace and the device copies of the
+ *    model tables.
+ *  - All work is enqueued on the stream given to inc_set_stream() (default: stream 0).
+ *    inc_simulate() ends with ONE small synchronous device-to-host copy (total number of
+ *    secondaries + error word), so on return the outputs are complete.
+ *  - Determinism: results depend only on (seed, global event index e = 0..n-1, E_in[e],
+ *    target_id[e], tables) — not on chunking, launch shape or GPU (R-R4).
+ *  - Units: MeV, MeV/c, fm.  Beam along +z (R-Q15); the caller rotates.
+ *  - There is NO CPU fallback: without a CUDA device every compute call returns INC_E_CUDA.
+ */
+#ifndef INC_H
+#define INC_H
+#include <stdint.h>
+
+#ifdef INC_REAL_IS_DOUBLE
+typedef double INC_REAL;
+#else
+typedef float INC_REAL;
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- error codes ------------------------------------------------------------------ */
+#define INC_OK 0
+#define INC_E_BADARG (-1)   /* null pointer, n < 0, unsupported (A,Z), E_in outside [20,250] MeV
+                               (found on device and reported, not clamped), unknown target_id */
+#define INC_E_TABLES (-2)   /* wrong version, non-monotone grid, or tables differ from the
+                               ones captured by the first inc_init                       */
+#define INC_E_CAPACITY (-3) /* out_secondaries->capacity too small: nothing is written past
+                               capacity, out_counts / residual are still complete, and
+                               inc_last_error() reports the needed size                   */
+#define INC_E_CUDA (-4)     /* a CUDA call failed; message in inc_last_error()            */
+#define INC_E_STATE (-5)    /* call order: inc_simulate before any inc_init, etc.         */
+
+/* ---- per-event status word (out_residual->status) ----------------------------------- */
+#define INC_ST_ATTEMPTS_MASK 0xFFu  /* bits 0-7: cascade attempts used (R-C6), saturating    */
+#define INC_ST_FAILED (1u << 8)     /* 256 attempts without a valid non-elastic event:
+                                       count = 0, residual = target at rest              */
+#define INC_ST_SEC_TRUNC (1u << 9)  /* more than INC_MAX_SEC secondaries: extra dropped (R-C5) */
+#define INC_ST_DEPTH_CAP (1u << 10) /* path code would exceed 24 bits (R-C3)              */
+#define INC_ST_SEG_CAP (1u << 11)   /* a track hit 1024 segments and was absorbed (R-C2)  */
+#define INC_ST_TRIAL_CAP (1u << 12) /* evaporation sampler hit 64 trials; chain stopped (R-E4) */
+#define INC_ST_QUEUE_OVF (1u << 13) /* implementation limit: pending-track storage overflowed;
+                                       never expected, tests assert it is never set       */
+
+#define INC_MAX_SEC 64        /* R-C5 */
+#define INC_MAX_TARGETS 16
+#define INC_E_MIN 20.0        /* P:9 "between 20 and 250 MeV" */
+#define INC_E_MAX 250.0
+
+/* ---- flags for inc_set_flags ---------------------------------------------------------- */
+#define INC_F_CASCADE_ONLY 1u      /* stop after the cascade epilogue: outputs are the cascade
+                                      secondaries and the post-cascade residual ("SoA of
+                                      excited nuclei")                                     */
+#define INC_F_KEEP_TRANSPARENT 2u  /* debug: accept attempts without a real collision       */
+#define INC_F_SAME_STREAM 4u       /* divergence probe of P:73-75: every event draws the random
+                                      stream of event 0                                     */
+#define INC_F_STATS 8u             /* accumulate the work counters of inc_get_stats         */
+#define INC_F_TIMING 32u           /* record CUDA events around each stage (inc_get_stage_times) */
+#define INC_F_LANE_PER_EVENT 16u   /* scheduling variant: no phase voting (baseline layout of
+                                      P:61, one lane runs one event straight through)      */
+
+/* ---- model inputs ("precalculated ... tables and other read-only input data") ----- */
+typedef struct inc_tables {   /* HOST memory, caller-owned, copied during inc_init           */
+  int32_t version;            /* = 1                                                         */
+  int32_t n_xs;               /* NN grid points (<= 4096); plab_k = k*plab_max/(n_xs-1) GeV/c */
+  double plab_max;
+  const double *sig_pp, *sig_np;    /* [n_xs] elastic NN cross sections, mb (pp also for nn) */
+  const double *B_pp, *B_np, *a_np; /* [n_xs] slope of exp(B t), (GeV/c)^-2; np backward weight    */
+  int32_t n_evz;                    /* Dostrovsky grid points (<= 16)                        */
+  const double *ev_Z, *ev_kp, *ev_cp, *ev_ka, *ev_ca; /* [n_evz] k, c vs daughter charge      */
+  double ws_c0, ws_delta, ws_rpad;  /* 1.07, 0.545, 2.5 (Eq. (1))                      */
+  int32_t n_shells;                 /* 15; 1..32                                      */
+  double semf[5];                   /* a_v a_s a_c a_a a_p, MeV ("semi-empirical mass formula") */
+  double evap_r0, evap_rj, evap_a_div; /* 1.5 fm, 1.2 fm, 8 (R-E1)                           */
+} inc_tables;
+
+/* inc_init — nuclear setup for one target (Woods-Saxon -> n_shells constant-density
+ * shells, Fermi momenta/energies, V = E_F + E_B, Coulomb barrier) done in fp64 on the host,
+ * uploaded once.  The first call also captures the NN / evaporation tables.
+ * Supported: 6 <= A <= 64, 2 <= Z <= A-2 (the separation energies need valid A-1 nuclei).  Returns target_id >= 0 (slot, < INC_MAX_TARGETS). */
+int inc_init(int A, int Z, const inc_tables *tables /*HOST*/);
+int inc_free_target(int target_id);
+void inc_shutdown(void);       /* frees every target, the tables and the workspace          */
+
+int inc_set_stream(void *cuda_stream /* cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream */);
+int inc_set_flags(uint32_t flags);
+/* Scheduling knob of the cascade kernel: a warp runs the collision phase when at least `coll`
+ * lanes wait for it, the epilogue+entry phase when at least `epi` lanes wait (1..32; default 8, 8).
+ * Results never depend on it. */
+int inc_set_vote_thresholds(int coll, int epi);
+/* Global index of the first event of the following inc_simulate calls (default 0): event i of a
+ * call uses the random stream of global event e = offset + i.  This is how a job is sharded over
+ * several GPUs or calls with bit-identical per-event results (R-R4). */
+int inc_set_event_offset(int64_t first_event);
+
+/* ---- outputs ---------------------------------------------------------------------------- */
+typedef struct inc_secondaries { /* DEVICE pointers, caller-owned, structure of arrays  */
+  uint8_t *species;              /* 0=n 1=p 2=d 3=t 4=3He 5=4He; bit 7 set = from evaporation */
+  INC_REAL *T;                   /* kinetic energy, MeV, lab                                  */
+  INC_REAL *ux, *uy, *uz;        /* unit direction                                            */
+  int64_t capacity;              /* elements available in each array                          */
+} inc_secondaries;
+
+typedef struct inc_residual {    /* DEVICE, structure of arrays of length n_events             */
+  int32_t *A, *Z;                /* final residual nucleus                                    */
+  INC_REAL *Estar;               /* leftover excitation, MeV (no photon model)          */
+  INC_REAL *px, *py, *pz;        /* lab momentum, MeV/c                                       */
+  uint32_t *status;              /* INC_ST_* bits                                             */
+} inc_residual;
+
+/* inc_simulate — the whole hot path for a batch (INC kernel, evaporation kernel;
+ * BASELINE.json north_star: entry, segment, boundary, collision, epilogue, evaporation,
+ * prefix-sum compaction).  Event e is a proton of kinetic energy E_in[e] on target
+ * target_id[e].  Secondaries of all events are written back to back in event order, inside
+ * an event in canonical order: cascade nucleons by ascending path code, then evaporation
+ * products in emission order.  out_counts[e] is the number of secondaries of event e.
+ * Returns the total number of secondaries (>= 0) or a negative INC_E_* code. */
+int64_t inc_simulate(int64_t n_events, const INC_REAL *E_in /*DEVICE, MeV*/,
+                     const int32_t *target_id /*DEVICE*/, uint64_t seed,
+                     inc_secondaries *out_secondaries /*HOST struct of DEVICE ptrs*/,
+                     int32_t *out_counts /*DEVICE [n_events]*/,
+                     inc_residual *out_residual /*HOST struct of DEVICE ptrs*/);
+
+/* inc_simulate_host — same computation with HOST buffers (every pointer, including those
+ * inside the two structs, is host memory).  The library stages inputs to the device,
+ * runs inc_simulate and copies the results back, all inside this call (used for the
+ * end-to-end number of bench.py).  Pinned host memory makes the copies faster but is not
+ * required. */
+int64_t inc_simulate_host(int64_t n_events, const INC_REAL *E_in /*HOST*/,
+                          const int32_t *target_id /*HOST*/, uint64_t seed,
+                          inc_secondaries *out_secondaries /*HOST ptrs*/,
+                          int32_t *out_counts /*HOST*/, inc_residual *out_residual /*HOST ptrs*/);
+
+/* Exclusive prefix sum of out_counts of the last inc_simulate: dev_offsets[e] is the index of
+ * the first secondary of event e, dev_offsets[n_events] the total. */
+int inc_get_offsets(int64_t *dev_offsets /*DEVICE [n_events+1]*/);
+
+/* Post-cascade nuclei of the last inc_simulate (the paper's "SoA of excited nuclei", P:69,
+ * P:83), for stage-level tests: any pointer may be NULL. */
+int inc_get_cascade_stage(int32_t *A /*DEVICE [n]*/, int32_t *Z, INC_REAL *Estar,
+                          INC_REAL *px, INC_REAL *py, INC_REAL *pz, int32_t *n_cascade_secondaries);
+
+typedef struct inc_stats {     /* work counters of the last inc_simulate (needs INC_F_STATS)   */
+  uint64_t events, failed, attempts, segments, boundaries, reflections, escapes;
+  uint64_t collisions, blocked, allowed, absorbed;
+  uint64_t evap_steps, evap_trials, evap_emitted;
+  uint64_t warp_iters_seg, warp_iters_coll, warp_iters_epi; /* scheduling: phase passes    */
+  uint64_t lane_slots_seg, lane_slots_coll, lane_slots_epi; /* active lanes summed over passes */
+} inc_stats;
+int inc_get_stats(inc_stats *host_out /*HOST*/);
+
+/* Device time of the stages of the last inc_simulate, summed over its chunks, in milliseconds:
+ * ms[0] cascade kernel, ms[1] evaporation kernel, ms[2] prefix-sum kernels, ms[3] compaction
+ * kernel; launches[0..3] the number of kernel launches of each stage.  Needs INC_F_TIMING. */
+int inc_get_stage_times(float ms[4] /*HOST*/, int32_t launches[4] /*HOST*/);
+
+/* Nuclear-setup record of a target, for tests of inc_init (all HOST, fp64, length n_shells
+ * except r, V_p, V_n which have n_shells+1; pointers may be NULL). */
+int inc_get_nucleus(int target_id, int32_t *A, int32_t *Z, int32_t *n_shells, double *R,
+                    double *E_C, double *EB_p, double *EB_n, double *r, double *rho_p,
+                    double *rho_n, double *pF_p, double *pF_n, double *EF_p, double *EF_n,
+                    double *V_p, double *V_n);
+
+/* Measured peak of the plain-ALU roofline: runs an FFMA (f32) or DFMA (f64) chain kernel at
+ * full occupancy on the current stream and returns lane-instructions per second (one FMA =
+ * one lane-instruction).  Used by bench.py for roofline.peak. */
+int inc_measure_issue_peak(double *lane_instr_per_s /*HOST*/, double *sm_clock_mhz /*HOST, may be NULL*/);
+
+/* Philox4x32-10 block, exposed for the RNG parity test (R-R1): out[4*i..] for counters
+ * ctr[4*i..] (DEVICE arrays of n blocks), key = (seed lo, seed hi). */
+int inc_philox_blocks(const uint32_t *ctr /*DEVICE [4n]*/, uint64_t seed, uint32_t *out /*DEVICE [4n]*/, int64_t n);
+
+const char *inc_last_error(void);
+const char *inc_build_info(void);   /* "f32 fast-math sm_100a ..." */
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,298 @@
+"""Thin ctypes binding of the C-ABI library (include/inc.h).  Argument marshalling only:
+every step of the hot path runs in the CUDA kernels of csrc/.  torch is used for device
+memory and streams.  There is no CPU fallback: loading fails loudly if the library has not
+been built, and every compute call fails if no CUDA device is present.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+# ---- constants mirrored from include/inc.h ----
+INC_E_BADARG, INC_E_TABLES, INC_E_CAPACITY, INC_E_CUDA, INC_E_STATE = -1, -2, -3, -4, -5
+ST_FAILED, ST_SEC_TRUNC, ST_DEPTH_CAP, ST_SEG_CAP, ST_TRIAL_CAP, ST_QUEUE_OVF = (1 << 8, 1 << 9, 1 << 10, 1 << 11, 1 << 12, 1 << 13)
+F_CASCADE_ONLY, F_KEEP_TRANSPARENT, F_SAME_STREAM, F_STATS, F_LANE_PER_EVENT, F_TIMING = 1, 2, 4, 8, 16, 32
+MAX_SEC = 64
+
+_DP = C.POINTER(C.c_double)
+
+
+class IncError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"inc error {code}: {msg}")
+        self.code = code
+
+
+class IncTables(C.Structure):
+    _fields_ = [
+        ("version", C.c_int32), ("n_xs", C.c_int32), ("plab_max", C.c_double),
+        ("sig_pp", _DP), ("sig_np", _DP), ("B_pp", _DP), ("B_np", _DP), ("a_np", _DP),
+        ("n_evz", C.c_int32), ("ev_Z", _DP), ("ev_kp", _DP), ("ev_cp", _DP), ("ev_ka", _DP), ("ev_ca", _DP),
+        ("ws_c0", C.c_double), ("ws_delta", C.c_double), ("ws_rpad", C.c_double), ("n_shells", C.c_int32),
+        ("semf", C.c_double * 5), ("evap_r0", C.c_double), ("evap_rj", C.c_double), ("evap_a_div", C.c_double),
+    ]
+
+
+class IncSecondaries(C.Structure):
+    _fields_ = [("species", C.c_void_p), ("T", C.c_void_p), ("ux", C.c_void_p), ("uy", C.c_void_p),
+                ("uz", C.c_void_p), ("capacity", C.c_int64)]
+
+
+class IncResidual(C.Structure):
+    _fields_ = [("A", C.c_void_p), ("Z", C.c_void_p), ("Estar", C.c_void_p), ("px", C.c_void_p),
+                ("py", C.c_void_p), ("pz", C.c_void_p), ("status", C.c_void_p)]
+
+
+_STAT_FIELDS = ["events", "failed", "attempts", "segments", "boundaries", "reflections", "escapes",
+                "collisions", "blocked", "allowed", "absorbed", "evap_steps", "evap_trials", "evap_emitted",
+                "warp_iters_seg", "warp_iters_coll", "warp_iters_epi",
+                "lane_slots_seg", "lane_slots_coll", "lane_slots_epi"]
+
+
+class IncStats(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in _STAT_FIELDS]
+
+
+def make_tables_struct(t: dict):
+    """dict (tables.default_tables) -> (IncTables, keepalive list)."""
+    s = IncTables()
+    keep = []
+    s.version, s.n_xs, s.plab_max = int(t["version"]), int(t["n_xs"]), float(t["plab_max"])
+    for name in ("sig_pp", "sig_np", "B_pp", "B_np", "a_np", "ev_Z", "ev_kp", "ev_cp", "ev_ka", "ev_ca"):
+        a = np.ascontiguousarray(t[name], dtype=np.float64)
+        keep.append(a)
+        setattr(s, name, a.ctypes.data_as(_DP))
+    s.n_evz = len(t["ev_Z"])
+    s.ws_c0, s.ws_delta, s.ws_rpad = float(t["ws_c0"]), float(t["ws_delta"]), float(t["ws_rpad"])
+    s.n_shells = int(t["n_shells"])
+    for i in range(5):
+        s.semf[i] = float(t["semf"][i])
+    s.evap_r0, s.evap_rj, s.evap_a_div = float(t["evap_r0"]), float(t["evap_rj"]), float(t["evap_a_div"])
+    return s, keep
+
+
+EXPORTS = ["inc_init", "inc_free_target", "inc_shutdown", "inc_set_stream", "inc_set_flags", "inc_set_event_offset",
+           "inc_get_stage_times", "inc_set_vote_thresholds", "inc_simulate",
+           "inc_simulate_host", "inc_get_offsets", "inc_get_cascade_stage", "inc_get_stats", "inc_get_nucleus",
+           "inc_measure_issue_peak", "inc_philox_blocks", "inc_last_error", "inc_build_info"]
+
+
+class IncLibrary:
+    """One loaded variant ('f32' production, 'f64' parity) of the C-ABI library."""
+
+    def __init__(self, variant: str = "f32", build_if_missing: bool = True):
+        if variant not in ("f32", "f64"):
+            raise ValueError(variant)
+        self.variant = variant
+        path = _build.lib_path(variant)
+        if not os.path.exists(path):
+            if not build_if_missing:
+                raise FileNotFoundError(path)
+            _build.build()
+        self.path = path
+        self.lib = L = C.CDLL(path, mode=C.RTLD_LOCAL)
+        self.real = np.float32 if variant == "f32" else np.float64
+        vp = C.c_void_p
+        L.inc_init.argtypes = [C.c_int, C.c_int, C.POINTER(IncTables)]
+        L.inc_init.restype = C.c_int
+        L.inc_free_target.argtypes = [C.c_int]
+        L.inc_shutdown.restype = None
+        L.inc_set_stream.argtypes = [vp]
+        L.inc_set_flags.argtypes = [C.c_uint32]
+        L.inc_set_event_offset.argtypes = [C.c_int64]
+        L.inc_get_stage_times.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_int32)]
+        for f in (L.inc_simulate, L.inc_simulate_host):
+            f.argtypes = [C.c_int64, vp, vp, C.c_uint64, C.POINTER(IncSecondaries), vp, C.POINTER(IncResidual)]
+            f.restype = C.c_int64
+        L.inc_get_offsets.argtypes = [vp]
+        L.inc_get_cascade_stage.argtypes = [vp] * 7
+        L.inc_get_stats.argtypes = [C.POINTER(IncStats)]
+        L.inc_get_nucleus.argtypes = [C.c_int] + [vp] * 16
+        L.inc_measure_issue_peak.argtypes = [_DP, _DP]
+        L.inc_philox_blocks.argtypes = [vp, C.c_uint64, vp, C.c_int64]
+        L.inc_last_error.restype = C.c_char_p
+        L.inc_build_info.restype = C.c_char_p
+        L.inc_set_vote_thresholds.argtypes = [C.c_int, C.c_int]
+        self._tables_keep = None
+
+    # ---- helpers ----
+    def _check(self, rc):
+        if rc < 0:
+            raise IncError(int(rc), self.lib.inc_last_error().decode())
+        return rc
+
+    def build_info(self) -> str:
+        return self.lib.inc_build_info().decode()
+
+    def last_error(self) -> str:
+        return self.lib.inc_last_error().decode()
+
+    # ---- ABI calls (same names as include/inc.h) ----
+    def inc_init(self, A: int, Z: int, tables: dict) -> int:
+        s, keep = make_tables_struct(tables)
+        self._tables_keep = (s, keep)
+        return self._check(self.lib.inc_init(int(A), int(Z), C.byref(s)))
+
+    def inc_free_target(self, tid: int):
+        self._check(self.lib.inc_free_target(int(tid)))
+
+    def inc_shutdown(self):
+        self.lib.inc_shutdown()
+
+    def inc_set_stream(self, stream=None):
+        import torch
+        st = torch.cuda.current_stream() if stream is None else stream
+        self._check(self.lib.inc_set_stream(C.c_void_p(st.cuda_stream)))
+
+    def inc_set_flags(self, flags: int):
+        self._check(self.lib.inc_set_flags(int(flags)))
+
+    def inc_set_event_offset(self, first_event: int):
+        self._check(self.lib.inc_set_event_offset(int(first_event)))
+
+    def inc_get_stage_times(self):
+        ms, nl = (C.c_float * 4)(), (C.c_int32 * 4)()
+        self._check(self.lib.inc_get_stage_times(ms, nl))
+        return dict(zip(("cascade", "evap", "scan", "compact"), [float(x) for x in ms])), [int(x) for x in nl]
+
+    def inc_set_vote_thresholds(self, coll: int, epi: int):
+        self._check(self.lib.inc_set_vote_thresholds(int(coll), int(epi)))
+
+    def torch_real(self):
+        import torch
+        return torch.float32 if self.variant == "f32" else torch.float64
+
+    def alloc_outputs(self, n: int, capacity: int, device="cuda"):
+        """Caller-owned output tensors (torch) for inc_simulate."""
+        import torch
+        r = self.torch_real()
+        pin = device == "cpu"
+        kw = dict(device=device, pin_memory=pin) if pin else dict(device=device)
+        return dict(
+            species=torch.empty(capacity, dtype=torch.uint8, **kw),
+            T=torch.empty(capacity, dtype=r, **kw), ux=torch.empty(capacity, dtype=r, **kw),
+            uy=torch.empty(capacity, dtype=r, **kw), uz=torch.empty(capacity, dtype=r, **kw),
+            counts=torch.empty(n, dtype=torch.int32, **kw),
+            A=torch.empty(n, dtype=torch.int32, **kw), Z=torch.empty(n, dtype=torch.int32, **kw),
+            Estar=torch.empty(n, dtype=r, **kw), px=torch.empty(n, dtype=r, **kw),
+            py=torch.empty(n, dtype=r, **kw), pz=torch.empty(n, dtype=r, **kw),
+            status=torch.empty(n, dtype=torch.int32, **kw))
+
+    def _structs(self, out):
+        sec = IncSecondaries(out["species"].data_ptr(), out["T"].data_ptr(), out["ux"].data_ptr(),
+                             out["uy"].data_ptr(), out["uz"].data_ptr(), out["species"].numel())
+        res = IncResidual(out["A"].data_ptr(), out["Z"].data_ptr(), out["Estar"].data_ptr(),
+                          out["px"].data_ptr(), out["py"].data_ptr(), out["pz"].data_ptr(), out["status"].data_ptr())
+        return sec, res
+
+    def inc_simulate(self, E_in, target_id, seed: int, out: dict, check: bool = True) -> int:
+        """E_in (real), target_id (int32): CUDA tensors.  out: alloc_outputs(...).  Returns total."""
+        n = E_in.numel()
+        assert E_in.is_cuda and target_id.is_cuda and E_in.dtype == self.torch_real()
+        sec, res = self._structs(out)
+        rc = self.lib.inc_simulate(n, C.c_void_p(E_in.data_ptr()), C.c_void_p(target_id.data_ptr()),
+                                   C.c_uint64(int(seed)), C.byref(sec), C.c_void_p(out["counts"].data_ptr()), C.byref(res))
+        return self._check(rc) if check else rc
+
+    def inc_simulate_host(self, E_in, target_id, seed: int, out: dict, check: bool = True) -> int:
+        """Same with HOST tensors (ideally pinned); copies happen inside the library call."""
+        n = E_in.numel()
+        assert not E_in.is_cuda and not target_id.is_cuda
+        sec, res = self._structs(out)
+        rc = self.lib.inc_simulate_host(n, C.c_void_p(E_in.data_ptr()), C.c_void_p(target_id.data_ptr()),
+                                        C.c_uint64(int(seed)), C.byref(sec), C.c_void_p(out["counts"].data_ptr()), C.byref(res))
+        return self._check(rc) if check else rc
+
+    def inc_get_offsets(self, n: int):
+        import torch
+        off = torch.empty(n + 1, dtype=torch.int64, device="cuda")
+        self._check(self.lib.inc_get_offsets(C.c_void_p(off.data_ptr())))
+        return off
+
+    def inc_get_cascade_stage(self, n: int):
+        import torch
+        r = self.torch_real()
+        d = dict(A=torch.empty(n, dtype=torch.int32, device="cuda"), Z=torch.empty(n, dtype=torch.int32, device="cuda"),
+                 Estar=torch.empty(n, dtype=r, device="cuda"), px=torch.empty(n, dtype=r, device="cuda"),
+                 py=torch.empty(n, dtype=r, device="cuda"), pz=torch.empty(n, dtype=r, device="cuda"),
+                 meta=torch.empty(n, dtype=torch.int32, device="cuda"))
+        self._check(self.lib.inc_get_cascade_stage(*[C.c_void_p(d[k].data_ptr()) for k in ("A", "Z", "Estar", "px", "py", "pz", "meta")]))
+        d["n_cascade"] = d["meta"] & 0xFF
+        return d
+
+    def inc_get_stats(self) -> dict:
+        s = IncStats()
+        self._check(self.lib.inc_get_stats(C.byref(s)))
+        return {n: int(getattr(s, n)) for n in _STAT_FIELDS}
+
+    def inc_get_nucleus(self, tid: int) -> dict:
+        A, Z, ns = C.c_int32(), C.c_int32(), C.c_int32()
+        R, EC, EBp, EBn = C.c_double(), C.c_double(), C.c_double(), C.c_double()
+        self._check(self.lib.inc_get_nucleus(tid, C.byref(A), C.byref(Z), C.byref(ns), C.byref(R), C.byref(EC),
+                                             C.byref(EBp), C.byref(EBn), *([None] * 9)))
+        n = ns.value
+        arr = {k: np.zeros(n + (1 if k in ("r", "V_p", "V_n") else 0)) for k in
+               ("r", "rho_p", "rho_n", "pF_p", "pF_n", "EF_p", "EF_n", "V_p", "V_n")}
+        ptr = lambda k: arr[k].ctypes.data_as(C.c_void_p)
+        self._check(self.lib.inc_get_nucleus(tid, None, None, None, None, None, None, None,
+                                             *[ptr(k) for k in ("r", "rho_p", "rho_n", "pF_p", "pF_n", "EF_p", "EF_n", "V_p", "V_n")]))
+        arr.update(A=A.value, Z=Z.value, n_shells=n, R=R.value, EC=EC.value, EB_p=EBp.value, EB_n=EBn.value)
+        return arr
+
+    def inc_measure_issue_peak(self):
+        a, b = C.c_double(), C.c_double()
+        self._check(self.lib.inc_measure_issue_peak(C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def inc_philox_blocks(self, ctr, seed: int):
+        import torch
+        out = torch.empty_like(ctr)
+        self._check(self.lib.inc_philox_blocks(C.c_void_p(ctr.data_ptr()), C.c_uint64(int(seed)),
+                                               C.c_void_p(out.data_ptr()), ctr.numel() // 4))
+        return out
+
+
+_cache = {}
+
+
+def load(variant: str = "f32") -> IncLibrary:
+    if variant not in _cache:
+        _cache[variant] = IncLibrary(variant)
+    return _cache[variant]
+
+
+def simulate(lib: IncLibrary, targets, E_in_np, target_idx_np, seed, tables: dict, flags: int = 0, capacity_per_event: int = 24):
+    """Convenience used by tests/bench: init targets, run on the GPU, return numpy arrays.
+    targets: list of (A,Z); target_idx_np indexes that list."""
+    import torch
+    lib.inc_shutdown()
+    slots = [lib.inc_init(a, z, tables) for a, z in targets]
+    slot_map = np.asarray(slots, dtype=np.int32)
+    n = len(E_in_np)
+    E = torch.as_tensor(np.asarray(E_in_np, dtype=lib.real), device="cuda")
+    tid = torch.as_tensor(slot_map[np.asarray(target_idx_np)], device="cuda")
+    lib.inc_set_stream()
+    lib.inc_set_flags(flags)
+    cap = max(64, n * capacity_per_event)
+    out = lib.alloc_outputs(n, cap)
+    total = lib.inc_simulate(E, tid, seed, out)
+    off = lib.inc_get_offsets(n)
+    res = {k: v.cpu().numpy() for k, v in out.items()}
+    for k in ("species", "T", "ux", "uy", "uz"):
+        res[k] = res[k][:total]
+    res["status"] = res["status"].view(np.uint32)
+    res["offsets"] = off.cpu().numpy()
+    res["total"] = total
+    if n <= (1 << 20):
+        st = lib.inc_get_cascade_stage(n)
+        res["casc_A"], res["casc_Z"] = st["A"].cpu().numpy(), st["Z"].cpu().numpy()
+        res["casc_Estar"] = st["Estar"].cpu().numpy()
+        res["casc_P"] = np.stack([st[k].cpu().numpy() for k in ("px", "py", "pz")], axis=1)
+        res["casc_count"] = st["n_cascade"].cpu().numpy()
+    if flags & F_STATS:
+        res["stats"] = lib.inc_get_stats()
+    return res

@@ -1,0 +1,55 @@
+"""Builds the two C-ABI libraries (libinc_f32.so, libinc_f64.so) in-tree with nvcc for sm_100a.
+
+    python -m paper_1309_7963_b200.build [--force] [--verbose]
+
+nvcc cross-compiles without a GPU.  The f64 parity build uses -fmad=false (BASELINE.json
+north_star, criterion (2)); the f32 production build uses explicit fast intrinsics in the
+source ("-use_fast_math" variant) and default flags otherwise.
+"""
+from __future__ import annotations
+
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+ROOT = os.path.dirname(HERE)
+SOURCES = [os.path.join(CSRC, "inc_lib.cu")]
+DEPS = SOURCES + [os.path.join(CSRC, "inc_device.cuh"), os.path.join(ROOT, "include", "inc.h")]
+
+COMMON = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+          "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=default"]
+VARIANTS = {
+    "f32": [],
+    "f64": ["-DINC_REAL_IS_DOUBLE", "-fmad=false"],
+}
+
+
+def lib_path(variant: str) -> str:
+    return os.path.join(HERE, f"libinc_{variant}.so")
+
+
+def _stale(out: str) -> bool:
+    if not os.path.exists(out):
+        return True
+    t = os.path.getmtime(out)
+    return any(os.path.getmtime(d) > t for d in DEPS)
+
+
+def build(force: bool = False, verbose: bool = False) -> dict:
+    nvcc = os.environ.get("NVCC", "nvcc")
+    out = {}
+    for variant, extra in VARIANTS.items():
+        dst = lib_path(variant)
+        if force or _stale(dst):
+            cmd = [nvcc] + COMMON + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", dst] + SOURCES
+            if verbose:
+                print(" ".join(cmd))
+            subprocess.check_call(cmd)
+        out[variant] = dst
+    return out
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

@@ -1,0 +1,714 @@
+// inc_lib.cu — host side of the C ABI declared in include/inc.h.
+//
+// Built twice: -DINC_REAL_IS_DOUBLE (parity build, -fmad=false) and default (float, production).
+// Host work: nuclear setup in fp64, model tables, workspace, kernel launches on the
+// caller's stream.  No CPU compute path exists: every compute entry point needs a CUDA device.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "inc_device.cuh"
+
+using namespace inc;
+typedef INC_REAL real;
+
+namespace {
+
+// ---- constants used by the host setup (standard values, R-K) ----------------------------------
+const double kHbarc = 197.3269804, kE2 = 1.43996448;
+const double kMp = 938.27208816, kMn = 939.56542052;
+const double kPi = 3.14159265358979323846;
+const int kEvA[6] = {1, 1, 2, 3, 3, 4};
+const int kEvZ[6] = {0, 1, 1, 1, 2, 2};
+const double kEvG[6] = {2, 2, 3, 2, 2, 1};
+
+struct HostNucleus {
+  bool live = false;
+  int A = 0, Z = 0, ns = 0;
+  double R = 0, dr = 0, EC = 0, EB_p = 0, EB_n = 0, Bt = 0;
+  std::vector<double> r, rho_p, rho_n, pF_p, pF_n, EF_p, EF_n, V_p, V_n;
+};
+
+struct TablesHost {
+  bool captured = false;
+  int n_xs = 0, n_evz = 0, n_shells = 0;
+  double plab_max = 0, ws_c0 = 0, ws_delta = 0, ws_rpad = 0, semf[5] = {0, 0, 0, 0, 0};
+  double evap_r0 = 0, evap_rj = 0, evap_a_div = 0;
+  std::vector<double> sig_pp, sig_np, B_pp, B_np, a_np, ev_Z, ev_kp, ev_cp, ev_ka, ev_ca;
+};
+
+struct State {
+  cudaStream_t stream = nullptr;
+  uint32_t flags = 0;
+  TablesHost tab;
+  HostNucleus nuc[INC_MAX_TARGETS];
+  // device model
+  real *d_tabS = nullptr, *d_tabC = nullptr, *d_bind = nullptr;
+  EvChan<real> *d_evch = nullptr;
+  NucDev<real> *d_nuc = nullptr;
+  DevCounters *d_ctr = nullptr;
+  // workspace
+  size_t ws_chunk = 0;
+  Workspace<real> ws{};
+  long long *d_offsets = nullptr; size_t offsets_cap = 0;
+  long long *d_tiles = nullptr; size_t tiles_cap = 0;
+  // host-buffer path
+  struct HostPath {
+    size_t n_cap = 0, sec_cap = 0;
+    real *E = nullptr; int32_t *tid = nullptr, *counts = nullptr, *A = nullptr, *Z = nullptr;
+    real *Es = nullptr, *px = nullptr, *py = nullptr, *pz = nullptr; uint32_t *status = nullptr;
+    uint8_t *sp = nullptr; real *T = nullptr, *ux = nullptr, *uy = nullptr, *uz = nullptr;
+  } hp;
+  // last call
+  long long last_n = -1;
+  long long last_total = 0;
+  long long event_offset = 0;
+  // stage timing (INC_F_TIMING)
+  cudaEvent_t tev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  float stage_ms[4] = {0, 0, 0, 0};
+  int stage_launches[4] = {0, 0, 0, 0};
+  std::vector<cudaEvent_t> pending_events;   // 5 per chunk, resolved after the stream sync
+  int vote_coll = 8, vote_epi = 8;
+  int sm_count = 0;
+  std::string err;
+};
+
+State g;
+
+int fail(int code, const std::string &msg) { g.err = msg; return code; }
+
+#define CU_TRY(expr)                                                                           \
+  do {                                                                                         \
+    cudaError_t _e = (expr);                                                                   \
+    if (_e != cudaSuccess)                                                                     \
+      return fail(INC_E_CUDA, std::string(#expr) + ": " + cudaGetErrorString(_e));            \
+  } while (0)
+
+// ---- mass model ("semi-empirical mass formula"; R-Q4) -------------------------------------
+bool valid_nucleus(int A, int Z) {
+  if (A < 1 || Z < 0 || Z > A) return false;
+  if (A >= 5 || A == 1) return true;
+  if (A == 2) return Z == 1;
+  if (A == 3) return Z == 1 || Z == 2;
+  return Z == 2;
+}
+
+double binding(int A, int Z, const TablesHost &t) {
+  static const double light[5][3] = {{0, 0, 0}, {0, 0, 0}, {0, 2.224566, 0}, {0, 8.481798, 7.718043}, {0, 0, 28.29566}};
+  if (A <= 4) return light[A][Z];
+  const double a = A, z = Z, a13 = std::cbrt(a);
+  double B = t.semf[0] * a - t.semf[1] * a13 * a13 - t.semf[2] * z * (z - 1.0) / a13 -
+             t.semf[3] * (a - 2.0 * z) * (a - 2.0 * z) / a;
+  const bool ze = (Z % 2) == 0, ne = ((A - Z) % 2) == 0;
+  if (ze && ne) B += t.semf[4] / std::sqrt(a);
+  else if (!ze && !ne) B -= t.semf[4] / std::sqrt(a);
+  return B;
+}
+
+// Gauss-Legendre nodes on [-1,1] by Newton iteration (for the shell integrals of Eq. (1))
+void gauss_legendre(int n, std::vector<double> &x, std::vector<double> &w) {
+  x.resize(n); w.resize(n);
+  for (int i = 0; i < n; ++i) {
+    double z = std::cos(kPi * (i + 0.75) / (n + 0.5)), pp = 1;
+    for (int it = 0; it < 100; ++it) {
+      double p1 = 1, p2 = 0;
+      for (int j = 0; j < n; ++j) { double p3 = p2; p2 = p1; p1 = ((2.0 * j + 1.0) * z * p2 - j * p3) / (j + 1.0); }
+      pp = n * (z * p1 - p2) / (z * z - 1.0);
+      const double dz = p1 / pp;
+      z -= dz;
+      if (std::fabs(dz) < 1e-16) break;
+    }
+    x[i] = z; w[i] = 2.0 / ((1.0 - z * z) * pp * pp);
+  }
+}
+
+double lerp_z(const std::vector<double> &zz, const std::vector<double> &y, double z) {
+  const int n = (int)zz.size();
+  if (z <= zz[0]) return y[0];
+  if (z >= zz[n - 1]) return y[n - 1];
+  int k = 0;
+  while (k < n - 2 && z > zz[k + 1]) ++k;
+  return y[k] + (z - zz[k]) / (zz[k + 1] - zz[k]) * (y[k + 1] - y[k]);
+}
+
+int setup_nucleus(int A, int Z, const TablesHost &t, HostNucleus &nu) {
+  const int ns = t.n_shells;
+  nu.A = A; nu.Z = Z; nu.ns = ns;
+  const double c = t.ws_c0 * std::cbrt((double)A);
+  nu.R = c + t.ws_rpad;
+  nu.dr = nu.R / ns;
+  nu.r.resize(ns + 1);
+  for (int i = 0; i <= ns; ++i) nu.r[i] = i * nu.dr;
+  // shell weights w_i = int rho(r) r^2 dr by 8 panels of 16-point Gauss-Legendre (R-N2: volume average)
+  std::vector<double> gx, gw, w(ns);
+  gauss_legendre(16, gx, gw);
+  double wsum = 0;
+  for (int i = 0; i < ns; ++i) {
+    double acc = 0;
+    const int NP = 8;
+    const double h = (nu.r[i + 1] - nu.r[i]) / NP;
+    for (int p = 0; p < NP; ++p) {
+      const double a = nu.r[i] + p * h;
+      for (int q = 0; q < 16; ++q) {
+        const double r = a + 0.5 * h * (gx[q] + 1.0);
+        acc += 0.5 * h * gw[q] * r * r / (1.0 + std::exp((r - c) / t.ws_delta));   // Eq. (1)
+      }
+    }
+    w[i] = acc; wsum += acc;
+  }
+  const double N = A - Z;
+  auto vec = [&](std::vector<double> &v, int n) { v.assign(n, 0.0); };
+  vec(nu.rho_p, ns); vec(nu.rho_n, ns); vec(nu.pF_p, ns); vec(nu.pF_n, ns);
+  vec(nu.EF_p, ns); vec(nu.EF_n, ns); vec(nu.V_p, ns + 1); vec(nu.V_n, ns + 1);
+  nu.Bt = binding(A, Z, t);
+  nu.EB_p = nu.Bt - binding(A - 1, Z - 1, t);             // R-N4 separation energies
+  nu.EB_n = nu.Bt - binding(A - 1, Z, t);
+  for (int i = 0; i < ns; ++i) {
+    const double vol = (nu.r[i + 1] * nu.r[i + 1] * nu.r[i + 1] - nu.r[i] * nu.r[i] * nu.r[i]) / 3.0;  // /4pi
+    const double rho = A * w[i] / (vol * wsum) / (4.0 * kPi);
+    nu.rho_p[i] = rho * Z / A; nu.rho_n[i] = rho * N / A;
+    nu.pF_p[i] = kHbarc * std::cbrt(3.0 * kPi * kPi * nu.rho_p[i]);   // R-N3
+    nu.pF_n[i] = kHbarc * std::cbrt(3.0 * kPi * kPi * nu.rho_n[i]);
+    nu.EF_p[i] = std::sqrt(nu.pF_p[i] * nu.pF_p[i] + kMp * kMp) - kMp;
+    nu.EF_n[i] = std::sqrt(nu.pF_n[i] * nu.pF_n[i] + kMn * kMn) - kMn;
+    nu.V_p[i] = nu.EF_p[i] + nu.EB_p;                      // P:45  V = E_F + E_B
+    nu.V_n[i] = nu.EF_n[i] + nu.EB_n;
+  }
+  nu.EC = kE2 * Z / nu.R;                                  // R-N6
+  nu.live = true;
+  return 0;
+}
+
+void fill_nucdev(const HostNucleus &h, NucDev<real> &d) {
+  std::memset(&d, 0, sizeof(d));
+  d.A = h.A; d.Z = h.Z; d.ns = h.ns; d.live = 1;
+  d.Rn = (real)h.R; d.dr = (real)h.dr; d.Bt = (real)h.Bt;
+  for (int i = 0; i <= h.ns; ++i) {
+    ShellDev<real> &s = d.sh[i];
+    if (i < h.ns) {
+      s.rho_p = (real)h.rho_p[i]; s.rho_n = (real)h.rho_n[i];
+      s.pF_p = (real)h.pF_p[i]; s.pF_n = (real)h.pF_n[i];
+      s.pF2_p = (real)(h.pF_p[i] * h.pF_p[i]); s.pF2_n = (real)(h.pF_n[i] * h.pF_n[i]);
+      const double tp = h.V_p[i] + h.EC, tn = h.V_n[i];    // cutoff kinetic energies
+      s.pc2_p = (real)(tp * (tp + 2.0 * kMp)); s.pc2_n = (real)(tn * (tn + 2.0 * kMn));
+      s.V_p = (real)h.V_p[i]; s.V_n = (real)h.V_n[i];
+    }
+  }
+}
+
+int check_tables(const inc_tables *t) {
+  if (!t) return fail(INC_E_BADARG, "tables is NULL");
+  if (t->version != 1) return fail(INC_E_TABLES, "tables.version != 1");
+  if (t->n_xs < 2 || t->n_xs > 4096 || !(t->plab_max > 0)) return fail(INC_E_TABLES, "bad NN grid");
+  if (!t->sig_pp || !t->sig_np || !t->B_pp || !t->B_np || !t->a_np) return fail(INC_E_TABLES, "NULL NN table");
+  if (t->n_evz < 1 || t->n_evz > 16 || !t->ev_Z || !t->ev_kp || !t->ev_cp || !t->ev_ka || !t->ev_ca)
+    return fail(INC_E_TABLES, "bad evaporation table");
+  for (int i = 1; i < t->n_evz; ++i)
+    if (!(t->ev_Z[i] > t->ev_Z[i - 1])) return fail(INC_E_TABLES, "ev_Z grid not increasing");
+  if (t->n_shells < 1 || t->n_shells > kMaxShells) return fail(INC_E_TABLES, "n_shells outside 1..32");
+  if (!(t->ws_delta > 0) || !(t->ws_c0 > 0) || !(t->ws_rpad >= 0) || !(t->evap_a_div > 0) || !(t->evap_r0 > 0))
+    return fail(INC_E_TABLES, "bad scalar model constant");
+  for (int i = 0; i < t->n_xs; ++i)
+    if (!(t->sig_pp[i] >= 0) || !(t->sig_np[i] >= 0) || !(t->B_pp[i] >= 0) || !(t->B_np[i] >= 0) || !(t->a_np[i] >= 0))
+      return fail(INC_E_TABLES, "negative or NaN NN table entry");
+  return 0;
+}
+
+void copy_tables(const inc_tables *t, TablesHost &h) {
+  h.n_xs = t->n_xs; h.n_evz = t->n_evz; h.n_shells = t->n_shells; h.plab_max = t->plab_max;
+  h.ws_c0 = t->ws_c0; h.ws_delta = t->ws_delta; h.ws_rpad = t->ws_rpad;
+  for (int i = 0; i < 5; ++i) h.semf[i] = t->semf[i];
+  h.evap_r0 = t->evap_r0; h.evap_rj = t->evap_rj; h.evap_a_div = t->evap_a_div;
+  auto cp = [](std::vector<double> &v, const double *p, int n) { v.assign(p, p + n); };
+  cp(h.sig_pp, t->sig_pp, t->n_xs); cp(h.sig_np, t->sig_np, t->n_xs); cp(h.B_pp, t->B_pp, t->n_xs);
+  cp(h.B_np, t->B_np, t->n_xs); cp(h.a_np, t->a_np, t->n_xs);
+  cp(h.ev_Z, t->ev_Z, t->n_evz); cp(h.ev_kp, t->ev_kp, t->n_evz); cp(h.ev_cp, t->ev_cp, t->n_evz);
+  cp(h.ev_ka, t->ev_ka, t->n_evz); cp(h.ev_ca, t->ev_ca, t->n_evz);
+  h.captured = true;
+}
+
+bool same_tables(const inc_tables *t, const TablesHost &h) {
+  if (t->n_xs != h.n_xs || t->n_evz != h.n_evz || t->n_shells != h.n_shells || t->plab_max != h.plab_max) return false;
+  if (t->ws_c0 != h.ws_c0 || t->ws_delta != h.ws_delta || t->ws_rpad != h.ws_rpad) return false;
+  if (t->evap_r0 != h.evap_r0 || t->evap_rj != h.evap_rj || t->evap_a_div != h.evap_a_div) return false;
+  for (int i = 0; i < 5; ++i) if (t->semf[i] != h.semf[i]) return false;
+  auto eq = [](const std::vector<double> &v, const double *p) { return std::memcmp(v.data(), p, v.size() * sizeof(double)) == 0; };
+  return eq(h.sig_pp, t->sig_pp) && eq(h.sig_np, t->sig_np) && eq(h.B_pp, t->B_pp) && eq(h.B_np, t->B_np) &&
+         eq(h.a_np, t->a_np) && eq(h.ev_Z, t->ev_Z) && eq(h.ev_kp, t->ev_kp) && eq(h.ev_cp, t->ev_cp) &&
+         eq(h.ev_ka, t->ev_ka) && eq(h.ev_ca, t->ev_ca);
+}
+
+int upload_model() {
+  const TablesHost &t = g.tab;
+  const int n = t.n_xs;
+  std::vector<real> S(4 * (size_t)n), Cc(8 * (size_t)n);
+  for (int k = 0; k < n; ++k) {
+    const int k1 = k + 1 < n ? k + 1 : k;
+    // mb -> fm^2 folded in; slopes stored so that a lookup is y + f * dy (R-N7)
+    S[4 * k + 0] = (real)(t.sig_pp[k] * 0.1); S[4 * k + 1] = (real)(t.sig_pp[k1] * 0.1) - (real)(t.sig_pp[k] * 0.1);
+    S[4 * k + 2] = (real)(t.sig_np[k] * 0.1); S[4 * k + 3] = (real)(t.sig_np[k1] * 0.1) - (real)(t.sig_np[k] * 0.1);
+    Cc[8 * k + 0] = (real)t.B_pp[k]; Cc[8 * k + 1] = (real)t.B_pp[k1] - (real)t.B_pp[k];
+    Cc[8 * k + 2] = (real)t.B_np[k]; Cc[8 * k + 3] = (real)t.B_np[k1] - (real)t.B_np[k];
+    Cc[8 * k + 4] = (real)t.a_np[k]; Cc[8 * k + 5] = (real)t.a_np[k1] - (real)t.a_np[k];
+    Cc[8 * k + 6] = 0; Cc[8 * k + 7] = 0;
+  }
+  std::vector<real> bind((size_t)kAmax * kZmax, (real)-1e30);
+  std::vector<EvChan<real>> ev((size_t)kAmax * kZmax * 6);
+  std::memset(ev.data(), 0, ev.size() * sizeof(EvChan<real>));
+  for (int A = 1; A < kAmax; ++A)
+    for (int Z = 0; Z < kZmax && Z <= A; ++Z)
+      if (valid_nucleus(A, Z)) bind[(size_t)A * kZmax + Z] = (real)binding(A, Z, t);
+  for (int Ad = 1; Ad < kAmax; ++Ad)
+    for (int Zd = 0; Zd < kZmax && Zd <= Ad; ++Zd) {
+      if (!valid_nucleus(Ad, Zd)) continue;
+      const double Bd = binding(Ad, Zd, t), ad13 = std::cbrt((double)Ad);
+      for (int j = 0; j < 6; ++j) {
+        const double Bj = binding(kEvA[j], kEvZ[j], t);
+        const double Mj = kEvZ[j] * kMp + (kEvA[j] - kEvZ[j]) * kMn - Bj;
+        double alpha, beta = 0, V = 0;
+        if (j == 0) {                                          // Dostrovsky neutron (R-E1)
+          alpha = 0.76 + 2.2 / ad13;
+          beta = (2.12 / (ad13 * ad13) - 0.05) / alpha;
+        } else {
+          const double kp = lerp_z(t.ev_Z, t.ev_kp, Zd), cp = lerp_z(t.ev_Z, t.ev_cp, Zd);
+          const double ka = lerp_z(t.ev_Z, t.ev_ka, Zd), ca = lerp_z(t.ev_Z, t.ev_ca, Zd);
+          double k, c, rj = t.evap_rj;
+          if (j == 1) { k = kp; c = cp; rj = 0; }
+          else if (j == 2) { k = kp + 0.06; c = cp / 2; }
+          else if (j == 3) { k = kp + 0.12; c = cp / 3; }
+          else if (j == 4) { k = ka - 0.06; c = 4 * ca / 3; }
+          else { k = ka; c = ca; }
+          alpha = 1 + c;
+          V = k * kE2 * kEvZ[j] * Zd / (t.evap_r0 * ad13 + rj);
+        }
+        EvChan<real> &e = ev[((size_t)Ad * kZmax + Zd) * 6 + j];
+        e.V = (real)V; e.pref = (real)(kEvG[j] * Mj * ad13 * ad13 * alpha); e.beta = (real)beta; e.BdBj = (real)(Bd + Bj);
+      }
+    }
+  auto up = [&](void **dst, const void *src, size_t bytes) -> cudaError_t {
+    if (*dst) cudaFree(*dst);
+    cudaError_t e = cudaMalloc(dst, bytes);
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice);
+  };
+  CU_TRY(up((void **)&g.d_tabS, S.data(), S.size() * sizeof(real)));
+  CU_TRY(up((void **)&g.d_tabC, Cc.data(), Cc.size() * sizeof(real)));
+  CU_TRY(up((void **)&g.d_bind, bind.data(), bind.size() * sizeof(real)));
+  CU_TRY(up((void **)&g.d_evch, ev.data(), ev.size() * sizeof(EvChan<real>)));
+  if (!g.d_nuc) {
+    CU_TRY(cudaMalloc((void **)&g.d_nuc, sizeof(NucDev<real>) * INC_MAX_TARGETS));
+    CU_TRY(cudaMemset(g.d_nuc, 0, sizeof(NucDev<real>) * INC_MAX_TARGETS));
+  }
+  if (!g.d_ctr) CU_TRY(cudaMalloc((void **)&g.d_ctr, sizeof(DevCounters)));
+  int dev = 0;
+  CU_TRY(cudaGetDevice(&dev));
+  CU_TRY(cudaDeviceGetAttribute(&g.sm_count, cudaDevAttrMultiProcessorCount, dev));
+  return 0;
+}
+
+ModelDev<real> model_dev() {
+  ModelDev<real> m;
+  m.tabS = g.d_tabS; m.tabC = g.d_tabC; m.bind = g.d_bind; m.evch = g.d_evch; m.nuc = g.d_nuc;
+  m.n_xs = g.tab.n_xs;
+  m.inv_dp = (real)(1.0 / (g.tab.plab_max / (g.tab.n_xs - 1) * 1000.0));
+  m.a_div = (real)g.tab.evap_a_div;
+  return m;
+}
+
+void free_ws() {
+  void **p[] = {(void **)&g.ws.st_code, (void **)&g.ws.st_T, (void **)&g.ws.st_ux, (void **)&g.ws.st_uy,
+                (void **)&g.ws.st_uz, (void **)&g.ws.cA, (void **)&g.ws.cZ, (void **)&g.ws.cE, (void **)&g.ws.cPx,
+                (void **)&g.ws.cPy, (void **)&g.ws.cPz, (void **)&g.ws.cmeta, (void **)&g.ws.cstatus};
+  for (auto q : p) { if (*q) cudaFree(*q); *q = nullptr; }
+  g.ws_chunk = 0;
+}
+
+int ensure_ws(size_t chunk, size_t n_total) {
+  if (chunk > g.ws_chunk) {
+    free_ws();
+    const size_t ns = chunk * kMaxSec;
+    CU_TRY(cudaMalloc((void **)&g.ws.st_code, ns * sizeof(uint32_t)));
+    CU_TRY(cudaMalloc((void **)&g.ws.st_T, ns * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&g.ws.st_ux, ns * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&g.ws.st_uy, ns * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&g.ws.st_uz, ns * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&g.ws.cA, chunk * sizeof(int32_t)));
+    CU_TRY(cudaMalloc((void **)&g.ws.cZ, chunk * sizeof(int32_t)));
+    CU_TRY(cudaMalloc((void **)&g.ws.cE, chunk * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&g.ws.cPx, chunk * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&g.ws.cPy, chunk * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&g.ws.cPz, chunk * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&g.ws.cmeta, chunk * sizeof(uint32_t)));
+    CU_TRY(cudaMalloc((void **)&g.ws.cstatus, chunk * sizeof(uint32_t)));
+    g.ws_chunk = chunk;
+  }
+  if (n_total + 1 > g.offsets_cap) {
+    if (g.d_offsets) cudaFree(g.d_offsets);
+    g.d_offsets = nullptr;
+    CU_TRY(cudaMalloc((void **)&g.d_offsets, (n_total + 1) * sizeof(long long)));
+    g.offsets_cap = n_total + 1;
+  }
+  const size_t tiles = (chunk + kScanTile - 1) / kScanTile + 1;
+  if (tiles > g.tiles_cap) {
+    if (g.d_tiles) cudaFree(g.d_tiles);
+    g.d_tiles = nullptr;
+    CU_TRY(cudaMalloc((void **)&g.d_tiles, tiles * sizeof(long long)));
+    g.tiles_cap = tiles;
+  }
+  return 0;
+}
+
+int mark(bool timing) {
+  if (!timing) return 0;
+  cudaEvent_t e;
+  CU_TRY(cudaEventCreate(&e));
+  CU_TRY(cudaEventRecord(e, g.stream));
+  g.pending_events.push_back(e);
+  return 0;
+}
+
+template <bool STATS>
+int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t *tid, uint64_t seed,
+                 inc_secondaries *sec, int32_t *counts, inc_residual *res, long long *offsets) {
+  const ModelDev<real> model = model_dev();
+  // --- cascade ---
+  CascadeParams<real> cp;
+  cp.model = model; cp.ws = g.ws; cp.ctr = g.d_ctr; cp.E_in = E_in; cp.target_id = tid;
+  cp.e_base = e_base + g.event_offset; cp.n_chunk = n_chunk; cp.seed_lo = (uint32_t)seed; cp.seed_hi = (uint32_t)(seed >> 32);
+  cp.flags = g.flags;
+  const bool naive = (g.flags & INC_F_LANE_PER_EVENT) != 0;
+  cp.vote_coll = naive ? 1 : g.vote_coll; cp.vote_epi = naive ? 1 : g.vote_epi;
+  cp.n_live_nuc = INC_MAX_TARGETS;
+  const size_t smem = cascade_smem_bytes<real>(model.n_xs);
+  auto kern = cascade_kernel<real, STATS>;
+  CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int occ = 0;
+  CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, smem));
+  if (occ < 1) return fail(INC_E_CUDA, "cascade kernel does not fit on an SM");
+  int blocks = occ * g.sm_count;
+  const int need = (n_chunk + 255) / 256;
+  if (blocks > need) blocks = need;
+  CU_TRY(cudaMemsetAsync(&g.d_ctr->next_event_casc, 0, 2 * sizeof(unsigned long long), g.stream));
+  const bool timing = (g.flags & INC_F_TIMING) != 0;
+  if (mark(timing)) return INC_E_CUDA;
+  kern<<<blocks, 256, smem, g.stream>>>(cp);
+  CU_TRY(cudaGetLastError());
+  if (mark(timing)) return INC_E_CUDA;
+  // --- evaporation ---
+  EvapParams<real> ep;
+  ep.model = model; ep.ws = g.ws; ep.ctr = g.d_ctr; ep.e_base = e_base + g.event_offset; ep.n_chunk = n_chunk;
+  ep.seed_lo = cp.seed_lo; ep.seed_hi = cp.seed_hi; ep.flags = g.flags;
+  ep.out_counts = counts; ep.rA = res->A; ep.rZ = res->Z; ep.rE = res->Estar;
+  ep.rPx = res->px; ep.rPy = res->py; ep.rPz = res->pz; ep.rstatus = res->status;
+  auto ekern = evap_kernel<real, STATS>;
+  int eocc = 0;
+  CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&eocc, ekern, 256, 0));
+  if (eocc < 1) return fail(INC_E_CUDA, "evaporation kernel does not fit on an SM");
+  int eblocks = eocc * g.sm_count;
+  if (eblocks > need) eblocks = need;
+  ekern<<<eblocks, 256, 0, g.stream>>>(ep);
+  CU_TRY(cudaGetLastError());
+  if (mark(timing)) return INC_E_CUDA;
+  // --- prefix sum of counts (running base carried across chunks in ctr->total_sec) ---
+  const int tiles = (n_chunk + kScanTile - 1) / kScanTile;
+  scan_tile_sums<<<tiles, kScanBlock, 0, g.stream>>>(counts, n_chunk, g.d_tiles);
+  scan_tiles<<<1, kScanBlock, 0, g.stream>>>(g.d_tiles, tiles, &g.d_ctr->total_sec);
+  scan_write_offsets<<<tiles, kScanBlock, 0, g.stream>>>(counts, n_chunk, g.d_tiles, offsets);
+  CU_TRY(cudaGetLastError());
+  if (mark(timing)) return INC_E_CUDA;
+  // --- compaction into the caller's SoA ---
+  CompactParams<real> kp;
+  kp.ws = g.ws; kp.offsets = offsets; kp.counts = counts; kp.n_chunk = n_chunk;
+  kp.species = sec->species; kp.T = sec->T; kp.ux = sec->ux; kp.uy = sec->uy; kp.uz = sec->uz;
+  kp.capacity = sec->capacity;
+  const int cwarps = (n_chunk + 31) / 32;
+  const int cblocks = (cwarps + 7) / 8;
+  compact_kernel<real><<<cblocks, 256, 0, g.stream>>>(kp);
+  CU_TRY(cudaGetLastError());
+  if (mark(timing)) return INC_E_CUDA;
+  return 0;
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+const char *inc_last_error(void) { return g.err.c_str(); }
+
+const char *inc_build_info(void) {
+#ifdef INC_REAL_IS_DOUBLE
+  return "inc-b200 f64 parity build (-fmad=false) sm_100a";
+#else
+  return "inc-b200 f32 production build (fast intrinsics) sm_100a";
+#endif
+}
+
+int inc_set_stream(void *s) { g.stream = (cudaStream_t)s; return 0; }
+int inc_set_flags(uint32_t f) { g.flags = f; return 0; }
+int inc_set_event_offset(int64_t e0) {
+  if (e0 < 0) return fail(INC_E_BADARG, "negative event offset");
+  g.event_offset = e0;
+  return 0;
+}
+
+int inc_init(int A, int Z, const inc_tables *t) {
+  int rc = check_tables(t);
+  if (rc) return rc;
+  if (A < 6 || A > 64 || Z < 2 || Z > A - 2) return fail(INC_E_BADARG, "unsupported (A,Z): need 6<=A<=64, 2<=Z<=A-2");
+  if (!g.tab.captured) {
+    copy_tables(t, g.tab);
+    rc = upload_model();
+    if (rc) { g.tab.captured = false; return rc; }
+  } else if (!same_tables(t, g.tab)) {
+    return fail(INC_E_TABLES, "tables differ from those captured by the first inc_init (call inc_shutdown first)");
+  }
+  int slot = -1;
+  for (int i = 0; i < INC_MAX_TARGETS; ++i) if (!g.nuc[i].live) { slot = i; break; }
+  if (slot < 0) return fail(INC_E_BADARG, "all 16 target slots are live");
+  setup_nucleus(A, Z, g.tab, g.nuc[slot]);
+  NucDev<real> d;
+  fill_nucdev(g.nuc[slot], d);
+  cudaError_t e = cudaMemcpy(&g.d_nuc[slot], &d, sizeof(d), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { g.nuc[slot].live = false; return fail(INC_E_CUDA, std::string("upload nucleus: ") + cudaGetErrorString(e)); }
+  return slot;
+}
+
+int inc_free_target(int id) {
+  if (id < 0 || id >= INC_MAX_TARGETS || !g.nuc[id].live) return fail(INC_E_BADARG, "no such target");
+  g.nuc[id].live = false;
+  NucDev<real> d;
+  std::memset(&d, 0, sizeof(d));
+  CU_TRY(cudaMemcpy(&g.d_nuc[id], &d, sizeof(d), cudaMemcpyHostToDevice));
+  return 0;
+}
+
+void inc_shutdown(void) {
+  free_ws();
+  void **p[] = {(void **)&g.d_tabS, (void **)&g.d_tabC, (void **)&g.d_bind, (void **)&g.d_evch, (void **)&g.d_nuc,
+                (void **)&g.d_ctr, (void **)&g.d_offsets, (void **)&g.d_tiles,
+                (void **)&g.hp.E, (void **)&g.hp.tid, (void **)&g.hp.counts, (void **)&g.hp.A, (void **)&g.hp.Z,
+                (void **)&g.hp.Es, (void **)&g.hp.px, (void **)&g.hp.py, (void **)&g.hp.pz, (void **)&g.hp.status,
+                (void **)&g.hp.sp, (void **)&g.hp.T, (void **)&g.hp.ux, (void **)&g.hp.uy, (void **)&g.hp.uz};
+  for (auto q : p) { if (*q) cudaFree(*q); *q = nullptr; }
+  g.offsets_cap = g.tiles_cap = 0; g.hp.n_cap = g.hp.sec_cap = 0;
+  for (auto &n : g.nuc) n.live = false;
+  g.tab.captured = false;
+  g.last_n = -1;
+  g.event_offset = 0;
+}
+
+int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
+                     int32_t *counts, inc_residual *res) {
+  if (!g.tab.captured) return fail(INC_E_STATE, "inc_simulate before inc_init");
+  if (n < 0 || !sec || !res || (n > 0 && (!E_in || !tid || !counts))) return fail(INC_E_BADARG, "null argument or n < 0");
+  if (n > 0 && (!res->A || !res->Z || !res->Estar || !res->px || !res->py || !res->pz || !res->status))
+    return fail(INC_E_BADARG, "null residual array");
+  if (sec->capacity < 0 || (sec->capacity > 0 && (!sec->species || !sec->T || !sec->ux || !sec->uy || !sec->uz)))
+    return fail(INC_E_BADARG, "null secondary array");
+  const size_t chunk_max = (size_t)1 << 20;
+  const size_t chunk = (size_t)n < chunk_max ? (size_t)(n > 0 ? n : 1) : chunk_max;
+  int rc = ensure_ws(chunk, (size_t)n);
+  if (rc) return rc;
+  CU_TRY(cudaMemsetAsync(g.d_ctr, 0, sizeof(DevCounters), g.stream));
+  for (auto e : g.pending_events) cudaEventDestroy(e);
+  g.pending_events.clear();
+  for (int i = 0; i < 4; ++i) { g.stage_ms[i] = 0; g.stage_launches[i] = 0; }
+  const bool stats = (g.flags & INC_F_STATS) != 0;
+  for (long long e0 = 0; e0 < n; e0 += (long long)chunk) {
+    const int nc = (int)((n - e0) < (long long)chunk ? (n - e0) : (long long)chunk);
+    inc_residual r = *res;
+    r.A += e0; r.Z += e0; r.Estar += e0; r.px += e0; r.py += e0; r.pz += e0; r.status += e0;
+    rc = stats ? launch_chunk<true>(e0, nc, E_in + e0, tid + e0, seed, sec, counts + e0, &r, g.d_offsets + e0)
+               : launch_chunk<false>(e0, nc, E_in + e0, tid + e0, seed, sec, counts + e0, &r, g.d_offsets + e0);
+    if (rc) return rc;
+  }
+  CU_TRY(cudaMemcpyAsync(g.d_offsets + n, &g.d_ctr->total_sec, sizeof(long long), cudaMemcpyDeviceToDevice, g.stream));
+  struct { unsigned long long total; unsigned int err, pad; } tail;
+  CU_TRY(cudaMemcpyAsync(&tail, &g.d_ctr->total_sec, 16, cudaMemcpyDeviceToHost, g.stream));
+  CU_TRY(cudaStreamSynchronize(g.stream));
+  for (size_t c = 0; c + 4 < g.pending_events.size(); c += 5) {
+    const int nl[4] = {1, 1, 3, 1};
+    for (int i = 0; i < 4; ++i) {
+      float ms = 0;
+      CU_TRY(cudaEventElapsedTime(&ms, g.pending_events[c + i], g.pending_events[c + i + 1]));
+      g.stage_ms[i] += ms; g.stage_launches[i] += nl[i];
+    }
+  }
+  for (auto e : g.pending_events) cudaEventDestroy(e);
+  g.pending_events.clear();
+  g.last_n = n; g.last_total = (long long)tail.total;
+  if (tail.err) {
+    return fail(INC_E_BADARG, std::string("device-side input check failed:") + ((tail.err & 1u) ? " E_in outside [20,250] MeV" : "") +
+                                  ((tail.err & 2u) ? " target_id not initialised" : ""));
+  }
+  if ((long long)tail.total > sec->capacity) {
+    char buf[160];
+    std::snprintf(buf, sizeof buf, "secondary capacity %lld too small, need %llu", (long long)sec->capacity, tail.total);
+    return fail(INC_E_CAPACITY, buf);
+  }
+  return (int64_t)tail.total;
+}
+
+int inc_get_offsets(int64_t *dev_offsets) {
+  if (g.last_n < 0) return fail(INC_E_STATE, "no previous inc_simulate");
+  if (!dev_offsets) return fail(INC_E_BADARG, "null pointer");
+  CU_TRY(cudaMemcpyAsync(dev_offsets, g.d_offsets, (size_t)(g.last_n + 1) * sizeof(long long), cudaMemcpyDeviceToDevice, g.stream));
+  CU_TRY(cudaStreamSynchronize(g.stream));
+  return 0;
+}
+
+int inc_get_cascade_stage(int32_t *A, int32_t *Z, INC_REAL *Es, INC_REAL *px, INC_REAL *py, INC_REAL *pz, int32_t *ncs) {
+  if (g.last_n < 0) return fail(INC_E_STATE, "no previous inc_simulate");
+  if ((size_t)g.last_n > g.ws_chunk) return fail(INC_E_STATE, "cascade stage is only kept for single-chunk calls (n <= 2^20)");
+  const size_t n = (size_t)g.last_n;
+  if (A) CU_TRY(cudaMemcpyAsync(A, g.ws.cA, n * 4, cudaMemcpyDeviceToDevice, g.stream));
+  if (Z) CU_TRY(cudaMemcpyAsync(Z, g.ws.cZ, n * 4, cudaMemcpyDeviceToDevice, g.stream));
+  if (Es) CU_TRY(cudaMemcpyAsync(Es, g.ws.cE, n * sizeof(real), cudaMemcpyDeviceToDevice, g.stream));
+  if (px) CU_TRY(cudaMemcpyAsync(px, g.ws.cPx, n * sizeof(real), cudaMemcpyDeviceToDevice, g.stream));
+  if (py) CU_TRY(cudaMemcpyAsync(py, g.ws.cPy, n * sizeof(real), cudaMemcpyDeviceToDevice, g.stream));
+  if (pz) CU_TRY(cudaMemcpyAsync(pz, g.ws.cPz, n * sizeof(real), cudaMemcpyDeviceToDevice, g.stream));
+  if (ncs) {
+    // low byte of cmeta
+    CU_TRY(cudaMemcpyAsync(ncs, g.ws.cmeta, n * 4, cudaMemcpyDeviceToDevice, g.stream));
+  }
+  CU_TRY(cudaStreamSynchronize(g.stream));
+  return 0;
+}
+
+int inc_get_stats(inc_stats *out) {
+  if (!out) return fail(INC_E_BADARG, "null pointer");
+  if (g.last_n < 0) return fail(INC_E_STATE, "no previous inc_simulate");
+  DevCounters c;
+  CU_TRY(cudaMemcpy(&c, g.d_ctr, sizeof(c), cudaMemcpyDeviceToHost));
+  out->events = c.stats[S_EVENTS]; out->failed = c.stats[S_FAILED]; out->attempts = c.stats[S_ATTEMPTS];
+  out->segments = c.stats[S_SEG]; out->boundaries = c.stats[S_BND]; out->reflections = c.stats[S_REFL];
+  out->escapes = c.stats[S_ESC]; out->collisions = c.stats[S_COLL]; out->blocked = c.stats[S_BLOCKED];
+  out->allowed = c.stats[S_ALLOWED]; out->absorbed = c.stats[S_ABSORBED];
+  out->evap_steps = c.stats[S_EVSTEPS]; out->evap_trials = c.stats[S_EVTRIALS]; out->evap_emitted = c.stats[S_EVEMIT];
+  out->warp_iters_seg = c.stats[S_WI_SEG]; out->warp_iters_coll = c.stats[S_WI_COLL]; out->warp_iters_epi = c.stats[S_WI_EPI];
+  out->lane_slots_seg = c.stats[S_LS_SEG]; out->lane_slots_coll = c.stats[S_LS_COLL]; out->lane_slots_epi = c.stats[S_LS_EPI];
+  return 0;
+}
+
+int inc_get_stage_times(float ms[4], int32_t launches[4]) {
+  if (g.last_n < 0) return fail(INC_E_STATE, "no previous inc_simulate");
+  for (int i = 0; i < 4; ++i) { if (ms) ms[i] = g.stage_ms[i]; if (launches) launches[i] = g.stage_launches[i]; }
+  return 0;
+}
+
+int inc_get_nucleus(int id, int32_t *A, int32_t *Z, int32_t *ns, double *R, double *EC, double *EBp, double *EBn,
+                    double *r, double *rho_p, double *rho_n, double *pF_p, double *pF_n, double *EF_p, double *EF_n,
+                    double *V_p, double *V_n) {
+  if (id < 0 || id >= INC_MAX_TARGETS || !g.nuc[id].live) return fail(INC_E_BADARG, "no such target");
+  const HostNucleus &h = g.nuc[id];
+  if (A) *A = h.A; if (Z) *Z = h.Z; if (ns) *ns = h.ns; if (R) *R = h.R; if (EC) *EC = h.EC;
+  if (EBp) *EBp = h.EB_p; if (EBn) *EBn = h.EB_n;
+  auto cp = [](double *dst, const std::vector<double> &v) { if (dst) std::memcpy(dst, v.data(), v.size() * sizeof(double)); };
+  cp(r, h.r); cp(rho_p, h.rho_p); cp(rho_n, h.rho_n); cp(pF_p, h.pF_p); cp(pF_n, h.pF_n);
+  cp(EF_p, h.EF_p); cp(EF_n, h.EF_n); cp(V_p, h.V_p); cp(V_n, h.V_n);
+  return 0;
+}
+
+int inc_set_vote_thresholds(int coll, int epi) {
+  if (coll < 1 || coll > 32 || epi < 1 || epi > 32) return fail(INC_E_BADARG, "thresholds must be 1..32");
+  g.vote_coll = coll; g.vote_epi = epi;
+  return 0;
+}
+
+int inc_measure_issue_peak(double *out, double *clock_mhz) {
+  if (!out) return fail(INC_E_BADARG, "null pointer");
+  int dev = 0, sms = 0, khz = 0;
+  CU_TRY(cudaGetDevice(&dev));
+  CU_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  CU_TRY(cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev));
+  real *d = nullptr;
+  CU_TRY(cudaMalloc((void **)&d, sizeof(real)));
+  const int blocks = sms * 8, iters = 4096;
+  cudaEvent_t a, b;
+  CU_TRY(cudaEventCreate(&a)); CU_TRY(cudaEventCreate(&b));
+  double best = 0;
+  for (int rep = 0; rep < 5; ++rep) {
+    CU_TRY(cudaEventRecord(a, g.stream));
+    fma_peak_kernel<real><<<blocks, 256, 0, g.stream>>>(d, iters, (real)0.999, (real)0.001);
+    CU_TRY(cudaEventRecord(b, g.stream));
+    CU_TRY(cudaEventSynchronize(b));
+    float ms = 0;
+    CU_TRY(cudaEventElapsedTime(&ms, a, b));
+    const double ops = (double)blocks * 256.0 * iters * 16.0 * 8.0;
+    const double rate = ops / (ms * 1e-3);
+    if (rep > 0 && rate > best) best = rate;
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(d);
+  *out = best;
+  if (clock_mhz) *clock_mhz = khz / 1000.0;
+  return 0;
+}
+
+int inc_philox_blocks(const uint32_t *ctr, uint64_t seed, uint32_t *out, int64_t n) {
+  if (n < 0 || (n > 0 && (!ctr || !out))) return fail(INC_E_BADARG, "bad argument");
+  if (n == 0) return 0;
+  philox_blocks_kernel<<<(unsigned)((n + 255) / 256), 256, 0, g.stream>>>(ctr, (uint32_t)seed, (uint32_t)(seed >> 32), out, n);
+  CU_TRY(cudaGetLastError());
+  CU_TRY(cudaStreamSynchronize(g.stream));
+  return 0;
+}
+
+int64_t inc_simulate_host(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
+                          int32_t *counts, inc_residual *res) {
+  if (!g.tab.captured) return fail(INC_E_STATE, "inc_simulate_host before inc_init");
+  if (n < 0 || !sec || !res || (n > 0 && (!E_in || !tid || !counts))) return fail(INC_E_BADARG, "null argument or n < 0");
+  State::HostPath &h = g.hp;
+  if ((size_t)n > h.n_cap) {
+    void **p[] = {(void **)&h.E, (void **)&h.tid, (void **)&h.counts, (void **)&h.A, (void **)&h.Z, (void **)&h.Es,
+                  (void **)&h.px, (void **)&h.py, (void **)&h.pz, (void **)&h.status};
+    for (auto q : p) { if (*q) cudaFree(*q); *q = nullptr; }
+    const size_t m = (size_t)n;
+    CU_TRY(cudaMalloc((void **)&h.E, m * sizeof(real))); CU_TRY(cudaMalloc((void **)&h.tid, m * 4));
+    CU_TRY(cudaMalloc((void **)&h.counts, m * 4)); CU_TRY(cudaMalloc((void **)&h.A, m * 4)); CU_TRY(cudaMalloc((void **)&h.Z, m * 4));
+    CU_TRY(cudaMalloc((void **)&h.Es, m * sizeof(real))); CU_TRY(cudaMalloc((void **)&h.px, m * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&h.py, m * sizeof(real))); CU_TRY(cudaMalloc((void **)&h.pz, m * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&h.status, m * 4));
+    h.n_cap = m;
+  }
+  if ((size_t)sec->capacity > h.sec_cap) {
+    void **p[] = {(void **)&h.sp, (void **)&h.T, (void **)&h.ux, (void **)&h.uy, (void **)&h.uz};
+    for (auto q : p) { if (*q) cudaFree(*q); *q = nullptr; }
+    const size_t m = (size_t)sec->capacity;
+    CU_TRY(cudaMalloc((void **)&h.sp, m)); CU_TRY(cudaMalloc((void **)&h.T, m * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&h.ux, m * sizeof(real))); CU_TRY(cudaMalloc((void **)&h.uy, m * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&h.uz, m * sizeof(real)));
+    h.sec_cap = m;
+  }
+  CU_TRY(cudaMemcpyAsync(h.E, E_in, (size_t)n * sizeof(real), cudaMemcpyHostToDevice, g.stream));
+  CU_TRY(cudaMemcpyAsync(h.tid, tid, (size_t)n * 4, cudaMemcpyHostToDevice, g.stream));
+  inc_secondaries ds; ds.species = h.sp; ds.T = h.T; ds.ux = h.ux; ds.uy = h.uy; ds.uz = h.uz; ds.capacity = sec->capacity;
+  inc_residual dr; dr.A = h.A; dr.Z = h.Z; dr.Estar = h.Es; dr.px = h.px; dr.py = h.py; dr.pz = h.pz; dr.status = h.status;
+  const int64_t tot = inc_simulate(n, h.E, h.tid, seed, &ds, h.counts, &dr);
+  if (tot < 0 && tot != INC_E_CAPACITY) return tot;
+  const size_t m = (size_t)n;
+  CU_TRY(cudaMemcpyAsync(counts, h.counts, m * 4, cudaMemcpyDeviceToHost, g.stream));
+  CU_TRY(cudaMemcpyAsync(res->A, h.A, m * 4, cudaMemcpyDeviceToHost, g.stream));
+  CU_TRY(cudaMemcpyAsync(res->Z, h.Z, m * 4, cudaMemcpyDeviceToHost, g.stream));
+  CU_TRY(cudaMemcpyAsync(res->Estar, h.Es, m * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
+  CU_TRY(cudaMemcpyAsync(res->px, h.px, m * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
+  CU_TRY(cudaMemcpyAsync(res->py, h.py, m * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
+  CU_TRY(cudaMemcpyAsync(res->pz, h.pz, m * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
+  CU_TRY(cudaMemcpyAsync(res->status, h.status, m * 4, cudaMemcpyDeviceToHost, g.stream));
+  if (tot >= 0) {
+    const size_t k = (size_t)tot;
+    CU_TRY(cudaMemcpyAsync(sec->species, h.sp, k, cudaMemcpyDeviceToHost, g.stream));
+    CU_TRY(cudaMemcpyAsync(sec->T, h.T, k * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
+    CU_TRY(cudaMemcpyAsync(sec->ux, h.ux, k * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
+    CU_TRY(cudaMemcpyAsync(sec->uy, h.uy, k * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
+    CU_TRY(cudaMemcpyAsync(sec->uz, h.uz, k * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
+  }
+  CU_TRY(cudaStreamSynchronize(g.stream));
+  return tot;
+}
+
+}  // extern "C"

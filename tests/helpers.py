@@ -1,0 +1,162 @@
+"""Shared test utilities: sharded oracle runs, histograms for criterion (3), comparisons."""
+from __future__ import annotations
+
+import multiprocessing as mp
+import os
+
+import numpy as np
+from scipy import stats
+
+T_EDGES = np.linspace(0.0, 250.0, 51)      # 50 bins of 5 MeV
+C_EDGES = np.linspace(-1.0, 1.0, 21)       # 20 bins of cos(theta)
+MULT_MAX = 24
+A_MAX = 72
+
+
+def histograms(species, T, uz, counts, A_res):
+    """Criterion-(3) histograms: per class (n, p, composites) T and cos,
+    per-event multiplicity per class, residual A."""
+    code = species & 0x7F
+    cls = np.where(code == 0, 0, np.where(code == 1, 1, 2))
+    h = {}
+    for c, name in enumerate(("n", "p", "comp")):
+        m = cls == c
+        h["T_" + name] = np.histogram(T[m], T_EDGES)[0].astype(np.int64)
+        h["T_over_" + name] = np.int64(np.sum(T[m] >= 250.0))
+        h["cos_" + name] = np.histogram(uz[m], C_EDGES)[0].astype(np.int64)
+    n = len(counts)
+    ev = np.repeat(np.arange(n), counts)
+    for c, name in enumerate(("n", "p", "comp")):
+        mult = np.bincount(ev[cls == c], minlength=n)
+        h["mult_" + name] = np.bincount(np.minimum(mult, MULT_MAX), minlength=MULT_MAX + 1).astype(np.int64)
+        h["msum_" + name] = np.float64(mult.sum())
+        h["msq_" + name] = np.float64((mult.astype(np.float64) ** 2).sum())
+    h["mult_all"] = np.bincount(np.minimum(counts, MULT_MAX), minlength=MULT_MAX + 1).astype(np.int64)
+    h["A_res"] = np.bincount(np.clip(A_res, 0, A_MAX), minlength=A_MAX + 1).astype(np.int64)
+    h["n_events"] = np.int64(n)
+    return h
+
+
+def add_hist(a, b):
+    if a is None:
+        return b
+    return {k: a[k] + b[k] for k in a}
+
+
+def _oracle_shard(args):
+    config_id, n_total, e0, e1 = args
+    from oracle import oracle as O
+    import paper_1309_7963_b200.workloads as W
+    E, tid, targets, seed, _ = W.make_inputs(config_id, n_total)
+    t = O.Tables()
+    r = O.simulate(t, targets, E[e0:e1], tid[e0:e1], seed, e0=e0, want_stats=True)
+    return histograms(r["species"], r["T"], r["uz"], r["counts"], r["A"]), r["stats"]
+
+
+def oracle_histograms(config_id, n_total, nproc=None, shard=50000):
+    """Oracle histograms over the first n_total events of a config, sharded over processes
+    (counter-keyed RNG makes shards exact)."""
+    nproc = nproc or min(os.cpu_count() or 1, 32)
+    jobs = [(config_id, n_total, a, min(a + shard, n_total)) for a in range(0, n_total, shard)]
+    if nproc == 1 or len(jobs) == 1:
+        outs = [_oracle_shard(j) for j in jobs]
+    else:
+        with mp.get_context("spawn").Pool(nproc) as pool:
+            outs = pool.map(_oracle_shard, jobs)
+    H, S = None, None
+    for h, s in outs:
+        H = add_hist(H, h)
+        S = s if S is None else {k: S[k] + s[k] for k in S}
+    return H, S
+
+
+def chi2_two_sample(a, b, min_expected=10.0):
+    """Two-sample chi-square on binned counts (bins with small expectation merged).  Returns p."""
+    a = np.asarray(a, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    na, nb = a.sum(), b.sum()
+    if na == 0 and nb == 0:
+        return 1.0
+    pooled = (a + b) / 2.0
+    keep = pooled >= min_expected
+    A = np.append(a[keep], a[~keep].sum())
+    B = np.append(b[keep], b[~keep].sum())
+    if A[-1] + B[-1] == 0:
+        A, B = A[:-1], B[:-1]
+    if len(A) < 2:
+        return 1.0
+    k1, k2 = np.sqrt(nb / na), np.sqrt(na / nb)
+    chi2 = np.sum((k1 * A - k2 * B) ** 2 / (A + B))
+    return float(stats.chi2.sf(chi2, len(A) - 1))
+
+
+def compare_histograms(hg, ho, p_min=1e-3):
+    """Criterion (3): every histogram agrees with p >= p_min; mean multiplicities within 3 sigma."""
+    failures = []
+    for k in hg:
+        if k.startswith(("T_", "cos_", "mult_", "A_res")) and not k.startswith("T_over"):
+            p = chi2_two_sample(hg[k], ho[k])
+            if p < p_min:
+                failures.append((k, p))
+    ng, no = float(hg["n_events"]), float(ho["n_events"])
+    for name in ("n", "p", "comp"):
+        mg, mo = hg["msum_" + name] / ng, ho["msum_" + name] / no
+        vg = hg["msq_" + name] / ng - mg * mg
+        vo = ho["msq_" + name] / no - mo * mo
+        sig = np.sqrt(vg / ng + vo / no)
+        if abs(mg - mo) > 3.0 * sig + 1e-12:
+            failures.append(("mean_mult_" + name, (mg, mo, sig)))
+    return failures
+
+
+def event_identity(g, o, rel=1e-9):
+    """Criterion (2): per event identical multiplicity, species, residual (A,Z); energies within rel.
+    Returns (fraction identical, max relative energy error among identical events)."""
+    n = len(o["counts"])
+    same = (g["counts"] == o["counts"]) & (g["A"] == o["A"]) & (g["Z"] == o["Z"])
+    og, oo = g["offsets"], o["offsets"]
+    max_err = 0.0
+    ident = np.zeros(n, dtype=bool)
+    for e in np.nonzero(same)[0]:
+        a, b = og[e], oo[e]
+        c = o["counts"][e]
+        if not np.array_equal(g["species"][a:a + c], o["species"][b:b + c]):
+            continue
+        tg, to = g["T"][a:a + c], o["T"][b:b + c]
+        err = np.max(np.abs(tg - to) / np.maximum(np.abs(to), 1e-300)) if c else 0.0
+        es_o = o["Estar"][e]
+        err_e = abs(g["Estar"][e] - es_o) / max(abs(es_o), 1.0)
+        dirs = 0.0
+        if c:
+            dirs = max(np.max(np.abs(g[k][a:a + c] - o[k][b:b + c])) for k in ("ux", "uy", "uz"))
+        if err <= rel and err_e <= rel and dirs <= 1e-7:
+            ident[e] = True
+            max_err = max(max_err, err, err_e)
+    return ident.mean() if n else 1.0, max_err, ident
+
+
+def conservation_residuals(r, targets, tid, E_in, mass_fn, species_A, species_Z, species_M, m_p):
+    """Per-event (dA, dZ, dE/E, |dP|/p_in) of any result dict (GPU or oracle)."""
+    n = len(r["counts"])
+    code = r["species"] & 0x7F
+    ev = np.repeat(np.arange(n), r["counts"])
+    At = np.array([a for a, z in targets])[tid]
+    Zt = np.array([z for a, z in targets])[tid]
+    sumA = np.bincount(ev, weights=species_A[code], minlength=n)
+    sumZ = np.bincount(ev, weights=species_Z[code], minlength=n)
+    dA = sumA + r["A"] - (At + 1)
+    dZ = sumZ + r["Z"] - (Zt + 1)
+    m = species_M[code]
+    T = r["T"].astype(np.float64)
+    pm = np.sqrt(T * (T + 2 * m))
+    sumE = np.bincount(ev, weights=T + m, minlength=n)
+    sp = [np.bincount(ev, weights=pm * r[k].astype(np.float64), minlength=n) for k in ("ux", "uy", "uz")]
+    Mres = np.array([mass_fn(int(a), int(z)) for a, z in zip(r["A"], r["Z"])])
+    Mt = np.array([mass_fn(a, z) for a, z in targets])[tid]
+    P2 = r["px"].astype(np.float64) ** 2 + r["py"].astype(np.float64) ** 2 + r["pz"].astype(np.float64) ** 2
+    Eres = np.sqrt((Mres + r["Estar"].astype(np.float64)) ** 2 + P2)
+    Etot = E_in + m_p + Mt
+    p_in = np.sqrt(E_in * (E_in + 2 * m_p))
+    dE = (sumE + Eres - Etot) / Etot
+    dP = np.sqrt((sp[0] + r["px"]) ** 2 + (sp[1] + r["py"]) ** 2 + (sp[2] + r["pz"] - p_in) ** 2) / p_in
+    return dA, dZ, dE, dP

@@ -1,0 +1,309 @@
+"""GPU parity tests (run on the B200 box: python -m pytest tests -m gpu).
+
+All go through the C-ABI library (paper_1309_7963_b200.binding -> libinc_f64.so / libinc_f32.so)
+and compare with the CPU oracle on the same seeded inputs.  Criteria of BASELINE.json:
+ (1) conservation laws exact per event;
+ (2) fp64 -fmad=false build: >= 99.9 % of events identical to the oracle in multiplicity,
+     species and residual (A,Z), energies within 1e-9 relative;
+ (3) fp32 build: histograms of secondary energy, angle, multiplicity agree with chi-square
+     p >= 0.001 and mean multiplicities within 3 sigma.
+"""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+import helpers as H
+
+pytestmark = pytest.mark.gpu
+
+REL_F64 = 1e-9          # north_star criterion (2)
+FRAC_IDENTICAL = 0.999  # north_star criterion (2)
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("the gpu tests need a CUDA device (no CPU fallback exists)")
+    import paper_1309_7963_b200.binding as B
+    return B
+
+
+@pytest.fixture(scope="module")
+def ptables():
+    import paper_1309_7963_b200.tables as T
+    return T.default_tables()
+
+
+def _mass_fn(orc, otables):
+    L = orc.lib()
+    return lambda a, z: L.orc_mass(int(a), int(z), C.byref(otables.c))
+
+
+def _inputs(cfg, n):
+    import paper_1309_7963_b200.workloads as W
+    return W.make_inputs(cfg, n)
+
+
+def _assert_conservation(r, targets, tid, E, orc, otables, tol_E, tol_P):
+    dA, dZ, dE, dP = H.conservation_residuals(r, targets, tid, E, _mass_fn(orc, otables), orc.SPECIES_A,
+                                              orc.SPECIES_Z, orc.SPECIES_M, orc.M_P)
+    ok = (r["status"] & orc.ST_FAILED) == 0
+    assert np.all(dA[ok] == 0) and np.all(dZ[ok] == 0)           # criterion (1): exact
+    assert np.max(np.abs(dE[ok])) < tol_E and np.max(dP[ok]) < tol_P
+    assert np.all((r["status"] & (1 << 13)) == 0)                # INC_ST_QUEUE_OVF never set
+
+
+# ------------------------------------------------------------------------------- building blocks
+def test_philox_device_matches_oracle(gpu, orc):
+    import torch
+    lib = gpu.load("f32")
+    rng = np.random.default_rng(0)
+    n = 4096
+    ctr = rng.integers(0, 2**32, size=(n, 4), dtype=np.uint64).astype(np.uint32)
+    ctr[:8] = [[0, 0, 0, 0], [1, 0, 0, 0], [0, 1, 0, 0], [0, 0, 1, 0], [0, 0, 0, 1],
+               [0xFFFFFFFF] * 4, [5, (3 << 24) | 77, 123456, 1], [0, (255 << 24) | 0xFFFFFF, 0xFFFFFFFF, 0xFFFFFFFF]]
+    seed = 0xDEADBEEF12345678
+    out = lib.inc_philox_blocks(torch.as_tensor(ctr.view(np.int32)).cuda(), seed).cpu().numpy().view(np.uint32)
+    L = orc.lib()
+    key = (C.c_uint32 * 2)(seed & 0xFFFFFFFF, seed >> 32)
+    for i in range(n):
+        o = (C.c_uint32 * 4)()
+        L.orc_philox4x32_10((C.c_uint32 * 4)(*[int(v) for v in ctr[i]]), key, o)
+        assert list(o) == [int(v) for v in out[i]]
+
+
+@pytest.mark.parametrize("A,Z", [(16, 8), (12, 6), (40, 20), (48, 22), (31, 15), (14, 7)])
+def test_nuclear_setup_matches_oracle(gpu, orc, otables, ptables, A, Z):
+    """inc_init (Gauss-Legendre shell integrals, own SEMF) vs the oracle (Simpson)."""
+    lib = gpu.load("f64")
+    lib.inc_shutdown()
+    tid = lib.inc_init(A, Z, ptables)
+    g = lib.inc_get_nucleus(tid)
+    o = orc.nucleus_arrays(orc.setup_nucleus(A, Z, otables))
+    for k in ("R", "EC", "EB_p", "EB_n"):
+        assert g[k] == pytest.approx(o[k], rel=1e-11)
+    for k in ("r", "rho_p", "rho_n", "pF_p", "pF_n", "EF_p", "EF_n", "V_p", "V_n"):
+        assert np.allclose(g[k], o[k], rtol=1e-10, atol=1e-13), k
+
+
+# ------------------------------------------------------------------------------- criterion (2)
+@pytest.mark.parametrize("cfg,n", [(1, 10000), (3, 10000), (4, 10000), (5, 10000)])
+def test_fp64_event_identity(gpu, orc, otables, ptables, cfg, n):
+    E, tid, targets, seed, _ = _inputs(cfg, n)
+    lib = gpu.load("f64")
+    g = gpu.simulate(lib, targets, E, tid, seed, ptables)
+    o = orc.simulate(otables, targets, E, tid, seed)
+    frac, max_err, ident = H.event_identity(g, o, rel=REL_F64)
+    assert frac >= FRAC_IDENTICAL, (frac, np.nonzero(~ident)[0][:10])
+    assert max_err <= REL_F64
+    assert np.array_equal(g["status"][ident], o["status"][ident])
+    assert np.array_equal(g["offsets"], np.concatenate([[0], np.cumsum(g["counts"])]))
+    # post-cascade stage ("SoA of excited nuclei")
+    same = ident
+    assert np.array_equal(g["casc_A"][same], o["casc_A"][same])
+    assert np.allclose(g["casc_Estar"][same], o["casc_Estar"][same], rtol=1e-9, atol=1e-9)
+    assert np.allclose(g["casc_P"][same], o["casc_P"][same], rtol=1e-9, atol=1e-7)
+    # criterion (1) on the GPU output itself
+    _assert_conservation(g, targets, tid, E, orc, otables, 1e-12, 1e-9)
+
+
+def test_fp64_ragged_sizes_and_empty(gpu, orc, otables, ptables):
+    """n = 0, 1, 31, 33, 257 (ragged tails of warps/blocks/scan tiles)."""
+    lib = gpu.load("f64")
+    for n in (0, 1, 31, 33, 257, 2049):
+        E, tid, targets, seed, _ = _inputs(1, n)
+        g = gpu.simulate(lib, targets, E, tid, seed, ptables)
+        assert g["total"] == int(np.sum(g["counts"])) and len(g["counts"]) == n
+        if n:
+            o = orc.simulate(otables, targets, E, tid, seed)
+            frac, _, _ = H.event_identity(g, o)
+            assert frac == 1.0 or frac >= 1 - 1.0 / n
+
+
+def test_fp64_cascade_only_and_flags(gpu, orc, otables, ptables):
+    E, tid, targets, seed, _ = _inputs(1, 3000)
+    lib = gpu.load("f64")
+    g = gpu.simulate(lib, targets, E, tid, seed, ptables, flags=gpu.F_CASCADE_ONLY)
+    o = orc.simulate(otables, targets, E, tid, seed, flags=orc.F_CASCADE_ONLY)
+    frac, err, _ = H.event_identity(g, o)
+    assert frac >= FRAC_IDENTICAL and np.all((g["species"] & 0x80) == 0)
+    # scheduling variants give bit-identical results (lane-per-event vs phase voting, thresholds)
+    base = gpu.simulate(lib, targets, E, tid, seed, ptables)
+    alt = gpu.simulate(lib, targets, E, tid, seed, ptables, flags=gpu.F_LANE_PER_EVENT)
+    lib.inc_set_vote_thresholds(3, 17)
+    alt2 = gpu.simulate(lib, targets, E, tid, seed, ptables)
+    lib.inc_set_vote_thresholds(8, 8)
+    for k in ("species", "T", "ux", "uz", "counts", "A", "Z", "Estar", "pz", "status"):
+        assert np.array_equal(base[k], alt[k]), k
+        assert np.array_equal(base[k], alt2[k]), k
+    # stats flag does not change results and the counters match the oracle's
+    st = gpu.simulate(lib, targets, E, tid, seed, ptables, flags=gpu.F_STATS)
+    assert np.array_equal(base["T"], st["T"])
+    os_ = orc.simulate(otables, targets, E, tid, seed)["stats"]
+    for k in ("attempts", "segments", "boundaries", "collisions", "blocked", "allowed", "escapes",
+              "evap_steps", "evap_emitted", "evap_trials"):
+        assert abs(st["stats"][k] - os_[k]) <= max(2, 1e-3 * os_[k]), (k, st["stats"][k], os_[k])
+
+
+def test_fp64_transparent_and_failed(gpu, orc, ptables):
+    """sigma = 0: KEEP_TRANSPARENT reproduces the oracle's refracted traversal (closed-form
+    pinned there); without the flag every event is FAILED with count 0."""
+    import paper_1309_7963_b200.tables as T
+    z = T.default_tables()
+    z["sig_pp"] = np.zeros_like(z["sig_pp"]); z["sig_np"] = np.zeros_like(z["sig_np"])
+    ot = orc.Tables(sigma_scale=0.0)
+    n = 500
+    E = np.full(n, 120.0); tid = np.zeros(n, dtype=np.int32)
+    lib = gpu.load("f64")
+    g = gpu.simulate(lib, [(40, 20)], E, tid, 7, z, flags=gpu.F_KEEP_TRANSPARENT | gpu.F_CASCADE_ONLY)
+    o = orc.simulate(ot, [(40, 20)], E, tid, 7, flags=orc.F_KEEP_TRANSPARENT | orc.F_CASCADE_ONLY)
+    assert np.all(g["counts"] == 1) and np.allclose(g["T"], 120.0, rtol=1e-12)
+    for k in ("ux", "uy", "uz"):
+        assert np.allclose(g[k], o[k], atol=1e-10)
+    g = gpu.simulate(lib, [(40, 20)], E[:8], tid[:8], 7, z)
+    assert np.all(g["status"] & gpu.ST_FAILED) and np.all(g["counts"] == 0) and g["total"] == 0
+    assert np.all(g["A"] == 40) and np.all(g["Z"] == 20) and np.all(g["Estar"] == 0)
+
+
+def test_error_paths(gpu, ptables):
+    import torch
+    lib = gpu.load("f32")
+    lib.inc_shutdown()
+    out = lib.alloc_outputs(4, 64)
+    E = torch.full((4,), 200.0, device="cuda"); tid = torch.zeros(4, dtype=torch.int32, device="cuda")
+    assert lib.inc_simulate(E, tid, 1, out, check=False) == gpu.INC_E_STATE          # before inc_init
+    with pytest.raises(gpu.IncError):
+        lib.inc_init(300, 8, ptables)
+    with pytest.raises(gpu.IncError):
+        lib.inc_init(4, 2, ptables)
+    bad = dict(ptables); bad["version"] = 2
+    with pytest.raises(gpu.IncError):
+        lib.inc_init(16, 8, bad)
+    t0 = lib.inc_init(16, 8, ptables)
+    other = dict(ptables); other["sig_pp"] = ptables["sig_pp"] * 1.01
+    with pytest.raises(gpu.IncError) as ei:
+        lib.inc_init(12, 6, other)
+    assert ei.value.code == gpu.INC_E_TABLES
+    lib.inc_set_stream(); lib.inc_set_flags(0)
+    # E_in out of range is reported, not clamped
+    Ebad = E.clone(); Ebad[2] = 300.0
+    assert lib.inc_simulate(Ebad, tid, 1, out, check=False) == gpu.INC_E_BADARG
+    assert "E_in" in lib.last_error()
+    tbad = tid.clone(); tbad[1] = 5
+    assert lib.inc_simulate(E, tbad, 1, out, check=False) == gpu.INC_E_BADARG
+    # capacity too small: counts still valid, nothing written past capacity
+    n = 2000
+    E = torch.full((n,), 200.0, device="cuda"); tid = torch.full((n,), t0, dtype=torch.int32, device="cuda")
+    big = lib.alloc_outputs(n, n * 24)
+    total = lib.inc_simulate(E, tid, 3, big)
+    small = lib.alloc_outputs(n, 100)
+    small["T"].fill_(-5.0)
+    assert lib.inc_simulate(E, tid, 3, small, check=False) == gpu.INC_E_CAPACITY
+    assert str(total) in lib.last_error()
+    assert torch.equal(small["counts"], big["counts"])
+    assert torch.equal(small["T"][:100], big["T"][:100])
+    lib.inc_free_target(t0)
+    assert lib.inc_simulate(E, tid, 3, big, check=False) == gpu.INC_E_BADARG
+
+
+def test_same_stream_probe_and_host_path(gpu, ptables):
+    """P:73-75 divergence probe: all events identical.  Host-buffer entry point == device one."""
+    import torch
+    lib = gpu.load("f32")
+    E, tid, targets, seed, _ = _inputs(1, 4096)
+    g = gpu.simulate(lib, targets, E, tid, seed, ptables, flags=gpu.F_SAME_STREAM)
+    assert np.all(g["counts"] == g["counts"][0]) and np.all(g["A"] == g["A"][0])
+    c = g["counts"][0]
+    assert np.all(g["T"].reshape(-1, c) == g["T"][:c])
+    ref = gpu.simulate(lib, targets, E, tid, seed, ptables)
+    n = len(E)
+    outh = lib.alloc_outputs(n, n * 24, device="cpu")
+    Eh = torch.as_tensor(E.astype(np.float32)).pin_memory()
+    th = torch.zeros(n, dtype=torch.int32).pin_memory()
+    lib.inc_set_flags(0)
+    tot = lib.inc_simulate_host(Eh, th, seed, outh)
+    assert tot == ref["total"]
+    assert np.array_equal(outh["counts"].numpy(), ref["counts"])
+    assert np.array_equal(outh["T"].numpy()[:tot], ref["T"])
+    assert np.array_equal(outh["species"].numpy()[:tot], ref["species"])
+    assert np.array_equal(outh["A"].numpy(), ref["A"])
+
+
+def test_chunk_boundary_determinism(gpu, orc, otables, ptables):
+    """n > 2^20 runs in two chunks; events around the boundary equal the oracle's (event index
+    keys the RNG, not the chunk)."""
+    n = (1 << 20) + 4000
+    E = np.full(n, 200.0); tid = np.zeros(n, dtype=np.int32)
+    lib = gpu.load("f64")
+    import torch
+    lib.inc_shutdown()
+    s = lib.inc_init(16, 8, ptables)
+    lib.inc_set_stream(); lib.inc_set_flags(0)
+    out = lib.alloc_outputs(n, n * 8)
+    tot = lib.inc_simulate(torch.as_tensor(E, device="cuda"), torch.full((n,), s, dtype=torch.int32, device="cuda"), 2, out)
+    off = lib.inc_get_offsets(n).cpu().numpy()
+    assert off[-1] == tot
+    lo, hi = (1 << 20) - 300, (1 << 20) + 300
+    o = orc.simulate(otables, [(16, 8)], E[lo:hi], tid[lo:hi], 2, e0=lo)
+    g = {k: out[k][lo:hi].cpu().numpy() for k in ("counts", "A", "Z", "Estar")}
+    a, b = off[lo], off[hi]
+    for k in ("species", "T", "ux", "uy", "uz"):
+        g[k] = out[k][a:b].cpu().numpy()
+    g["offsets"] = off[lo:hi + 1] - off[lo]
+    frac, err, _ = H.event_identity(g, o)
+    assert frac >= 0.995 and err <= REL_F64
+
+
+# ------------------------------------------------------------------------------- criteria (1), (3)
+@pytest.mark.parametrize("cfg", [2, 3, 5, 4])
+def test_fp32_histograms_full_size(gpu, orc, otables, ptables, cfg):
+    """Full BASELINE.json sizes, production build, in the launch configuration bench.py times."""
+    import paper_1309_7963_b200.workloads as W
+    n = W.CONFIGS[cfg]["n"]
+    E, tid, targets, seed, _ = _inputs(cfg, n)
+    lib = gpu.load("f32")
+    hg = None
+    # the GPU result is histogrammed in slices to bound host memory (config 4: 1e7 events)
+    import torch
+    lib.inc_shutdown()
+    slots = np.array([lib.inc_init(a, z, ptables) for a, z in targets], dtype=np.int32)
+    lib.inc_set_stream(); lib.inc_set_flags(0)
+    Ed = torch.as_tensor(E.astype(np.float32), device="cuda")
+    td = torch.as_tensor(slots[tid], device="cuda")
+    out = lib.alloc_outputs(n, n * 10)
+    tot = lib.inc_simulate(Ed, td, seed, out)
+    g = {k: out[k].cpu().numpy() for k in ("counts", "A", "Z", "Estar", "px", "py", "pz")}
+    g["status"] = out["status"].cpu().numpy().view(np.uint32)
+    for k in ("species", "T", "ux", "uy", "uz"):
+        g[k] = out[k][:tot].cpu().numpy()
+    assert not np.any(g["status"] & (gpu.ST_FAILED | gpu.ST_QUEUE_OVF))
+    hg = H.histograms(g["species"], g["T"].astype(np.float64), g["uz"].astype(np.float64), g["counts"], g["A"])
+    ho, _ = H.oracle_histograms(cfg, n)
+    fails = H.compare_histograms(hg, ho)
+    assert not fails, fails
+    # criterion (1) on a 2e5-event slice (exact A, Z; 4-momentum to fp32 accuracy)
+    m = min(n, 200000)
+    sl = {k: g[k][:m] for k in ("counts", "A", "Z", "Estar", "px", "py", "pz", "status")}
+    k_end = int(np.sum(g["counts"][:m]))
+    for k in ("species", "T", "ux", "uy", "uz"):
+        sl[k] = g[k][:k_end]
+    _assert_conservation(sl, targets, tid[:m], E[:m], orc, otables, 2e-6, 2e-4)
+    # sampled events against the oracle one by one: identical discrete outcome in most events
+    o = orc.simulate(otables, targets, E[:2000], tid[:2000], seed)
+    same = (g["counts"][:2000] == o["counts"]) & (g["A"][:2000] == o["A"]) & (g["Z"][:2000] == o["Z"])
+    assert same.mean() > 0.97
+
+
+def test_fp32_independent_sample(gpu, orc, otables, ptables):
+    """Same workload, different GPU seed: an INDEPENDENT sample must still match the oracle's
+    distributions (guards against a test that passes only because the streams are shared)."""
+    n = 200000
+    E, tid, targets, seed, _ = _inputs(2, n)
+    lib = gpu.load("f32")
+    g = gpu.simulate(lib, targets, E, tid, seed + 1000, ptables)
+    hg = H.histograms(g["species"], g["T"].astype(np.float64), g["uz"].astype(np.float64), g["counts"], g["A"])
+    ho, _ = H.oracle_histograms(2, n)
+    fails = H.compare_histograms(hg, ho, p_min=1e-4)
+    assert not fails, fails
