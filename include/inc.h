@@ -74,8 +74,11 @@ extern "C" {
                                       stream of event 0                                     */
 #define INC_F_STATS 8u             /* accumulate the work counters of inc_get_stats         */
 #define INC_F_TIMING 32u           /* record CUDA events around each stage (inc_get_stage_times) */
-#define INC_F_LANE_PER_EVENT 16u   /* scheduling variant: no phase voting (baseline layout of
-                                      P:61, one lane runs one event straight through)      */
+#define INC_F_LANE_PER_EVENT 16u   /* scheduling variant: one lane runs one event straight through,
+                                      no phase voting (the layout of P:61, for comparison)  */
+#define INC_F_LANE_STATE_MACHINE 64u /* scheduling variant: lane-per-event state machine with
+                                      warp-voted phases instead of the default per-warp
+                                      wavefront queues.  Results never depend on the variant. */
 
 /* ---- model inputs ("precalculated ... tables and other read-only input data") ----- */
 typedef struct inc_tables {   /* HOST memory, caller-owned, copied during inc_init           */

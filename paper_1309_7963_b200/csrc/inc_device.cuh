@@ -4,12 +4,21 @@
 // double: parity build compiled with -fmad=false).  Citations: P:NN = PAPER.md line,
 // R-xx = reading in DESIGN.md section 3.
 //
+// Physics steps (device functions, used by both cascade kernels)
+//   entry_step      C0  uniform-disc entry, potential step into the outermost shell
+//   seg_step        C2  Fermi-sea partner, NN cross sections, exponential path, shell geometry,
+//                   C4  refraction / reflection / escape at the shell boundary
+//   coll_step       C3  relativistic two-body scatter, Pauli blocking, cutoff
+//   epilogue_eval   C6  residual nucleus and excitation energy from 4-momentum balance
 // Kernels
-//   cascade_kernel   persistent warps; every lane owns one event at a time and runs a small
-//                    state machine {SEG, COLL, EPI}.  Each warp pass executes ONE phase, chosen
-//                    by warp vote, so the expensive rare steps (collision, epilogue+entry) are
-//                    deferred until several lanes need them instead of diverging every pass.
-//   evap_kernel      persistent lanes, one Weisskopf-Ewing emission step per pass.
+//   cascade_wavefront_kernel  DEFAULT.  Per-warp wavefront: tracks of ~48 events in flight live in
+//                   per-warp shared-memory queues, sorted by the kind of step they need next
+//                   (segment / collision / epilogue+entry).  Every warp pass pops up to 32 items of
+//                   ONE kind, so lanes execute the same step; queue indices come from warp votes
+//                   (__ballot_sync + popc), per-event bookkeeping from shared-memory integer atomics.
+//   cascade_lane_kernel       INC_F_LANE_STATE_MACHINE.  One lane owns one event at a time and runs a
+//                   {SEG, COLL, EPI} state machine; the warp votes which phase to run each pass.
+//   evap_kernel     persistent lanes, one Weisskopf-Ewing emission step per pass.
 //   scan_* / compact_kernel   exclusive prefix sum of counts, canonical-order SoA output.
 #pragma once
 #include <cuda_runtime.h>
@@ -24,7 +33,7 @@ constexpr int kMaxSeg = 1024;      // R-C2
 constexpr int kMaxAttempt = 256;   // R-C6
 constexpr int kMaxTrial = 64;      // R-E4
 constexpr int kMaxSec = INC_MAX_SEC;
-constexpr int kStackCap = 16;      // pending tracks per event (implementation limit, INC_ST_QUEUE_OVF)
+constexpr int kStackCap = 16;      // lane kernel: pending tracks per event (INC_ST_QUEUE_OVF beyond)
 constexpr int kAmax = 72;          // binding / channel tables cover 0..kAmax-1
 constexpr int kZmax = 40;
 constexpr unsigned kFull = 0xFFFFFFFFu;
@@ -33,26 +42,29 @@ constexpr unsigned kFull = 0xFFFFFFFFu;
 template <typename R> struct K {
   static constexpr R mp = R(938.27208816);
   static constexpr R mn = R(939.56542052);
-  static constexpr R two_pi = R(6.283185307179586476925286766559);
+  static constexpr R imp = R(1.0 / 938.27208816);
+  static constexpr R imn = R(1.0 / 939.56542052);
 };
 
 // ---- device-resident model data ----------------------------------------------------------
-template <typename R> struct ShellDev {   // one constant-density shell
+template <typename R> struct ShellDev {   // one constant-density shell; 16 reals
   R rho_p, rho_n;      // fm^-3
   R pF_p, pF_n;        // Fermi momenta, MeV/c
   R pF2_p, pF2_n;      // Pauli threshold on |p'|^2  (T' > E_F  <=>  p'^2 > pF^2)
   R pc2_p, pc2_n;      // cutoff threshold on |p'|^2 (T' - V <= cut <=> p'^2 <= pc2)
   R V_p, V_n;          // well depth E_F + E_B, MeV
+  R r_in, r_out;       // shell radii i*dr, (i+1)*dr
+  R ir_in, ir_out;     // reciprocals (ir_in = 0 for the innermost shell)
   R pad0, pad1;
 };
 
 template <typename R> struct NucDev {
   int32_t A, Z, ns, live;
-  R Rn, dr, Bt, pad;                       // radius, shell thickness, target binding energy
+  R Rn, dr, Bt, iRn;                       // radius, shell thickness, target binding energy, 1/R
   ShellDev<R> sh[kMaxShells + 1];          // [ns] = outside: V = 0
 };
 
-template <typename R> struct EvChan {        // per (A_d, Z_d, channel j): R-E1/E2 constants
+template <typename R> struct __align__(16) EvChan {        // per (A_d, Z_d, channel j): R-E1/E2 constants
   R V;        // Coulomb barrier of the channel
   R pref;     // g_j M_j A_d^(2/3) alpha_j   (0 => channel closed: daughter invalid)
   R beta;     // Dostrovsky beta (neutron) or 0
@@ -71,7 +83,7 @@ template <typename R> struct ModelDev {
 };
 
 template <typename R> struct Workspace {   // per-chunk internal buffers (DEVICE)
-  uint32_t *st_code;      // [chunk][kMaxSec]  path code | type << 24 | evap << 31 (evap: species<<24 | seq)
+  uint32_t *st_code;      // [chunk][kMaxSec]  path code | type << 24 ; evap: 1<<31 | species<<24 | seq
   R *st_T, *st_ux, *st_uy, *st_uz;
   int32_t *cA, *cZ;       // post-cascade nucleus ("SoA of excited nuclei")
   R *cE, *cPx, *cPy, *cPz;
@@ -91,7 +103,29 @@ enum StatIdx { S_EVENTS = 0, S_FAILED, S_ATTEMPTS, S_SEG, S_BND, S_REFL, S_ESC, 
                S_ALLOWED, S_ABSORBED, S_EVSTEPS, S_EVTRIALS, S_EVEMIT, S_WI_SEG, S_WI_COLL, S_WI_EPI,
                S_LS_SEG, S_LS_COLL, S_LS_EPI, S_NSTAT };
 
-// ---- math wrappers: exact library calls for double, fast intrinsics for float ---------------
+template <bool ON> struct LaneStats {
+  unsigned long long c[ON ? S_NSTAT : 1];
+  __device__ __forceinline__ void clear() {
+    if (ON) {
+#pragma unroll
+      for (int i = 0; i < S_NSTAT; ++i) c[i] = 0;
+    }
+  }
+  __device__ __forceinline__ void add(int i, unsigned long long v = 1) { if (ON) c[i] += v; }
+  __device__ __forceinline__ void flush(DevCounters *ctr, int lane) {
+    if (ON) {
+#pragma unroll
+      for (int i = 0; i < S_NSTAT; ++i) {
+        unsigned long long v = c[i];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+        if (lane == 0 && v) atomicAdd(&ctr->stats[i], v);
+      }
+    }
+  }
+};
+
+// ---- math wrappers: exact library calls for double, MUFU-based approximations for float ------
 template <typename R> struct M;
 template <> struct M<double> {
   static __device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
@@ -105,30 +139,51 @@ template <> struct M<double> {
     sincos(6.283185307179586476925286766559 * u, s, c);
   }
   static __device__ __forceinline__ double div_(double a, double b) { return a / b; }
+  static __device__ __forceinline__ double rcp_(double a) { return 1.0 / a; }
   static __device__ __forceinline__ double u01(uint32_t x) {   // R-R3 (fp64): (x + 1/2) 2^-32
     return ((double)x + 0.5) * (1.0 / 4294967296.0);
   }
-  static __device__ __forceinline__ double floor_(double x) { return floor(x); }
+  // x >= 0 -> integer part k (clamped to kmax) and fraction
+  static __device__ __forceinline__ void split(double x, int kmax, int &k, double &f) {
+    int kk = (int)x;
+    kk = kk > kmax ? kmax : kk;
+    k = kk; f = x - (double)kk;
+  }
   static constexpr int kSeriesTerms = 24;
 };
 template <> struct M<float> {
-  static __device__ __forceinline__ float sqrt_(float x) { return __fsqrt_rn(x); }
-  static __device__ __forceinline__ float rsqrt_(float x) { return rsqrtf(x); }
-  static __device__ __forceinline__ float log_(float x) { return __logf(x); }
-  static __device__ __forceinline__ float exp_(float x) { return __expf(x); }
-  static __device__ __forceinline__ float cbrt_(float x) { return cbrtf(x); }
+  static __device__ __forceinline__ float sqrt_(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+  static __device__ __forceinline__ float rsqrt_(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+  static __device__ __forceinline__ float lg2_(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+  static __device__ __forceinline__ float ex2_(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+  static __device__ __forceinline__ float log_(float x) { return 0.6931471805599453f * lg2_(x); }
+  static __device__ __forceinline__ float exp_(float x) { return ex2_(1.4426950408889634f * x); }
+  static __device__ __forceinline__ float cbrt_(float x) { return ex2_(0.3333333333f * lg2_(x)); }   // x in (0,1)
   static __device__ __forceinline__ float log1p_(float x) { return log1pf(x); }
   static __device__ __forceinline__ float expm1_(float x) { return expm1f(x); }
   static __device__ __forceinline__ void sincos2pi(float u, float *s, float *c) {
+    // sin.approx / cos.approx scale their argument by 1/(2 pi) before MUFU: feed radians
     float a = 6.283185307179586f * u;
-    *s = __sinf(a);
-    *c = __cosf(a);
+    float ss, cc;
+    asm("sin.approx.ftz.f32 %0, %1;" : "=f"(ss) : "f"(a));
+    asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cc) : "f"(a));
+    *s = ss; *c = cc;
   }
-  static __device__ __forceinline__ float div_(float a, float b) { return __fdividef(a, b); }
-  static __device__ __forceinline__ float u01(uint32_t x) {    // R-R3 (fp32): ((x>>9) + 1/2) 2^-23, exact
-    return ((float)(x >> 9) + 0.5f) * (1.0f / 8388608.0f);
+  static __device__ __forceinline__ float rcp_(float a) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(a)); return y; }
+  static __device__ __forceinline__ float div_(float a, float b) { return a * rcp_(b); }
+  static __device__ __forceinline__ float u01(uint32_t x) {
+    // R-R3 (fp32): ((x>>9) + 1/2) 2^-23, built from the mantissa bits (no int->float conversion)
+    return __uint_as_float(0x3F800000u | (x >> 9)) - 0.99999994f;
   }
-  static __device__ __forceinline__ float floor_(float x) { return floorf(x); }
+  static __device__ __forceinline__ void split(float x, int kmax, int &k, float &f) {
+    // round-to-nearest of (x - 1/2) by the 2^23 trick: stays on the FMA/ALU pipes.  A knot that is
+    // mis-assigned by one ulp gives f just outside [0,1]; the interpolant is continuous there.
+    float y = (x - 0.49999997f) + 8388608.0f;
+    int kk = __float_as_int(y) - 0x4B000000;
+    kk = kk < 0 ? 0 : (kk > kmax ? kmax : kk);
+    k = kk; f = x - (y - 8388608.0f);
+    f = kk == kmax ? x - (float)kmax : f;
+  }
   static constexpr int kSeriesTerms = 13;
 };
 
@@ -137,8 +192,10 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
                                                uint32_t k0, uint32_t k1) {
 #pragma unroll
   for (int r = 0; r < 10; ++r) {
-    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;   // one IMAD.WIDE each
+    const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
+    const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
     c0 = hi1 ^ c1 ^ k0;
     c1 = lo1;
     c2 = hi0 ^ c3 ^ k1;
@@ -165,39 +222,294 @@ __device__ __forceinline__ void draw4(const RngKey &g, uint32_t attempt, uint32_
 template <typename R>
 __device__ __forceinline__ void grid_pos(R plab_mev, R inv_dp, int n_xs, int &k, R &f) {
   R x = plab_mev * inv_dp;
-  R xmax = R(n_xs - 1);
+  const R xmax = R(n_xs - 1);
   x = x > xmax ? xmax : x;
-  int kk = (int)x;            // x >= 0
-  kk = kk > n_xs - 2 ? n_xs - 2 : kk;
-  k = kk;
-  f = x - R(kk);
+  M<R>::split(x, n_xs - 2, k, f);
 }
 
 template <typename R> __device__ __forceinline__ R nucleon_mass(int type) { return type ? K<R>::mp : K<R>::mn; }
+template <typename R> __device__ __forceinline__ R nucleon_imass(int type) { return type ? K<R>::imp : K<R>::imn; }
 
-// momentum of particle 1 (mass m1, kinetic T1, momentum vector dotted with partner direction = pn)
-// in the rest frame of a partner of momentum magnitude q along n (mass m2), MeV/c.  Equivalent to
-// sqrt(E_lab^2 - m1^2) with E_lab = (s - m1^2 - m2^2)/(2 m2), written without cancellation.
+// Momentum of particle 1 (mass m1, total energy E1) in the rest frame of a partner with momentum q n
+// (mass m2, 1/m2 = im2); pn = p1 . n.  E_lab = (E1 E2 - p1.p2)/m2 is the invariant s expression
+// (s - m1^2 - m2^2)/(2 m2) of R-C2; p_lab = sqrt(T_lab (T_lab + 2 m1)), MeV/c.
 template <typename R>
-__device__ __forceinline__ R plab_of(R m1, R T1, R pn, R q, R m2) {
-  R q2 = q * q;
-  R E2 = M<R>::sqrt_(q2 + m2 * m2);
-  R T2 = M<R>::div_(q2, E2 + m2);
-  R Tlab = M<R>::div_(m1 * T2 + m2 * T1 + T1 * T2 - q * pn, m2);
+__device__ __forceinline__ R plab_of(R m1, R E1, R pn, R q, R m2, R im2) {
+  const R E2 = M<R>::sqrt_(q * q + m2 * m2);
+  const R Tlab = (E1 * E2 - q * pn) * im2 - m1;
   R a = Tlab * (Tlab + R(2) * m1);
   a = a > R(0) ? a : R(0);
   return M<R>::sqrt_(a);
 }
 
-// ---- lane state ------------------------------------------------------------------------------
-enum LaneState : int { ST_SEG = 0, ST_COLL = 1, ST_EPI = 2, ST_DONE = 3 };
-
-template <typename R> struct TrackRec {   // pending track (local-memory stack)
-  R x, y, z, px, py, pz;
-  uint32_t pi;
-  uint32_t meta;   // type | shell << 1
+// ---- track state ---------------------------------------------------------------------------------
+template <typename R> struct Track {
+  R x, y, z;          // position, fm
+  R px, py, pz;       // momentum, MeV/c
+  R T;                // kinetic energy, MeV (kept consistent with |p|)
+  uint32_t pi;        // path code (R-R2)
+  uint32_t k;         // next Philox block of this track's stream
+  int nseg;           // segments done (R-C2 cap)
+  int type, shell;    // 1 = proton, 0 = neutron; shell index
 };
 
+template <typename R> struct CollCarry { R f, nx, ny, nz, Sp, Sig; };   // SEG -> COLL hand-over
+template <typename R> struct Escape { R T, ux, uy, uz; };
+
+enum SegOutcome : int { SEG_CONT = 0, SEG_COLLIDE = 1, SEG_ESCAPE = 2, SEG_CAP = 3 };
+
+// ---------- C0: entry — uniform disc, beam along +z (R-Q15), potential step into the last shell ----------
+template <typename R>
+__device__ __forceinline__ void entry_step(Track<R> &t, const NucDev<R> &nu, R E_in, const RngKey &g, uint32_t attempt,
+                                           R &p_in) {
+  R u[4];
+  draw4<R>(g, attempt, 1u, 0u, u);
+  const R b = nu.Rn * M<R>::sqrt_(u[0]);
+  R sb, cb;
+  M<R>::sincos2pi(u[1], &sb, &cb);
+  t.x = b * cb; t.y = b * sb;
+  const R zz = nu.Rn * nu.Rn - b * b;
+  t.z = -M<R>::sqrt_(zz > R(0) ? zz : R(0));
+  p_in = M<R>::sqrt_(E_in * (E_in + R(2) * K<R>::mp));
+  // potential step (cannot reflect: V rises inward)
+  const R ux = t.x * nu.iRn, uy = t.y * nu.iRn, uz = t.z * nu.iRn;
+  const R pr = p_in * uz;
+  const R dV = nu.sh[nu.ns - 1].V_p;
+  const R Tj = E_in + dV;
+  const R prj2 = pr * pr + dV * (E_in + Tj + R(2) * K<R>::mp);
+  const R prj = -M<R>::sqrt_(prj2 > R(0) ? prj2 : R(0));
+  const R dp = prj - pr;
+  t.px = dp * ux; t.py = dp * uy; t.pz = p_in + dp * uz;
+  t.T = Tj;
+  t.type = 1; t.shell = nu.ns - 1; t.pi = 1u; t.k = 1u; t.nseg = 0;
+}
+
+// ---------- C2 + C4: one segment (R-Q8 partner first, then the path) ----------
+template <typename R, bool STATS>
+__device__ __forceinline__ int seg_step(Track<R> &t, const NucDev<R> &nu, const R *s_tabS, int n_xs, R inv_dp,
+                                        const RngKey &g, uint32_t attempt, CollCarry<R> &cc, Escape<R> &esc,
+                                        LaneStats<STATS> &st) {
+  if (t.nseg >= kMaxSeg) { st.add(S_ABSORBED); return SEG_CAP; }    // R-C2 cap
+  t.nseg++;
+  st.add(S_SEG);
+  R u[4];
+  draw4<R>(g, attempt, t.pi, t.k++, u);
+  const ShellDev<R> &sh = nu.sh[t.shell];
+  const R m1 = nucleon_mass<R>(t.type);
+  const R E1 = t.T + m1;
+  const R p1sq = t.px * t.px + t.py * t.py + t.pz * t.pz;
+  // partner direction and magnitude fraction ("quadratic distribution")
+  const R cth = R(2) * u[1] - R(1);
+  R s2 = R(1) - cth * cth;
+  s2 = s2 > R(0) ? s2 : R(0);
+  const R sth = M<R>::sqrt_(s2);
+  R sph, cph;
+  M<R>::sincos2pi(u[2], &sph, &cph);
+  const R nx = sth * cph, ny = sth * sph, nz = cth;
+  const R f = M<R>::cbrt_(u[0]);
+  const R pn = t.px * nx + t.py * ny + t.pz * nz;
+  // cross sections against a proton and a neutron partner (same n, f: R-C2)
+  const R plab_p = plab_of<R>(m1, E1, pn, sh.pF_p * f, K<R>::mp, K<R>::imp);
+  const R plab_n = plab_of<R>(m1, E1, pn, sh.pF_n * f, K<R>::mn, K<R>::imn);
+  int kp, kn; R fp, fn;
+  grid_pos<R>(plab_p, inv_dp, n_xs, kp, fp);
+  grid_pos<R>(plab_n, inv_dp, n_xs, kn, fn);
+  // tabS row {sig_pp, d, sig_np, d}: vs a proton pp if the track is a proton else np; vs a neutron the opposite
+  const R *rp = s_tabS + 4 * kp + (t.type ? 0 : 2);
+  const R *rn = s_tabS + 4 * kn + (t.type ? 2 : 0);
+  const R Sp = sh.rho_p * (rp[0] + fp * rp[1]);
+  const R Sn = sh.rho_n * (rn[0] + fn * rn[1]);
+  const R Sig = Sp + Sn;
+  const R nlu = -M<R>::log_(u[3]);                  // d_coll = nlu / Sig
+  // geometry: distances to the shell spheres along the flight direction
+  const R ip = M<R>::rsqrt_(p1sq);
+  const R dx = t.px * ip, dy = t.py * ip, dz = t.pz * ip;
+  const R beta = t.x * dx + t.y * dy + t.z * dz;
+  const R r2 = t.x * t.x + t.y * t.y + t.z * t.z;
+  const R bb = beta * beta - r2;
+  R disc_out = bb + sh.r_out * sh.r_out;
+  disc_out = disc_out > R(0) ? disc_out : R(0);
+  const R d_out = -beta + M<R>::sqrt_(disc_out);
+  R d_in = R(1e30);
+  if (t.shell > 0 && beta < R(0)) {
+    const R D = bb + sh.r_in * sh.r_in;
+    if (D > R(0)) d_in = -beta - M<R>::sqrt_(D);
+  }
+  const bool inward = d_in < d_out;
+  const R d_min = inward ? d_in : d_out;
+  if (nlu < Sig * d_min) {
+    // collision point reached first (d_coll < d_min): hand over to the collision step
+    const R d_coll = M<R>::div_(nlu, Sig);
+    t.x += d_coll * dx; t.y += d_coll * dy; t.z += d_coll * dz;
+    cc.f = f; cc.nx = nx; cc.ny = ny; cc.nz = nz; cc.Sp = Sp; cc.Sig = Sig;
+    return SEG_COLLIDE;
+  }
+  // ---------- C4: shell boundary, potential step (P:49 refraction / reflection) ----------
+  st.add(S_BND);
+  const int j = inward ? t.shell - 1 : t.shell + 1;
+  const R rb = inward ? sh.r_in : sh.r_out;
+  const R irb = inward ? sh.ir_in : sh.ir_out;
+  R x = t.x + d_min * dx, y = t.y + d_min * dy, z = t.z + d_min * dz;
+  // renormalise onto the sphere: one Newton step of 1/sqrt around |x|^2 = rb^2 (|x| is within rounding of rb)
+  const R corr = R(1.5) - R(0.5) * (x * x + y * y + z * z) * irb * irb;
+  x *= corr; y *= corr; z *= corr;
+  t.x = x; t.y = y; t.z = z;
+  const R ux = x * irb, uy = y * irb, uz = z * irb;              // outward normal
+  const R pr = t.px * ux + t.py * uy + t.pz * uz;
+  const R Vi = t.type ? sh.V_p : sh.V_n;
+  const R Vj = t.type ? nu.sh[j].V_p : nu.sh[j].V_n;
+  const R dV = Vj - Vi;
+  const R Tj = t.T + dV;
+  const R prj2 = pr * pr + dV * (t.T + Tj + R(2) * m1);          // p_j^2 - p_t^2
+  if (Tj <= R(0) || prj2 <= R(0)) {
+    st.add(S_REFL);
+    const R t2 = R(2) * pr;
+    t.px -= t2 * ux; t.py -= t2 * uy; t.pz -= t2 * uz;            // specular reflection
+    return SEG_CONT;
+  }
+  const R sq = M<R>::sqrt_(prj2);
+  const R dp = (pr >= R(0) ? sq : -sq) - pr;
+  t.px += dp * ux; t.py += dp * uy; t.pz += dp * uz;
+  t.T = Tj;
+  t.shell = j;
+  if (j == nu.ns) {                                               // escape ("exiting particles")
+    st.add(S_ESC);
+    const R ipj = M<R>::rsqrt_(Tj * (Tj + R(2) * m1));
+    esc.T = Tj; esc.ux = t.px * ipj; esc.uy = t.py * ipj; esc.uz = t.pz * ipj;
+    return SEG_ESCAPE;
+  }
+  return SEG_CONT;
+}
+
+// ---------- C3: collision.  Returns false if Pauli-blocked (track t continues, k advanced) ----------
+template <typename R, bool STATS>
+__device__ __forceinline__ bool coll_step(Track<R> &t, const CollCarry<R> &cc, const NucDev<R> &nu, const R *tabC,
+                                          int n_xs, R inv_dp, const RngKey &g, uint32_t attempt,
+                                          Track<R> &c2, bool &keep1, bool &keep2, uint32_t &status, LaneStats<STATS> &st) {
+  st.add(S_COLL);
+  const ShellDev<R> &sh = nu.sh[t.shell];
+  R u[4];
+  draw4<R>(g, attempt, t.pi, t.k++, u);
+  const int t2 = (u[0] * cc.Sig < cc.Sp) ? 1 : 0;
+  const R m1 = nucleon_mass<R>(t.type), m2 = nucleon_mass<R>(t2);
+  const R q = (t2 ? sh.pF_p : sh.pF_n) * cc.f;
+  const R p2x = q * cc.nx, p2y = q * cc.ny, p2z = q * cc.nz;
+  const R E1 = t.T + m1;
+  const R E2 = M<R>::sqrt_(q * q + m2 * m2);
+  const R pn = t.px * cc.nx + t.py * cc.ny + t.pz * cc.nz;
+  const R Tlab = (E1 * E2 - q * pn) * nucleon_imass<R>(t2) - m1;
+  R pl2 = Tlab * (Tlab + R(2) * m1);
+  const R plab = M<R>::sqrt_(pl2 > R(0) ? pl2 : R(0));
+  int kk; R ff;
+  grid_pos<R>(plab, inv_dp, n_xs, kk, ff);
+  const bool same = (t2 == t.type);
+  const R *row = tabC + 8 * kk;
+  const R B = same ? (__ldg(row + 0) + ff * __ldg(row + 1)) : (__ldg(row + 2) + ff * __ldg(row + 3));
+  const R ab = same ? R(0) : (__ldg(row + 4) + ff * __ldg(row + 5));
+  // boost to the CM frame
+  const R Px = t.px + p2x, Py = t.py + p2y, Pz = t.pz + p2z;
+  const R E = E1 + E2;
+  const R s = E * E - (Px * Px + Py * Py + Pz * Pz);
+  const R iE = M<R>::rcp_(E);
+  const R bx = Px * iE, by = Py * iE, bz = Pz * iE;
+  const R gam = E * M<R>::rsqrt_(s);
+  const R gfac = M<R>::div_(gam * gam, gam + R(1));      // (gamma - 1) / beta^2
+  const R pb = t.px * bx + t.py * by + t.pz * bz;
+  const R fb = gfac * pb - gam * E1;
+  const R qx = t.px + fb * bx, qy = t.py + fb * by, qz = t.pz + fb * bz;   // p1 in the CM frame
+  const R pcm2 = qx * qx + qy * qy + qz * qz;
+  const R ipcm = M<R>::rsqrt_(pcm2);
+  const R pcm = pcm2 * ipcm;
+  // scattering angle: dsigma/dt ~ exp(B t), t in (GeV/c)^2 (R-Q10)
+  const R pg2 = pcm2 * R(1e-6);
+  const R tmin = R(-4) * pg2;
+  R tt;
+  if (B * (-tmin) < R(1e-9)) tt = u[1] * tmin;
+  else tt = M<R>::div_(M<R>::log1p_(-u[1] * (-M<R>::expm1_(B * tmin))), B);
+  R ct = R(1) + M<R>::div_(tt, R(2) * pg2);
+  ct = ct < R(-1) ? R(-1) : (ct > R(1) ? R(1) : ct);
+  if (!same && u[2] * (R(1) + ab) < ab) ct = -ct;       // np backward term
+  const R st2 = R(1) - ct * ct;
+  const R stt = M<R>::sqrt_(st2 > R(0) ? st2 : R(0));
+  R sphi, cphi;
+  M<R>::sincos2pi(u[3], &sphi, &cphi);
+  // rotation frame around n = q/|q|
+  const R n0 = qx * ipcm, n1 = qy * ipcm, n2 = qz * ipcm;
+  const R q2 = n0 * n0 + n1 * n1;
+  R e1x, e1y, e1z, e2x, e2y;
+  if (q2 > R(1e-24)) {
+    const R iq = M<R>::rsqrt_(q2);
+    e1x = n0 * n2 * iq; e1y = n1 * n2 * iq; e1z = -q2 * iq;
+    e2x = -n1 * iq; e2y = n0 * iq;
+  } else {
+    e1x = R(1); e1y = R(0); e1z = R(0);
+    e2x = R(0); e2y = n2 >= R(0) ? R(1) : R(-1);
+  }
+  const R a1 = stt * cphi, a2 = stt * sphi;
+  const R w1x = pcm * (a1 * e1x + a2 * e2x + ct * n0);
+  const R w1y = pcm * (a1 * e1y + a2 * e2y + ct * n1);
+  const R w1z = pcm * (a1 * e1z + ct * n2);
+  // boost back; partner by momentum conservation
+  const R E1cm = M<R>::sqrt_(pcm2 + m1 * m1);
+  const R wb = w1x * bx + w1y * by + w1z * bz;
+  const R fo = gfac * wb + gam * E1cm;
+  const R o1x = w1x + fo * bx, o1y = w1y + fo * by, o1z = w1z + fo * bz;
+  const R o2x = Px - o1x, o2y = Py - o1y, o2z = Pz - o1z;
+  const R o1sq = o1x * o1x + o1y * o1y + o1z * o1z;
+  const R o2sq = o2x * o2x + o2y * o2y + o2z * o2z;
+  // Pauli blocking: both products above their Fermi energies (strict, R-Q12)
+  const R pF2_1 = t.type ? sh.pF2_p : sh.pF2_n;
+  const R pF2_2 = t2 ? sh.pF2_p : sh.pF2_n;
+  if (!(o1sq > pF2_1 && o2sq > pF2_2)) {
+    st.add(S_BLOCKED);
+    return false;                                     // projectile continues unchanged (R-Q13)
+  }
+  st.add(S_ALLOWED);
+  keep1 = false; keep2 = false;
+  if (2u * t.pi + 1u >= (1u << 24)) {                 // depth cap (R-C3)
+    status |= INC_ST_DEPTH_CAP;
+    st.add(S_ABSORBED, 2);
+  } else {
+    // cutoff: E_F + E_B (n), E_F + E_B + E_C (p)
+    keep1 = o1sq > (t.type ? sh.pc2_p : sh.pc2_n);
+    keep2 = o2sq > (t2 ? sh.pc2_p : sh.pc2_n);
+    st.add(S_ABSORBED, (keep1 ? 0 : 1) + (keep2 ? 0 : 1));
+  }
+  // children: scattered projectile keeps the lane's track slot (pi' = 2 pi), recoil is c2 (pi' = 2 pi + 1)
+  c2.x = t.x; c2.y = t.y; c2.z = t.z; c2.px = o2x; c2.py = o2y; c2.pz = o2z;
+  c2.T = M<R>::div_(o2sq, M<R>::sqrt_(o2sq + m2 * m2) + m2);
+  c2.pi = 2u * t.pi + 1u; c2.k = 0u; c2.nseg = 0; c2.type = t2; c2.shell = t.shell;
+  t.px = o1x; t.py = o1y; t.pz = o1z;
+  t.T = M<R>::div_(o1sq, M<R>::sqrt_(o1sq + m1 * m1) + m1);
+  t.pi = 2u * t.pi; t.k = 0u; t.nseg = 0;
+  return true;
+}
+
+// ---------- C6: epilogue ("excitation energy ... through energy conservation") ----------
+// Eavail = E_in - sum T_k, (Prx,Pry,Prz) = p_in - sum p_k.  Returns true if the attempt is accepted.
+template <typename R>
+__device__ __forceinline__ bool epilogue_eval(const NucDev<R> &nu, const R *bind, int n_esc, int n_p, int n_real,
+                                              R Eavail, R Prx, R Pry, R Prz, bool keep_transparent,
+                                              int &A_res, int &Z_res, R &Estar) {
+  A_res = nu.A + 1 - n_esc; Z_res = nu.Z + 1 - n_p;
+  Estar = R(0);
+  if (!((n_real > 0) || keep_transparent)) return false;       // transparent: not a non-elastic event
+  R Bres = R(-1e30);
+  if (A_res >= 1 && A_res < kAmax && Z_res >= 0 && Z_res < kZmax) Bres = __ldg(bind + A_res * kZmax + Z_res);
+  if (Bres < R(-1e29)) return false;                            // no such nucleus
+  // E_res - M_res = X with the nucleon masses cancelled analytically; E* = M* - M_res in rationalised form
+  const R X = Eavail + Bres - nu.Bt;
+  const R Mres = R(Z_res) * K<R>::mp + R(A_res - Z_res) * K<R>::mn - Bres;
+  const R P2 = Prx * Prx + Pry * Pry + Prz * Prz;
+  const R Er = Mres + X;
+  const R M2 = Er * Er - P2;
+  const R Mstar = M2 > R(0) ? M<R>::sqrt_(M2) : R(0);
+  Estar = (R(2) * Mres * X + X * X - P2) / (Mstar + Mres);
+  if (Estar < R(0) && !(keep_transparent && n_real == 0)) return false;
+  return true;
+}
+
+// ---- kernel parameters ------------------------------------------------------------------------------
 template <typename R> struct CascadeParams {
   ModelDev<R> model;
   Workspace<R> ws;
@@ -208,34 +520,84 @@ template <typename R> struct CascadeParams {
   int n_chunk;
   uint32_t seed_lo, seed_hi;
   uint32_t flags;
-  int vote_coll, vote_epi;  // phase-vote thresholds
-  int n_live_nuc;           // nuclei slots to stage into shared memory (0..INC_MAX_TARGETS)
+  int vote_coll, vote_epi;  // lane kernel: phase-vote thresholds
+  int n_stage;              // nuclei slots staged into shared memory (target_id must be < n_stage)
 };
 
-// shared-memory layout: [NucDev x INC_MAX_TARGETS (only live ones filled)] [tabS n_xs*4]
-template <typename R> __host__ __device__ inline size_t cascade_smem_bytes(int n_xs) {
-  return sizeof(NucDev<R>) * INC_MAX_TARGETS + sizeof(R) * 4 * (size_t)n_xs;
+// shared-memory staging of the model: [NucDev x n_stage] [tabS n_xs*4]   (n_stage = highest live slot + 1)
+template <typename R> __host__ __device__ inline size_t model_smem_bytes(int n_xs, int n_stage) {
+  return sizeof(NucDev<R>) * (size_t)n_stage + sizeof(R) * 4 * (size_t)n_xs;
 }
 
+template <typename R>
+__device__ __forceinline__ void stage_model(const ModelDev<R> &model, int n_stage, NucDev<R> *s_nuc, R *s_tabS) {
+  const int nw = (int)(sizeof(NucDev<R>) / 4);
+  for (int t = 0; t < n_stage; ++t) {
+    if (!model.nuc[t].live) { if (threadIdx.x == 0) s_nuc[t].live = 0; continue; }
+    const uint32_t *src = reinterpret_cast<const uint32_t *>(&model.nuc[t]);
+    uint32_t *dst = reinterpret_cast<uint32_t *>(&s_nuc[t]);
+    for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
+  }
+  const int nt = model.n_xs * 4;
+  for (int i = threadIdx.x; i < nt; i += blockDim.x) s_tabS[i] = model.tabS[i];
+  __syncthreads();
+}
+
+// validate an event's inputs; on failure write neutral outputs and raise the device error word
+template <typename R>
+__device__ __forceinline__ bool check_inputs(const CascadeParams<R> &P, const NucDev<R> *s_nuc, int ev, R E_in, int tgt) {
+  unsigned err = 0;
+  if (!(E_in >= R(INC_E_MIN) && E_in <= R(INC_E_MAX))) err |= 1u;
+  if (tgt < 0 || tgt >= P.n_stage) err |= 2u;
+  else if (!s_nuc[tgt].live) err |= 2u;
+  if (!err) return true;
+  atomicOr(&P.ctr->error_word, err);
+  P.ws.cA[ev] = 0; P.ws.cZ[ev] = 0; P.ws.cE[ev] = R(0);
+  P.ws.cPx[ev] = R(0); P.ws.cPy[ev] = R(0); P.ws.cPz[ev] = R(0);
+  P.ws.cmeta[ev] = (1u << 16); P.ws.cstatus[ev] = INC_ST_FAILED;
+  return false;
+}
+
+template <typename R>
+__device__ __forceinline__ void write_cascade_result(const Workspace<R> &ws, int ev, int A, int Z, R Es, R Px, R Py, R Pz,
+                                                     uint32_t meta, uint32_t status) {
+  ws.cA[ev] = A; ws.cZ[ev] = Z; ws.cE[ev] = Es;
+  ws.cPx[ev] = Px; ws.cPy[ev] = Py; ws.cPz[ev] = Pz;
+  ws.cmeta[ev] = meta; ws.cstatus[ev] = status;
+}
+
+// Order-independent sums (escaped energy and momentum): fixed point, so that any processing order of
+// an event's tracks gives bit-identical residuals.  double: int64, unit 2^-40 MeV; float: int32, unit
+// 2^-20 MeV (|values| < 2048 MeV, resolution below the fp32 rounding of the addends).
+template <typename R> struct Fx;
+template <> struct Fx<double> {
+  typedef long long T; typedef unsigned long long U;
+  static __device__ __forceinline__ T to(double v) { return __double2ll_rn(v * 1099511627776.0); }
+  static __device__ __forceinline__ double from(T v) { return (double)v * (1.0 / 1099511627776.0); }
+};
+template <> struct Fx<float> {
+  typedef int T; typedef unsigned int U;
+  static __device__ __forceinline__ T to(float v) { return __float2int_rn(v * 1048576.0f); }
+  static __device__ __forceinline__ float from(T v) { return (float)v * (1.0f / 1048576.0f); }
+};
+
+// =================================================================================================
+// Cascade kernel A: lane-per-event state machine with warp-voted phases
+// =================================================================================================
+enum LaneState : int { ST_SEG = 0, ST_COLL = 1, ST_EPI = 2, ST_DONE = 3 };
+
+template <typename R> struct TrackRec {   // pending track (local-memory stack)
+  R x, y, z, px, py, pz, T;
+  uint32_t pi;
+  uint32_t meta;   // type | shell << 1
+};
+
 template <typename R, bool STATS>
-__global__ void __launch_bounds__(256, 2) cascade_kernel(const CascadeParams<R> P) {
+__global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParams<R> P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   NucDev<R> *s_nuc = reinterpret_cast<NucDev<R> *>(smem_raw);
-  R *s_tabS = reinterpret_cast<R *>(smem_raw + sizeof(NucDev<R>) * INC_MAX_TARGETS);
-
-  // ---- stage the model into shared memory (read-only afterwards) ----
-  {
-    const int nw = (int)(sizeof(NucDev<R>) / 4);
-    for (int t = 0; t < INC_MAX_TARGETS; ++t) {
-      if (!P.model.nuc[t].live) { if (threadIdx.x == 0) s_nuc[t].live = 0; continue; }
-      const uint32_t *src = reinterpret_cast<const uint32_t *>(&P.model.nuc[t]);
-      uint32_t *dst = reinterpret_cast<uint32_t *>(&s_nuc[t]);
-      for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
-    }
-    const int nt = P.model.n_xs * 4;
-    for (int i = threadIdx.x; i < nt; i += blockDim.x) s_tabS[i] = P.model.tabS[i];
-  }
-  __syncthreads();
+  R *s_tabS = reinterpret_cast<R *>(smem_raw + sizeof(NucDev<R>) * P.n_stage);
+  stage_model<R>(P.model, P.n_stage, s_nuc, s_tabS);
 
   const int lane = threadIdx.x & 31;
   const int n_xs = P.model.n_xs;
@@ -243,37 +605,38 @@ __global__ void __launch_bounds__(256, 2) cascade_kernel(const CascadeParams<R> 
   const bool keep_transparent = (P.flags & INC_F_KEEP_TRANSPARENT) != 0;
   const bool same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
 
-  // ---- lane registers ----
   int state = ST_EPI;
-  int ev = -1;                  // chunk-local event index
-  int tgt = 0;
+  int ev = -1, tgt = 0;
   uint32_t attempt = 0;
   R E_in = R(0);
   RngKey g;
   g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = 0; g.e1 = 0;
-  // current track
-  R x = 0, y = 0, z = 0, px = 0, py = 0, pz = 0;
-  uint32_t pi = 0, kblk = 0;
-  int type = 0, shell = 0, nseg = 0;
-  // event accumulators
-  R Eavail = 0, Prx = 0, Pry = 0, Prz = 0;
+  Track<R> t;
+  t.x = t.y = t.z = t.px = t.py = t.pz = t.T = R(0); t.pi = 0; t.k = 0; t.nseg = 0; t.type = 0; t.shell = 0;
+  typename Fx<R>::T fxE = 0, fxX = 0, fxY = 0, fxZ = 0;   // fixed-point E_in - sum T, p_in - sum p
   int n_esc = 0, n_p = 0, n_real = 0;
   uint32_t st_try = 0;
-  // pending stack
   TrackRec<R> stack[kStackCap];
   int sp = 0;
-  // carry from SEG to COLL
-  R c_f = 0, c_nx = 0, c_ny = 0, c_nz = 0, c_Sp = 0, c_Sig = 0;
-  // stats
-  unsigned long long stc[S_NSTAT];
-  if (STATS) {
-#pragma unroll
-    for (int i = 0; i < S_NSTAT; ++i) stc[i] = 0;
-  }
+  CollCarry<R> cc;
+  cc.f = cc.nx = cc.ny = cc.nz = cc.Sp = cc.Sig = R(0);
+  LaneStats<STATS> st;
+  st.clear();
+
+  auto pop_or_finish = [&]() {
+    if (sp > 0) {
+      const TrackRec<R> &r = stack[--sp];
+      t.x = r.x; t.y = r.y; t.z = r.z; t.px = r.px; t.py = r.py; t.pz = r.pz; t.T = r.T;
+      t.pi = r.pi; t.type = r.meta & 1; t.shell = (int)(r.meta >> 1);
+      t.k = 0; t.nseg = 0;
+      state = ST_SEG;
+    } else {
+      state = ST_EPI;
+    }
+  };
 
   for (;;) {
     __syncwarp();
-    // ---- phase vote ----
     const unsigned mS = __ballot_sync(kFull, state == ST_SEG);
     const unsigned mC = __ballot_sync(kFull, state == ST_COLL);
     const unsigned mE = __ballot_sync(kFull, state == ST_EPI);
@@ -285,294 +648,75 @@ __global__ void __launch_bounds__(256, 2) cascade_kernel(const CascadeParams<R> 
     else phase = ST_SEG;
 
     if (phase == ST_SEG) {
-      if (STATS && lane == 0) { stc[S_WI_SEG]++; stc[S_LS_SEG] += nS; }
+      if (lane == 0) { st.add(S_WI_SEG); st.add(S_LS_SEG, nS); }
       if (state == ST_SEG) {
-        bool dead = false;
-        const NucDev<R> &nu = s_nuc[tgt];
-        if (nseg >= kMaxSeg) {                       // R-C2 cap
+        Escape<R> esc;
+        const int out = seg_step<R, STATS>(t, s_nuc[tgt], s_tabS, n_xs, inv_dp, g, attempt, cc, esc, st);
+        if (out == SEG_COLLIDE) state = ST_COLL;
+        else if (out == SEG_ESCAPE) {
+          if (n_esc < kMaxSec) {
+            const size_t o = (size_t)ev * kMaxSec + n_esc;
+            P.ws.st_code[o] = t.pi | ((uint32_t)t.type << 24);
+            P.ws.st_T[o] = esc.T; P.ws.st_ux[o] = esc.ux; P.ws.st_uy[o] = esc.uy; P.ws.st_uz[o] = esc.uz;
+            n_esc++; n_p += t.type;
+            fxE -= Fx<R>::to(esc.T); fxX -= Fx<R>::to(t.px); fxY -= Fx<R>::to(t.py); fxZ -= Fx<R>::to(t.pz);
+          } else {
+            st_try |= INC_ST_SEC_TRUNC;
+          }
+          pop_or_finish();
+        } else if (out == SEG_CAP) {
           st_try |= INC_ST_SEG_CAP;
-          if (STATS) stc[S_ABSORBED]++;
-          dead = true;
-        } else {
-          nseg++;
-          if (STATS) stc[S_SEG]++;
-          // ---------- C2: segment (R-Q8 partner first, then the path) ----------
-          R u[4];
-          draw4<R>(g, attempt, pi, kblk++, u);
-          const ShellDev<R> &sh = nu.sh[shell];
-          const R m1 = nucleon_mass<R>(type);
-          const R p1sq = px * px + py * py + pz * pz;
-          const R E1 = M<R>::sqrt_(p1sq + m1 * m1);
-          const R T1 = M<R>::div_(p1sq, E1 + m1);
-          // partner direction and magnitude fraction ("quadratic distribution")
-          const R cth = R(2) * u[1] - R(1);
-          R s2 = R(1) - cth * cth;
-          s2 = s2 > R(0) ? s2 : R(0);
-          const R sth = M<R>::sqrt_(s2);
-          R sph, cph;
-          M<R>::sincos2pi(u[2], &sph, &cph);
-          const R nx = sth * cph, ny = sth * sph, nz = cth;
-          const R f = M<R>::cbrt_(u[0]);
-          const R pn = px * nx + py * ny + pz * nz;
-          // cross sections against a proton and a neutron partner (same n, f: R-C2)
-          const R plab_p = plab_of<R>(m1, T1, pn, sh.pF_p * f, K<R>::mp);
-          const R plab_n = plab_of<R>(m1, T1, pn, sh.pF_n * f, K<R>::mn);
-          int kp, kn; R fp, fn;
-          grid_pos<R>(plab_p, inv_dp, n_xs, kp, fp);
-          grid_pos<R>(plab_n, inv_dp, n_xs, kn, fn);
-          // tabS row: {sig_pp, d, sig_np, d}; vs proton: pp if type==1 else np; vs neutron: opposite
-          const R *rp = s_tabS + 4 * kp + (type ? 0 : 2);
-          const R *rn = s_tabS + 4 * kn + (type ? 2 : 0);
-          const R sig_p = rp[0] + fp * rp[1];
-          const R sig_n = rn[0] + fn * rn[1];
-          const R Sp = sh.rho_p * sig_p, Sn = sh.rho_n * sig_n;
-          const R Sig = Sp + Sn;
-          const R d_coll = Sig > R(0) ? M<R>::div_(-M<R>::log_(u[3]), Sig) : R(1e30);
-          // geometry: distances to the shell spheres along the flight direction
-          const R ip = M<R>::rsqrt_(p1sq);
-          const R dx = px * ip, dy = py * ip, dz = pz * ip;
-          const R beta = x * dx + y * dy + z * dz;
-          const R r2 = x * x + y * y + z * z;
-          const R r_in = R(shell) * nu.dr, r_out = R(shell + 1) * nu.dr;
-          R disc_out = beta * beta - r2 + r_out * r_out;
-          disc_out = disc_out > R(0) ? disc_out : R(0);
-          const R d_out = -beta + M<R>::sqrt_(disc_out);
-          R d_in = R(1e30);
-          if (shell > 0 && beta < R(0)) {
-            const R D = beta * beta - r2 + r_in * r_in;
-            if (D > R(0)) d_in = -beta - M<R>::sqrt_(D);
-          }
-          const bool inward = d_in < d_out;
-          const R d_min = inward ? d_in : d_out;
-          if (d_coll < d_min) {
-            // collision point reached first: defer the collision to the COLL phase
-            x += d_coll * dx; y += d_coll * dy; z += d_coll * dz;
-            c_f = f; c_nx = nx; c_ny = ny; c_nz = nz; c_Sp = Sp; c_Sig = Sig;
-            state = ST_COLL;
-          } else {
-            // ---------- C4: shell boundary, potential step (P:49 refraction/reflection) ----------
-            if (STATS) stc[S_BND]++;
-            const int j = inward ? shell - 1 : shell + 1;
-            const R rb = inward ? r_in : r_out;
-            x += d_min * dx; y += d_min * dy; z += d_min * dz;
-            const R irr = M<R>::rsqrt_(x * x + y * y + z * z);
-            const R ux = x * irr, uy = y * irr, uz = z * irr;   // outward normal
-            x = ux * rb; y = uy * rb; z = uz * rb;                // renormalise onto the sphere
-            const R pr = px * ux + py * uy + pz * uz;
-            const R Vi = type ? sh.V_p : sh.V_n;
-            const R Vj = type ? nu.sh[j].V_p : nu.sh[j].V_n;
-            const R dV = Vj - Vi;
-            const R Tj = T1 + dV;
-            const R prj2 = pr * pr + dV * (T1 + Tj + R(2) * m1);  // p_j^2 - p_t^2
-            if (Tj <= R(0) || prj2 <= R(0)) {
-              if (STATS) stc[S_REFL]++;
-              const R t2 = R(2) * pr;
-              px -= t2 * ux; py -= t2 * uy; pz -= t2 * uz;         // specular reflection
-            } else {
-              const R prj = pr >= R(0) ? M<R>::sqrt_(prj2) : -M<R>::sqrt_(prj2);
-              const R dp = prj - pr;
-              px += dp * ux; py += dp * uy; pz += dp * uz;
-              shell = j;
-              if (j == nu.ns) {
-                // escape: append to the event's list ("SoA ... exiting particles")
-                if (STATS) stc[S_ESC]++;
-                dead = true;
-                if (n_esc < kMaxSec) {
-                  const R ipj = M<R>::rsqrt_(px * px + py * py + pz * pz);
-                  const size_t o = (size_t)ev * kMaxSec + n_esc;
-                  P.ws.st_code[o] = pi | ((uint32_t)type << 24);
-                  P.ws.st_T[o] = Tj;
-                  P.ws.st_ux[o] = px * ipj; P.ws.st_uy[o] = py * ipj; P.ws.st_uz[o] = pz * ipj;
-                  n_esc++; n_p += type;
-                  Eavail -= Tj; Prx -= px; Pry -= py; Prz -= pz;
-                } else {
-                  st_try |= INC_ST_SEC_TRUNC;
-                }
-              }
-            }
-          }
-        }
-        if (dead) {
-          if (sp > 0) {
-            const TrackRec<R> &t = stack[--sp];
-            x = t.x; y = t.y; z = t.z; px = t.px; py = t.py; pz = t.pz;
-            pi = t.pi; type = t.meta & 1; shell = (int)(t.meta >> 1);
-            kblk = 0; nseg = 0;
-          } else {
-            state = ST_EPI;
-          }
+          pop_or_finish();
         }
       }
     } else if (phase == ST_COLL) {
-      if (STATS && lane == 0) { stc[S_WI_COLL]++; stc[S_LS_COLL] += nC; }
+      if (lane == 0) { st.add(S_WI_COLL); st.add(S_LS_COLL, nC); }
       if (state == ST_COLL) {
-        // ---------- C3: collision ----------
-        if (STATS) stc[S_COLL]++;
-        const NucDev<R> &nu = s_nuc[tgt];
-        const ShellDev<R> &sh = nu.sh[shell];
-        R u[4];
-        draw4<R>(g, attempt, pi, kblk++, u);
-        const int t2 = (u[0] * c_Sig < c_Sp) ? 1 : 0;
-        const R m1 = nucleon_mass<R>(type), m2 = nucleon_mass<R>(t2);
-        const R q = (t2 ? sh.pF_p : sh.pF_n) * c_f;
-        const R p2x = q * c_nx, p2y = q * c_ny, p2z = q * c_nz;
-        const R p1sq = px * px + py * py + pz * pz;
-        const R E1 = M<R>::sqrt_(p1sq + m1 * m1);
-        const R T1 = M<R>::div_(p1sq, E1 + m1);
-        const R E2 = M<R>::sqrt_(q * q + m2 * m2);
-        const R pn = px * c_nx + py * c_ny + pz * c_nz;
-        const R plab = plab_of<R>(m1, T1, pn, q, m2);
-        int kk; R ff;
-        grid_pos<R>(plab, inv_dp, n_xs, kk, ff);
-        const bool same = (t2 == type);
-        const R *row = P.model.tabC + 8 * kk;
-        const R B = same ? (__ldg(row + 0) + ff * __ldg(row + 1)) : (__ldg(row + 2) + ff * __ldg(row + 3));
-        const R ab = same ? R(0) : (__ldg(row + 4) + ff * __ldg(row + 5));
-        // boost to the CM frame
-        const R Px = px + p2x, Py = py + p2y, Pz = pz + p2z;
-        const R E = E1 + E2;
-        const R s = E * E - (Px * Px + Py * Py + Pz * Pz);
-        const R iE = R(1) / E;
-        const R bx = Px * iE, by = Py * iE, bz = Pz * iE;
-        const R gam = E * M<R>::rsqrt_(s);
-        const R gfac = gam * gam / (gam + R(1));        // (gamma - 1) / beta^2
-        const R pb = px * bx + py * by + pz * bz;
-        const R fb = gfac * pb - gam * E1;
-        const R qx = px + fb * bx, qy = py + fb * by, qz = pz + fb * bz;   // p1 in the CM frame
-        const R pcm2 = qx * qx + qy * qy + qz * qz;
-        const R ipcm = M<R>::rsqrt_(pcm2);
-        const R pcm = pcm2 * ipcm;
-        // scattering angle: dsigma/dt ~ exp(B t), t in (GeV/c)^2 (R-Q10)
-        const R pg2 = pcm2 * R(1e-6);
-        const R tmin = R(-4) * pg2;
-        R t;
-        if (B * (-tmin) < R(1e-9)) t = u[1] * tmin;
-        else t = M<R>::log1p_(-u[1] * (-M<R>::expm1_(B * tmin))) / B;
-        R ct = R(1) + t / (R(2) * pg2);
-        ct = ct < R(-1) ? R(-1) : (ct > R(1) ? R(1) : ct);
-        if (!same && u[2] * (R(1) + ab) < ab) ct = -ct;       // np backward term
-        R st2 = R(1) - ct * ct;
-        const R stt = M<R>::sqrt_(st2 > R(0) ? st2 : R(0));
-        R sphi, cphi;
-        M<R>::sincos2pi(u[3], &sphi, &cphi);
-        // rotation frame around n = q/|q|
-        const R n0 = qx * ipcm, n1 = qy * ipcm, n2 = qz * ipcm;
-        const R q2 = n0 * n0 + n1 * n1;
-        R e1x, e1y, e1z, e2x, e2y;
-        if (q2 > R(1e-24)) {
-          const R iq = M<R>::rsqrt_(q2);
-          e1x = n0 * n2 * iq; e1y = n1 * n2 * iq; e1z = -q2 * iq;
-          e2x = -n1 * iq; e2y = n0 * iq;
-        } else {
-          e1x = R(1); e1y = R(0); e1z = R(0);
-          e2x = R(0); e2y = n2 >= R(0) ? R(1) : R(-1);
-        }
-        const R a1 = stt * cphi, a2 = stt * sphi;
-        const R w1x = pcm * (a1 * e1x + a2 * e2x + ct * n0);
-        const R w1y = pcm * (a1 * e1y + a2 * e2y + ct * n1);
-        const R w1z = pcm * (a1 * e1z + ct * n2);
-        // boost back; partner by momentum conservation
-        const R E1cm = M<R>::sqrt_(pcm2 + m1 * m1);
-        const R wb = w1x * bx + w1y * by + w1z * bz;
-        const R fo = gfac * wb + gam * E1cm;
-        const R o1x = w1x + fo * bx, o1y = w1y + fo * by, o1z = w1z + fo * bz;
-        const R o2x = Px - o1x, o2y = Py - o1y, o2z = Pz - o1z;
-        const R o1sq = o1x * o1x + o1y * o1y + o1z * o1z;
-        const R o2sq = o2x * o2x + o2y * o2y + o2z * o2z;
-        // Pauli blocking: both products above their Fermi energies (strict, R-Q12)
-        const R pF2_1 = type ? sh.pF2_p : sh.pF2_n;
-        const R pF2_2 = t2 ? sh.pF2_p : sh.pF2_n;
-        if (!(o1sq > pF2_1 && o2sq > pF2_2)) {
-          if (STATS) stc[S_BLOCKED]++;
-          state = ST_SEG;                                  // projectile continues unchanged (R-Q13)
-        } else {
+        Track<R> c2;
+        bool keep1 = false, keep2 = false;
+        const bool allowed = coll_step<R, STATS>(t, cc, s_nuc[tgt], P.model.tabC, n_xs, inv_dp, g, attempt, c2, keep1, keep2, st_try, st);
+        if (!allowed) state = ST_SEG;
+        else {
           n_real++;
-          if (STATS) stc[S_ALLOWED]++;
-          bool keep1 = false, keep2 = false;
-          if (2u * pi + 1u >= (1u << 24)) {                // depth cap (R-C3)
-            st_try |= INC_ST_DEPTH_CAP;
-            if (STATS) stc[S_ABSORBED] += 2;
-          } else {
-            // cutoff: E_F + E_B (n), E_F + E_B + E_C (p)
-            keep1 = o1sq > (type ? sh.pc2_p : sh.pc2_n);
-            keep2 = o2sq > (t2 ? sh.pc2_p : sh.pc2_n);
-            if (STATS) stc[S_ABSORBED] += (keep1 ? 0 : 1) + (keep2 ? 0 : 1);
-          }
-          const uint32_t pi0 = 2u * pi, pi1 = 2u * pi + 1u;
           if (keep1 && keep2) {
             if (sp < kStackCap) {
-              TrackRec<R> &t = stack[sp++];
-              t.x = x; t.y = y; t.z = z; t.px = o2x; t.py = o2y; t.pz = o2z;
-              t.pi = pi1; t.meta = (uint32_t)t2 | ((uint32_t)shell << 1);
+              TrackRec<R> &r = stack[sp++];
+              r.x = c2.x; r.y = c2.y; r.z = c2.z; r.px = c2.px; r.py = c2.py; r.pz = c2.pz; r.T = c2.T;
+              r.pi = c2.pi; r.meta = (uint32_t)c2.type | ((uint32_t)c2.shell << 1);
             } else {
               st_try |= INC_ST_QUEUE_OVF;
             }
-          }
-          if (keep1) {
-            px = o1x; py = o1y; pz = o1z; pi = pi0; kblk = 0; nseg = 0;
             state = ST_SEG;
-          } else if (keep2) {
-            px = o2x; py = o2y; pz = o2z; pi = pi1; type = t2; kblk = 0; nseg = 0;
-            state = ST_SEG;
-          } else if (sp > 0) {
-            const TrackRec<R> &t = stack[--sp];
-            x = t.x; y = t.y; z = t.z; px = t.px; py = t.py; pz = t.pz;
-            pi = t.pi; type = t.meta & 1; shell = (int)(t.meta >> 1);
-            kblk = 0; nseg = 0;
-            state = ST_SEG;
-          } else {
-            state = ST_EPI;
-          }
+          } else if (keep1) state = ST_SEG;
+          else if (keep2) { t = c2; state = ST_SEG; }
+          else pop_or_finish();
         }
       }
-    } else {  // ---------- EPI phase: epilogue of the finished attempt, then entry of the next ----------
-      if (STATS && lane == 0) { stc[S_WI_EPI]++; stc[S_LS_EPI] += nE; }
+    } else {  // EPI phase: epilogue of the finished attempt, then entry of the next attempt / event
+      if (lane == 0) { st.add(S_WI_EPI); st.add(S_LS_EPI, nE); }
       bool want_event = false;
       if (state == ST_EPI) {
         if (ev >= 0) {
-          // ---------- C6: epilogue ("excitation energy ... through energy conservation") ----------
           const NucDev<R> &nu = s_nuc[tgt];
-          const int A_res = nu.A + 1 - n_esc, Z_res = nu.Z + 1 - n_p;
-          bool ok = (n_real > 0) || keep_transparent;
-          R Estar = R(0);
+          int A_res, Z_res;
+          R Estar;
+          const R Eavail = Fx<R>::from(fxE), Prx = Fx<R>::from(fxX), Pry = Fx<R>::from(fxY), Prz = Fx<R>::from(fxZ);
+          const bool ok = epilogue_eval<R>(nu, P.model.bind, n_esc, n_p, n_real, Eavail, Prx, Pry, Prz, keep_transparent, A_res, Z_res, Estar);
           if (ok) {
-            R Bres = R(-1e30);
-            if (A_res >= 1 && A_res < kAmax && Z_res >= 0 && Z_res < kZmax) Bres = __ldg(P.model.bind + A_res * kZmax + Z_res);
-            if (Bres < R(-1e29)) ok = false;                 // no such nucleus: retry
-            else {
-              // E_res - M_res = X, with the nucleon masses cancelled analytically
-              const R X = Eavail + Bres - nu.Bt;
-              const R Mres = R(Z_res) * K<R>::mp + R(A_res - Z_res) * K<R>::mn - Bres;
-              const R P2 = Prx * Prx + Pry * Pry + Prz * Prz;
-              const R Er = Mres + X;
-              const R M2 = Er * Er - P2;
-              const R Mstar = M2 > R(0) ? M<R>::sqrt_(M2) : R(0);
-              Estar = (R(2) * Mres * X + X * X - P2) / (Mstar + Mres);
-              if (Estar < R(0) && !(keep_transparent && n_real == 0)) ok = false;
-            }
-          }
-          if (ok) {
-            P.ws.cA[ev] = A_res; P.ws.cZ[ev] = Z_res; P.ws.cE[ev] = Estar;
-            P.ws.cPx[ev] = Prx; P.ws.cPy[ev] = Pry; P.ws.cPz[ev] = Prz;
-            P.ws.cmeta[ev] = (uint32_t)n_esc | (attempt << 8);
             const uint32_t used = attempt + 1u > 255u ? 255u : attempt + 1u;
-            P.ws.cstatus[ev] = st_try | used;
+            write_cascade_result<R>(P.ws, ev, A_res, Z_res, Estar, Prx, Pry, Prz, (uint32_t)n_esc | (attempt << 8), st_try | used);
             ev = -1;
           } else {
             attempt++;
             if (attempt >= (uint32_t)kMaxAttempt) {          // FAILED: count 0, target at rest
-              P.ws.cA[ev] = nu.A; P.ws.cZ[ev] = nu.Z; P.ws.cE[ev] = R(0);
-              P.ws.cPx[ev] = R(0); P.ws.cPy[ev] = R(0); P.ws.cPz[ev] = R(0);
-              P.ws.cmeta[ev] = (1u << 16);
-              P.ws.cstatus[ev] = INC_ST_FAILED | 0xFFu;
-              if (STATS) stc[S_FAILED]++;
+              write_cascade_result<R>(P.ws, ev, nu.A, nu.Z, R(0), R(0), R(0), R(0), (1u << 16), INC_ST_FAILED | 0xFFu);
+              st.add(S_FAILED);
               ev = -1;
             }
           }
         }
         want_event = (ev < 0);
       }
-      // ---- warp-aggregated event fetch (convergent) ----
       const unsigned need = __ballot_sync(kFull, want_event);
       if (need) {
         const int leader = __ffs(need) - 1;
@@ -586,21 +730,11 @@ __global__ void __launch_bounds__(256, 2) cascade_kernel(const CascadeParams<R> 
             attempt = 0;
             E_in = P.E_in[ev];
             tgt = P.target_id[ev];
-            unsigned err = 0;
-            if (!(E_in >= R(INC_E_MIN) && E_in <= R(INC_E_MAX))) err |= 1u;
-            if (tgt < 0 || tgt >= INC_MAX_TARGETS || !s_nuc[tgt < 0 ? 0 : (tgt >= INC_MAX_TARGETS ? 0 : tgt)].live) err |= 2u;
-            if (err) {
-              atomicOr(&P.ctr->error_word, err);
-              // neutral outputs; the call returns INC_E_BADARG
-              P.ws.cA[ev] = 0; P.ws.cZ[ev] = 0; P.ws.cE[ev] = R(0);
-              P.ws.cPx[ev] = R(0); P.ws.cPy[ev] = R(0); P.ws.cPz[ev] = R(0);
-              P.ws.cmeta[ev] = (1u << 16); P.ws.cstatus[ev] = INC_ST_FAILED;
-              ev = -1;
-              state = ST_EPI;    // try again for another event on the next EPI pass
-            } else {
+            if (!check_inputs<R>(P, s_nuc, ev, E_in, tgt)) { ev = -1; tgt = 0; }
+            else {
               const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
               g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
-              if (STATS) stc[S_EVENTS]++;
+              st.add(S_EVENTS);
             }
           } else {
             state = ST_DONE;
@@ -608,45 +742,342 @@ __global__ void __launch_bounds__(256, 2) cascade_kernel(const CascadeParams<R> 
         }
       }
       if (state == ST_EPI && ev >= 0) {
-        // ---------- C0: entry — uniform disc, beam along +z (R-Q15) ----------
-        if (STATS) stc[S_ATTEMPTS]++;
-        const NucDev<R> &nu = s_nuc[tgt];
-        R u[4];
-        draw4<R>(g, attempt, 1u, 0u, u);
-        const R b = nu.Rn * M<R>::sqrt_(u[0]);
-        R sb, cb;
-        M<R>::sincos2pi(u[1], &sb, &cb);
-        x = b * cb; y = b * sb;
-        R zz = nu.Rn * nu.Rn - b * b;
-        z = -M<R>::sqrt_(zz > R(0) ? zz : R(0));
-        const R p_in = M<R>::sqrt_(E_in * (E_in + R(2) * K<R>::mp));
-        // potential step into the outermost shell (cannot reflect: V rises inward)
-        const R ir = R(1) / nu.Rn;
-        const R ux = x * ir, uy = y * ir, uz = z * ir;
-        const R pr = p_in * uz;
-        const R dV = nu.sh[nu.ns - 1].V_p;
-        const R Tj = E_in + dV;
-        const R prj2 = pr * pr + dV * (E_in + Tj + R(2) * K<R>::mp);
-        const R prj = -M<R>::sqrt_(prj2 > R(0) ? prj2 : R(0));
-        const R dp = prj - pr;
-        px = dp * ux; py = dp * uy; pz = p_in + dp * uz;
-        type = 1; shell = nu.ns - 1; pi = 1u; kblk = 1u; nseg = 0;
-        Eavail = E_in; Prx = R(0); Pry = R(0); Prz = p_in;
+        st.add(S_ATTEMPTS);
+        R p_in;
+        entry_step<R>(t, s_nuc[tgt], E_in, g, attempt, p_in);
+        fxE = Fx<R>::to(E_in); fxX = 0; fxY = 0; fxZ = Fx<R>::to(p_in);
         n_esc = 0; n_p = 0; n_real = 0; st_try = 0; sp = 0;
         state = ST_SEG;
       }
     }
   }
+  st.flush(P.ctr, lane);
+}
 
-  if (STATS) {
-#pragma unroll
-    for (int i = 0; i < S_NSTAT; ++i) {
-      unsigned long long v = stc[i];
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
-      if (lane == 0 && v) atomicAdd(&P.ctr->stats[i], v);
+// =================================================================================================
+// Cascade kernel B (default): per-warp wavefront with shared-memory queues
+// =================================================================================================
+
+template <typename R, int NS, int QS, int QC> struct WarpMem {
+  // event slots (32 B each in the f32 build)
+  int32_t ev[NS];
+  uint32_t info[NS];        // n_esc | n_p << 8 | attempt << 16 | tgt << 24
+  uint32_t cnt[NS];         // pending tracks of the attempt (low 16) | real collisions (high 16)
+  uint32_t status[NS];
+  typename Fx<R>::T acc[4][NS];   // fixed-point E_in - sum T, p_in - sum p (x, y, z)
+  // segment queue (structure of arrays: lane-consecutive addresses)
+  R qx[QS], qy[QS], qz[QS], qpx[QS], qpy[QS], qpz[QS], qT[QS];
+  uint32_t qpi[QS], qkn[QS], qmeta[QS];   // qkn = k | nseg << 16 ; qmeta = type | shell << 1 | slot << 8
+  // collision queue
+  R cx[QC], cy[QC], cz[QC], cpx[QC], cpy[QC], cpz[QC], cT[QC];
+  uint32_t cpi[QC], ckn[QC], cmeta[QC];
+  R cf[QC], cnx[QC], cny[QC], cnz[QC], cSp[QC], cSig[QC];
+  // slot lists
+  uint8_t epi_q[NS], free_q[NS];
+};
+
+template <typename R> struct WaveCfg;
+template <> struct WaveCfg<float> { static constexpr int NS = 80, QS = 128, QC = 64, WARPS = 16; };
+template <> struct WaveCfg<double> { static constexpr int NS = 64, QS = 128, QC = 64, WARPS = 8; };
+
+template <typename R> __host__ __device__ inline size_t wave_smem_bytes(int n_xs, int n_stage) {
+  typedef WaveCfg<R> C;
+  return model_smem_bytes<R>(n_xs, n_stage) + 16 + sizeof(WarpMem<R, C::NS, C::QS, C::QC>) * C::WARPS;
+}
+
+template <typename R, bool STATS>
+__global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_kernel(const CascadeParams<R> P) {
+  typedef WaveCfg<R> C;
+  typedef WarpMem<R, C::NS, C::QS, C::QC> WM;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  NucDev<R> *s_nuc = reinterpret_cast<NucDev<R> *>(smem_raw);
+  R *s_tabS = reinterpret_cast<R *>(smem_raw + sizeof(NucDev<R>) * P.n_stage);
+  const size_t off = (model_smem_bytes<R>(P.model.n_xs, P.n_stage) + 15) & ~(size_t)15;
+  WM &w = reinterpret_cast<WM *>(smem_raw + off)[threadIdx.x >> 5];
+  stage_model<R>(P.model, P.n_stage, s_nuc, s_tabS);
+
+  const int lane = threadIdx.x & 31;
+  const unsigned lt = (1u << lane) - 1u;
+  const int n_xs = P.model.n_xs;
+  const R inv_dp = P.model.inv_dp;
+  const bool keep_transparent = (P.flags & INC_F_KEEP_TRANSPARENT) != 0;
+  const bool same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
+  LaneStats<STATS> st;
+  st.clear();
+
+  // warp-uniform queue sizes (every queue operation is warp-collective, so all lanes agree)
+  int nSeg = 0, nColl = 0, nEpi = 0, nFree = C::NS;
+  bool exhausted = false;
+  for (int i = lane; i < C::NS; i += 32) { w.free_q[i] = (uint8_t)i; w.ev[i] = -1; }
+  __syncwarp();
+
+  auto load_key = [&](int slot, RngKey &g, uint32_t &attempt, int &tgt, int &ev) {
+    ev = w.ev[slot];
+    const uint32_t m = w.info[slot];
+    attempt = (m >> 16) & 0xFFu; tgt = (int)(m >> 24);
+    const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
+    g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
+  };
+  auto push_seg = [&](bool pred, const Track<R> &t, int slot) {
+    const unsigned m = __ballot_sync(kFull, pred);
+    if (pred) {
+      const int i = nSeg + __popc(m & lt);
+      w.qx[i] = t.x; w.qy[i] = t.y; w.qz[i] = t.z; w.qpx[i] = t.px; w.qpy[i] = t.py; w.qpz[i] = t.pz; w.qT[i] = t.T;
+      w.qpi[i] = t.pi; w.qkn[i] = t.k | ((uint32_t)t.nseg << 16);
+      w.qmeta[i] = (uint32_t)t.type | ((uint32_t)t.shell << 1) | ((uint32_t)slot << 8);
+    }
+    nSeg += __popc(m);
+  };
+  auto push_epi = [&](bool pred, int slot) {
+    const unsigned m = __ballot_sync(kFull, pred);
+    if (pred) w.epi_q[nEpi + __popc(m & lt)] = (uint8_t)slot;
+    nEpi += __popc(m);
+  };
+
+  // lane-resident segment track: stays in registers across consecutive segment passes; only lanes whose
+  // track left the segment state (collision, escape, cap) touch the queues
+  Track<R> rt;
+  rt.x = rt.y = rt.z = rt.px = rt.py = rt.pz = rt.T = R(0); rt.pi = 0; rt.k = 0; rt.nseg = 0; rt.type = 0; rt.shell = 0;
+  int rslot = 0, rev = 0, rtgt = 0;
+  uint32_t rattempt = 0;
+  bool rhas = false;
+  int nRes = 0;   // warp-uniform count of resident tracks
+
+  for (;;) {
+    __syncwarp();
+    // ---- choose the kind of step of this pass (warp-uniform) ----
+    const int nSegT = nSeg + nRes;
+    const int availE = nEpi + (exhausted ? 0 : nFree);
+    int phase;
+    if (nColl >= 32) phase = ST_COLL;
+    else if (nSegT >= 32) phase = ST_SEG;
+    else if (availE >= 32) phase = ST_EPI;
+    else {
+      // nothing fills a whole pass: take the fullest queue (ties: entry first, it creates work)
+      if (availE > 0 && availE >= nSegT && availE >= nColl) phase = ST_EPI;
+      else if (nColl > 0 && nColl >= nSegT) phase = ST_COLL;
+      else if (nSegT > 0) phase = ST_SEG;
+      else break;
+    }
+    // capacity guards: a collision pass can add 2 tracks per item, an entry pass 1 track per item
+    if (phase == ST_COLL && nSegT + 2 * (nColl < 32 ? nColl : 32) > C::QS) phase = ST_SEG;
+    if (phase == ST_EPI && nSegT + nColl > 64) phase = nSegT > 0 ? ST_SEG : ST_COLL;   // admission control
+
+    if (phase == ST_SEG) {
+      // refill lanes without a resident track from the top of the segment queue
+      {
+        const bool need = !rhas;
+        const unsigned mk = __ballot_sync(kFull, need);
+        int take = __popc(mk);
+        take = take < nSeg ? take : nSeg;
+        const int r = __popc(mk & lt);
+        if (need && r < take) {
+          const int i = nSeg - 1 - r;
+          rt.x = w.qx[i]; rt.y = w.qy[i]; rt.z = w.qz[i]; rt.px = w.qpx[i]; rt.py = w.qpy[i]; rt.pz = w.qpz[i]; rt.T = w.qT[i];
+          rt.pi = w.qpi[i];
+          const uint32_t kn = w.qkn[i], mt = w.qmeta[i];
+          rt.k = kn & 0xFFFFu; rt.nseg = (int)(kn >> 16);
+          rt.type = mt & 1u; rt.shell = (int)((mt >> 1) & 0x7Fu); rslot = (int)(mt >> 8);
+          rev = w.ev[rslot];
+          const uint32_t inf = w.info[rslot];
+          rattempt = (inf >> 16) & 0xFFu; rtgt = (int)(inf >> 24);
+          rhas = true;
+        }
+        nSeg -= take; nRes += take;
+      }
+      if (lane == 0) { st.add(S_WI_SEG); st.add(S_LS_SEG, nRes); }
+      int out = -1;
+      CollCarry<R> cc;
+      Escape<R> esc;
+      if (rhas) {
+        RngKey g;
+        const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + rev);
+        g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
+        out = seg_step<R, STATS>(rt, s_nuc[rtgt], s_tabS, n_xs, inv_dp, g, rattempt, cc, esc, st);
+      }
+      const unsigned left = __ballot_sync(kFull, out > SEG_CONT);     // tracks that leave the segment state
+      if (left) {
+        {   // collisions -> collision queue
+          const bool pc = out == SEG_COLLIDE;
+          const unsigned mk = __ballot_sync(kFull, pc);
+          if (pc) {
+            const int i = nColl + __popc(mk & lt);
+            w.cx[i] = rt.x; w.cy[i] = rt.y; w.cz[i] = rt.z; w.cpx[i] = rt.px; w.cpy[i] = rt.py; w.cpz[i] = rt.pz; w.cT[i] = rt.T;
+            w.cpi[i] = rt.pi; w.ckn[i] = rt.k | ((uint32_t)rt.nseg << 16);
+            w.cmeta[i] = (uint32_t)rt.type | ((uint32_t)rt.shell << 1) | ((uint32_t)rslot << 8);
+            w.cf[i] = cc.f; w.cnx[i] = cc.nx; w.cny[i] = cc.ny; w.cnz[i] = cc.nz; w.cSp[i] = cc.Sp; w.cSig[i] = cc.Sig;
+          }
+          nColl += __popc(mk);
+        }
+        bool finished = false;
+        if (out == SEG_ESCAPE || out == SEG_CAP) {
+          if (out == SEG_ESCAPE) {
+            const uint32_t old = atomicAdd(&w.info[rslot], 1u + ((uint32_t)rt.type << 8));
+            const int idx = (int)(old & 0xFFu);
+            if (idx < kMaxSec) {
+              const size_t o = (size_t)rev * kMaxSec + idx;
+              P.ws.st_code[o] = rt.pi | ((uint32_t)rt.type << 24);
+              P.ws.st_T[o] = esc.T; P.ws.st_ux[o] = esc.ux; P.ws.st_uy[o] = esc.uy; P.ws.st_uz[o] = esc.uz;
+              typedef typename Fx<R>::U FU;
+              atomicAdd((FU *)&w.acc[0][rslot], (FU)(-Fx<R>::to(esc.T)));
+              atomicAdd((FU *)&w.acc[1][rslot], (FU)(-Fx<R>::to(rt.px)));
+              atomicAdd((FU *)&w.acc[2][rslot], (FU)(-Fx<R>::to(rt.py)));
+              atomicAdd((FU *)&w.acc[3][rslot], (FU)(-Fx<R>::to(rt.pz)));
+            } else {
+              atomicSub(&w.info[rslot], 1u + ((uint32_t)rt.type << 8));
+              atomicOr(&w.status[rslot], INC_ST_SEC_TRUNC);
+            }
+          } else {
+            atomicOr(&w.status[rslot], INC_ST_SEG_CAP);
+          }
+          finished = (atomicSub(&w.cnt[rslot], 1u) & 0xFFFFu) == 1u;
+        }
+        push_epi(finished, rslot);
+        if (out > SEG_CONT) rhas = false;
+        nRes -= __popc(left);
+      }
+      continue;
+    }
+
+    // any other pass: park the resident tracks in the segment queue first
+    if (nRes > 0) {
+      push_seg(rhas, rt, rslot);
+      rhas = false; nRes = 0;
+    }
+
+    if (phase == ST_COLL) {
+      int m = nColl < 32 ? nColl : 32;
+      if (2 * m > C::QS - nSeg) m = (C::QS - nSeg) / 2;
+      if (m <= 0) {   // both queues full: implementation limit exceeded -> fail loudly, never hang
+        if (lane == 0) atomicOr(&P.ctr->error_word, 4u);
+        break;
+      }
+      if (lane == 0) { st.add(S_WI_COLL); st.add(S_LS_COLL, m); }
+      const bool has = lane < m;
+      Track<R> t, c2;
+      CollCarry<R> cc;
+      int slot = 0;
+      if (has) {
+        const int i = nColl - 1 - lane;
+        t.x = w.cx[i]; t.y = w.cy[i]; t.z = w.cz[i]; t.px = w.cpx[i]; t.py = w.cpy[i]; t.pz = w.cpz[i]; t.T = w.cT[i];
+        t.pi = w.cpi[i];
+        const uint32_t kn = w.ckn[i], mt = w.cmeta[i];
+        t.k = kn & 0xFFFFu; t.nseg = (int)(kn >> 16);
+        t.type = mt & 1u; t.shell = (int)((mt >> 1) & 0x7Fu); slot = (int)(mt >> 8);
+        cc.f = w.cf[i]; cc.nx = w.cnx[i]; cc.ny = w.cny[i]; cc.nz = w.cnz[i]; cc.Sp = w.cSp[i]; cc.Sig = w.cSig[i];
+      }
+      nColl -= m;
+      __syncwarp();
+      bool keep1 = false, keep2 = false, allowed = false, finished = false;
+      if (has) {
+        RngKey g;
+        uint32_t attempt;
+        int tgt, ev;
+        load_key(slot, g, attempt, tgt, ev);
+        uint32_t stbits = 0;
+        allowed = coll_step<R, STATS>(t, cc, s_nuc[tgt], P.model.tabC, n_xs, inv_dp, g, attempt, c2, keep1, keep2, stbits, st);
+        if (stbits) atomicOr(&w.status[slot], stbits);
+        if (allowed) {
+          // one real collision (high half) and the change of the pending count (low half) in one atomic
+          const uint32_t delta = (1u << 16) + (keep1 ? 1u : 0u) + (keep2 ? 1u : 0u) - 1u;
+          finished = ((atomicAdd(&w.cnt[slot], delta) + delta) & 0xFFFFu) == 0u;
+        } else {
+          keep1 = true;   // blocked: the projectile continues from the collision point
+        }
+      }
+      push_seg(has && keep1, t, slot);
+      push_seg(has && allowed && keep2, c2, slot);
+      push_epi(finished, slot);
+      continue;
+    }
+
+    // ---------- EPI pass: epilogue of finished attempts, event fetch, entry ----------
+    {
+      int m = availE < 32 ? availE : 32;
+      if (m > C::QS - nSeg) m = C::QS - nSeg;
+      const int mE = nEpi < m ? nEpi : m;          // finished slots first, then free slots
+      const int mF = m - mE;
+      if (lane == 0) { st.add(S_WI_EPI); st.add(S_LS_EPI, m); }
+      const bool has = lane < m;
+      int slot = 0;
+      if (has) slot = lane < mE ? w.epi_q[nEpi - 1 - lane] : w.free_q[nFree - 1 - (lane - mE)];
+      nEpi -= mE; nFree -= mF;
+      __syncwarp();
+      bool want_event = has && lane >= mE;
+      bool do_entry = false;
+      int ev = -1, tgt = 0;
+      uint32_t attempt = 0;
+      R E_in = R(0);
+      if (has && lane < mE) {
+        ev = w.ev[slot];
+        const uint32_t ne = w.info[slot];
+        attempt = (ne >> 16) & 0xFFu; tgt = (int)(ne >> 24);
+        E_in = P.E_in[ev];
+        const NucDev<R> &nu = s_nuc[tgt];
+        const int n_esc = (int)(ne & 0xFFu), n_p = (int)((ne >> 8) & 0xFFu);
+        const R Eavail = Fx<R>::from(w.acc[0][slot]);
+        const R Prx = Fx<R>::from(w.acc[1][slot]), Pry = Fx<R>::from(w.acc[2][slot]), Prz = Fx<R>::from(w.acc[3][slot]);
+        int A_res, Z_res;
+        R Estar;
+        const bool ok = epilogue_eval<R>(nu, P.model.bind, n_esc, n_p, (int)(w.cnt[slot] >> 16), Eavail, Prx, Pry, Prz, keep_transparent, A_res, Z_res, Estar);
+        if (ok) {
+          const uint32_t used = attempt + 1u > 255u ? 255u : attempt + 1u;
+          write_cascade_result<R>(P.ws, ev, A_res, Z_res, Estar, Prx, Pry, Prz, (uint32_t)n_esc | (attempt << 8), w.status[slot] | used);
+          want_event = true;
+        } else if (attempt + 1u >= (uint32_t)kMaxAttempt) {    // FAILED: count 0, target at rest
+          write_cascade_result<R>(P.ws, ev, nu.A, nu.Z, R(0), R(0), R(0), R(0), (1u << 16), INC_ST_FAILED | 0xFFu);
+          st.add(S_FAILED);
+          want_event = true;
+        } else {
+          attempt++;
+          do_entry = true;
+        }
+      }
+      // ---- warp-aggregated event fetch ----
+      const unsigned need = __ballot_sync(kFull, want_event && !exhausted);
+      bool got_none = false;
+      if (need) {
+        const int leader = __ffs(need) - 1;
+        unsigned long long base = 0;
+        if (lane == leader) base = atomicAdd(&P.ctr->next_event_casc, (unsigned long long)__popc(need));
+        base = __shfl_sync(kFull, base, leader);
+        if (want_event) {
+          const unsigned long long mine = base + (unsigned long long)__popc(need & lt);
+          if (mine < (unsigned long long)P.n_chunk) {
+            ev = (int)mine;
+            attempt = 0;
+            E_in = P.E_in[ev];
+            tgt = P.target_id[ev];
+            if (check_inputs<R>(P, s_nuc, ev, E_in, tgt)) { do_entry = true; st.add(S_EVENTS); }
+          } else {
+            got_none = true;
+          }
+        }
+      }
+      if (__ballot_sync(kFull, got_none)) exhausted = true;
+      // slots that did not get work go back to the free list
+      {
+        const bool fr = has && !do_entry;
+        const unsigned mk = __ballot_sync(kFull, fr);
+        if (fr) { w.free_q[nFree + __popc(mk & lt)] = (uint8_t)slot; w.ev[slot] = -1; }
+        nFree += __popc(mk);
+      }
+      Track<R> t;
+      if (do_entry) {
+        st.add(S_ATTEMPTS);
+        RngKey g;
+        const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
+        g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
+        R p_in;
+        entry_step<R>(t, s_nuc[tgt], E_in, g, attempt, p_in);
+        w.ev[slot] = ev; w.info[slot] = (attempt << 16) | ((uint32_t)tgt << 24);
+        w.cnt[slot] = 1u; w.status[slot] = 0;
+        w.acc[0][slot] = Fx<R>::to(E_in); w.acc[1][slot] = 0; w.acc[2][slot] = 0; w.acc[3][slot] = Fx<R>::to(p_in);
+      }
+      push_seg(do_entry, t, slot);
     }
   }
+  st.flush(P.ctr, lane);
 }
 
 // =================================================================================================

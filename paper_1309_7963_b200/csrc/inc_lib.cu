@@ -186,10 +186,12 @@ int setup_nucleus(int A, int Z, const TablesHost &t, HostNucleus &nu) {
 void fill_nucdev(const HostNucleus &h, NucDev<real> &d) {
   std::memset(&d, 0, sizeof(d));
   d.A = h.A; d.Z = h.Z; d.ns = h.ns; d.live = 1;
-  d.Rn = (real)h.R; d.dr = (real)h.dr; d.Bt = (real)h.Bt;
+  d.Rn = (real)h.R; d.dr = (real)h.dr; d.Bt = (real)h.Bt; d.iRn = (real)(1.0 / h.R);
   for (int i = 0; i <= h.ns; ++i) {
     ShellDev<real> &s = d.sh[i];
     if (i < h.ns) {
+      s.r_in = (real)h.r[i]; s.r_out = (real)h.r[i + 1];
+      s.ir_in = i > 0 ? (real)(1.0 / h.r[i]) : (real)0; s.ir_out = (real)(1.0 / h.r[i + 1]);
       s.rho_p = (real)h.rho_p[i]; s.rho_n = (real)h.rho_n[i];
       s.pF_p = (real)h.pF_p[i]; s.pF_n = (real)h.pF_n[i];
       s.pF2_p = (real)(h.pF_p[i] * h.pF_p[i]); s.pF2_n = (real)(h.pF_n[i] * h.pF_n[i]);
@@ -382,20 +384,41 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   cp.flags = g.flags;
   const bool naive = (g.flags & INC_F_LANE_PER_EVENT) != 0;
   cp.vote_coll = naive ? 1 : g.vote_coll; cp.vote_epi = naive ? 1 : g.vote_epi;
-  cp.n_live_nuc = INC_MAX_TARGETS;
-  const size_t smem = cascade_smem_bytes<real>(model.n_xs);
-  auto kern = cascade_kernel<real, STATS>;
-  CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  int occ = 0;
-  CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, smem));
-  if (occ < 1) return fail(INC_E_CUDA, "cascade kernel does not fit on an SM");
-  int blocks = occ * g.sm_count;
-  const int need = (n_chunk + 255) / 256;
-  if (blocks > need) blocks = need;
-  CU_TRY(cudaMemsetAsync(&g.d_ctr->next_event_casc, 0, 2 * sizeof(unsigned long long), g.stream));
+  int n_stage = 0;
+  for (int i = 0; i < INC_MAX_TARGETS; ++i) if (g.nuc[i].live) n_stage = i + 1;
+  cp.n_stage = n_stage;
   const bool timing = (g.flags & INC_F_TIMING) != 0;
+  const int need = (n_chunk + 255) / 256;
+  int dev = 0, smem_max = 0;
+  CU_TRY(cudaGetDevice(&dev));
+  CU_TRY(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  const size_t wsmem = wave_smem_bytes<real>(model.n_xs, n_stage);
+  const bool lane_kernel = naive || (g.flags & INC_F_LANE_STATE_MACHINE) != 0 || wsmem > (size_t)smem_max;
+  CU_TRY(cudaMemsetAsync(&g.d_ctr->next_event_casc, 0, 2 * sizeof(unsigned long long), g.stream));
   if (mark(timing)) return INC_E_CUDA;
-  kern<<<blocks, 256, smem, g.stream>>>(cp);
+  if (lane_kernel) {
+    const size_t smem = model_smem_bytes<real>(model.n_xs, n_stage);
+    auto kern = cascade_lane_kernel<real, STATS>;
+    CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, smem));
+    if (occ < 1) return fail(INC_E_CUDA, "cascade kernel does not fit on an SM");
+    int blocks = occ * g.sm_count;
+    if (blocks > need) blocks = need;
+    kern<<<blocks, 256, smem, g.stream>>>(cp);
+  } else {
+    // one persistent CTA per SM; each warp keeps WaveCfg::NS events in flight in its shared-memory queues
+    auto kern = cascade_wavefront_kernel<real, STATS>;
+    const int threads = WaveCfg<real>::WARPS * 32;
+    CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wsmem));
+    int occ = 0;
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, wsmem));
+    if (occ < 1) return fail(INC_E_CUDA, "wavefront cascade kernel does not fit on an SM");
+    int blocks = occ * g.sm_count;
+    const int wneed = (n_chunk + threads - 1) / threads;
+    if (blocks > wneed) blocks = wneed;
+    kern<<<blocks, threads, wsmem, g.stream>>>(cp);
+  }
   CU_TRY(cudaGetLastError());
   if (mark(timing)) return INC_E_CUDA;
   // --- evaporation ---
@@ -542,6 +565,7 @@ int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64
   for (auto e : g.pending_events) cudaEventDestroy(e);
   g.pending_events.clear();
   g.last_n = n; g.last_total = (long long)tail.total;
+  if (tail.err & 4u) return fail(INC_E_STATE, "internal track-queue overflow in the wavefront cascade kernel (results invalid)");
   if (tail.err) {
     return fail(INC_E_BADARG, std::string("device-side input check failed:") + ((tail.err & 1u) ? " E_in outside [20,250] MeV" : "") +
                                   ((tail.err & 2u) ? " target_id not initialised" : ""));

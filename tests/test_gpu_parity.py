@@ -104,7 +104,7 @@ def test_fp64_event_identity(gpu, orc, otables, ptables, cfg, n):
     same = ident
     assert np.array_equal(g["casc_A"][same], o["casc_A"][same])
     assert np.allclose(g["casc_Estar"][same], o["casc_Estar"][same], rtol=1e-9, atol=1e-9)
-    assert np.allclose(g["casc_P"][same], o["casc_P"][same], rtol=1e-9, atol=1e-7)
+    assert np.allclose(g["casc_P"][same], o["casc_P"][same], rtol=1e-9, atol=1e-6)   # 1e-9 of the ~1 GeV/c scale
     # criterion (1) on the GPU output itself
     _assert_conservation(g, targets, tid, E, orc, otables, 1e-12, 1e-9)
 
@@ -129,15 +129,17 @@ def test_fp64_cascade_only_and_flags(gpu, orc, otables, ptables):
     o = orc.simulate(otables, targets, E, tid, seed, flags=orc.F_CASCADE_ONLY)
     frac, err, _ = H.event_identity(g, o)
     assert frac >= FRAC_IDENTICAL and np.all((g["species"] & 0x80) == 0)
-    # scheduling variants give bit-identical results (lane-per-event vs phase voting, thresholds)
+    # scheduling variants give bit-identical results in the fp64 build (no FMA contraction):
+    # default per-warp wavefront queues, lane state machine (two vote settings), plain lane-per-event
     base = gpu.simulate(lib, targets, E, tid, seed, ptables)
     alt = gpu.simulate(lib, targets, E, tid, seed, ptables, flags=gpu.F_LANE_PER_EVENT)
     lib.inc_set_vote_thresholds(3, 17)
-    alt2 = gpu.simulate(lib, targets, E, tid, seed, ptables)
+    alt2 = gpu.simulate(lib, targets, E, tid, seed, ptables, flags=gpu.F_LANE_STATE_MACHINE)
     lib.inc_set_vote_thresholds(8, 8)
+    alt3 = gpu.simulate(lib, targets, E, tid, seed, ptables, flags=gpu.F_LANE_STATE_MACHINE)
     for k in ("species", "T", "ux", "uz", "counts", "A", "Z", "Estar", "pz", "status"):
-        assert np.array_equal(base[k], alt[k]), k
-        assert np.array_equal(base[k], alt2[k]), k
+        for other in (alt, alt2, alt3):
+            assert np.array_equal(base[k], other[k]), k
     # stats flag does not change results and the counters match the oracle's
     st = gpu.simulate(lib, targets, E, tid, seed, ptables, flags=gpu.F_STATS)
     assert np.array_equal(base["T"], st["T"])
