@@ -29,8 +29,9 @@ METRIC = "200 MeV p-16O non-elastic events/sec on 1 B200; % of FP32 issue roofli
 UNIT = "events/s"
 
 # Algorithmic work model: lane-instructions per step kind, hand-counted
-# from the formulas (FMA = 1), times the per-event step counts measured by the work counters.
-WORK = dict(segment=330.0, boundary=45.0, collision=340.0, epilogue=120.0, evap_step=520.0, evap_trial=150.0)
+# from the formulas (FMA = 1, MUFU = 1, Philox block = 72), times the per-event step counts
+# measured by the work counters.  Queue management, addressing and votes are NOT counted.
+WORK = dict(segment=190.0, boundary=42.0, collision=255.0, epilogue=135.0, evap_step=430.0, evap_trial=90.0)
 
 
 def work_per_event(stats: dict) -> dict:
