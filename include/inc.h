@@ -80,6 +80,9 @@ extern "C" {
                                       warp-voted phases instead of the default per-warp
                                       wavefront queues.  Results never depend on the variant. */
 
+#define INC_F_NO_DRAIN_HELPERS 256u /* scheduling variant: every track stays with the warp that owns its
+                                      event (no drain helpers).  Results never depend on it.   */
+
 /* ---- model inputs ("precalculated ... tables and other read-only input data") ----- */
 typedef struct inc_tables {   /* HOST memory, caller-owned, copied during inc_init           */
   int32_t version;            /* = 1                                                         */
@@ -109,6 +112,11 @@ int inc_set_flags(uint32_t flags);
  * lanes wait for it, the epilogue+entry phase when at least `epi` lanes wait (1..32; default 8, 8).
  * Results never depend on it. */
 int inc_set_vote_thresholds(int coll, int epi);
+/* Scheduling knob of the default (wavefront) cascade kernel: a track that has run `n_segments`
+ * segments may be handed to a warp that has finished its own events, which evaluates 32 consecutive
+ * segments of the one track per pass along its collision-free path (drain helpers, DESIGN.md
+ * section 6).  0 restores the default (128).  Results never depend on it. */
+int inc_set_long_track_threshold(int n_segments);
 /* Global index of the first event of the following inc_simulate calls (default 0): event i of a
  * call uses the random stream of global event e = offset + i.  This is how a job is sharded over
  * several GPUs or calls with bit-identical per-event results (R-R4). */
@@ -174,6 +182,13 @@ int inc_get_stats(inc_stats *host_out /*HOST*/);
  * ms[0] cascade kernel, ms[1] evaporation kernel, ms[2] prefix-sum kernels, ms[3] compaction
  * kernel; launches[0..3] the number of kernel launches of each stage.  Needs INC_F_TIMING. */
 int inc_get_stage_times(float ms[4] /*HOST*/, int32_t launches[4] /*HOST*/);
+
+/* Drain timeline of the cascade kernel of the last inc_simulate (last chunk; needs INC_F_TIMING),
+ * in milliseconds after the first warp started: ms[0] mean over warps of the moment the event
+ * counter ran out for the warp, ms[1] mean warp exit, ms[2] last warp exit, ms[3] first warp
+ * exit.  Diagnostic for the tail of the persistent kernel; wavefront
+ * kernel only, zeros otherwise. */
+int inc_get_drain_timeline(double ms[4] /*HOST*/);
 
 /* Nuclear-setup record of a target, for tests of inc_init (all HOST, fp64, length n_shells
  * except r, V_p, V_n which have n_shells+1; pointers may be NULL). */

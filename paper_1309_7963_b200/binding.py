@@ -16,6 +16,7 @@ from . import build as _build
 INC_E_BADARG, INC_E_TABLES, INC_E_CAPACITY, INC_E_CUDA, INC_E_STATE = -1, -2, -3, -4, -5
 ST_FAILED, ST_SEC_TRUNC, ST_DEPTH_CAP, ST_SEG_CAP, ST_TRIAL_CAP, ST_QUEUE_OVF = (1 << 8, 1 << 9, 1 << 10, 1 << 11, 1 << 12, 1 << 13)
 F_CASCADE_ONLY, F_KEEP_TRANSPARENT, F_SAME_STREAM, F_STATS, F_LANE_PER_EVENT, F_TIMING, F_LANE_STATE_MACHINE = 1, 2, 4, 8, 16, 32, 64
+F_NO_DRAIN_HELPERS = 256
 MAX_SEC = 64
 
 _DP = C.POINTER(C.c_double)
@@ -76,7 +77,7 @@ def make_tables_struct(t: dict):
 
 
 EXPORTS = ["inc_init", "inc_free_target", "inc_shutdown", "inc_set_stream", "inc_set_flags", "inc_set_event_offset",
-           "inc_get_stage_times", "inc_set_vote_thresholds", "inc_simulate",
+           "inc_get_stage_times", "inc_get_drain_timeline", "inc_set_vote_thresholds", "inc_set_long_track_threshold", "inc_simulate",
            "inc_simulate_host", "inc_get_offsets", "inc_get_cascade_stage", "inc_get_stats", "inc_get_nucleus",
            "inc_measure_issue_peak", "inc_philox_blocks", "inc_last_error", "inc_build_info"]
 
@@ -158,6 +159,14 @@ class IncLibrary:
         ms, nl = (C.c_float * 4)(), (C.c_int32 * 4)()
         self._check(self.lib.inc_get_stage_times(ms, nl))
         return dict(zip(("cascade", "evap", "scan", "compact"), [float(x) for x in ms])), [int(x) for x in nl]
+
+    def inc_set_long_track_threshold(self, n_segments: int):
+        self._check(self.lib.inc_set_long_track_threshold(int(n_segments)))
+
+    def inc_get_drain_timeline(self):
+        ms = (C.c_double * 4)()
+        self._check(self.lib.inc_get_drain_timeline(ms))
+        return dict(zip(("exhausted_mean", "exit_mean", "exit_last", "exit_first"), [float(x) for x in ms]))
 
     def inc_set_vote_thresholds(self, coll: int, epi: int):
         self._check(self.lib.inc_set_vote_thresholds(int(coll), int(epi)))

@@ -21,7 +21,10 @@ DEPS = SOURCES + [os.path.join(CSRC, "inc_device.cuh"), os.path.join(ROOT, "incl
 COMMON = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
           "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=default"]
 VARIANTS = {
-    "f32": [],
+    # -fmad=false in the f32 build too: the wavefront kernel instantiates its pass twice (steady state / drain) and
+    # the drain helpers a third copy of the segment step; without contraction every copy rounds identically, so
+    # results cannot depend on which copy ran.  The hot segment step carries its FMAs explicitly (M<R>::fma_).
+    "f32": ["-fmad=false"],
     "f64": ["-DINC_REAL_IS_DOUBLE", "-fmad=false"],
 }
 

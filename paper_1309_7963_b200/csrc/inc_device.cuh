@@ -23,6 +23,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <type_traits>
 
 #include "../../include/inc.h"
 
@@ -97,7 +98,16 @@ struct DevCounters {       // device scalars
   unsigned int error_word;   // bit0: E_in out of range, bit1: bad target id
   unsigned int pad;
   unsigned long long stats[24];
+  // drain timeline of the wavefront kernel (INC_F_TIMING), %globaltimer ns (low 40 bits): [0] max of ~start
+  // (= ~earliest start), [1] sum over warps of the time the event counter ran out for them, [2] sum of warp
+  // exit times, [3] latest warp exit, [4] number of warps, [5] max of ~exit (= ~earliest exit)
+  unsigned long long tl[6];
 };
+__device__ __forceinline__ unsigned long long global_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  return t & 0xFFFFFFFFFFull;     // 40 bits (18 minutes): sums over a few thousand warps stay far below 2^64
+}
 
 enum StatIdx { S_EVENTS = 0, S_FAILED, S_ATTEMPTS, S_SEG, S_BND, S_REFL, S_ESC, S_COLL, S_BLOCKED,
                S_ALLOWED, S_ABSORBED, S_EVSTEPS, S_EVTRIALS, S_EVEMIT, S_WI_SEG, S_WI_COLL, S_WI_EPI,
@@ -150,27 +160,33 @@ template <> struct M<double> {
     k = kk; f = x - (double)kk;
   }
   static constexpr int kSeriesTerms = 24;
+  // pinned arithmetic: never re-contracted by the compiler, so an inlined function gives the same bits at every
+  // call site.  fp64: product and sum rounded separately, like the oracle (-ffp-contract=off).
+  static __device__ __forceinline__ double mul_(double a, double b) { return __dmul_rn(a, b); }
+  static __device__ __forceinline__ double add_(double a, double b) { return __dadd_rn(a, b); }
+  static __device__ __forceinline__ double sub_(double a, double b) { return __dsub_rn(a, b); }
+  static __device__ __forceinline__ double fma_(double a, double b, double c) { return __dadd_rn(__dmul_rn(a, b), c); }
 };
 template <> struct M<float> {
   static __device__ __forceinline__ float sqrt_(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
   static __device__ __forceinline__ float rsqrt_(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
   static __device__ __forceinline__ float lg2_(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
   static __device__ __forceinline__ float ex2_(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-  static __device__ __forceinline__ float log_(float x) { return 0.6931471805599453f * lg2_(x); }
+  static __device__ __forceinline__ float log_(float x) { return __fmul_rn(0.6931471805599453f, lg2_(x)); }
   static __device__ __forceinline__ float exp_(float x) { return ex2_(1.4426950408889634f * x); }
-  static __device__ __forceinline__ float cbrt_(float x) { return ex2_(0.3333333333f * lg2_(x)); }   // x in (0,1)
+  static __device__ __forceinline__ float cbrt_(float x) { return ex2_(__fmul_rn(0.3333333333f, lg2_(x))); }   // x in (0,1)
   static __device__ __forceinline__ float log1p_(float x) { return log1pf(x); }
   static __device__ __forceinline__ float expm1_(float x) { return expm1f(x); }
   static __device__ __forceinline__ void sincos2pi(float u, float *s, float *c) {
     // sin.approx / cos.approx scale their argument by 1/(2 pi) before MUFU: feed radians
-    float a = 6.283185307179586f * u;
+    float a = __fmul_rn(6.283185307179586f, u);
     float ss, cc;
     asm("sin.approx.ftz.f32 %0, %1;" : "=f"(ss) : "f"(a));
     asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cc) : "f"(a));
     *s = ss; *c = cc;
   }
   static __device__ __forceinline__ float rcp_(float a) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(a)); return y; }
-  static __device__ __forceinline__ float div_(float a, float b) { return a * rcp_(b); }
+  static __device__ __forceinline__ float div_(float a, float b) { return __fmul_rn(a, rcp_(b)); }
   static __device__ __forceinline__ float u01(uint32_t x) {
     // R-R3 (fp32): ((x>>9) + 1/2) 2^-23, built from the mantissa bits (no int->float conversion)
     return __uint_as_float(0x3F800000u | (x >> 9)) - 0.99999994f;
@@ -185,6 +201,10 @@ template <> struct M<float> {
     f = kk == kmax ? x - (float)kmax : f;
   }
   static constexpr int kSeriesTerms = 13;
+  static __device__ __forceinline__ float mul_(float a, float b) { return __fmul_rn(a, b); }
+  static __device__ __forceinline__ float add_(float a, float b) { return __fadd_rn(a, b); }
+  static __device__ __forceinline__ float sub_(float a, float b) { return __fsub_rn(a, b); }
+  static __device__ __forceinline__ float fma_(float a, float b, float c) { return __fmaf_rn(a, b, c); }
 };
 
 // ---- R-R1: Philox4x32-10 ---------------------------------------------------------------------
@@ -221,7 +241,7 @@ __device__ __forceinline__ void draw4(const RngKey &g, uint32_t attempt, uint32_
 // ---- table lookup (R-N7): y_k + f (y_{k+1} - y_k), clamped to the grid -------------------------
 template <typename R>
 __device__ __forceinline__ void grid_pos(R plab_mev, R inv_dp, int n_xs, int &k, R &f) {
-  R x = plab_mev * inv_dp;
+  R x = M<R>::mul_(plab_mev, inv_dp);
   const R xmax = R(n_xs - 1);
   x = x > xmax ? xmax : x;
   M<R>::split(x, n_xs - 2, k, f);
@@ -256,7 +276,7 @@ template <typename R> struct Track {
 template <typename R> struct CollCarry { R f, nx, ny, nz, Sp, Sig; };   // SEG -> COLL hand-over
 template <typename R> struct Escape { R T, ux, uy, uz; };
 
-enum SegOutcome : int { SEG_CONT = 0, SEG_COLLIDE = 1, SEG_ESCAPE = 2, SEG_CAP = 3 };
+enum SegOutcome : int { SEG_REFLECT = -1, SEG_CONT = 0, SEG_COLLIDE = 1, SEG_ESCAPE = 2, SEG_CAP = 3 };
 
 // ---------- C0: entry — uniform disc, beam along +z (R-Q15), potential step into the last shell ----------
 template <typename R>
@@ -285,10 +305,89 @@ __device__ __forceinline__ void entry_step(Track<R> &t, const NucDev<R> &nu, R E
 }
 
 // ---------- C2 + C4: one segment (R-Q8 partner first, then the path) ----------
+// Written in pinned arithmetic (M<R>::fma_/mul_/add_/sub_, never re-contracted): the wavefront kernel runs a
+// segment at two call sites (its own segment pass and the drain helpers' look-ahead), and both must give the
+// same bits in the f32 build too.  The f64 operation order is the oracle's.
+template <typename R> struct SegGeom { R dx, dy, dz, d_min; bool inward; };
+
+// R-C2 geometry: distances to the shell spheres along the flight direction
+template <typename R>
+__device__ __forceinline__ void seg_geometry(const Track<R> &t, const ShellDev<R> &sh, SegGeom<R> &gm) {
+  typedef M<R> m;
+  const R p1sq = m::fma_(t.pz, t.pz, m::fma_(t.py, t.py, m::mul_(t.px, t.px)));
+  const R ip = m::rsqrt_(p1sq);
+  gm.dx = m::mul_(t.px, ip); gm.dy = m::mul_(t.py, ip); gm.dz = m::mul_(t.pz, ip);
+  const R beta = m::fma_(t.z, gm.dz, m::fma_(t.y, gm.dy, m::mul_(t.x, gm.dx)));
+  const R r2 = m::fma_(t.z, t.z, m::fma_(t.y, t.y, m::mul_(t.x, t.x)));
+  const R bb = m::sub_(m::mul_(beta, beta), r2);
+  R disc_out = m::fma_(sh.r_out, sh.r_out, bb);
+  disc_out = disc_out > R(0) ? disc_out : R(0);
+  const R d_out = m::sub_(m::sqrt_(disc_out), beta);
+  R d_in = R(1e30);
+  if (t.shell > 0 && beta < R(0)) {
+    const R D = m::fma_(sh.r_in, sh.r_in, bb);
+    if (D > R(0)) d_in = m::sub_(-beta, m::sqrt_(D));
+  }
+  gm.inward = d_in < d_out;
+  gm.d_min = gm.inward ? d_in : d_out;
+}
+
+// R-C4 shell boundary, potential step (P:49 refraction / reflection).  Returns SEG_CONT (refracted into the
+// next shell), SEG_REFLECT (total reflection, shell unchanged) or SEG_ESCAPE (left the nucleus; esc filled).
+template <typename R>
+__device__ __forceinline__ int seg_boundary(Track<R> &t, const NucDev<R> &nu, const ShellDev<R> &sh, const SegGeom<R> &gm,
+                                            Escape<R> &esc) {
+  typedef M<R> m;
+  const int j = gm.inward ? t.shell - 1 : t.shell + 1;
+  const R irb = gm.inward ? sh.ir_in : sh.ir_out;
+  const R m1 = nucleon_mass<R>(t.type);
+  R x = m::fma_(gm.d_min, gm.dx, t.x), y = m::fma_(gm.d_min, gm.dy, t.y), z = m::fma_(gm.d_min, gm.dz, t.z);
+  // renormalise onto the sphere: one Newton step of 1/sqrt around |x|^2 = rb^2 (|x| is within rounding of rb)
+  const R rr = m::fma_(z, z, m::fma_(y, y, m::mul_(x, x)));
+  const R corr = m::sub_(R(1.5), m::mul_(m::mul_(m::mul_(R(0.5), rr), irb), irb));
+  x = m::mul_(x, corr); y = m::mul_(y, corr); z = m::mul_(z, corr);
+  t.x = x; t.y = y; t.z = z;
+  const R ux = m::mul_(x, irb), uy = m::mul_(y, irb), uz = m::mul_(z, irb);              // outward normal
+  const R pr = m::fma_(t.pz, uz, m::fma_(t.py, uy, m::mul_(t.px, ux)));
+  const R Vi = t.type ? sh.V_p : sh.V_n;
+  const R Vj = t.type ? nu.sh[j].V_p : nu.sh[j].V_n;
+  const R dV = m::sub_(Vj, Vi);
+  const R Tj = m::add_(t.T, dV);
+  const R prj2 = m::fma_(dV, m::add_(m::add_(t.T, Tj), m::mul_(R(2), m1)), m::mul_(pr, pr));   // p_j^2 - p_t^2
+  if (Tj <= R(0) || prj2 <= R(0)) {
+    const R t2 = m::mul_(R(-2), pr);
+    t.px = m::fma_(t2, ux, t.px); t.py = m::fma_(t2, uy, t.py); t.pz = m::fma_(t2, uz, t.pz);   // specular reflection
+    return SEG_REFLECT;
+  }
+  const R sq = m::sqrt_(prj2);
+  const R dp = m::sub_(pr >= R(0) ? sq : -sq, pr);
+  t.px = m::fma_(dp, ux, t.px); t.py = m::fma_(dp, uy, t.py); t.pz = m::fma_(dp, uz, t.pz);
+  t.T = Tj;
+  t.shell = j;
+  if (j == nu.ns) {                                               // escape ("exiting particles")
+    const R ipj = m::rsqrt_(m::mul_(Tj, m::fma_(R(2), m1, Tj)));
+    esc.T = Tj; esc.ux = m::mul_(t.px, ipj); esc.uy = m::mul_(t.py, ipj); esc.uz = m::mul_(t.pz, ipj);
+    return SEG_ESCAPE;
+  }
+  return SEG_CONT;
+}
+
+// momentum of the track in the rest frame of a partner with momentum q n (plab_of in pinned arithmetic)
+template <typename R>
+__device__ __forceinline__ R plab_pinned(R m1, R E1, R pn, R q, R m2, R im2) {
+  typedef M<R> m;
+  const R E2 = m::sqrt_(m::fma_(q, q, m::mul_(m2, m2)));
+  const R Tlab = m::fma_(m::fma_(E1, E2, -m::mul_(q, pn)), im2, -m1);
+  R a = m::mul_(Tlab, m::fma_(R(2), m1, Tlab));
+  a = a > R(0) ? a : R(0);
+  return m::sqrt_(a);
+}
+
 template <typename R, bool STATS>
 __device__ __forceinline__ int seg_step(Track<R> &t, const NucDev<R> &nu, const R *s_tabS, int n_xs, R inv_dp,
                                         const RngKey &g, uint32_t attempt, CollCarry<R> &cc, Escape<R> &esc,
                                         LaneStats<STATS> &st) {
+  typedef M<R> m;
   if (t.nseg >= kMaxSeg) { st.add(S_ABSORBED); return SEG_CAP; }    // R-C2 cap
   t.nseg++;
   st.add(S_SEG);
@@ -296,86 +395,70 @@ __device__ __forceinline__ int seg_step(Track<R> &t, const NucDev<R> &nu, const 
   draw4<R>(g, attempt, t.pi, t.k++, u);
   const ShellDev<R> &sh = nu.sh[t.shell];
   const R m1 = nucleon_mass<R>(t.type);
-  const R E1 = t.T + m1;
-  const R p1sq = t.px * t.px + t.py * t.py + t.pz * t.pz;
+  const R E1 = m::add_(t.T, m1);
   // partner direction and magnitude fraction ("quadratic distribution")
-  const R cth = R(2) * u[1] - R(1);
-  R s2 = R(1) - cth * cth;
+  const R cth = m::fma_(R(2), u[1], R(-1));
+  R s2 = m::fma_(-cth, cth, R(1));
   s2 = s2 > R(0) ? s2 : R(0);
-  const R sth = M<R>::sqrt_(s2);
+  const R sth = m::sqrt_(s2);
   R sph, cph;
-  M<R>::sincos2pi(u[2], &sph, &cph);
-  const R nx = sth * cph, ny = sth * sph, nz = cth;
-  const R f = M<R>::cbrt_(u[0]);
-  const R pn = t.px * nx + t.py * ny + t.pz * nz;
+  m::sincos2pi(u[2], &sph, &cph);
+  const R nx = m::mul_(sth, cph), ny = m::mul_(sth, sph), nz = cth;
+  const R f = m::cbrt_(u[0]);
+  const R pn = m::fma_(t.pz, nz, m::fma_(t.py, ny, m::mul_(t.px, nx)));
   // cross sections against a proton and a neutron partner (same n, f: R-C2)
-  const R plab_p = plab_of<R>(m1, E1, pn, sh.pF_p * f, K<R>::mp, K<R>::imp);
-  const R plab_n = plab_of<R>(m1, E1, pn, sh.pF_n * f, K<R>::mn, K<R>::imn);
+  const R plab_p = plab_pinned<R>(m1, E1, pn, m::mul_(sh.pF_p, f), K<R>::mp, K<R>::imp);
+  const R plab_n = plab_pinned<R>(m1, E1, pn, m::mul_(sh.pF_n, f), K<R>::mn, K<R>::imn);
   int kp, kn; R fp, fn;
   grid_pos<R>(plab_p, inv_dp, n_xs, kp, fp);
   grid_pos<R>(plab_n, inv_dp, n_xs, kn, fn);
   // tabS row {sig_pp, d, sig_np, d}: vs a proton pp if the track is a proton else np; vs a neutron the opposite
   const R *rp = s_tabS + 4 * kp + (t.type ? 0 : 2);
   const R *rn = s_tabS + 4 * kn + (t.type ? 2 : 0);
-  const R Sp = sh.rho_p * (rp[0] + fp * rp[1]);
-  const R Sn = sh.rho_n * (rn[0] + fn * rn[1]);
-  const R Sig = Sp + Sn;
-  const R nlu = -M<R>::log_(u[3]);                  // d_coll = nlu / Sig
-  // geometry: distances to the shell spheres along the flight direction
-  const R ip = M<R>::rsqrt_(p1sq);
-  const R dx = t.px * ip, dy = t.py * ip, dz = t.pz * ip;
-  const R beta = t.x * dx + t.y * dy + t.z * dz;
-  const R r2 = t.x * t.x + t.y * t.y + t.z * t.z;
-  const R bb = beta * beta - r2;
-  R disc_out = bb + sh.r_out * sh.r_out;
-  disc_out = disc_out > R(0) ? disc_out : R(0);
-  const R d_out = -beta + M<R>::sqrt_(disc_out);
-  R d_in = R(1e30);
-  if (t.shell > 0 && beta < R(0)) {
-    const R D = bb + sh.r_in * sh.r_in;
-    if (D > R(0)) d_in = -beta - M<R>::sqrt_(D);
-  }
-  const bool inward = d_in < d_out;
-  const R d_min = inward ? d_in : d_out;
-  if (nlu < Sig * d_min) {
+  const R Sp = m::mul_(sh.rho_p, m::fma_(fp, rp[1], rp[0]));
+  const R Sn = m::mul_(sh.rho_n, m::fma_(fn, rn[1], rn[0]));
+  const R Sig = m::add_(Sp, Sn);
+  const R nlu = -m::log_(u[3]);                  // d_coll = nlu / Sig
+  SegGeom<R> gm;
+  seg_geometry<R>(t, sh, gm);
+  if (nlu < m::mul_(Sig, gm.d_min)) {
     // collision point reached first (d_coll < d_min): hand over to the collision step
-    const R d_coll = M<R>::div_(nlu, Sig);
-    t.x += d_coll * dx; t.y += d_coll * dy; t.z += d_coll * dz;
+    const R d_coll = m::div_(nlu, Sig);
+    t.x = m::fma_(d_coll, gm.dx, t.x); t.y = m::fma_(d_coll, gm.dy, t.y); t.z = m::fma_(d_coll, gm.dz, t.z);
     cc.f = f; cc.nx = nx; cc.ny = ny; cc.nz = nz; cc.Sp = Sp; cc.Sig = Sig;
     return SEG_COLLIDE;
   }
-  // ---------- C4: shell boundary, potential step (P:49 refraction / reflection) ----------
+  // ---------- C4: shell boundary, potential step (same pinned expressions as seg_boundary) ----------
   st.add(S_BND);
-  const int j = inward ? t.shell - 1 : t.shell + 1;
-  const R rb = inward ? sh.r_in : sh.r_out;
-  const R irb = inward ? sh.ir_in : sh.ir_out;
-  R x = t.x + d_min * dx, y = t.y + d_min * dy, z = t.z + d_min * dz;
-  // renormalise onto the sphere: one Newton step of 1/sqrt around |x|^2 = rb^2 (|x| is within rounding of rb)
-  const R corr = R(1.5) - R(0.5) * (x * x + y * y + z * z) * irb * irb;
-  x *= corr; y *= corr; z *= corr;
+  const int j = gm.inward ? t.shell - 1 : t.shell + 1;
+  const R irb = gm.inward ? sh.ir_in : sh.ir_out;
+  R x = m::fma_(gm.d_min, gm.dx, t.x), y = m::fma_(gm.d_min, gm.dy, t.y), z = m::fma_(gm.d_min, gm.dz, t.z);
+  const R rr = m::fma_(z, z, m::fma_(y, y, m::mul_(x, x)));
+  const R corr = m::sub_(R(1.5), m::mul_(m::mul_(m::mul_(R(0.5), rr), irb), irb));
+  x = m::mul_(x, corr); y = m::mul_(y, corr); z = m::mul_(z, corr);
   t.x = x; t.y = y; t.z = z;
-  const R ux = x * irb, uy = y * irb, uz = z * irb;              // outward normal
-  const R pr = t.px * ux + t.py * uy + t.pz * uz;
+  const R ux = m::mul_(x, irb), uy = m::mul_(y, irb), uz = m::mul_(z, irb);              // outward normal
+  const R pr = m::fma_(t.pz, uz, m::fma_(t.py, uy, m::mul_(t.px, ux)));
   const R Vi = t.type ? sh.V_p : sh.V_n;
   const R Vj = t.type ? nu.sh[j].V_p : nu.sh[j].V_n;
-  const R dV = Vj - Vi;
-  const R Tj = t.T + dV;
-  const R prj2 = pr * pr + dV * (t.T + Tj + R(2) * m1);          // p_j^2 - p_t^2
+  const R dV = m::sub_(Vj, Vi);
+  const R Tj = m::add_(t.T, dV);
+  const R prj2 = m::fma_(dV, m::add_(m::add_(t.T, Tj), m::mul_(R(2), m1)), m::mul_(pr, pr));   // p_j^2 - p_t^2
   if (Tj <= R(0) || prj2 <= R(0)) {
     st.add(S_REFL);
-    const R t2 = R(2) * pr;
-    t.px -= t2 * ux; t.py -= t2 * uy; t.pz -= t2 * uz;            // specular reflection
+    const R t2 = m::mul_(R(-2), pr);
+    t.px = m::fma_(t2, ux, t.px); t.py = m::fma_(t2, uy, t.py); t.pz = m::fma_(t2, uz, t.pz);   // specular reflection
     return SEG_CONT;
   }
-  const R sq = M<R>::sqrt_(prj2);
-  const R dp = (pr >= R(0) ? sq : -sq) - pr;
-  t.px += dp * ux; t.py += dp * uy; t.pz += dp * uz;
+  const R sq = m::sqrt_(prj2);
+  const R dp = m::sub_(pr >= R(0) ? sq : -sq, pr);
+  t.px = m::fma_(dp, ux, t.px); t.py = m::fma_(dp, uy, t.py); t.pz = m::fma_(dp, uz, t.pz);
   t.T = Tj;
   t.shell = j;
   if (j == nu.ns) {                                               // escape ("exiting particles")
     st.add(S_ESC);
-    const R ipj = M<R>::rsqrt_(Tj * (Tj + R(2) * m1));
-    esc.T = Tj; esc.ux = t.px * ipj; esc.uy = t.py * ipj; esc.uz = t.pz * ipj;
+    const R ipj = m::rsqrt_(m::mul_(Tj, m::fma_(R(2), m1, Tj)));
+    esc.T = Tj; esc.ux = m::mul_(t.px, ipj); esc.uy = m::mul_(t.py, ipj); esc.uz = m::mul_(t.pz, ipj);
     return SEG_ESCAPE;
   }
   return SEG_CONT;
@@ -521,6 +604,7 @@ template <typename R> struct CascadeParams {
   uint32_t seed_lo, seed_hi;
   uint32_t flags;
   int vote_coll, vote_epi;  // lane kernel: phase-vote thresholds
+  int long_seg;             // wavefront kernel: tracks with this many segments behind them may go to a drain helper
   int n_stage;              // nuclei slots staged into shared memory (target_id must be < n_stage)
 };
 
@@ -758,6 +842,35 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
 // Cascade kernel B (default): per-warp wavefront with shared-memory queues
 // =================================================================================================
 
+// ---- drain helpers ---------------------------------------------------------------------------------
+// A track that orbits in the outer shells (nearly tangential, reflected at every surface hit, short chords,
+// hardly any collision) runs up to kMaxSeg = 1024 segments, one per pass of its warp; the last such tracks of a
+// launch kept single lanes busy for ~0.5 ms while the rest of the GPU idled.  Between collisions the path is
+// deterministic, so a warp that has finished its own events (a "helper") takes such a track over: every lane
+// walks the collision-free path (seg_geometry + seg_boundary only) and lane j keeps the state at the start of
+// segment j; then the 32 lanes run seg_step on their segments in parallel.  If all 32 simply continue, the track
+// has advanced 32 segments in one pass; otherwise the state at the start of the first segment that does not
+// continue (collision, escape, cap) goes back to the owner, which runs that segment in the ordinary way.  The
+// owner's bookkeeping is never touched by a helper.  seg_step is written in pinned arithmetic, so the helper's
+// path is bit-identical to the owner's: results do not depend on whether, or when, a track was helped.
+constexpr int kCtaLongQ = 32;      // hand-over queue owners -> helpers (per CTA)
+constexpr int kRetQ = 8;           // returns helpers -> owner (per warp) = max tracks an owner has out at a time
+constexpr int kLongSegDefault = 128;
+
+template <typename R> struct CtaLong {
+  int credits;              // free entries of q (producers reserve with atomicSub, consumers give back)
+  int avail;                // published, not yet taken entries
+  uint32_t tail, head;      // producer / consumer tickets
+  uint32_t n_helpers;       // warps that have finished their own events
+  uint32_t lock;            // consumers take entries one at a time, in ticket order: the ring frees in order, so a
+                            // producer that holds a credit always finds the entry of its ticket free
+  int idle;                 // helpers waiting for an entry: owners hand a track over only to a helper that is free
+  uint32_t pad;
+  uint32_t valid[kCtaLongQ];
+  R q[7][kCtaLongQ];        // x y z px py pz T
+  uint32_t qi[5][kCtaLongQ];   // pi, k | nseg << 16, meta (type | shell << 1 | slot << 8), event, attempt | tgt << 8 | owner << 16
+};
+
 template <typename R, int NS, int QS, int QC> struct WarpMem {
   // event slots (32 B each in the f32 build)
   int32_t ev[NS];
@@ -774,6 +887,11 @@ template <typename R, int NS, int QS, int QC> struct WarpMem {
   R cf[QC], cnx[QC], cny[QC], cnz[QC], cSp[QC], cSig[QC];
   // slot lists
   uint8_t epi_q[NS], free_q[NS];
+  // tracks coming back from the drain helpers
+  uint32_t r_tail;
+  uint32_t r_valid[kRetQ];
+  R rq[7][kRetQ];
+  uint32_t rqi[3][kRetQ];
 };
 
 template <typename R> struct WaveCfg;
@@ -782,7 +900,98 @@ template <> struct WaveCfg<double> { static constexpr int NS = 64, QS = 128, QC 
 
 template <typename R> __host__ __device__ inline size_t wave_smem_bytes(int n_xs, int n_stage) {
   typedef WaveCfg<R> C;
-  return model_smem_bytes<R>(n_xs, n_stage) + 16 + sizeof(WarpMem<R, C::NS, C::QS, C::QC>) * C::WARPS;
+  return model_smem_bytes<R>(n_xs, n_stage) + 32 + sizeof(CtaLong<R>) + sizeof(WarpMem<R, C::NS, C::QS, C::QC>) * C::WARPS;
+}
+
+// One warp, done with its own events, serves the CTA's hand-over queue until every warp of the CTA is done.
+template <typename R, typename WM>
+__device__ __forceinline__ void help_long_tracks(const CascadeParams<R> &P, const NucDev<R> *s_nuc, const R *s_tabS, WM *wm,
+                                              CtaLong<R> &cq, int n_warps) {
+  const int lane = threadIdx.x & 31;
+  const bool same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
+  LaneStats<false> st;      // the STATS build never hands tracks over (its counters would see the speculative lanes)
+  bool idle = false;
+  for (;;) {
+    // ---- take an entry (under the CTA's consumer lock) ----
+    int h = -1;
+    if (lane == 0) {
+      if (atomicSub(&cq.avail, 1) > 0) {
+        while (atomicCAS(&cq.lock, 0u, 1u) != 0u) { }
+        h = (int)(*(volatile uint32_t *)&cq.head & (kCtaLongQ - 1));
+        while (((volatile uint32_t *)cq.valid)[h] == 0u) { }      // its producer is just publishing it
+      } else {
+        atomicAdd(&cq.avail, 1);
+      }
+    }
+    h = __shfl_sync(kFull, h, 0);
+    if (h < 0) {
+      if (*(volatile uint32_t *)&cq.n_helpers == (uint32_t)n_warps) break;     // nobody has a track out any more
+      if (!idle) { idle = true; if (lane == 0) atomicAdd(&cq.idle, 1); }
+      __nanosleep(64);
+      continue;
+    }
+    if (idle) { idle = false; if (lane == 0) atomicSub(&cq.idle, 1); }
+    __threadfence_block();
+    Track<R> cur;
+    cur.x = cq.q[0][h]; cur.y = cq.q[1][h]; cur.z = cq.q[2][h]; cur.px = cq.q[3][h]; cur.py = cq.q[4][h]; cur.pz = cq.q[5][h];
+    cur.T = cq.q[6][h]; cur.pi = cq.qi[0][h];
+    const uint32_t kn = cq.qi[1][h], mt = cq.qi[2][h], ev = cq.qi[3][h], ao = cq.qi[4][h];
+    cur.k = kn & 0xFFFFu; cur.nseg = (int)(kn >> 16);
+    cur.type = mt & 1u; cur.shell = (int)((mt >> 1) & 0x7Fu);
+    __syncwarp();
+    if (lane == 0) {
+      ((volatile uint32_t *)cq.valid)[h] = 0u;
+      *(volatile uint32_t *)&cq.head = *(volatile uint32_t *)&cq.head + 1u;
+      __threadfence_block();
+      atomicAdd(&cq.credits, 1);
+      atomicExch(&cq.lock, 0u);
+    }
+    const uint32_t attempt = ao & 0xFFu;
+    const NucDev<R> &nu = s_nuc[(ao >> 8) & 0xFFu];
+    RngKey g;
+    const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + (long long)ev);
+    g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
+    // ---- advance it up to 32 segments per pass while every segment just continues (8 in the first pass: a
+    // track that has only just become long often collides within a few segments) ----
+    int depth = 8;
+    for (;;) {
+      Track<R> mine = cur;
+      int n_look = depth;
+#pragma unroll 1
+      for (int j = 0; j < depth; ++j) {
+        if (j == lane) mine = cur;
+        if (cur.nseg >= kMaxSeg) { n_look = j + 1; break; }       // segment j ends at the cap
+        cur.nseg++; cur.k++;
+        const ShellDev<R> &sh = nu.sh[cur.shell];
+        SegGeom<R> gm;
+        Escape<R> e;
+        seg_geometry<R>(cur, sh, gm);
+        if (seg_boundary<R>(cur, nu, sh, gm, e) == SEG_ESCAPE) { n_look = j + 1; break; }   // segment j ends outside
+      }
+      int out = -1;
+      if (lane < n_look) {
+        Track<R> post = mine;
+        CollCarry<R> cc;
+        Escape<R> esc;
+        out = seg_step<R, false>(post, nu, s_tabS, P.model.n_xs, P.model.inv_dp, g, attempt, cc, esc, st);
+      }
+      const unsigned ended = __ballot_sync(kFull, out > SEG_CONT);
+      if (ended == 0u && n_look == depth) { depth = 32; continue; }     // cur = the state after `depth` continuing segments
+      // the start of the first segment that does not continue goes back to the owner (were the walk and seg_step
+      // ever to disagree about an escape or the cap, the start of the last walked segment does)
+      const int f = ended ? __ffs(ended) - 1 : n_look - 1;
+      if (lane == f) {
+        WM &o = wm[ao >> 16];
+        const int i = (int)(atomicAdd(&o.r_tail, 1u) & (kRetQ - 1));
+        o.rq[0][i] = mine.x; o.rq[1][i] = mine.y; o.rq[2][i] = mine.z; o.rq[3][i] = mine.px; o.rq[4][i] = mine.py; o.rq[5][i] = mine.pz;
+        o.rq[6][i] = mine.T; o.rqi[0][i] = mine.pi; o.rqi[1][i] = mine.k | ((uint32_t)mine.nseg << 16);
+        o.rqi[2][i] = (uint32_t)mine.type | ((uint32_t)mine.shell << 1) | (mt & 0xFFFFFF00u);
+        __threadfence_block();
+        ((volatile uint32_t *)o.r_valid)[i] = 1u;
+      }
+      break;
+    }
+  }
 }
 
 template <typename R, bool STATS>
@@ -793,10 +1002,16 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   NucDev<R> *s_nuc = reinterpret_cast<NucDev<R> *>(smem_raw);
   R *s_tabS = reinterpret_cast<R *>(smem_raw + sizeof(NucDev<R>) * P.n_stage);
   const size_t off = (model_smem_bytes<R>(P.model.n_xs, P.n_stage) + 15) & ~(size_t)15;
-  WM &w = reinterpret_cast<WM *>(smem_raw + off)[threadIdx.x >> 5];
-  stage_model<R>(P.model, P.n_stage, s_nuc, s_tabS);
-
+  CtaLong<R> &cq = *reinterpret_cast<CtaLong<R> *>(smem_raw + off);
+  WM *wm = reinterpret_cast<WM *>(smem_raw + off + ((sizeof(CtaLong<R>) + 15) & ~(size_t)15));
+  WM &w = wm[threadIdx.x >> 5];
   const int lane = threadIdx.x & 31;
+  if (lane < kRetQ) w.r_valid[lane] = 0u;
+  if (lane == 0) w.r_tail = 0u;
+  if (threadIdx.x < kCtaLongQ) cq.valid[threadIdx.x] = 0u;
+  if (threadIdx.x == 0) { cq.credits = kCtaLongQ; cq.avail = 0; cq.tail = 0u; cq.head = 0u; cq.n_helpers = 0u; cq.lock = 0u; cq.idle = 0; }
+  stage_model<R>(P.model, P.n_stage, s_nuc, s_tabS);      // ends with __syncthreads()
+
   const unsigned lt = (1u << lane) - 1u;
   const int n_xs = P.model.n_xs;
   const R inv_dp = P.model.inv_dp;
@@ -808,8 +1023,16 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   // warp-uniform queue sizes (every queue operation is warp-collective, so all lanes agree)
   int nSeg = 0, nColl = 0, nEpi = 0, nFree = C::NS;
   bool exhausted = false;
+  // drain helpers: a track with long_seg segments behind it is handed to a warp that has finished its own events
+  // (if there is one).  The STATS build keeps every track (a helper's speculative lanes would be counted).
+  const bool helpers_on = !STATS && (P.flags & INC_F_NO_DRAIN_HELPERS) == 0;
+  const int long_seg = helpers_on ? P.long_seg : (1 << 30);
+  int n_out = 0;              // tracks of ours that are with helpers
+  uint32_t r_head = 0u;       // returns consumed
   for (int i = lane; i < C::NS; i += 32) { w.free_q[i] = (uint8_t)i; w.ev[i] = -1; }
   __syncwarp();
+  const bool timeline = (P.flags & INC_F_TIMING) != 0;
+  if (timeline && lane == 0) { atomicMax(&P.ctr->tl[0], ~global_ns()); atomicAdd(&P.ctr->tl[4], 1ull); }
 
   auto load_key = [&](int slot, RngKey &g, uint32_t &attempt, int &tgt, int &ev) {
     ev = w.ev[slot];
@@ -843,8 +1066,32 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   bool rhas = false;
   int nRes = 0;   // warp-uniform count of resident tracks
 
-  for (;;) {
+  // One pass of the warp (returns true when the warp has nothing left to do).  Two instances: the steady state,
+  // and the drain phase (after the event counter has run out for this warp), which alone carries the hand-over
+  // of long tracks to drain helpers -- so that code costs the steady-state loop nothing (registers, uniform
+  // registers, instructions).
+  auto pass = [&](auto drain_tag) -> bool {
+    constexpr bool DRAIN = decltype(drain_tag)::value;
     __syncwarp();
+    if (DRAIN && n_out > 0) {
+      // ---- a track back from a helper: it continues here, at the segment that ends its collision-free run ----
+      const int i = (int)(r_head & (kRetQ - 1));
+      // (votes make the loaded flags warp-uniform for the compiler as well)
+      const bool back = __ballot_sync(kFull, ((volatile uint32_t *)w.r_valid)[i] != 0u) == kFull;
+      if (back && nSeg + nRes < C::QS) {
+        __threadfence_block();
+        Track<R> t;
+        t.x = w.rq[0][i]; t.y = w.rq[1][i]; t.z = w.rq[2][i]; t.px = w.rq[3][i]; t.py = w.rq[4][i]; t.pz = w.rq[5][i];
+        t.T = w.rq[6][i]; t.pi = w.rqi[0][i];
+        const uint32_t kn = w.rqi[1][i], mt = w.rqi[2][i];
+        t.k = kn & 0xFFFFu; t.nseg = (int)(kn >> 16);
+        t.type = mt & 1u; t.shell = (int)((mt >> 1) & 0x7Fu);
+        __syncwarp();
+        if (lane == 0) ((volatile uint32_t *)w.r_valid)[i] = 0u;
+        push_seg(lane == 0, t, (int)(mt >> 8));
+        r_head++; n_out--;
+      }
+    }
     // ---- choose the kind of step of this pass (warp-uniform) ----
     const int nSegT = nSeg + nRes;
     const int availE = nEpi + (exhausted ? 0 : nFree);
@@ -857,10 +1104,13 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       if (availE > 0 && availE >= nSegT && availE >= nColl) phase = ST_EPI;
       else if (nColl > 0 && nColl >= nSegT) phase = ST_COLL;
       else if (nSegT > 0) phase = ST_SEG;
-      else break;
+      else if (DRAIN && n_out > 0) { __nanosleep(100); return false; }      // our last tracks are with helpers
+      else return true;
     }
-    // capacity guards: a collision pass can add 2 tracks per item, an entry pass 1 track per item
-    if (phase == ST_COLL && nSegT + 2 * (nColl < 32 ? nColl : 32) > C::QS) phase = ST_SEG;
+    // capacity guards: a collision pass can add 2 tracks per item, an entry pass 1 track per item.  While a full
+    // collision pass does not fit, segment passes make room first -- unless the collision queue could then
+    // overflow (a segment pass adds up to one item per lane): then a partial collision pass runs.
+    if (phase == ST_COLL && nSegT + 2 * (nColl < 32 ? nColl : 32) > C::QS && nColl <= C::QC - 32) phase = ST_SEG;
     if (phase == ST_EPI && nSegT + nColl > 64) phase = nSegT > 0 ? ST_SEG : ST_COLL;   // admission control
 
     if (phase == ST_SEG) {
@@ -894,6 +1144,36 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
         const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + rev);
         g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
         out = seg_step<R, STATS>(rt, s_nuc[rtgt], s_tabS, n_xs, inv_dp, g, rattempt, cc, esc, st);
+      }
+      {
+        // long tracks go to a helper, if there is one and its queue and our return queue have room
+        const bool wl = DRAIN && rhas && out == SEG_CONT && rt.nseg >= long_seg;
+        const unsigned ml = __ballot_sync(kFull, wl);
+        if (ml) {
+          bool moved = false;
+          // only to helpers that are free right now: a track never waits in the queue behind another one
+          const int free_helpers = *(volatile int *)&cq.idle - *(volatile int *)&cq.avail;
+          const int room = free_helpers < kRetQ - n_out ? free_helpers : kRetQ - n_out;
+          if (wl && __popc(ml & lt) < room) {
+            if (atomicSub(&cq.credits, 1) > 0) {
+              const int i = (int)(atomicAdd(&cq.tail, 1u) & (kCtaLongQ - 1));
+              cq.q[0][i] = rt.x; cq.q[1][i] = rt.y; cq.q[2][i] = rt.z; cq.q[3][i] = rt.px; cq.q[4][i] = rt.py; cq.q[5][i] = rt.pz;
+              cq.q[6][i] = rt.T; cq.qi[0][i] = rt.pi; cq.qi[1][i] = rt.k | ((uint32_t)rt.nseg << 16);
+              cq.qi[2][i] = (uint32_t)rt.type | ((uint32_t)rt.shell << 1) | ((uint32_t)rslot << 8);
+              cq.qi[3][i] = (uint32_t)rev;
+              cq.qi[4][i] = rattempt | ((uint32_t)rtgt << 8) | ((uint32_t)(threadIdx.x >> 5) << 16);
+              __threadfence_block();
+              ((volatile uint32_t *)cq.valid)[i] = 1u;
+              atomicAdd(&cq.avail, 1);
+              moved = true;
+            } else {
+              atomicAdd(&cq.credits, 1);
+            }
+          }
+          const unsigned mm = __ballot_sync(kFull, moved);
+          if (moved) rhas = false;
+          nRes -= __popc(mm); n_out += __popc(mm);
+        }
       }
       const unsigned left = __ballot_sync(kFull, out > SEG_CONT);     // tracks that leave the segment state
       if (left) {
@@ -936,7 +1216,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
         if (out > SEG_CONT) rhas = false;
         nRes -= __popc(left);
       }
-      continue;
+      return false;
     }
 
     // any other pass: park the resident tracks in the segment queue first
@@ -950,7 +1230,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       if (2 * m > C::QS - nSeg) m = (C::QS - nSeg) / 2;
       if (m <= 0) {   // both queues full: implementation limit exceeded -> fail loudly, never hang
         if (lane == 0) atomicOr(&P.ctr->error_word, 4u);
-        break;
+        return true;
       }
       if (lane == 0) { st.add(S_WI_COLL); st.add(S_LS_COLL, m); }
       const bool has = lane < m;
@@ -988,7 +1268,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       push_seg(has && keep1, t, slot);
       push_seg(has && allowed && keep2, c2, slot);
       push_epi(finished, slot);
-      continue;
+      return false;
     }
 
     // ---------- EPI pass: epilogue of finished attempts, event fetch, entry ----------
@@ -1054,7 +1334,9 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
           }
         }
       }
-      if (__ballot_sync(kFull, got_none)) exhausted = true;
+      const bool ran_out = __ballot_sync(kFull, got_none) != 0u;
+      if (timeline && ran_out && !exhausted && lane == 0) atomicAdd(&P.ctr->tl[1], global_ns());
+      if (ran_out) exhausted = true;
       // slots that did not get work go back to the free list
       {
         const bool fr = has && !do_entry;
@@ -1076,8 +1358,20 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       }
       push_seg(do_entry, t, slot);
     }
+    return false;
+  };
+  bool done = false;
+  while (!exhausted && !done) done = pass(std::false_type());
+  while (!done) done = pass(std::true_type());
+  if (timeline && lane == 0) {
+    const unsigned long long t = global_ns();
+    atomicAdd(&P.ctr->tl[2], t); atomicMax(&P.ctr->tl[3], t); atomicMax(&P.ctr->tl[5], ~t);
   }
   st.flush(P.ctr, lane);
+  if (helpers_on) {
+    if (lane == 0) { __threadfence_block(); atomicAdd(&cq.n_helpers, 1u); }
+    help_long_tracks<R, WM>(P, s_nuc, s_tabS, wm, cq, C::WARPS);
+  }
 }
 
 // =================================================================================================

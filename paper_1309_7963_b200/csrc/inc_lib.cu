@@ -73,6 +73,7 @@ struct State {
   int stage_launches[4] = {0, 0, 0, 0};
   std::vector<cudaEvent_t> pending_events;   // 5 per chunk, resolved after the stream sync
   int vote_coll = 8, vote_epi = 8;
+  int long_seg = kLongSegDefault;
   int sm_count = 0;
   std::string err;
 };
@@ -384,6 +385,7 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   cp.flags = g.flags;
   const bool naive = (g.flags & INC_F_LANE_PER_EVENT) != 0;
   cp.vote_coll = naive ? 1 : g.vote_coll; cp.vote_epi = naive ? 1 : g.vote_epi;
+  cp.long_seg = g.long_seg;
   int n_stage = 0;
   for (int i = 0; i < INC_MAX_TARGETS; ++i) if (g.nuc[i].live) n_stage = i + 1;
   cp.n_stage = n_stage;
@@ -619,6 +621,21 @@ int inc_get_stats(inc_stats *out) {
   return 0;
 }
 
+int inc_get_drain_timeline(double ms[4]) {
+  if (!ms) return fail(INC_E_BADARG, "null pointer");
+  if (g.last_n < 0) return fail(INC_E_STATE, "no previous inc_simulate");
+  DevCounters c;
+  CU_TRY(cudaMemcpy(&c, g.d_ctr, sizeof(c), cudaMemcpyDeviceToHost));
+  ms[0] = ms[1] = ms[2] = ms[3] = 0;
+  if (c.tl[4] == 0) return 0;
+  const double t0 = (double)(~c.tl[0]), nw = (double)c.tl[4];
+  ms[0] = ((double)c.tl[1] / nw - t0) * 1e-6;
+  ms[1] = ((double)c.tl[2] / nw - t0) * 1e-6;
+  ms[2] = ((double)c.tl[3] - t0) * 1e-6;
+  ms[3] = ((double)(~c.tl[5]) - t0) * 1e-6;
+  return 0;
+}
+
 int inc_get_stage_times(float ms[4], int32_t launches[4]) {
   if (g.last_n < 0) return fail(INC_E_STATE, "no previous inc_simulate");
   for (int i = 0; i < 4; ++i) { if (ms) ms[i] = g.stage_ms[i]; if (launches) launches[i] = g.stage_launches[i]; }
@@ -641,6 +658,12 @@ int inc_get_nucleus(int id, int32_t *A, int32_t *Z, int32_t *ns, double *R, doub
 int inc_set_vote_thresholds(int coll, int epi) {
   if (coll < 1 || coll > 32 || epi < 1 || epi > 32) return fail(INC_E_BADARG, "thresholds must be 1..32");
   g.vote_coll = coll; g.vote_epi = epi;
+  return 0;
+}
+
+int inc_set_long_track_threshold(int n_segments) {
+  if (n_segments < 0) return fail(INC_E_BADARG, "threshold must be >= 0");
+  g.long_seg = n_segments == 0 ? kLongSegDefault : n_segments;
   return 0;
 }
 

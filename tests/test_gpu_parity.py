@@ -149,6 +149,32 @@ def test_fp64_cascade_only_and_flags(gpu, orc, otables, ptables):
         assert abs(st["stats"][k] - os_[k]) <= max(2, 1e-3 * os_[k]), (k, st["stats"][k], os_[k])
 
 
+@pytest.mark.parametrize("variant", ["f64", "f32"])
+@pytest.mark.parametrize("cfg,n", [(1, 6000), (4, 300000), (5, 4000)])
+def test_drain_helpers_change_nothing(gpu, orc, otables, ptables, variant, cfg, n):
+    """Drain helpers: a warp that has finished its own events advances long tracks of
+    other warps 32 segments per pass along their collision-free path.  With the threshold at 2 segments
+    almost every track of the drain phase goes through a helper; the outputs must be bit-identical to the
+    default threshold and to helpers switched off, in both builds (pinned arithmetic), and the fp64
+    build must still equal the oracle."""
+    E, tid, targets, seed, _ = _inputs(cfg, n)
+    lib = gpu.load(variant)
+    runs = []
+    try:
+        for thr, flags in ((2, 0), (0, 0), (0, gpu.F_NO_DRAIN_HELPERS), (16, 0)):
+            lib.inc_set_long_track_threshold(thr)
+            runs.append(gpu.simulate(lib, targets, E, tid, seed, ptables, flags=flags))
+    finally:
+        lib.inc_set_long_track_threshold(0)
+    for other in runs[1:]:
+        for k in ("species", "T", "ux", "uy", "uz", "counts", "A", "Z", "Estar", "px", "py", "pz", "status", "offsets"):
+            assert np.array_equal(runs[0][k], other[k]), k
+    if variant == "f64" and n <= 10000:
+        o = orc.simulate(otables, targets, E, tid, seed)
+        frac, max_err, _ = H.event_identity(runs[0], o, rel=REL_F64)
+        assert frac >= FRAC_IDENTICAL and max_err <= REL_F64
+
+
 def test_fp64_transparent_and_failed(gpu, orc, ptables):
     """sigma = 0: KEEP_TRANSPARENT reproduces the oracle's refracted traversal (closed-form
     pinned there); without the flag every event is FAILED with count 0."""
