@@ -115,7 +115,7 @@ int inc_set_vote_thresholds(int coll, int epi);
 /* Scheduling knob of the default (wavefront) cascade kernel: a track that has run `n_segments`
  * segments may be handed to a warp that has finished its own events, which evaluates 32 consecutive
  * segments of the one track per pass along its collision-free path (drain helpers, DESIGN.md
- * section 6).  0 restores the default (128).  Results never depend on it. */
+ * section 6).  0 restores the default (48).  Results never depend on it. */
 int inc_set_long_track_threshold(int n_segments);
 /* Global index of the first event of the following inc_simulate calls (default 0): event i of a
  * call uses the random stream of global event e = offset + i.  This is how a job is sharded over

@@ -855,7 +855,7 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
 // path is bit-identical to the owner's: results do not depend on whether, or when, a track was helped.
 constexpr int kCtaLongQ = 32;      // hand-over queue owners -> helpers (per CTA)
 constexpr int kRetQ = 8;           // returns helpers -> owner (per warp) = max tracks an owner has out at a time
-constexpr int kLongSegDefault = 128;
+constexpr int kLongSegDefault = 48;
 
 template <typename R> struct CtaLong {
   int credits;              // free entries of q (producers reserve with atomicSub, consumers give back)
@@ -1147,7 +1147,9 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       }
       {
         // long tracks go to a helper, if there is one and its queue and our return queue have room
-        const bool wl = DRAIN && rhas && out == SEG_CONT && rt.nseg >= long_seg;
+        // ... and only tracks that have hardly collided so far (k - nseg = collisions <= nseg / 16): those are the
+        // orbits whose collision-free runs are long enough for a helper to pay off
+        const bool wl = DRAIN && rhas && out == SEG_CONT && rt.nseg >= long_seg && ((int)rt.k - rt.nseg) * 16 <= rt.nseg;
         const unsigned ml = __ballot_sync(kFull, wl);
         if (ml) {
           bool moved = false;
