@@ -83,14 +83,29 @@ template <typename R> struct ModelDev {
   R a_div;                // level density a = A_d / a_div
 };
 
+// One staged secondary.  f32: 32 bytes = one DRAM sector, so an event with n secondaries touches n sectors when it
+// is written (cascade escapes, evaporation emissions) and when the compaction kernel reads it back; the earlier
+// layout (five [chunk][64] arrays) touched 5-10 sectors per event and made the compaction the one HBM-bound kernel.
+template <typename R> struct __align__(16) StageRec {
+  R T, ux, uy, uz;
+  uint32_t code;          // path code | type << 24 ; evaporation: 1 << 31 | species << 24 | sequence number
+  uint32_t pad[3];
+};
+
 template <typename R> struct Workspace {   // per-chunk internal buffers (DEVICE)
-  uint32_t *st_code;      // [chunk][kMaxSec]  path code | type << 24 ; evap: 1<<31 | species<<24 | seq
-  R *st_T, *st_ux, *st_uy, *st_uz;
+  StageRec<R> *st;        // [chunk][kMaxSec] staged secondaries, one record per secondary
   int32_t *cA, *cZ;       // post-cascade nucleus ("SoA of excited nuclei")
   R *cE, *cPx, *cPy, *cPz;
   uint32_t *cmeta;        // n_casc | attempt << 8 | failed << 16
   uint32_t *cstatus;
 };
+
+template <typename R>
+__device__ __forceinline__ void stage_write(StageRec<R> *dst, R T, R ux, R uy, R uz, uint32_t code) {
+  StageRec<R> r;
+  r.T = T; r.ux = ux; r.uy = uy; r.uz = uz; r.code = code; r.pad[0] = 0u; r.pad[1] = 0u; r.pad[2] = 0u;
+  *dst = r;               // 16-byte vector stores
+}
 
 struct DevCounters {       // device scalars
   unsigned long long next_event_casc, next_event_evap;
@@ -740,8 +755,7 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
         else if (out == SEG_ESCAPE) {
           if (n_esc < kMaxSec) {
             const size_t o = (size_t)ev * kMaxSec + n_esc;
-            P.ws.st_code[o] = t.pi | ((uint32_t)t.type << 24);
-            P.ws.st_T[o] = esc.T; P.ws.st_ux[o] = esc.ux; P.ws.st_uy[o] = esc.uy; P.ws.st_uz[o] = esc.uz;
+            stage_write<R>(P.ws.st + o, esc.T, esc.ux, esc.uy, esc.uz, t.pi | ((uint32_t)t.type << 24));
             n_esc++; n_p += t.type;
             fxE -= Fx<R>::to(esc.T); fxX -= Fx<R>::to(t.px); fxY -= Fx<R>::to(t.py); fxZ -= Fx<R>::to(t.pz);
           } else {
@@ -1198,8 +1212,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
             const int idx = (int)(old & 0xFFu);
             if (idx < kMaxSec) {
               const size_t o = (size_t)rev * kMaxSec + idx;
-              P.ws.st_code[o] = rt.pi | ((uint32_t)rt.type << 24);
-              P.ws.st_T[o] = esc.T; P.ws.st_ux[o] = esc.ux; P.ws.st_uy[o] = esc.uy; P.ws.st_uz[o] = esc.uz;
+              stage_write<R>(P.ws.st + o, esc.T, esc.ux, esc.uy, esc.uz, rt.pi | ((uint32_t)rt.type << 24));
               typedef typename Fx<R>::U FU;
               atomicAdd((FU *)&w.acc[0][rslot], (FU)(-Fx<R>::to(esc.T)));
               atomicAdd((FU *)&w.acc[1][rslot], (FU)(-Fx<R>::to(rt.px)));
@@ -1421,7 +1434,7 @@ __device__ __forceinline__ void G13_scaled(R s, R s_ref, R &g1, R &g3) {
 }
 
 template <typename R, bool STATS>
-__global__ void __launch_bounds__(256, 2) evap_kernel(const EvapParams<R> P) {
+__global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const EvapParams<R> P) {
   const int lane = threadIdx.x & 31;
   const bool cascade_only = (P.flags & INC_F_CASCADE_ONLY) != 0;
   const bool same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
@@ -1582,9 +1595,7 @@ __global__ void __launch_bounds__(256, 2) evap_kernel(const EvapParams<R> P) {
             const R Tl = l2 / (El + Mj);
             const R il = M<R>::rsqrt_(l2);
             const size_t o = (size_t)ev * kMaxSec + count;
-            P.ws.st_code[o] = 0x80000000u | ((uint32_t)jsel << 24) | (uint32_t)count;
-            P.ws.st_T[o] = Tl;
-            P.ws.st_ux[o] = lx * il; P.ws.st_uy[o] = ly * il; P.ws.st_uz[o] = lz * il;
+            stage_write<R>(P.ws.st + o, Tl, lx * il, ly * il, lz * il, 0x80000000u | ((uint32_t)jsel << 24) | (uint32_t)count);
             count++;
             if (STATS) n_emit++;
             A = Ad; Z = Zd; Es = Esd;
@@ -1745,7 +1756,9 @@ __global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) 
       const int el = e0 + lo;
       const int j = i - ex_l;
       const size_t sbase = (size_t)el * kMaxSec;
-      const uint32_t code = P.ws.st_code[sbase + j];
+      const StageRec<R> *row = P.ws.st + sbase;
+      const StageRec<R> rec = row[j];
+      const uint32_t code = rec.code;
       int rank = j;
       uint8_t sp;
       if (code & 0x80000000u) {
@@ -1755,15 +1768,12 @@ __global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) 
         const uint32_t key = code & 0xFFFFFFu;
         const int n_casc = (int)(P.ws.cmeta[el] & 0xFFu);
         rank = 0;
-        for (int l = 0; l < n_casc; ++l) rank += ((P.ws.st_code[sbase + l] & 0xFFFFFFu) < key) ? 1 : 0;
+        for (int l = 0; l < n_casc; ++l) rank += ((row[l].code & 0xFFFFFFu) < key) ? 1 : 0;
       }
       const long long dst = off_l + rank;
       if (dst < P.capacity) {
         P.species[dst] = sp;
-        P.T[dst] = P.ws.st_T[sbase + j];
-        P.ux[dst] = P.ws.st_ux[sbase + j];
-        P.uy[dst] = P.ws.st_uy[sbase + j];
-        P.uz[dst] = P.ws.st_uz[sbase + j];
+        P.T[dst] = rec.T; P.ux[dst] = rec.ux; P.uy[dst] = rec.uy; P.uz[dst] = rec.uz;
       }
     }
   }

@@ -323,8 +323,7 @@ ModelDev<real> model_dev() {
 }
 
 void free_ws() {
-  void **p[] = {(void **)&g.ws.st_code, (void **)&g.ws.st_T, (void **)&g.ws.st_ux, (void **)&g.ws.st_uy,
-                (void **)&g.ws.st_uz, (void **)&g.ws.cA, (void **)&g.ws.cZ, (void **)&g.ws.cE, (void **)&g.ws.cPx,
+  void **p[] = {(void **)&g.ws.st, (void **)&g.ws.cA, (void **)&g.ws.cZ, (void **)&g.ws.cE, (void **)&g.ws.cPx,
                 (void **)&g.ws.cPy, (void **)&g.ws.cPz, (void **)&g.ws.cmeta, (void **)&g.ws.cstatus};
   for (auto q : p) { if (*q) cudaFree(*q); *q = nullptr; }
   g.ws_chunk = 0;
@@ -334,11 +333,7 @@ int ensure_ws(size_t chunk, size_t n_total) {
   if (chunk > g.ws_chunk) {
     free_ws();
     const size_t ns = chunk * kMaxSec;
-    CU_TRY(cudaMalloc((void **)&g.ws.st_code, ns * sizeof(uint32_t)));
-    CU_TRY(cudaMalloc((void **)&g.ws.st_T, ns * sizeof(real)));
-    CU_TRY(cudaMalloc((void **)&g.ws.st_ux, ns * sizeof(real)));
-    CU_TRY(cudaMalloc((void **)&g.ws.st_uy, ns * sizeof(real)));
-    CU_TRY(cudaMalloc((void **)&g.ws.st_uz, ns * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&g.ws.st, ns * sizeof(StageRec<real>)));
     CU_TRY(cudaMalloc((void **)&g.ws.cA, chunk * sizeof(int32_t)));
     CU_TRY(cudaMalloc((void **)&g.ws.cZ, chunk * sizeof(int32_t)));
     CU_TRY(cudaMalloc((void **)&g.ws.cE, chunk * sizeof(real)));
