@@ -207,6 +207,19 @@ def main():
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     value = world * n * args.steps / (ms_total * 1e-3)
 
+    # ---- extras (outside the timed region): drain timeline of the last cascade launch, on-device tallies ----
+    timeline = lib.inc_get_drain_timeline()
+    off_d = lib.inc_get_offsets(n)
+    tspec, tall = lib.alloc_tallies()
+    lib.inc_tally(out, off_d, tspec, tall)
+    tev0, tev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    tev0.record()
+    for _ in range(5):
+        lib.inc_tally(out, off_d, tspec, tall)
+    tev1.record()
+    torch.cuda.synchronize()
+    tally_ms = tev0.elapsed_time(tev1) / 5
+
     # ---- end to end through the host-buffer entry point (pinned host memory) ----
     lib.inc_set_flags(args.flags)
     E_h = torch.as_tensor(E.astype(lib.real)).pin_memory()
@@ -269,11 +282,13 @@ def main():
                 dtype=args.variant, data="synthetic",
                 config=dict(workload=f"config {cfg}: {name}", events_per_step_per_gpu=n, seed=seed,
                             secondaries_per_step=int(total), build=lib.build_info(),
-                            l2="no flush: each step rewrites a 1.4 GB staging area and ~0.1 GB of outputs, far above the 126 MB L2",
+                            l2="no flush: each step writes and re-reads ~0.3 GB (staging records, post-cascade records, outputs; new seed every step), above the 126 MB L2",
                             parallelism=f"dp{world} (independent event ranges, no collective)"),
                 clocks=clocks, e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                                         steps=e2e_steps),
                 gpu_launches=int(launches), roofline=roofline, cpu_baseline=cpu_baseline,
+                cascade_drain_timeline_ms=timeline,
+                tally=dict(ms=tally_ms, note="inc_tally over the step's outputs (dd spectra 3x20x51, multiplicities, nuclide chart, yields); not part of the step"),
                 work_counters_per_event={k: stats[k] / max(stats["events"], 1) for k in
                                          ("attempts", "segments", "boundaries", "collisions", "allowed", "evap_steps", "evap_trials")},
                 lane_utilisation=dict(seg=stats["lane_slots_seg"] / max(32 * stats["warp_iters_seg"], 1),

@@ -206,6 +206,41 @@ int inc_measure_issue_peak(double *lane_instr_per_s /*HOST*/, double *sm_clock_m
  * ctr[4*i..] (DEVICE arrays of n blocks), key = (seed lo, seed hi). */
 int inc_philox_blocks(const uint32_t *ctr /*DEVICE [4n]*/, uint64_t seed, uint32_t *out /*DEVICE [4n]*/, int64_t n);
 
+/* ---- on-device tallies --------------------------------------------------
+ * The quantities the paper shows for its results: secondary yields and double-differential
+ * spectra ("double differential yields at 7.5, 30, 60 and 150 degrees", Figs. 1-2)
+ * and the residual nuclides, whose positron emitters are the paper's named application ("very
+ * fast calculation of the yield of positron emitters for range verification").  inc_tally
+ * reduces the outputs of an inc_simulate call on the device, so that a study needs O(bins) instead
+ * of O(events) to come back to the host.  All tallies are unsigned 64-bit counts in DEVICE memory,
+ * caller-owned, and are ACCUMULATED into (the caller zeroes them once and may call inc_tally after
+ * every batch).  Classes: 0 = neutrons, 1 = protons, 2 = composites (d, t, 3He, 4He).
+ *   dd[c][a][t]     c < 3, a < n_cos, t <= n_T : secondaries of class c with
+ *                   a = min(floor((uz + 1) * n_cos / 2), n_cos - 1)   (uz = cos of the polar angle to the beam)
+ *                   t = min(floor(T * n_T / T_max), n_T)               (t = n_T: overflow T >= T_max)
+ *                   both products evaluated in INC_REAL, one rounding each.
+ *   mult[c][m]      c < 4 (3 = all secondaries), m <= mult_max: events with min(multiplicity of class c, mult_max) = m
+ *   nuclide[A][Z]   A <= A_max, Z <= Z_max: events whose final residual is (A, Z); others are not counted
+ *   yield[s][o]     s < 6 species, o = 0 cascade / 1 evaporation (bit 7 of the species byte)
+ * Events are all n_events of the call; offsets = exclusive prefix sum of counts ([n_events + 1], e.g. from
+ * inc_get_offsets).  Returns 0 or INC_E_BADARG (null pointer, n < 0, non-positive bin counts) / INC_E_CUDA. */
+typedef struct inc_tally_spec {
+  int32_t n_T; double T_max;     /* energy bins of width T_max / n_T, MeV, plus one overflow bin */
+  int32_t n_cos;                 /* bins of cos(theta) on [-1, 1]                                */
+  int32_t mult_max;              /* multiplicities are clamped to this                           */
+  int32_t A_max, Z_max;          /* extent of the nuclide chart                                  */
+} inc_tally_spec;
+typedef struct inc_tallies {     /* DEVICE pointers, caller-owned, accumulated                   */
+  unsigned long long *dd;        /* [3][n_cos][n_T + 1]                                          */
+  unsigned long long *mult;      /* [4][mult_max + 1]                                            */
+  unsigned long long *nuclide;   /* [A_max + 1][Z_max + 1]                                       */
+  unsigned long long *yield;     /* [6][2]                                                       */
+} inc_tallies;
+int inc_tally(int64_t n_events, const inc_secondaries *sec /*HOST struct of DEVICE pointers*/,
+              const int32_t *counts /*DEVICE [n]*/, const int64_t *offsets /*DEVICE [n+1]*/,
+              const inc_residual *res /*HOST struct of DEVICE pointers*/, const inc_tally_spec *spec /*HOST*/,
+              const inc_tallies *out /*HOST struct of DEVICE pointers*/);
+
 const char *inc_last_error(void);
 const char *inc_build_info(void);   /* "f32 fast-math sm_100a ..." */
 

@@ -286,3 +286,39 @@ def simulate(tables: Tables, nuclei, E_in, target, seed, e0=0, flags=0, want_sta
                 offsets=offsets, A=rA, Z=rZ, Estar=rE, px=rpx, py=rpy, pz=rpz, status=status,
                 casc_A=cA, casc_Z=cZ, casc_Estar=cE, casc_P=cP, casc_count=cN,
                 stats=st.as_dict() if want_stats else None, total=int(tot))
+
+
+def tally_reference(species, T, uz, counts, A_res, Z_res, n_T=50, T_max=250.0, n_cos=20, mult_max=24,
+                    A_max=72, Z_max=36, real=np.float64):
+    """The tallies of include/inc.h `inc_tally` written out as the
+    plain definition: histograms over the outputs of a simulate call.  Classes 0 = n, 1 = p, 2 = composites.
+    `real` is the precision in which the two bin coordinates are formed (one rounding per operation, as the
+    library does): np.float64 for the parity build and the oracle, np.float32 for the production build."""
+    species = np.asarray(species); counts = np.asarray(counts)
+    code = (species & 0x7).astype(np.int64)
+    origin = (species >> 7).astype(np.int64)
+    cls = np.minimum(code, 2)
+    cos_scale = real(n_cos / 2.0)
+    T_scale = real(n_T / T_max)
+    a = ((np.asarray(uz, dtype=real) + real(1)) * cos_scale).astype(np.int64)      # truncation, like the (int) cast
+    a = np.clip(a, 0, n_cos - 1)
+    tt = np.asarray(T, dtype=real) * T_scale
+    t = np.where(tt >= real(n_T), n_T, tt.astype(np.int64))
+    t = np.maximum(t, 0)
+    dd = np.zeros((3, n_cos, n_T + 1), dtype=np.int64)
+    np.add.at(dd, (cls, a, t), 1)
+    n = len(counts)
+    ev = np.repeat(np.arange(n), counts)
+    mult = np.zeros((4, mult_max + 1), dtype=np.int64)
+    for c in range(3):
+        m = np.bincount(ev[cls == c], minlength=n)
+        mult[c] = np.bincount(np.minimum(m, mult_max), minlength=mult_max + 1)
+    mult[3] = np.bincount(np.minimum(counts, mult_max), minlength=mult_max + 1)
+    nuclide = np.zeros((A_max + 1, Z_max + 1), dtype=np.int64)
+    A_res = np.asarray(A_res); Z_res = np.asarray(Z_res)
+    ok = (A_res >= 0) & (A_res <= A_max) & (Z_res >= 0) & (Z_res <= Z_max)
+    np.add.at(nuclide, (A_res[ok], Z_res[ok]), 1)
+    yields = np.zeros((6, 2), dtype=np.int64)
+    ok6 = code < 6
+    np.add.at(yields, (code[ok6], origin[ok6]), 1)
+    return dict(dd=dd, mult=mult, nuclide=nuclide, yields=yields)

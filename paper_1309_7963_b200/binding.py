@@ -79,7 +79,16 @@ def make_tables_struct(t: dict):
 EXPORTS = ["inc_init", "inc_free_target", "inc_shutdown", "inc_set_stream", "inc_set_flags", "inc_set_event_offset",
            "inc_get_stage_times", "inc_get_drain_timeline", "inc_set_vote_thresholds", "inc_set_long_track_threshold", "inc_simulate",
            "inc_simulate_host", "inc_get_offsets", "inc_get_cascade_stage", "inc_get_stats", "inc_get_nucleus",
-           "inc_measure_issue_peak", "inc_philox_blocks", "inc_last_error", "inc_build_info"]
+           "inc_measure_issue_peak", "inc_philox_blocks", "inc_tally", "inc_last_error", "inc_build_info"]
+
+
+class IncTallySpec(C.Structure):
+    _fields_ = [("n_T", C.c_int32), ("T_max", C.c_double), ("n_cos", C.c_int32), ("mult_max", C.c_int32),
+                ("A_max", C.c_int32), ("Z_max", C.c_int32)]
+
+
+class IncTallies(C.Structure):
+    _fields_ = [("dd", C.c_void_p), ("mult", C.c_void_p), ("nuclide", C.c_void_p), ("yield_", C.c_void_p)]
 
 
 class IncLibrary:
@@ -215,6 +224,22 @@ class IncLibrary:
         rc = self.lib.inc_simulate_host(n, C.c_void_p(E_in.data_ptr()), C.c_void_p(target_id.data_ptr()),
                                         C.c_uint64(int(seed)), C.byref(sec), C.c_void_p(out["counts"].data_ptr()), C.byref(res))
         return self._check(rc) if check else rc
+
+    def alloc_tallies(self, n_T=50, T_max=250.0, n_cos=20, mult_max=24, A_max=72, Z_max=36):
+        """Zeroed caller-owned tally tensors (torch int64 on the device) + the spec, for inc_tally."""
+        import torch
+        spec = IncTallySpec(n_T, T_max, n_cos, mult_max, A_max, Z_max)
+        z = lambda *shape: torch.zeros(shape, dtype=torch.int64, device="cuda")
+        return spec, dict(dd=z(3, n_cos, n_T + 1), mult=z(4, mult_max + 1), nuclide=z(A_max + 1, Z_max + 1), yields=z(6, 2))
+
+    def inc_tally(self, out: dict, offsets, spec, tallies: dict, n=None):
+        """Accumulates the tallies of the outputs `out` (alloc_outputs, filled by inc_simulate) into `tallies`."""
+        n = out["counts"].numel() if n is None else n
+        sec, res = self._structs(out)
+        t = IncTallies(tallies["dd"].data_ptr(), tallies["mult"].data_ptr(), tallies["nuclide"].data_ptr(), tallies["yields"].data_ptr())
+        rc = self.lib.inc_tally(C.c_int64(n), C.byref(sec), C.c_void_p(out["counts"].data_ptr()), C.c_void_p(offsets.data_ptr()),
+                                C.byref(res), C.byref(spec), C.byref(t))
+        return self._check(rc)
 
     def inc_get_offsets(self, n: int):
         import torch

@@ -1109,23 +1109,24 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
     // ---- choose the kind of step of this pass (warp-uniform) ----
     const int nSegT = nSeg + nRes;
     const int availE = nEpi + (exhausted ? 0 : nFree);
-    int phase;
-    if (nColl >= 32) phase = ST_COLL;
-    else if (nSegT >= 32) phase = ST_SEG;
-    else if (availE >= 32) phase = ST_EPI;
-    else {
-      // nothing fills a whole pass: take the fullest queue (ties: entry first, it creates work)
-      if (availE > 0 && availE >= nSegT && availE >= nColl) phase = ST_EPI;
-      else if (nColl > 0 && nColl >= nSegT) phase = ST_COLL;
-      else if (nSegT > 0) phase = ST_SEG;
-      else if (DRAIN && n_out > 0) { __nanosleep(100); return false; }      // our last tracks are with helpers
-      else return true;
+    int phase = ST_SEG;
+    if (!(nColl < 32 && nSegT >= 32)) {        // (the common case needs none of what follows)
+      if (nColl >= 32) phase = ST_COLL;
+      else if (availE >= 32) phase = ST_EPI;
+      else {
+        // nothing fills a whole pass: take the fullest queue (ties: entry first, it creates work)
+        if (availE > 0 && availE >= nSegT && availE >= nColl) phase = ST_EPI;
+        else if (nColl > 0 && nColl >= nSegT) phase = ST_COLL;
+        else if (nSegT > 0) phase = ST_SEG;
+        else if (DRAIN && n_out > 0) { __nanosleep(100); return false; }      // our last tracks are with helpers
+        else return true;
+      }
+      // capacity guards: a collision pass can add 2 tracks per item, an entry pass 1 track per item.  While a full
+      // collision pass does not fit, segment passes make room first -- unless the collision queue could then
+      // overflow (a segment pass adds up to one item per lane): then a partial collision pass runs.
+      if (phase == ST_COLL && nSegT + 2 * (nColl < 32 ? nColl : 32) > C::QS && nColl <= C::QC - 32) phase = ST_SEG;
+      if (phase == ST_EPI && nSegT + nColl > 64) phase = nSegT > 0 ? ST_SEG : ST_COLL;   // admission control
     }
-    // capacity guards: a collision pass can add 2 tracks per item, an entry pass 1 track per item.  While a full
-    // collision pass does not fit, segment passes make room first -- unless the collision queue could then
-    // overflow (a segment pass adds up to one item per lane): then a partial collision pass runs.
-    if (phase == ST_COLL && nSegT + 2 * (nColl < 32 ? nColl : 32) > C::QS && nColl <= C::QC - 32) phase = ST_SEG;
-    if (phase == ST_EPI && nSegT + nColl > 64) phase = nSegT > 0 ? ST_SEG : ST_COLL;   // admission control
 
     if (phase == ST_SEG) {
       // refill lanes without a resident track from the top of the segment queue
@@ -1774,6 +1775,78 @@ __global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) 
       if (dst < P.capacity) {
         P.species[dst] = sp;
         P.T[dst] = rec.T; P.ux[dst] = rec.ux; P.uy[dst] = rec.uy; P.uz[dst] = rec.uz;
+      }
+    }
+  }
+}
+
+// =================================================================================================
+// On-device tallies (inc_tally): double-differential spectra per
+// class, multiplicities, residual nuclide chart, yields.  One thread per event (grid-stride); each block
+// histograms into 32-bit shared-memory bins and adds its non-zero bins to the caller's 64-bit tallies at the end
+// (smem = 0: straight to the global tallies, for bin counts that do not fit in shared memory).
+// =================================================================================================
+template <typename R> struct TallyParams {
+  const uint8_t *species; const R *T, *uz;
+  const int32_t *counts; const long long *offsets;
+  const int32_t *rA, *rZ;
+  long long n_events;
+  int n_T, n_cos, mult_max, A_max, Z_max;
+  R T_scale, cos_scale;          // n_T / T_max and n_cos / 2, rounded once to R
+  unsigned long long *dd, *mult, *nuclide, *yield;
+  int smem;                      // 1 = shared-memory bins
+};
+
+template <typename R>
+__global__ void __launch_bounds__(256) tally_kernel(const TallyParams<R> P) {
+  extern __shared__ unsigned int s_bins[];
+  const int n_dd = 3 * P.n_cos * (P.n_T + 1), n_mult = 4 * (P.mult_max + 1), n_nuc = (P.A_max + 1) * (P.Z_max + 1);
+  const int o_mult = n_dd, o_nuc = n_dd + n_mult, o_y = o_nuc + n_nuc, n_all = o_y + 12;
+  if (P.smem) {
+    for (int i = threadIdx.x; i < n_all; i += blockDim.x) s_bins[i] = 0u;
+    __syncthreads();
+  }
+  auto bump = [&](int bin) {
+    if (P.smem) atomicAdd(&s_bins[bin], 1u);
+    else {
+      unsigned long long *g = bin < o_mult ? P.dd + bin : bin < o_nuc ? P.mult + (bin - o_mult)
+                            : bin < o_y ? P.nuclide + (bin - o_nuc) : P.yield + (bin - o_y);
+      atomicAdd(g, 1ull);
+    }
+  };
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < P.n_events; e += (long long)gridDim.x * blockDim.x) {
+    const long long b = P.offsets[e];
+    const int n = P.counts[e];
+    int m[3] = {0, 0, 0};
+    for (int k = 0; k < n; ++k) {
+      const unsigned sp = P.species[b + k];
+      const int code = (int)(sp & 0x7u);
+      const int c = code < 2 ? code : 2;
+      m[c]++;
+      int a = (int)((P.uz[b + k] + R(1)) * P.cos_scale);
+      a = a < 0 ? 0 : (a > P.n_cos - 1 ? P.n_cos - 1 : a);
+      const R tt = P.T[b + k] * P.T_scale;
+      int t = tt >= R(P.n_T) ? P.n_T : (int)tt;
+      t = t < 0 ? 0 : t;
+      bump((c * P.n_cos + a) * (P.n_T + 1) + t);
+      if (code < 6) bump(o_y + code * 2 + (int)(sp >> 7));
+    }
+    const int mm = P.mult_max;
+    bump(o_mult + 0 * (mm + 1) + (m[0] < mm ? m[0] : mm));
+    bump(o_mult + 1 * (mm + 1) + (m[1] < mm ? m[1] : mm));
+    bump(o_mult + 2 * (mm + 1) + (m[2] < mm ? m[2] : mm));
+    bump(o_mult + 3 * (mm + 1) + (n < mm ? n : mm));
+    const int A = P.rA[e], Z = P.rZ[e];
+    if (A >= 0 && A <= P.A_max && Z >= 0 && Z <= P.Z_max) bump(o_nuc + A * (P.Z_max + 1) + Z);
+  }
+  if (P.smem) {
+    __syncthreads();
+    for (int i = threadIdx.x; i < n_all; i += blockDim.x) {
+      const unsigned int v = s_bins[i];
+      if (v) {
+        unsigned long long *g = i < o_mult ? P.dd + i : i < o_nuc ? P.mult + (i - o_mult)
+                              : i < o_y ? P.nuclide + (i - o_nuc) : P.yield + (i - o_y);
+        atomicAdd(g, (unsigned long long)v);
       }
     }
   }

@@ -691,6 +691,34 @@ int inc_measure_issue_peak(double *out, double *clock_mhz) {
   return 0;
 }
 
+int inc_tally(int64_t n, const inc_secondaries *sec, const int32_t *counts, const int64_t *offsets,
+              const inc_residual *res, const inc_tally_spec *spec, const inc_tallies *out) {
+  if (n < 0 || !sec || !res || !spec || !out) return fail(INC_E_BADARG, "null pointer or n < 0");
+  if (spec->n_T < 1 || spec->n_cos < 1 || spec->mult_max < 0 || spec->A_max < 0 || spec->Z_max < 0 || !(spec->T_max > 0.0))
+    return fail(INC_E_BADARG, "tally spec: bin counts must be positive");
+  if (!out->dd || !out->mult || !out->nuclide || !out->yield) return fail(INC_E_BADARG, "null tally pointer");
+  if (n == 0) return 0;
+  if (!counts || !offsets || !sec->species || !sec->T || !sec->uz || !res->A || !res->Z) return fail(INC_E_BADARG, "null pointer");
+  TallyParams<real> tp;
+  tp.species = sec->species; tp.T = sec->T; tp.uz = sec->uz; tp.counts = counts;
+  tp.offsets = reinterpret_cast<const long long *>(offsets); tp.rA = res->A; tp.rZ = res->Z; tp.n_events = n;
+  tp.n_T = spec->n_T; tp.n_cos = spec->n_cos; tp.mult_max = spec->mult_max; tp.A_max = spec->A_max; tp.Z_max = spec->Z_max;
+  tp.T_scale = (real)((double)spec->n_T / spec->T_max); tp.cos_scale = (real)((double)spec->n_cos / 2.0);
+  tp.dd = out->dd; tp.mult = out->mult; tp.nuclide = out->nuclide; tp.yield = out->yield;
+  const size_t bins = (size_t)3 * spec->n_cos * (spec->n_T + 1) + (size_t)4 * (spec->mult_max + 1) +
+                      (size_t)(spec->A_max + 1) * (spec->Z_max + 1) + 12;
+  const size_t smem = bins * sizeof(unsigned int);
+  tp.smem = smem <= 96 * 1024 ? 1 : 0;
+  auto kern = tally_kernel<real>;
+  if (tp.smem && smem > 48 * 1024) CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  long long blocks = (n + 255) / 256;
+  const long long cap = (long long)g.sm_count * 4;
+  if (g.sm_count > 0 && blocks > cap) blocks = cap;
+  kern<<<(unsigned)blocks, 256, tp.smem ? smem : 0, g.stream>>>(tp);
+  CU_TRY(cudaGetLastError());
+  return 0;
+}
+
 int inc_philox_blocks(const uint32_t *ctr, uint64_t seed, uint32_t *out, int64_t n) {
   if (n < 0 || (n > 0 && (!ctr || !out))) return fail(INC_E_BADARG, "bad argument");
   if (n == 0) return 0;

@@ -179,3 +179,34 @@ def test_golden_digest(orc, otables):
     assert r["species"].tolist() == g["species"]
     assert np.allclose(r["T"], g["T"], rtol=1e-9)
     assert np.allclose(r["Estar"], g["Estar"], rtol=1e-9, atol=1e-9)
+
+
+def test_tally_reference_against_brute_force(orc, otables):
+    """oracle.tally_reference (the definition of inc_tally's histograms) against a pure-Python loop over the
+    events of a small oracle run, and its invariants: every secondary is in exactly one dd bin and one yield
+    bin, every event in one multiplicity bin per class and (valid residual) one nuclide bin."""
+    import paper_1309_7963_b200.workloads as W
+    E, tid, targets, seed, _ = W.make_inputs(1, 300)
+    o = orc.simulate(otables, targets, E, tid, seed)
+    kw = dict(n_T=10, T_max=100.0, n_cos=4, mult_max=3, A_max=20, Z_max=10)
+    t = orc.tally_reference(o["species"], o["T"], o["uz"], o["counts"], o["A"], o["Z"], **kw)
+    dd = np.zeros((3, 4, 11), dtype=np.int64); mult = np.zeros((4, 4), dtype=np.int64)
+    nuc = np.zeros((21, 11), dtype=np.int64); yl = np.zeros((6, 2), dtype=np.int64)
+    for e in range(len(o["counts"])):
+        m = [0, 0, 0]
+        for k in range(o["offsets"][e], o["offsets"][e + 1]):
+            sp = int(o["species"][k]); code = sp & 7; c = min(code, 2); m[c] += 1
+            a = min(max(int((o["uz"][k] + 1.0) * 2.0), 0), 3)
+            tt = o["T"][k] * 0.1
+            tb = 10 if tt >= 10 else int(tt)
+            dd[c, a, tb] += 1; yl[code, sp >> 7] += 1
+        for c in range(3):
+            mult[c, min(m[c], 3)] += 1
+        mult[3, min(int(o["counts"][e]), 3)] += 1
+        if 0 <= o["A"][e] <= 20 and 0 <= o["Z"][e] <= 10:
+            nuc[o["A"][e], o["Z"][e]] += 1
+    assert np.array_equal(t["dd"], dd) and np.array_equal(t["mult"], mult)
+    assert np.array_equal(t["nuclide"], nuc) and np.array_equal(t["yields"], yl)
+    assert t["dd"].sum() == o["total"] == t["yields"].sum()
+    assert np.all(t["mult"].sum(axis=1) == len(o["counts"]))
+    assert t["nuclide"].sum() == len(o["counts"])          # 16O residuals all fit a 20 x 10 chart
