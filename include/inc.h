@@ -112,6 +112,11 @@ int inc_set_flags(uint32_t flags);
  * lanes wait for it, the epilogue+entry phase when at least `epi` lanes wait (1..32; default 8, 8).
  * Results never depend on it. */
 int inc_set_vote_thresholds(int coll, int epi);
+/* A call is processed in chunks of at most `n` events (default 2^22; 0 restores it; 1024 .. 2^24): the
+ * library's staging workspace is sized for one chunk (64 records of 32 bytes per event in the f32
+ * build: 8.6 GB at the default) and every chunk is one launch of each kernel, so large chunks mean
+ * few drain phases of the persistent cascade kernel.  Results never depend on it (R-R4). */
+int inc_set_chunk_events(int64_t n);
 /* Scheduling knob of the default (wavefront) cascade kernel: a track that has run `n_segments`
  * segments may be handed to a warp that has finished its own events, which evaluates 32 consecutive
  * segments of the one track per pass along its collision-free path (drain helpers, DESIGN.md

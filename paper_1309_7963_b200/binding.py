@@ -77,7 +77,7 @@ def make_tables_struct(t: dict):
 
 
 EXPORTS = ["inc_init", "inc_free_target", "inc_shutdown", "inc_set_stream", "inc_set_flags", "inc_set_event_offset",
-           "inc_get_stage_times", "inc_get_drain_timeline", "inc_set_vote_thresholds", "inc_set_long_track_threshold", "inc_simulate",
+           "inc_get_stage_times", "inc_get_drain_timeline", "inc_set_vote_thresholds", "inc_set_long_track_threshold", "inc_set_chunk_events", "inc_simulate",
            "inc_simulate_host", "inc_get_offsets", "inc_get_cascade_stage", "inc_get_stats", "inc_get_nucleus",
            "inc_measure_issue_peak", "inc_philox_blocks", "inc_tally", "inc_last_error", "inc_build_info"]
 
@@ -168,6 +168,9 @@ class IncLibrary:
         ms, nl = (C.c_float * 4)(), (C.c_int32 * 4)()
         self._check(self.lib.inc_get_stage_times(ms, nl))
         return dict(zip(("cascade", "evap", "scan", "compact"), [float(x) for x in ms])), [int(x) for x in nl]
+
+    def inc_set_chunk_events(self, n: int):
+        self._check(self.lib.inc_set_chunk_events(C.c_int64(int(n))))
 
     def inc_set_long_track_threshold(self, n_segments: int):
         self._check(self.lib.inc_set_long_track_threshold(int(n_segments)))
@@ -299,7 +302,8 @@ def load(variant: str = "f32") -> IncLibrary:
     return _cache[variant]
 
 
-def simulate(lib: IncLibrary, targets, E_in_np, target_idx_np, seed, tables: dict, flags: int = 0, capacity_per_event: int = 24):
+def simulate(lib: IncLibrary, targets, E_in_np, target_idx_np, seed, tables: dict, flags: int = 0, capacity_per_event: int = 24,
+             chunk_events: int = 1 << 22):
     """Convenience used by tests/bench: init targets, run on the GPU, return numpy arrays.
     targets: list of (A,Z); target_idx_np indexes that list."""
     import torch
@@ -321,7 +325,7 @@ def simulate(lib: IncLibrary, targets, E_in_np, target_idx_np, seed, tables: dic
     res["status"] = res["status"].view(np.uint32)
     res["offsets"] = off.cpu().numpy()
     res["total"] = total
-    if n <= (1 << 20):
+    if n <= chunk_events:
         st = lib.inc_get_cascade_stage(n)
         res["casc_A"], res["casc_Z"] = st["A"].cpu().numpy(), st["Z"].cpu().numpy()
         res["casc_Estar"] = st["Estar"].cpu().numpy()

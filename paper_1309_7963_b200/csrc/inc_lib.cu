@@ -74,6 +74,7 @@ struct State {
   std::vector<cudaEvent_t> pending_events;   // 5 per chunk, resolved after the stream sync
   int vote_coll = 8, vote_epi = 8;
   int long_seg = kLongSegDefault;
+  size_t chunk_events = (size_t)1 << 22;
   int sm_count = 0;
   std::string err;
 };
@@ -530,7 +531,7 @@ int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64
     return fail(INC_E_BADARG, "null residual array");
   if (sec->capacity < 0 || (sec->capacity > 0 && (!sec->species || !sec->T || !sec->ux || !sec->uy || !sec->uz)))
     return fail(INC_E_BADARG, "null secondary array");
-  const size_t chunk_max = (size_t)1 << 20;
+  const size_t chunk_max = g.chunk_events;
   const size_t chunk = (size_t)n < chunk_max ? (size_t)(n > 0 ? n : 1) : chunk_max;
   int rc = ensure_ws(chunk, (size_t)n);
   if (rc) return rc;
@@ -585,7 +586,7 @@ int inc_get_offsets(int64_t *dev_offsets) {
 
 int inc_get_cascade_stage(int32_t *A, int32_t *Z, INC_REAL *Es, INC_REAL *px, INC_REAL *py, INC_REAL *pz, int32_t *ncs) {
   if (g.last_n < 0) return fail(INC_E_STATE, "no previous inc_simulate");
-  if ((size_t)g.last_n > g.ws_chunk) return fail(INC_E_STATE, "cascade stage is only kept for single-chunk calls (n <= 2^20)");
+  if ((size_t)g.last_n > g.ws_chunk) return fail(INC_E_STATE, "cascade stage is only kept for single-chunk calls (n <= the chunk size, inc_set_chunk_events)");
   const size_t n = (size_t)g.last_n;
   if (A) CU_TRY(cudaMemcpyAsync(A, g.ws.cA, n * 4, cudaMemcpyDeviceToDevice, g.stream));
   if (Z) CU_TRY(cudaMemcpyAsync(Z, g.ws.cZ, n * 4, cudaMemcpyDeviceToDevice, g.stream));
@@ -653,6 +654,12 @@ int inc_get_nucleus(int id, int32_t *A, int32_t *Z, int32_t *ns, double *R, doub
 int inc_set_vote_thresholds(int coll, int epi) {
   if (coll < 1 || coll > 32 || epi < 1 || epi > 32) return fail(INC_E_BADARG, "thresholds must be 1..32");
   g.vote_coll = coll; g.vote_epi = epi;
+  return 0;
+}
+
+int inc_set_chunk_events(int64_t n) {
+  if (n < 0 || (n > 0 && n < 1024) || n > ((int64_t)1 << 24)) return fail(INC_E_BADARG, "chunk size must be 0 (default) or 1024 .. 2^24");
+  g.chunk_events = n == 0 ? ((size_t)1 << 22) : (size_t)n;
   return 0;
 }
 

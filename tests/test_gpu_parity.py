@@ -260,28 +260,43 @@ def test_same_stream_probe_and_host_path(gpu, ptables):
 
 
 def test_chunk_boundary_determinism(gpu, orc, otables, ptables):
-    """n > 2^20 runs in two chunks; events around the boundary equal the oracle's (event index
-    keys the RNG, not the chunk)."""
-    n = (1 << 20) + 4000
+    """A call longer than the chunk size (inc_set_chunk_events) runs as several launches with a carried
+    offset; events around every boundary equal the oracle's (the event index keys the RNG, not the chunk) and
+    the whole output is bit-identical to the single-chunk run."""
+    import torch
+    chunk = 1 << 16
+    n = 3 * chunk + 4000
     E = np.full(n, 200.0); tid = np.zeros(n, dtype=np.int32)
     lib = gpu.load("f64")
-    import torch
     lib.inc_shutdown()
     s = lib.inc_init(16, 8, ptables)
     lib.inc_set_stream(); lib.inc_set_flags(0)
-    out = lib.alloc_outputs(n, n * 8)
-    tot = lib.inc_simulate(torch.as_tensor(E, device="cuda"), torch.full((n,), s, dtype=torch.int32, device="cuda"), 2, out)
-    off = lib.inc_get_offsets(n).cpu().numpy()
+    Ed = torch.as_tensor(E, device="cuda"); td = torch.full((n,), s, dtype=torch.int32, device="cuda")
+    try:
+        lib.inc_set_chunk_events(chunk)
+        out = lib.alloc_outputs(n, n * 8)
+        tot = lib.inc_simulate(Ed, td, 2, out)
+        off = lib.inc_get_offsets(n).cpu().numpy()
+    finally:
+        lib.inc_set_chunk_events(0)
     assert off[-1] == tot
-    lo, hi = (1 << 20) - 300, (1 << 20) + 300
-    o = orc.simulate(otables, [(16, 8)], E[lo:hi], tid[lo:hi], 2, e0=lo)
-    g = {k: out[k][lo:hi].cpu().numpy() for k in ("counts", "A", "Z", "Estar")}
-    a, b = off[lo], off[hi]
+    one = lib.alloc_outputs(n, n * 8)
+    assert lib.inc_simulate(Ed, td, 2, one) == tot
+    assert np.array_equal(lib.inc_get_offsets(n).cpu().numpy(), off)
+    for k in ("counts", "A", "Z", "Estar", "px", "status"):
+        assert torch.equal(out[k], one[k]), k
     for k in ("species", "T", "ux", "uy", "uz"):
-        g[k] = out[k][a:b].cpu().numpy()
-    g["offsets"] = off[lo:hi + 1] - off[lo]
-    frac, err, _ = H.event_identity(g, o)
-    assert frac >= 0.995 and err <= REL_F64
+        assert torch.equal(out[k][:tot], one[k][:tot]), k
+    for bnd in (chunk, 2 * chunk, 3 * chunk):
+        lo, hi = bnd - 200, bnd + 200
+        o = orc.simulate(otables, [(16, 8)], E[lo:hi], tid[lo:hi], 2, e0=lo)
+        g = {k: out[k][lo:hi].cpu().numpy() for k in ("counts", "A", "Z", "Estar")}
+        a, b = off[lo], off[hi]
+        for k in ("species", "T", "ux", "uy", "uz"):
+            g[k] = out[k][a:b].cpu().numpy()
+        g["offsets"] = off[lo:hi + 1] - off[lo]
+        frac, err, _ = H.event_identity(g, o)
+        assert frac >= 0.995 and err <= REL_F64
 
 
 # ------------------------------------------------------------------------------- criteria (1), (3)
