@@ -1421,9 +1421,9 @@ __device__ __forceinline__ void G13_scaled(R s, R s_ref, R &g1, R &g3) {
     R a1 = R(0), a3 = R(0);
 #pragma unroll 1
     for (int k = 0; k < M<R>::kSeriesTerms; ++k) {
-      a1 += term / R(k + 2);
-      a3 += term * s * s / R(k + 4);
-      term *= s / R(k + 1);
+      a1 += M<R>::div_(term, R(k + 2));
+      a3 += M<R>::div_(term * s * s, R(k + 4));
+      term *= M<R>::div_(s, R(k + 1));
     }
     const R e = M<R>::exp_(-s_ref);
     g1 = a1 * e; g3 = a3 * e;
@@ -1498,7 +1498,7 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
             if (X > R(0)) {
               ch[j] = c;
               Xj[j] = X;
-              aj[j] = R(Ad) / P.model.a_div;
+              aj[j] = M<R>::div_(R(Ad), P.model.a_div);
               sj[j] = R(2) * M<R>::sqrt_(aj[j] * X);
               s_ref = sj[j] > s_ref ? sj[j] : s_ref;
               any = true;
@@ -1518,8 +1518,8 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
           if (Xj[j] > R(0)) {
             R g1, g3;
             G13_scaled<R>(sj[j], s_ref, g1, g3);
-            const R I0 = g1 / (R(2) * aj[j]);
-            const R I1 = Xj[j] * I0 - g3 / (R(8) * aj[j] * aj[j]);
+            const R I0 = M<R>::div_(g1, R(2) * aj[j]);
+            const R I1 = Xj[j] * I0 - M<R>::div_(g3, R(8) * aj[j] * aj[j]);
             R w = ch[j].pref * (I1 + ch[j].beta * I0);
             W[j] = w > R(0) ? w : R(0);
             Wsum += W[j];
@@ -1543,7 +1543,7 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
           for (int j = 0; j < 6; ++j) if (j == jsel) { X = Xj[j]; a = aj[j]; beta = ch[j].beta; V = ch[j].V; BdBj = ch[j].BdBj; }
           // ---------- E4: rejection sampling of x (two envelopes, R-E4) ----------
           const R s = R(2) * M<R>::sqrt_(a * X);
-          const R T = M<R>::sqrt_(X / a);
+          const R T = M<R>::sqrt_(M<R>::div_(X, a));
           const R areaA = T * (T + beta), areaB = R(0.5) * X * X + beta * X;
           R xs = R(-1);
 #pragma unroll 1
@@ -1560,7 +1560,7 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
             } else {
               if (v[0] * (T + beta) < T) xx = -T * M<R>::log_(v[1] * v[2]);
               else xx = -T * M<R>::log_(v[1]);
-              if (xx < X && M<R>::log_(v[3]) < R(2) * M<R>::sqrt_(a * (X - xx)) - s + xx / T) { xs = xx; break; }
+              if (xx < X && M<R>::log_(v[3]) < R(2) * M<R>::sqrt_(a * (X - xx)) - s + M<R>::div_(xx, T)) { xs = xx; break; }
             }
           }
           if (xs < R(0)) { status |= INC_ST_TRIAL_CAP; finish = true; }
@@ -1575,7 +1575,7 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
             const R Mds = R(Zd) * K<R>::mp + R(Ad - Zd) * K<R>::mn - Bd + Esd;
             const R Mpar = R(Z) * K<R>::mp + R(A - Z) * K<R>::mn - Bpar + Es;
             const R eps = V + xs;   // total kinetic energy released in the parent frame
-            const R p2 = eps * (R(2) * Mpar - eps) * (R(2) * Mds + eps) * (R(2) * Mj + eps) / (R(4) * Mpar * Mpar);
+            const R p2 = M<R>::div_(eps * (R(2) * Mpar - eps) * (R(2) * Mds + eps) * (R(2) * Mj + eps), R(4) * Mpar * Mpar);
             const R pm = M<R>::sqrt_(p2 > R(0) ? p2 : R(0));
             const R Ej = M<R>::sqrt_(p2 + Mj * Mj);
             const R cth = R(2) * u[1] - R(1);
@@ -1585,15 +1585,15 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
             M<R>::sincos2pi(u[2], &sph, &cph);
             const R qx = pm * sth * cph, qy = pm * sth * sph, qz = pm * cth;
             const R Epar = M<R>::sqrt_(Mpar * Mpar + Px * Px + Py * Py + Pz * Pz);
-            const R iEp = R(1) / Epar;
+            const R iEp = M<R>::rcp_(Epar);
             const R bx = Px * iEp, by = Py * iEp, bz = Pz * iEp;
-            const R gam = Epar / Mpar;
-            const R gfac = gam * gam / (gam + R(1));
+            const R gam = M<R>::div_(Epar, Mpar);
+            const R gfac = M<R>::div_(gam * gam, gam + R(1));
             const R fo = gfac * (qx * bx + qy * by + qz * bz) + gam * Ej;
             const R lx = qx + fo * bx, ly = qy + fo * by, lz = qz + fo * bz;
             const R l2 = lx * lx + ly * ly + lz * lz;
             const R El = M<R>::sqrt_(l2 + Mj * Mj);
-            const R Tl = l2 / (El + Mj);
+            const R Tl = M<R>::div_(l2, El + Mj);
             const R il = M<R>::rsqrt_(l2);
             const size_t o = (size_t)ev * kMaxSec + count;
             stage_write<R>(P.ws.st + o, Tl, lx * il, ly * il, lz * il, 0x80000000u | ((uint32_t)jsel << 24) | (uint32_t)count);
