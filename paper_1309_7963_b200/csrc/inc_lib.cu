@@ -370,6 +370,15 @@ int mark(bool timing) {
   return 0;
 }
 
+// R-R1: the ten round keys of the call's seed, to constant memory (ordered on the stream like everything else)
+int set_round_keys(uint64_t seed) {
+  RoundKeys rk;
+  uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) { rk.k0[r] = k0; rk.k1[r] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+  CU_TRY(cudaMemcpyToSymbolAsync(c_rk, &rk, sizeof(rk), 0, cudaMemcpyHostToDevice, g.stream));
+  return 0;
+}
+
 template <bool STATS>
 int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t *tid, uint64_t seed,
                  inc_secondaries *sec, int32_t *counts, inc_residual *res, long long *offsets) {
@@ -536,6 +545,7 @@ int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64
   int rc = ensure_ws(chunk, (size_t)n);
   if (rc) return rc;
   CU_TRY(cudaMemsetAsync(g.d_ctr, 0, sizeof(DevCounters), g.stream));
+  if (int rk_rc = set_round_keys(seed)) return rk_rc;
   for (auto e : g.pending_events) cudaEventDestroy(e);
   g.pending_events.clear();
   for (int i = 0; i < 4; ++i) { g.stage_ms[i] = 0; g.stage_launches[i] = 0; }
@@ -729,7 +739,8 @@ int inc_tally(int64_t n, const inc_secondaries *sec, const int32_t *counts, cons
 int inc_philox_blocks(const uint32_t *ctr, uint64_t seed, uint32_t *out, int64_t n) {
   if (n < 0 || (n > 0 && (!ctr || !out))) return fail(INC_E_BADARG, "bad argument");
   if (n == 0) return 0;
-  philox_blocks_kernel<<<(unsigned)((n + 255) / 256), 256, 0, g.stream>>>(ctr, (uint32_t)seed, (uint32_t)(seed >> 32), out, n);
+  if (int rc = set_round_keys(seed)) return rc;
+  philox_blocks_kernel<<<(unsigned)((n + 255) / 256), 256, 0, g.stream>>>(ctr, out, n);
   CU_TRY(cudaGetLastError());
   CU_TRY(cudaStreamSynchronize(g.stream));
   return 0;
