@@ -189,9 +189,12 @@ def main():
     stage = dict(cascade=0.0, evap=0.0, scan=0.0, compact=0.0)
     launches = 0
     t_wall0 = time.time()
+    step_ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     ev0.record()
+    step_ev[0].record()
     for k in range(args.steps):
         lib.inc_simulate(E_d, tid_d, seed + k, out)
+        step_ev[k + 1].record()
         ms, nl = lib.inc_get_stage_times()
         for kk in stage:
             stage[kk] += ms[kk]
@@ -207,7 +210,20 @@ def main():
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     value = world * n * args.steps / (ms_total * 1e-3)
 
-    # ---- extras (outside the timed region): drain timeline of the last cascade launch, on-device tallies ----
+    per_step = sorted(step_ev[k].elapsed_time(step_ev[k + 1]) for k in range(args.steps))
+    # ---- extras (outside the timed region) ----
+    # divergence-free ceiling: every event draws the random stream of event 0
+    lib.inc_set_flags(args.flags | B.F_SAME_STREAM)
+    lib.inc_simulate(E_d, tid_d, seed, out)
+    pev0, pev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    pev0.record()
+    lib.inc_simulate(E_d, tid_d, seed, out)
+    pev1.record()
+    torch.cuda.synchronize()
+    same_stream_ms = pev0.elapsed_time(pev1)
+    lib.inc_set_flags(args.flags | B.F_TIMING)
+    lib.inc_simulate(E_d, tid_d, seed + args.steps - 1, out)
+    # drain timeline of the last cascade launch, on-device tallies
     timeline = lib.inc_get_drain_timeline()
     off_d = lib.inc_get_offsets(n)
     tspec, tall = lib.alloc_tallies()
@@ -287,6 +303,10 @@ def main():
                 clocks=clocks, e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                                         steps=e2e_steps),
                 gpu_launches=int(launches), roofline=roofline, cpu_baseline=cpu_baseline,
+                per_step_ms=dict(best=per_step[0], median=per_step[len(per_step) // 2]),
+                same_stream_probe=dict(ms=same_stream_ms, events_per_s=n / (same_stream_ms * 1e-3),
+                                       note="INC_F_SAME_STREAM: all events identical, no divergence (the paper's probe, P:73-75)"),
+                paper_time_split="GTX680, 200 MeV p-16O: INC 72 %, evaporation 23 %, RNG init 3 % (P:142); see roofline.kernel_share",
                 cascade_drain_timeline_ms=timeline,
                 tally=dict(ms=tally_ms, note="inc_tally over the step's outputs (dd spectra 3x20x51, multiplicities, nuclide chart, yields); not part of the step"),
                 work_counters_per_event={k: stats[k] / max(stats["events"], 1) for k in
