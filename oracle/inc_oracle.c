@@ -464,7 +464,7 @@ static int cmp_esc(const void *a, const void *b) {
 
 /* One cascade attempt (C0-C5).  Returns n_real; fills esc[0..*n_esc). */
 static int cascade_attempt(const orc_tables *t, const orc_nucleus *nu, const rng_ctx *g,
-                           uint32_t attempt, double E_in, uint32_t flags,
+                           uint32_t attempt, double E_in, int proj, uint32_t flags,
                            esc_rec *esc, int *n_esc, uint32_t *status, orc_stats *st) {
   int ns = nu->n_shells;
   int n_real = 0;
@@ -480,10 +480,13 @@ static int cascade_attempt(const orc_tables *t, const orc_nucleus *nu, const rng
   track tr;
   tr.x[0] = b * cos(phib); tr.x[1] = b * sin(phib);
   { double zz = nu->R * nu->R - b * b; if (zz < 0.0) zz = 0.0; tr.x[2] = -sqrt(zz); }
-  tr.p[0] = 0.0; tr.p[1] = 0.0; tr.p[2] = sqrt(E_in * (E_in + 2.0 * M_P));
-  tr.type = 1; tr.pi = 1u; tr.k = 1u; tr.nseg = 0;
+  /* NEXT-3 ("nucleon-nucleus interaction"): the incident nucleon is a proton (proj = 1) or a neutron
+     (proj = 0); it enters with its own mass and feels its own species' potential */
+  const double m0 = nucleon_mass(proj);
+  tr.p[0] = 0.0; tr.p[1] = 0.0; tr.p[2] = sqrt(E_in * (E_in + 2.0 * m0));
+  tr.type = proj; tr.pi = 1u; tr.k = 1u; tr.nseg = 0;
   {
-    int refl = orc_boundary(tr.x, tr.p, M_P, 0.0, nu->V_p[ns - 1], NULL);
+    int refl = orc_boundary(tr.x, tr.p, m0, 0.0, proj ? nu->V_p[ns - 1] : nu->V_n[ns - 1], NULL);
     (void)refl; /* cannot reflect: V rises inward */
     tr.shell = ns - 1;
   }
@@ -600,7 +603,7 @@ int64_t orc_simulate(const orc_tables *t, const orc_nucleus *nuc, int n_nuc,
                      int32_t *res_A, int32_t *res_Z, double *res_Estar, double *res_px,
                      double *res_py, double *res_pz, uint32_t *status,
                      int32_t *casc_A, int32_t *casc_Z, double *casc_Estar, double *casc_P,
-                     int32_t *casc_count, orc_stats *stats) {
+                     int32_t *casc_count, orc_stats *stats, const uint8_t *projectile) {
   if (!t || !nuc || n < 0 || !E_in || !target || !counts) return -1;
   int64_t total = 0;
   if (stats) memset(stats, 0, sizeof(*stats));
@@ -623,11 +626,14 @@ int64_t orc_simulate(const orc_tables *t, const orc_nucleus *nuc, int n_nuc,
     int A_res = nu->A, Z_res = nu->Z;
     double Estar = 0.0, Pres[3] = {0, 0, 0};
     uint32_t attempt = 0;
-    double p_in = sqrt(Ein * (Ein + 2.0 * M_P));
+    const int proj = projectile ? (int)projectile[idx] : 1;      /* NULL: protons (the paper's case, P:9) */
+    if (proj != 0 && proj != 1) return -1;
+    const double m_in = nucleon_mass(proj);
+    double p_in = sqrt(Ein * (Ein + 2.0 * m_in));
     for (attempt = 0; attempt < ORC_MAX_ATTEMPT; ++attempt) {
       if (stats) stats->attempts++;
       uint32_t st_try = 0;
-      int n_real = cascade_attempt(t, nu, &g, attempt, Ein, flags, esc, &n_esc, &st_try, stats);
+      int n_real = cascade_attempt(t, nu, &g, attempt, Ein, proj, flags, esc, &n_esc, &st_try, stats);
       /* C6: epilogue — sums in ascending path-code order */
       qsort(esc, (size_t)n_esc, sizeof(esc_rec), cmp_esc);
       int n_p = 0;
@@ -638,8 +644,8 @@ int64_t orc_simulate(const orc_tables *t, const orc_nucleus *nuc, int n_nuc,
         for (int q = 0; q < 3; ++q) sumP[q] += esc[k].p[q];
       }
       A_res = nu->A + 1 - n_esc;
-      Z_res = nu->Z + 1 - n_p;
-      double Eres = Ein + M_P + nu->M - sumE;
+      Z_res = nu->Z + proj - n_p;
+      double Eres = Ein + m_in + nu->M - sumE;
       Pres[0] = -sumP[0]; Pres[1] = -sumP[1]; Pres[2] = p_in - sumP[2];
       int transparent = (n_real == 0);
       if (transparent && !(flags & ORC_F_KEEP_TRANSPARENT)) { if (stats) stats->retry_transparent++; continue; }

@@ -93,7 +93,8 @@ int64_t orc_simulate(const orc_tables *t, const orc_nucleus *nuc, int n_nuc,
                      int32_t *res_A, int32_t *res_Z, double *res_Estar, double *res_px,
                      double *res_py, double *res_pz, uint32_t *status,
                      int32_t *casc_A, int32_t *casc_Z, double *casc_Estar, double *casc_P,
-                     int32_t *casc_count, orc_stats *stats);
+                     int32_t *casc_count, orc_stats *stats,
+                     const uint8_t *projectile /* [n] 0 = neutron, 1 = proton; NULL = all protons (NEXT-3) */);
 
 /* ---- single steps, exported so the pins can test each in isolation ----------- */
 void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);

@@ -114,7 +114,7 @@ def lib():
         C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32,
         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p,
         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
-        C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(OrcStats)]
+        C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(OrcStats), C.c_void_p]
     L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
     L.orc_philox4x32_10.restype = None
     L.orc_u01.argtypes = [C.c_uint32]
@@ -247,13 +247,17 @@ def nucleus_arrays(nu: OrcNucleus) -> dict:
     return out
 
 
-def simulate(tables: Tables, nuclei, E_in, target, seed, e0=0, flags=0, want_stats=True):
-    """Run the oracle on events e0..e0+n-1.  nuclei: list of (A,Z) or OrcNucleus."""
+def simulate(tables: Tables, nuclei, E_in, target, seed, e0=0, flags=0, want_stats=True, projectile=None):
+    """Run the oracle on events e0..e0+n-1.  nuclei: list of (A,Z) or OrcNucleus.
+    projectile: None (protons, the paper's case) or per-event uint8 array, 0 = neutron, 1 = proton (NEXT-3)."""
     L = lib()
     nus = (OrcNucleus * len(nuclei))()
     for i, nz in enumerate(nuclei):
         nus[i] = nz if isinstance(nz, OrcNucleus) else setup_nucleus(nz[0], nz[1], tables)
     E_in = np.ascontiguousarray(E_in, dtype=np.float64)
+    if projectile is not None:
+        projectile = np.ascontiguousarray(projectile, dtype=np.uint8)
+        assert len(projectile) == len(E_in)
     target = np.ascontiguousarray(target, dtype=np.int32)
     n = len(E_in)
     cap = n * MAX_SEC
@@ -273,7 +277,8 @@ def simulate(tables: Tables, nuclei, E_in, target, seed, e0=0, flags=0, want_sta
                              C.c_uint64(int(seed)), C.c_uint32(int(flags)),
                              vp(sp), vp(T), vp(ux), vp(uy), vp(uz), int(cap), vp(counts),
                              vp(rA), vp(rZ), vp(rE), vp(rpx), vp(rpy), vp(rpz), vp(status),
-                             vp(cA), vp(cZ), vp(cE), vp(cP), vp(cN), C.byref(st))
+                             vp(cA), vp(cZ), vp(cE), vp(cP), vp(cN), C.byref(st),
+                             None if projectile is None else vp(projectile))
         if tot == -3 and cap < n * MAX_SEC:
             cap = n * MAX_SEC
             continue

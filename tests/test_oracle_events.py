@@ -15,7 +15,7 @@ def _run(orc, otables, A, Z, E, n, seed, **kw):
     return orc.simulate(otables, [(A, Z)], np.full(n, float(E)), np.zeros(n, dtype=np.int32), seed, **kw)
 
 
-def _check_conservation(orc, otables, r, A, Z, E_in, rel=1e-9):
+def _check_conservation(orc, otables, r, A, Z, E_in, rel=1e-9, proj=1):
     L = orc.lib()
     t = C.byref(otables.c)
     n = len(r["counts"])
@@ -28,15 +28,16 @@ def _check_conservation(orc, otables, r, A, Z, E_in, rel=1e-9):
     ok = (r["status"] & orc.ST_FAILED) == 0
     # (1) exact baryon number and charge
     assert np.all((sumA + r["A"])[ok] == A + 1)
-    assert np.all((sumZ + r["Z"])[ok] == Z + 1)
+    assert np.all((sumZ + r["Z"])[ok] == (Z + np.asarray(proj))[ok] if np.ndim(proj) else (sumZ + r["Z"])[ok] == Z + proj)
     # 4-momentum
     sumE = np.bincount(seg, weights=r["T"] + mass, minlength=n)
     sp = [np.bincount(seg, weights=pmag * r[k], minlength=n) for k in ("ux", "uy", "uz")]
     Mres = np.array([L.orc_mass(int(a), int(z), t) for a, z in zip(r["A"], r["Z"])])
     Pres2 = r["px"] ** 2 + r["py"] ** 2 + r["pz"] ** 2
     Eres = np.sqrt((Mres + r["Estar"]) ** 2 + Pres2)
-    E_tot = E_in + orc.M_P + L.orc_mass(A, Z, t)
-    p_in = np.sqrt(E_in * (E_in + 2 * orc.M_P))
+    m_in = np.where(np.asarray(proj) == 1, orc.M_P, orc.M_N)
+    E_tot = E_in + m_in + L.orc_mass(A, Z, t)
+    p_in = np.sqrt(E_in * (E_in + 2 * m_in))
     assert np.allclose((sumE + Eres)[ok], E_tot[ok] if np.ndim(E_tot) else E_tot, rtol=rel, atol=0)
     assert np.allclose((sp[0] + r["px"])[ok], 0.0, atol=rel * np.max(p_in))
     assert np.allclose((sp[1] + r["py"])[ok], 0.0, atol=rel * np.max(p_in))
@@ -210,3 +211,29 @@ def test_tally_reference_against_brute_force(orc, otables):
     assert t["dd"].sum() == o["total"] == t["yields"].sum()
     assert np.all(t["mult"].sum(axis=1) == len(o["counts"]))
     assert t["nuclide"].sum() == len(o["counts"])          # 16O residuals all fit a 20 x 10 chart
+
+
+def test_neutron_projectile(orc, otables):
+    """NEXT-3 ("nucleon-nucleus"): an incident neutron.  Pins: exact baryon number A + 1 and charge Z + 0,
+    4-momentum with the neutron mass, a mixed batch equals the two homogeneous batches event by event (the
+    projectile is a per-event input like E_in), and the two species really differ (Coulomb cutoff, potentials)."""
+    n = 3000
+    E = np.full(n, 150.0); tid = np.zeros(n, dtype=np.int32)
+    rn = orc.simulate(otables, [(40, 20)], E, tid, 11, projectile=np.zeros(n, dtype=np.uint8))
+    rp = orc.simulate(otables, [(40, 20)], E, tid, 11, projectile=np.ones(n, dtype=np.uint8))
+    r1 = orc.simulate(otables, [(40, 20)], E, tid, 11)
+    assert not np.any(rn["status"] & orc.ST_FAILED)
+    _check_conservation(orc, otables, rn, 40, 20, np.float64(150.0), proj=0)
+    for k in ("species", "T", "counts", "A", "Z", "Estar"):
+        assert np.array_equal(rp[k], r1[k]), k                      # projectile = 1 is the default
+    mix = (np.arange(n) % 3 == 0).astype(np.uint8)
+    rm = orc.simulate(otables, [(40, 20)], E, tid, 11, projectile=mix)
+    for e in range(0, n, 7):
+        ref = rp if mix[e] else rn
+        a, b = rm["offsets"][e], rm["offsets"][e + 1]
+        c, d = ref["offsets"][e], ref["offsets"][e + 1]
+        assert b - a == d - c and np.array_equal(rm["T"][a:b], ref["T"][c:d]) and rm["Z"][e] == ref["Z"][e]
+    assert np.mean(rn["Z"]) < np.mean(rp["Z"])                    # one unit of charge less came in
+    # the leading particle keeps its species more often than not: more fast neutrons out for neutrons in
+    fast_n = lambda r: np.sum(((r["species"] & 0xFF) == 0) & (r["T"] > 75.0))
+    assert fast_n(rn) > 1.5 * fast_n(rp)
