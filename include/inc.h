@@ -112,6 +112,13 @@ int inc_set_flags(uint32_t flags);
  * lanes wait for it, the epilogue+entry phase when at least `epi` lanes wait (1..32; default 8, 8).
  * Results never depend on it. */
 int inc_set_vote_thresholds(int coll, int epi);
+/* Incident nucleon species (the paper's model is a "nucleon-nucleus" one, and is
+ * applied to protons, P:9): projectile[i] = 1 proton, 0 neutron for event i of the following inc_simulate /
+ * inc_simulate_host calls.  DEVICE array, caller-owned, at least as long as the calls' n_events; it must stay
+ * valid until those calls have returned.  NULL (the default) = all protons.  A neutron enters with its own mass
+ * and feels the neutron potential; the residual then has charge Z - n_p instead of Z + 1 - n_p.  Any other
+ * value is an input error (INC_E_BADARG, found on the device like E_in out of range). */
+int inc_set_projectiles(const uint8_t *projectile /*DEVICE [n] or NULL*/);
 /* A call is processed in chunks of at most `n` events (default 2^22; 0 restores it; 1024 .. 2^24): the
  * library's staging workspace is sized for one chunk (64 records of 32 bytes per event in the f32
  * build: 8.6 GB at the default) and every chunk is one launch of each kernel, so large chunks mean

@@ -77,7 +77,7 @@ def make_tables_struct(t: dict):
 
 
 EXPORTS = ["inc_init", "inc_free_target", "inc_shutdown", "inc_set_stream", "inc_set_flags", "inc_set_event_offset",
-           "inc_get_stage_times", "inc_get_drain_timeline", "inc_set_vote_thresholds", "inc_set_long_track_threshold", "inc_set_chunk_events", "inc_simulate",
+           "inc_get_stage_times", "inc_get_drain_timeline", "inc_set_vote_thresholds", "inc_set_long_track_threshold", "inc_set_chunk_events", "inc_set_projectiles", "inc_simulate",
            "inc_simulate_host", "inc_get_offsets", "inc_get_cascade_stage", "inc_get_stats", "inc_get_nucleus",
            "inc_measure_issue_peak", "inc_philox_blocks", "inc_tally", "inc_last_error", "inc_build_info"]
 
@@ -168,6 +168,11 @@ class IncLibrary:
         ms, nl = (C.c_float * 4)(), (C.c_int32 * 4)()
         self._check(self.lib.inc_get_stage_times(ms, nl))
         return dict(zip(("cascade", "evap", "scan", "compact"), [float(x) for x in ms])), [int(x) for x in nl]
+
+    def inc_set_projectiles(self, projectile=None):
+        """projectile: CUDA uint8 tensor (1 proton, 0 neutron per event) or None (protons).  Keep it alive."""
+        self._projectile = projectile
+        self._check(self.lib.inc_set_projectiles(C.c_void_p(0 if projectile is None else projectile.data_ptr())))
 
     def inc_set_chunk_events(self, n: int):
         self._check(self.lib.inc_set_chunk_events(C.c_int64(int(n))))
@@ -303,7 +308,7 @@ def load(variant: str = "f32") -> IncLibrary:
 
 
 def simulate(lib: IncLibrary, targets, E_in_np, target_idx_np, seed, tables: dict, flags: int = 0, capacity_per_event: int = 24,
-             chunk_events: int = 1 << 22):
+             chunk_events: int = 1 << 22, projectile=None):
     """Convenience used by tests/bench: init targets, run on the GPU, return numpy arrays.
     targets: list of (A,Z); target_idx_np indexes that list."""
     import torch
@@ -315,9 +320,13 @@ def simulate(lib: IncLibrary, targets, E_in_np, target_idx_np, seed, tables: dic
     tid = torch.as_tensor(slot_map[np.asarray(target_idx_np)], device="cuda")
     lib.inc_set_stream()
     lib.inc_set_flags(flags)
+    lib.inc_set_projectiles(None if projectile is None else torch.as_tensor(np.asarray(projectile, dtype=np.uint8), device="cuda"))
     cap = max(64, n * capacity_per_event)
     out = lib.alloc_outputs(n, cap)
-    total = lib.inc_simulate(E, tid, seed, out)
+    try:
+        total = lib.inc_simulate(E, tid, seed, out)
+    finally:
+        lib.inc_set_projectiles(None)
     off = lib.inc_get_offsets(n)
     res = {k: v.cpu().numpy() for k, v in out.items()}
     for k in ("species", "T", "ux", "uy", "uz"):

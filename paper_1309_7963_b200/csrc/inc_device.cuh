@@ -298,8 +298,8 @@ enum SegOutcome : int { SEG_REFLECT = -1, SEG_CONT = 0, SEG_COLLIDE = 1, SEG_ESC
 
 // ---------- C0: entry — uniform disc, beam along +z (R-Q15), potential step into the last shell ----------
 template <typename R>
-__device__ __forceinline__ void entry_step(Track<R> &t, const NucDev<R> &nu, R E_in, const RngKey &g, uint32_t attempt,
-                                           R &p_in) {
+__device__ __forceinline__ void entry_step(Track<R> &t, const NucDev<R> &nu, R E_in, int ptype, const RngKey &g,
+                                           uint32_t attempt, R &p_in) {
   R u[4];
   draw4<R>(g, attempt, 1u, 0u, u);
   const R b = nu.Rn * M<R>::sqrt_(u[0]);
@@ -308,18 +308,20 @@ __device__ __forceinline__ void entry_step(Track<R> &t, const NucDev<R> &nu, R E
   t.x = b * cb; t.y = b * sb;
   const R zz = nu.Rn * nu.Rn - b * b;
   t.z = -M<R>::sqrt_(zz > R(0) ? zz : R(0));
-  p_in = M<R>::sqrt_(E_in * (E_in + R(2) * K<R>::mp));
+  // the incident nucleon: proton (ptype 1, the paper's case P:9) or neutron (NEXT-3), with its own mass and potential
+  const R m0 = nucleon_mass<R>(ptype);
+  p_in = M<R>::sqrt_(E_in * (E_in + R(2) * m0));
   // potential step (cannot reflect: V rises inward)
   const R ux = t.x * nu.iRn, uy = t.y * nu.iRn, uz = t.z * nu.iRn;
   const R pr = p_in * uz;
-  const R dV = nu.sh[nu.ns - 1].V_p;
+  const R dV = ptype ? nu.sh[nu.ns - 1].V_p : nu.sh[nu.ns - 1].V_n;
   const R Tj = E_in + dV;
-  const R prj2 = pr * pr + dV * (E_in + Tj + R(2) * K<R>::mp);
+  const R prj2 = pr * pr + dV * (E_in + Tj + R(2) * m0);
   const R prj = -M<R>::sqrt_(prj2 > R(0) ? prj2 : R(0));
   const R dp = prj - pr;
   t.px = dp * ux; t.py = dp * uy; t.pz = p_in + dp * uz;
   t.T = Tj;
-  t.type = 1; t.shell = nu.ns - 1; t.pi = 1u; t.k = 1u; t.nseg = 0;
+  t.type = ptype; t.shell = nu.ns - 1; t.pi = 1u; t.k = 1u; t.nseg = 0;
 }
 
 // ---------- C2 + C4: one segment (R-Q8 partner first, then the path) ----------
@@ -589,10 +591,10 @@ __device__ __forceinline__ bool coll_step(Track<R> &t, const CollCarry<R> &cc, c
 // ---------- C6: epilogue ("excitation energy ... through energy conservation") ----------
 // Eavail = E_in - sum T_k, (Prx,Pry,Prz) = p_in - sum p_k.  Returns true if the attempt is accepted.
 template <typename R>
-__device__ __forceinline__ bool epilogue_eval(const NucDev<R> &nu, const R *bind, int n_esc, int n_p, int n_real,
+__device__ __forceinline__ bool epilogue_eval(const NucDev<R> &nu, const R *bind, int ptype, int n_esc, int n_p, int n_real,
                                               R Eavail, R Prx, R Pry, R Prz, bool keep_transparent,
                                               int &A_res, int &Z_res, R &Estar) {
-  A_res = nu.A + 1 - n_esc; Z_res = nu.Z + 1 - n_p;
+  A_res = nu.A + 1 - n_esc; Z_res = nu.Z + ptype - n_p;   // (the nucleon masses cancel for either projectile)
   Estar = R(0);
   if (!((n_real > 0) || keep_transparent)) return false;       // transparent: not a non-elastic event
   R Bres = R(-1e30);
@@ -617,6 +619,7 @@ template <typename R> struct CascadeParams {
   DevCounters *ctr;
   const R *E_in;            // chunk base
   const int32_t *target_id; // chunk base
+  const uint8_t *projectile; // chunk base; 0 = neutron, 1 = proton; nullptr = all protons
   long long e_base;         // global index of the chunk's first event
   int n_chunk;
   uint32_t seed_lo, seed_hi;
@@ -647,8 +650,9 @@ __device__ __forceinline__ void stage_model(const ModelDev<R> &model, int n_stag
 
 // validate an event's inputs; on failure write neutral outputs and raise the device error word
 template <typename R>
-__device__ __forceinline__ bool check_inputs(const CascadeParams<R> &P, const NucDev<R> *s_nuc, int ev, R E_in, int tgt) {
+__device__ __forceinline__ bool check_inputs(const CascadeParams<R> &P, const NucDev<R> *s_nuc, int ev, R E_in, int tgt, int ptype) {
   unsigned err = 0;
+  if (ptype != 0 && ptype != 1) err |= 8u;
   if (!(E_in >= R(INC_E_MIN) && E_in <= R(INC_E_MAX))) err |= 1u;
   if (tgt < 0 || tgt >= P.n_stage) err |= 2u;
   else if (!s_nuc[tgt].live) err |= 2u;
@@ -708,7 +712,7 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
   const bool same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
 
   int state = ST_EPI;
-  int ev = -1, tgt = 0;
+  int ev = -1, tgt = 0, ptype = 1;
   uint32_t attempt = 0;
   R E_in = R(0);
   RngKey g;
@@ -802,7 +806,7 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
           int A_res, Z_res;
           R Estar;
           const R Eavail = Fx<R>::from(fxE), Prx = Fx<R>::from(fxX), Pry = Fx<R>::from(fxY), Prz = Fx<R>::from(fxZ);
-          const bool ok = epilogue_eval<R>(nu, P.model.bind, n_esc, n_p, n_real, Eavail, Prx, Pry, Prz, keep_transparent, A_res, Z_res, Estar);
+          const bool ok = epilogue_eval<R>(nu, P.model.bind, ptype, n_esc, n_p, n_real, Eavail, Prx, Pry, Prz, keep_transparent, A_res, Z_res, Estar);
           if (ok) {
             const uint32_t used = attempt + 1u > 255u ? 255u : attempt + 1u;
             write_cascade_result<R>(P.ws, ev, A_res, Z_res, Estar, Prx, Pry, Prz, (uint32_t)n_esc | (attempt << 8), st_try | used);
@@ -831,7 +835,8 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
             attempt = 0;
             E_in = P.E_in[ev];
             tgt = P.target_id[ev];
-            if (!check_inputs<R>(P, s_nuc, ev, E_in, tgt)) { ev = -1; tgt = 0; }
+            ptype = P.projectile ? (int)P.projectile[ev] : 1;
+            if (!check_inputs<R>(P, s_nuc, ev, E_in, tgt, ptype)) { ev = -1; tgt = 0; }
             else {
               const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
               g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
@@ -845,7 +850,7 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
       if (state == ST_EPI && ev >= 0) {
         st.add(S_ATTEMPTS);
         R p_in;
-        entry_step<R>(t, s_nuc[tgt], E_in, g, attempt, p_in);
+        entry_step<R>(t, s_nuc[tgt], E_in, ptype, g, attempt, p_in);
         fxE = Fx<R>::to(E_in); fxX = 0; fxY = 0; fxZ = Fx<R>::to(p_in);
         n_esc = 0; n_p = 0; n_real = 0; st_try = 0; sp = 0;
         state = ST_SEG;
@@ -891,7 +896,7 @@ template <typename R> struct CtaLong {
 template <typename R, int NS, int QS, int QC> struct WarpMem {
   // event slots (32 B each in the f32 build)
   int32_t ev[NS];
-  uint32_t info[NS];        // n_esc | n_p << 8 | attempt << 16 | tgt << 24
+  uint32_t info[NS];        // n_esc | n_p << 8 | attempt << 16 | tgt << 24 (7 bits) | projectile type << 31
   uint32_t cnt[NS];         // pending tracks of the attempt (low 16) | real collisions (high 16)
   uint32_t status[NS];
   typename Fx<R>::T acc[4][NS];   // fixed-point E_in - sum T, p_in - sum p (x, y, z)
@@ -1054,7 +1059,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   auto load_key = [&](int slot, RngKey &g, uint32_t &attempt, int &tgt, int &ev) {
     ev = w.ev[slot];
     const uint32_t m = w.info[slot];
-    attempt = (m >> 16) & 0xFFu; tgt = (int)(m >> 24);
+    attempt = (m >> 16) & 0xFFu; tgt = (int)((m >> 24) & 0x7Fu);
     const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
     g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
   };
@@ -1148,7 +1153,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
           rt.type = mt & 1u; rt.shell = (int)((mt >> 1) & 0x7Fu); rslot = (int)(mt >> 8);
           rev = w.ev[rslot];
           const uint32_t inf = w.info[rslot];
-          rattempt = (inf >> 16) & 0xFFu; rtgt = (int)(inf >> 24);
+          rattempt = (inf >> 16) & 0xFFu; rtgt = (int)((inf >> 24) & 0x7Fu);
           rhas = true;
         }
         nSeg -= take; nRes += take;
@@ -1304,13 +1309,13 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       __syncwarp();
       bool want_event = has && lane >= mE;
       bool do_entry = false;
-      int ev = -1, tgt = 0;
+      int ev = -1, tgt = 0, ptype = 1;
       uint32_t attempt = 0;
       R E_in = R(0);
       if (has && lane < mE) {
         ev = w.ev[slot];
         const uint32_t ne = w.info[slot];
-        attempt = (ne >> 16) & 0xFFu; tgt = (int)(ne >> 24);
+        attempt = (ne >> 16) & 0xFFu; tgt = (int)((ne >> 24) & 0x7Fu); ptype = (int)(ne >> 31);
         E_in = P.E_in[ev];
         const NucDev<R> &nu = s_nuc[tgt];
         const int n_esc = (int)(ne & 0xFFu), n_p = (int)((ne >> 8) & 0xFFu);
@@ -1318,7 +1323,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
         const R Prx = Fx<R>::from(w.acc[1][slot]), Pry = Fx<R>::from(w.acc[2][slot]), Prz = Fx<R>::from(w.acc[3][slot]);
         int A_res, Z_res;
         R Estar;
-        const bool ok = epilogue_eval<R>(nu, P.model.bind, n_esc, n_p, (int)(w.cnt[slot] >> 16), Eavail, Prx, Pry, Prz, keep_transparent, A_res, Z_res, Estar);
+        const bool ok = epilogue_eval<R>(nu, P.model.bind, ptype, n_esc, n_p, (int)(w.cnt[slot] >> 16), Eavail, Prx, Pry, Prz, keep_transparent, A_res, Z_res, Estar);
         if (ok) {
           const uint32_t used = attempt + 1u > 255u ? 255u : attempt + 1u;
           write_cascade_result<R>(P.ws, ev, A_res, Z_res, Estar, Prx, Pry, Prz, (uint32_t)n_esc | (attempt << 8), w.status[slot] | used);
@@ -1347,7 +1352,8 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
             attempt = 0;
             E_in = P.E_in[ev];
             tgt = P.target_id[ev];
-            if (check_inputs<R>(P, s_nuc, ev, E_in, tgt)) { do_entry = true; st.add(S_EVENTS); }
+            ptype = P.projectile ? (int)P.projectile[ev] : 1;
+            if (check_inputs<R>(P, s_nuc, ev, E_in, tgt, ptype)) { do_entry = true; st.add(S_EVENTS); }
           } else {
             got_none = true;
           }
@@ -1370,8 +1376,8 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
         const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
         g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
         R p_in;
-        entry_step<R>(t, s_nuc[tgt], E_in, g, attempt, p_in);
-        w.ev[slot] = ev; w.info[slot] = (attempt << 16) | ((uint32_t)tgt << 24);
+        entry_step<R>(t, s_nuc[tgt], E_in, ptype, g, attempt, p_in);
+        w.ev[slot] = ev; w.info[slot] = (attempt << 16) | ((uint32_t)tgt << 24) | ((uint32_t)ptype << 31);
         w.cnt[slot] = 1u; w.status[slot] = 0;
         w.acc[0][slot] = Fx<R>::to(E_in); w.acc[1][slot] = 0; w.acc[2][slot] = 0; w.acc[3][slot] = Fx<R>::to(p_in);
       }

@@ -75,6 +75,7 @@ struct State {
   int vote_coll = 8, vote_epi = 8;
   int long_seg = kLongSegDefault;
   size_t chunk_events = (size_t)1 << 22;
+  const uint8_t *projectile = nullptr;   // DEVICE, caller-owned; nullptr = protons
   int sm_count = 0;
   std::string err;
 };
@@ -380,12 +381,12 @@ int set_round_keys(uint64_t seed) {
 }
 
 template <bool STATS>
-int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t *tid, uint64_t seed,
+int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t *tid, const uint8_t *proj, uint64_t seed,
                  inc_secondaries *sec, int32_t *counts, inc_residual *res, long long *offsets) {
   const ModelDev<real> model = model_dev();
   // --- cascade ---
   CascadeParams<real> cp;
-  cp.model = model; cp.ws = g.ws; cp.ctr = g.d_ctr; cp.E_in = E_in; cp.target_id = tid;
+  cp.model = model; cp.ws = g.ws; cp.ctr = g.d_ctr; cp.E_in = E_in; cp.target_id = tid; cp.projectile = proj;
   cp.e_base = e_base + g.event_offset; cp.n_chunk = n_chunk; cp.seed_lo = (uint32_t)seed; cp.seed_hi = (uint32_t)(seed >> 32);
   cp.flags = g.flags;
   const bool naive = (g.flags & INC_F_LANE_PER_EVENT) != 0;
@@ -554,8 +555,9 @@ int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64
     const int nc = (int)((n - e0) < (long long)chunk ? (n - e0) : (long long)chunk);
     inc_residual r = *res;
     r.A += e0; r.Z += e0; r.Estar += e0; r.px += e0; r.py += e0; r.pz += e0; r.status += e0;
-    rc = stats ? launch_chunk<true>(e0, nc, E_in + e0, tid + e0, seed, sec, counts + e0, &r, g.d_offsets + e0)
-               : launch_chunk<false>(e0, nc, E_in + e0, tid + e0, seed, sec, counts + e0, &r, g.d_offsets + e0);
+    const uint8_t *pj = g.projectile ? g.projectile + e0 : nullptr;
+    rc = stats ? launch_chunk<true>(e0, nc, E_in + e0, tid + e0, pj, seed, sec, counts + e0, &r, g.d_offsets + e0)
+               : launch_chunk<false>(e0, nc, E_in + e0, tid + e0, pj, seed, sec, counts + e0, &r, g.d_offsets + e0);
     if (rc) return rc;
   }
   CU_TRY(cudaMemcpyAsync(g.d_offsets + n, &g.d_ctr->total_sec, sizeof(long long), cudaMemcpyDeviceToDevice, g.stream));
@@ -576,7 +578,8 @@ int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64
   if (tail.err & 4u) return fail(INC_E_STATE, "internal track-queue overflow in the wavefront cascade kernel (results invalid)");
   if (tail.err) {
     return fail(INC_E_BADARG, std::string("device-side input check failed:") + ((tail.err & 1u) ? " E_in outside [20,250] MeV" : "") +
-                                  ((tail.err & 2u) ? " target_id not initialised" : ""));
+                                  ((tail.err & 2u) ? " target_id not initialised" : "") +
+                                  ((tail.err & 8u) ? " projectile not 0 or 1" : ""));
   }
   if ((long long)tail.total > sec->capacity) {
     char buf[160];
@@ -664,6 +667,11 @@ int inc_get_nucleus(int id, int32_t *A, int32_t *Z, int32_t *ns, double *R, doub
 int inc_set_vote_thresholds(int coll, int epi) {
   if (coll < 1 || coll > 32 || epi < 1 || epi > 32) return fail(INC_E_BADARG, "thresholds must be 1..32");
   g.vote_coll = coll; g.vote_epi = epi;
+  return 0;
+}
+
+int inc_set_projectiles(const uint8_t *projectile) {
+  g.projectile = projectile;
   return 0;
 }
 

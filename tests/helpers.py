@@ -135,7 +135,7 @@ def event_identity(g, o, rel=1e-9):
     return ident.mean() if n else 1.0, max_err, ident
 
 
-def conservation_residuals(r, targets, tid, E_in, mass_fn, species_A, species_Z, species_M, m_p):
+def conservation_residuals(r, targets, tid, E_in, mass_fn, species_A, species_Z, species_M, m_p, projectile=None, m_n=None):
     """Per-event (dA, dZ, dE/E, |dP|/p_in) of any result dict (GPU or oracle)."""
     n = len(r["counts"])
     code = r["species"] & 0x7F
@@ -145,7 +145,8 @@ def conservation_residuals(r, targets, tid, E_in, mass_fn, species_A, species_Z,
     sumA = np.bincount(ev, weights=species_A[code], minlength=n)
     sumZ = np.bincount(ev, weights=species_Z[code], minlength=n)
     dA = sumA + r["A"] - (At + 1)
-    dZ = sumZ + r["Z"] - (Zt + 1)
+    proj = np.ones(n, dtype=np.int64) if projectile is None else np.asarray(projectile, dtype=np.int64)
+    dZ = sumZ + r["Z"] - (Zt + proj)
     m = species_M[code]
     T = r["T"].astype(np.float64)
     pm = np.sqrt(T * (T + 2 * m))
@@ -155,8 +156,9 @@ def conservation_residuals(r, targets, tid, E_in, mass_fn, species_A, species_Z,
     Mt = np.array([mass_fn(a, z) for a, z in targets])[tid]
     P2 = r["px"].astype(np.float64) ** 2 + r["py"].astype(np.float64) ** 2 + r["pz"].astype(np.float64) ** 2
     Eres = np.sqrt((Mres + r["Estar"].astype(np.float64)) ** 2 + P2)
-    Etot = E_in + m_p + Mt
-    p_in = np.sqrt(E_in * (E_in + 2 * m_p))
+    m_in = m_p if projectile is None else np.where(proj == 1, m_p, m_n)
+    Etot = E_in + m_in + Mt
+    p_in = np.sqrt(E_in * (E_in + 2 * m_in))
     dE = (sumE + Eres - Etot) / Etot
     dP = np.sqrt((sp[0] + r["px"]) ** 2 + (sp[1] + r["py"]) ** 2 + (sp[2] + r["pz"] - p_in) ** 2) / p_in
     return dA, dZ, dE, dP

@@ -46,9 +46,9 @@ def _inputs(cfg, n):
     return W.make_inputs(cfg, n)
 
 
-def _assert_conservation(r, targets, tid, E, orc, otables, tol_E, tol_P):
+def _assert_conservation(r, targets, tid, E, orc, otables, tol_E, tol_P, projectile=None):
     dA, dZ, dE, dP = H.conservation_residuals(r, targets, tid, E, _mass_fn(orc, otables), orc.SPECIES_A,
-                                              orc.SPECIES_Z, orc.SPECIES_M, orc.M_P)
+                                              orc.SPECIES_Z, orc.SPECIES_M, orc.M_P, projectile=projectile, m_n=orc.M_N)
     ok = (r["status"] & orc.ST_FAILED) == 0
     assert np.all(dA[ok] == 0) and np.all(dZ[ok] == 0)           # criterion (1): exact
     assert np.max(np.abs(dE[ok])) < tol_E and np.max(dP[ok]) < tol_P
@@ -393,3 +393,40 @@ def test_tallies(gpu, orc, otables, ptables, variant, cfg, n):
         lib.inc_tally(out, off, spec, tl)
         torch.cuda.synchronize()
         assert np.array_equal(tl["dd"].cpu().numpy(), 2 * g["dd"]) and np.array_equal(tl["nuclide"].cpu().numpy(), 2 * g["nuclide"])
+
+
+# ------------------------------------------------------------------------------- NEXT-3: incident neutrons
+@pytest.mark.parametrize("cfg,n", [(3, 6000), (4, 20000)])
+def test_neutron_projectiles(gpu, orc, otables, ptables, cfg, n):
+    """inc_set_projectiles ("nucleon-nucleus"): a mixed proton / neutron batch.  fp64 build identical to the
+    oracle event by event, conservation with the projectile's charge and mass in both builds, scheduling
+    variants identical, the default (no array) unchanged, and a bad species byte is an input error."""
+    import torch
+    E, tid, targets, seed, _ = _inputs(cfg, n)
+    proj = (np.random.default_rng(7).random(n) < 0.5).astype(np.uint8)
+    proj[:64] = 0
+    lib = gpu.load("f64")
+    g = gpu.simulate(lib, targets, E, tid, seed, ptables, projectile=proj)
+    o = orc.simulate(otables, targets, E, tid, seed, projectile=proj)
+    frac, max_err, ident = H.event_identity(g, o, rel=REL_F64)
+    assert frac >= FRAC_IDENTICAL and max_err <= REL_F64
+    assert np.array_equal(g["status"][ident], o["status"][ident])
+    _assert_conservation(g, targets, tid, E, orc, otables, 1e-12, 1e-9, projectile=proj)
+    alt = gpu.simulate(lib, targets, E, tid, seed, ptables, projectile=proj, flags=gpu.F_LANE_STATE_MACHINE)
+    for k in ("species", "T", "counts", "A", "Z", "Estar", "status"):
+        assert np.array_equal(g[k], alt[k]), k
+    # all-ones array == no array
+    a = gpu.simulate(lib, targets, E[:2000], tid[:2000], seed, ptables, projectile=np.ones(2000, dtype=np.uint8))
+    b = gpu.simulate(lib, targets, E[:2000], tid[:2000], seed, ptables)
+    for k in ("species", "T", "counts", "A", "Z", "Estar"):
+        assert np.array_equal(a[k], b[k]), k
+    # production build: conservation and the same discrete outcome for nearly all events
+    lib32 = gpu.load("f32")
+    g32 = gpu.simulate(lib32, targets, E, tid, seed, ptables, projectile=proj)
+    _assert_conservation(g32, targets, tid, E, orc, otables, 2e-6, 2e-4, projectile=proj)
+    same = (g32["counts"] == o["counts"]) & (g32["A"] == o["A"]) & (g32["Z"] == o["Z"])
+    assert same.mean() > 0.95
+    bad = proj.copy(); bad[100] = 2
+    with pytest.raises(gpu.IncError) as ei:
+        gpu.simulate(lib32, targets, E, tid, seed, ptables, projectile=bad)
+    assert ei.value.code == -1 and "projectile" in str(ei.value)
