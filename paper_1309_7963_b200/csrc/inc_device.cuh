@@ -1485,12 +1485,19 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
       }
     }
     if (__ballot_sync(kFull, ev >= 0) == 0) break;
-    if (ev < 0) continue;
-
-    bool finish = cascade_only || !(Es > R(0)) || (status & INC_ST_FAILED);
-    if (!finish) {
+    // The step is written as stages that every lane of the warp walks through, each under its own predicate, with
+    // the rejection loop ended by a vote: the warp is converged again before the two-body kinematics.  (With the
+    // loop left by `break`, the compiler ran everything behind it once per group of lanes that left the loop
+    // together: 2.9 executions per pass at 6 lanes instead of one at 20.)
+    const bool have = ev >= 0;
+    bool finish = have && (cascade_only || !(Es > R(0)) || (status & INC_ST_FAILED));
+    bool sampling = false;      // stage 2 runs for this lane
+    R Bpar = R(0), X = R(0), a = R(1), beta = R(0), V = R(0), BdBj = R(0), s = R(0), T = R(1), areaA = R(0), areaB = R(0);
+    R u1 = R(0), u2 = R(0);
+    int jsel = -1;
+    if (have && !finish) {
       // ---------- E1/E2: channel widths ----------
-      const R Bpar = __ldg(P.model.bind + A * kZmax + Z);
+      Bpar = __ldg(P.model.bind + A * kZmax + Z);
       R Xj[6], sj[6], aj[6];
       EvChan<R> ch[6];
       R s_ref = R(0);
@@ -1503,12 +1510,12 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
         if (Ad >= 1 && Zd >= 0 && Zd <= Ad) {
           const EvChan<R> c = P.model.evch[(Ad * kZmax + Zd) * 6 + j];
           if (c.pref > R(0)) {
-            const R X = Es - Bpar + c.BdBj - c.V;
-            if (X > R(0)) {
+            const R Xc = Es - Bpar + c.BdBj - c.V;
+            if (Xc > R(0)) {
               ch[j] = c;
-              Xj[j] = X;
+              Xj[j] = Xc;
               aj[j] = M<R>::div_(R(Ad), P.model.a_div);
-              sj[j] = R(2) * M<R>::sqrt_(aj[j] * X);
+              sj[j] = R(2) * M<R>::sqrt_(aj[j] * Xc);
               s_ref = sj[j] > s_ref ? sj[j] : s_ref;
               any = true;
             }
@@ -1539,7 +1546,7 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
           // ---------- E3: choose the channel ----------
           R u[4];
           draw4<R>(g, attempt, 0u, kblk++, u);
-          int jsel = -1;
+          u1 = u[1]; u2 = u[2];
           R cum = R(0);
           const R thr = u[0] * Wsum;
           bool done = false;
@@ -1547,71 +1554,78 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
           for (int j = 0; j < 6; ++j) {
             if (!done && W[j] > R(0)) { cum += W[j]; jsel = j; if (thr < cum) done = true; }
           }
-          R X = R(0), a = R(1), beta = R(0), V = R(0), BdBj = R(0);
 #pragma unroll
           for (int j = 0; j < 6; ++j) if (j == jsel) { X = Xj[j]; a = aj[j]; beta = ch[j].beta; V = ch[j].V; BdBj = ch[j].BdBj; }
-          // ---------- E4: rejection sampling of x (two envelopes, R-E4) ----------
-          const R s = R(2) * M<R>::sqrt_(a * X);
-          const R T = M<R>::sqrt_(M<R>::div_(X, a));
-          const R areaA = T * (T + beta), areaB = R(0.5) * X * X + beta * X;
-          R xs = R(-1);
-#pragma unroll 1
-          for (int n = 0; n < kMaxTrial; ++n) {
-            R v[4];
-            draw4<R>(g, attempt, 0u, kblk++, v);
-            if (STATS) n_trials++;
-            R xx;
-            if (areaB < areaA) {
-              xx = -beta + M<R>::sqrt_(beta * beta + v[1] * (X * X + R(2) * beta * X));
-              R rem = X - xx;
-              rem = rem > R(0) ? rem : R(0);
-              if (M<R>::log_(v[3]) < R(2) * M<R>::sqrt_(a * rem) - s) { xs = xx < X ? xx : X; break; }
-            } else {
-              if (v[0] * (T + beta) < T) xx = -T * M<R>::log_(v[1] * v[2]);
-              else xx = -T * M<R>::log_(v[1]);
-              if (xx < X && M<R>::log_(v[3]) < R(2) * M<R>::sqrt_(a * (X - xx)) - s + M<R>::div_(xx, T)) { xs = xx; break; }
-            }
-          }
-          if (xs < R(0)) { status |= INC_ST_TRIAL_CAP; finish = true; }
-          else {
-            // ---------- E5: two-body decay in the parent rest frame, isotropic, boost to lab ----------
-            const int Aj = c_evA[jsel], Zj = c_evZ[jsel];
-            const int Ad = A - Aj, Zd = Z - Zj;
-            const R Bj = __ldg(P.model.bind + Aj * kZmax + Zj);
-            const R Mj = R(Zj) * K<R>::mp + R(Aj - Zj) * K<R>::mn - Bj;
-            const R Bd = BdBj - Bj;
-            const R Esd = X - xs;
-            const R Mds = R(Zd) * K<R>::mp + R(Ad - Zd) * K<R>::mn - Bd + Esd;
-            const R Mpar = R(Z) * K<R>::mp + R(A - Z) * K<R>::mn - Bpar + Es;
-            const R eps = V + xs;   // total kinetic energy released in the parent frame
-            const R p2 = M<R>::div_(eps * (R(2) * Mpar - eps) * (R(2) * Mds + eps) * (R(2) * Mj + eps), R(4) * Mpar * Mpar);
-            const R pm = M<R>::sqrt_(p2 > R(0) ? p2 : R(0));
-            const R Ej = M<R>::sqrt_(p2 + Mj * Mj);
-            const R cth = R(2) * u[1] - R(1);
-            R s2 = R(1) - cth * cth;
-            const R sth = M<R>::sqrt_(s2 > R(0) ? s2 : R(0));
-            R sph, cph;
-            M<R>::sincos2pi(u[2], &sph, &cph);
-            const R qx = pm * sth * cph, qy = pm * sth * sph, qz = pm * cth;
-            const R Epar = M<R>::sqrt_(Mpar * Mpar + Px * Px + Py * Py + Pz * Pz);
-            const R iEp = M<R>::rcp_(Epar);
-            const R bx = Px * iEp, by = Py * iEp, bz = Pz * iEp;
-            const R gam = M<R>::div_(Epar, Mpar);
-            const R gfac = M<R>::div_(gam * gam, gam + R(1));
-            const R fo = gfac * (qx * bx + qy * by + qz * bz) + gam * Ej;
-            const R lx = qx + fo * bx, ly = qy + fo * by, lz = qz + fo * bz;
-            const R l2 = lx * lx + ly * ly + lz * lz;
-            const R El = M<R>::sqrt_(l2 + Mj * Mj);
-            const R Tl = M<R>::div_(l2, El + Mj);
-            const R il = M<R>::rsqrt_(l2);
-            const size_t o = (size_t)ev * kMaxSec + count;
-            stage_write<R>(P.ws.st + o, Tl, lx * il, ly * il, lz * il, 0x80000000u | ((uint32_t)jsel << 24) | (uint32_t)count);
-            count++;
-            if (STATS) n_emit++;
-            A = Ad; Z = Zd; Es = Esd;
-            Px -= lx; Py -= ly; Pz -= lz;
-          }
+          s = R(2) * M<R>::sqrt_(a * X);
+          T = M<R>::sqrt_(M<R>::div_(X, a));
+          areaA = T * (T + beta); areaB = R(0.5) * X * X + beta * X;
+          sampling = true;
         }
+      }
+    }
+    // ---------- E4: rejection sampling of x (two envelopes, R-E4); warp-uniform loop ----------
+    R xs = R(-1);
+    bool pending = sampling;
+#pragma unroll 1
+    for (int n = 0; n < kMaxTrial; ++n) {
+      if (__ballot_sync(kFull, pending) == 0u) break;
+      if (pending) {
+        R v[4];
+        draw4<R>(g, attempt, 0u, kblk++, v);
+        if (STATS) n_trials++;
+        R xx;
+        if (areaB < areaA) {
+          xx = -beta + M<R>::sqrt_(beta * beta + v[1] * (X * X + R(2) * beta * X));
+          R rem = X - xx;
+          rem = rem > R(0) ? rem : R(0);
+          if (M<R>::log_(v[3]) < R(2) * M<R>::sqrt_(a * rem) - s) { xs = xx < X ? xx : X; pending = false; }
+        } else {
+          if (v[0] * (T + beta) < T) xx = -T * M<R>::log_(v[1] * v[2]);
+          else xx = -T * M<R>::log_(v[1]);
+          if (xx < X && M<R>::log_(v[3]) < R(2) * M<R>::sqrt_(a * (X - xx)) - s + M<R>::div_(xx, T)) { xs = xx; pending = false; }
+        }
+      }
+    }
+    __syncwarp();
+    if (sampling) {
+      if (xs < R(0)) { status |= INC_ST_TRIAL_CAP; finish = true; }
+      else {
+        // ---------- E5: two-body decay in the parent rest frame, isotropic, boost to lab ----------
+        const int Aj = c_evA[jsel], Zj = c_evZ[jsel];
+        const int Ad = A - Aj, Zd = Z - Zj;
+        const R Bj = __ldg(P.model.bind + Aj * kZmax + Zj);
+        const R Mj = R(Zj) * K<R>::mp + R(Aj - Zj) * K<R>::mn - Bj;
+        const R Bd = BdBj - Bj;
+        const R Esd = X - xs;
+        const R Mds = R(Zd) * K<R>::mp + R(Ad - Zd) * K<R>::mn - Bd + Esd;
+        const R Mpar = R(Z) * K<R>::mp + R(A - Z) * K<R>::mn - Bpar + Es;
+        const R eps = V + xs;   // total kinetic energy released in the parent frame
+        const R p2 = M<R>::div_(eps * (R(2) * Mpar - eps) * (R(2) * Mds + eps) * (R(2) * Mj + eps), R(4) * Mpar * Mpar);
+        const R pm = M<R>::sqrt_(p2 > R(0) ? p2 : R(0));
+        const R Ej = M<R>::sqrt_(p2 + Mj * Mj);
+        const R cth = R(2) * u1 - R(1);
+        R s2 = R(1) - cth * cth;
+        const R sth = M<R>::sqrt_(s2 > R(0) ? s2 : R(0));
+        R sph, cph;
+        M<R>::sincos2pi(u2, &sph, &cph);
+        const R qx = pm * sth * cph, qy = pm * sth * sph, qz = pm * cth;
+        const R Epar = M<R>::sqrt_(Mpar * Mpar + Px * Px + Py * Py + Pz * Pz);
+        const R iEp = M<R>::rcp_(Epar);
+        const R bx = Px * iEp, by = Py * iEp, bz = Pz * iEp;
+        const R gam = M<R>::div_(Epar, Mpar);
+        const R gfac = M<R>::div_(gam * gam, gam + R(1));
+        const R fo = gfac * (qx * bx + qy * by + qz * bz) + gam * Ej;
+        const R lx = qx + fo * bx, ly = qy + fo * by, lz = qz + fo * bz;
+        const R l2 = lx * lx + ly * ly + lz * lz;
+        const R El = M<R>::sqrt_(l2 + Mj * Mj);
+        const R Tl = M<R>::div_(l2, El + Mj);
+        const R il = M<R>::rsqrt_(l2);
+        const size_t o = (size_t)ev * kMaxSec + count;
+        stage_write<R>(P.ws.st + o, Tl, lx * il, ly * il, lz * il, 0x80000000u | ((uint32_t)jsel << 24) | (uint32_t)count);
+        count++;
+        if (STATS) n_emit++;
+        A = Ad; Z = Zd; Es = Esd;
+        Px -= lx; Py -= ly; Pz -= lz;
       }
     }
     if (finish) {
