@@ -1084,7 +1084,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   Track<R> rt;
   rt.x = rt.y = rt.z = rt.px = rt.py = rt.pz = rt.T = R(0); rt.pi = 0; rt.k = 0; rt.nseg = 0; rt.type = 0; rt.shell = 0;
   int rslot = 0, rev = 0, rtgt = 0;
-  uint32_t rattempt = 0;
+  uint32_t rattempt = 0, rge0 = 0, rge1 = 0;
   bool rhas = false;
   int nRes = 0;   // warp-uniform count of resident tracks
 
@@ -1152,6 +1152,10 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
           rt.k = kn & 0xFFFFu; rt.nseg = (int)(kn >> 16);
           rt.type = mt & 1u; rt.shell = (int)((mt >> 1) & 0x7Fu); rslot = (int)(mt >> 8);
           rev = w.ev[rslot];
+          {
+            const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + rev);
+            rge0 = (uint32_t)ge; rge1 = (uint32_t)(ge >> 32);       // counter words 2, 3 of this track's event
+          }
           const uint32_t inf = w.info[rslot];
           rattempt = (inf >> 16) & 0xFFu; rtgt = (int)((inf >> 24) & 0x7Fu);
           rhas = true;
@@ -1164,8 +1168,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       Escape<R> esc;
       if (rhas) {
         RngKey g;
-        const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + rev);
-        g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
+        g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = rge0; g.e1 = rge1;
         out = seg_step<R, STATS>(rt, s_nuc[rtgt], s_tabS, n_xs, inv_dp, g, rattempt, cc, esc, st);
       }
       {
