@@ -165,8 +165,11 @@ int64_t inc_simulate(int64_t n_events, const INC_REAL *E_in /*DEVICE, MeV*/,
 /* inc_simulate_host — same computation with HOST buffers (every pointer, including those
  * inside the two structs, is host memory).  The library stages inputs to the device,
  * runs inc_simulate and copies the results back, all inside this call (used for the
- * end-to-end number of bench.py).  Pinned host memory makes the copies faster but is not
- * required. */
+ * end-to-end number of bench.py).  It streams: the call runs in chunks of at
+ * most 2^19 events (2^20 for calls above 2^21 events; or inc_set_chunk_events, if smaller), and while one chunk computes on the
+ * caller's stream the outputs of the previous one travel to the host on a second stream, so a
+ * long call costs about max(compute, copy) instead of their sum.  Pinned host memory is what
+ * makes the copies asynchronous; pageable memory works, without the overlap. */
 int64_t inc_simulate_host(int64_t n_events, const INC_REAL *E_in /*HOST*/,
                           const int32_t *target_id /*HOST*/, uint64_t seed,
                           inc_secondaries *out_secondaries /*HOST ptrs*/,

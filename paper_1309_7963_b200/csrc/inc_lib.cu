@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <functional>
 #include <string>
 #include <vector>
 
@@ -62,7 +63,14 @@ struct State {
     real *E = nullptr; int32_t *tid = nullptr, *counts = nullptr, *A = nullptr, *Z = nullptr;
     real *Es = nullptr, *px = nullptr, *py = nullptr, *pz = nullptr; uint32_t *status = nullptr;
     uint8_t *sp = nullptr; real *T = nullptr, *ux = nullptr, *uy = nullptr, *uz = nullptr;
+    // pipelined copies (inc_simulate_host): copy stream, per-chunk events, running totals in pinned host memory
+    cudaStream_t copy_stream = nullptr;
+    unsigned long long *h_tot = nullptr;      // pinned, [kMaxHostChunks]
+    std::vector<cudaEvent_t> ev;
   } hp;
+  size_t host_chunk_events = (size_t)1 << 19;
+  // per-chunk hook of the running call (inc_simulate_host): called after chunk c has been enqueued
+  std::function<int(int, long long, int)> chunk_hook;
   // last call
   long long last_n = -1;
   long long last_total = 0;
@@ -527,6 +535,10 @@ void inc_shutdown(void) {
                 (void **)&g.hp.sp, (void **)&g.hp.T, (void **)&g.hp.ux, (void **)&g.hp.uy, (void **)&g.hp.uz};
   for (auto q : p) { if (*q) cudaFree(*q); *q = nullptr; }
   g.offsets_cap = g.tiles_cap = 0; g.hp.n_cap = g.hp.sec_cap = 0;
+  for (auto e : g.hp.ev) cudaEventDestroy(e);
+  g.hp.ev.clear();
+  if (g.hp.copy_stream) { cudaStreamDestroy(g.hp.copy_stream); g.hp.copy_stream = nullptr; }
+  if (g.hp.h_tot) { cudaFreeHost(g.hp.h_tot); g.hp.h_tot = nullptr; }
   for (auto &n : g.nuc) n.live = false;
   g.tab.captured = false;
   g.last_n = -1;
@@ -541,7 +553,10 @@ int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64
     return fail(INC_E_BADARG, "null residual array");
   if (sec->capacity < 0 || (sec->capacity > 0 && (!sec->species || !sec->T || !sec->ux || !sec->uy || !sec->uz)))
     return fail(INC_E_BADARG, "null secondary array");
-  const size_t chunk_max = g.chunk_events;
+  // inc_simulate_host pipelines chunks against their copies: 2^19 events per chunk, 2^20 for long calls (a chunk
+  // costs one drain phase of the cascade kernel, so they should not be smaller than the copies need)
+  const size_t host_chunk = (size_t)n > ((size_t)1 << 21) ? 2 * g.host_chunk_events : g.host_chunk_events;
+  const size_t chunk_max = g.chunk_hook ? (host_chunk < g.chunk_events ? host_chunk : g.chunk_events) : g.chunk_events;
   const size_t chunk = (size_t)n < chunk_max ? (size_t)(n > 0 ? n : 1) : chunk_max;
   int rc = ensure_ws(chunk, (size_t)n);
   if (rc) return rc;
@@ -559,6 +574,7 @@ int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64
     rc = stats ? launch_chunk<true>(e0, nc, E_in + e0, tid + e0, pj, seed, sec, counts + e0, &r, g.d_offsets + e0)
                : launch_chunk<false>(e0, nc, E_in + e0, tid + e0, pj, seed, sec, counts + e0, &r, g.d_offsets + e0);
     if (rc) return rc;
+    if (g.chunk_hook) { rc = g.chunk_hook((int)(e0 / (long long)chunk), e0, nc); if (rc) return rc; }
   }
   CU_TRY(cudaMemcpyAsync(g.d_offsets + n, &g.d_ctr->total_sec, sizeof(long long), cudaMemcpyDeviceToDevice, g.stream));
   struct { unsigned long long total; unsigned int err, pad; } tail;
@@ -784,25 +800,65 @@ int64_t inc_simulate_host(int64_t n, const INC_REAL *E_in, const int32_t *tid, u
   CU_TRY(cudaMemcpyAsync(h.tid, tid, (size_t)n * 4, cudaMemcpyHostToDevice, g.stream));
   inc_secondaries ds; ds.species = h.sp; ds.T = h.T; ds.ux = h.ux; ds.uy = h.uy; ds.uz = h.uz; ds.capacity = sec->capacity;
   inc_residual dr; dr.A = h.A; dr.Z = h.Z; dr.Estar = h.Es; dr.px = h.px; dr.py = h.py; dr.pz = h.pz; dr.status = h.status;
+  // Streaming: the call runs in chunks of <= 2^19 events; while chunk c+1 computes on the
+  // caller's stream, the outputs of chunk c travel to the host on a second stream.  After each chunk its running
+  // total of secondaries is read back (8 bytes, pinned) behind an event: that is the range of its list.
+  constexpr int kMaxHostChunks = 4096;
+  if (!h.copy_stream) CU_TRY(cudaStreamCreateWithFlags(&h.copy_stream, cudaStreamNonBlocking));
+  if (!h.h_tot) CU_TRY(cudaMallocHost((void **)&h.h_tot, kMaxHostChunks * sizeof(unsigned long long)));
+  struct Pending { long long e0; int nc; int c; };
+  std::vector<Pending> pend;
+  auto copy_chunk = [&](const Pending &q) -> int {
+    CU_TRY(cudaEventSynchronize(h.ev[q.c]));
+    const unsigned long long t1 = h.h_tot[q.c], t0 = q.c ? h.h_tot[q.c - 1] : 0ull;
+    const size_t m = (size_t)q.nc, o = (size_t)q.e0;
+    cudaStream_t cs = h.copy_stream;
+    CU_TRY(cudaMemcpyAsync(counts + o, h.counts + o, m * 4, cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->A + o, h.A + o, m * 4, cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->Z + o, h.Z + o, m * 4, cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->Estar + o, h.Es + o, m * sizeof(real), cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->px + o, h.px + o, m * sizeof(real), cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->py + o, h.py + o, m * sizeof(real), cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->pz + o, h.pz + o, m * sizeof(real), cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->status + o, h.status + o, m * 4, cudaMemcpyDeviceToHost, cs));
+    const unsigned long long cap = (unsigned long long)sec->capacity;
+    const unsigned long long a0 = t0 < cap ? t0 : cap, a1 = t1 < cap ? t1 : cap;     // nothing is written past the capacity
+    if (a1 > a0) {
+      const size_t k = (size_t)(a1 - a0), f = (size_t)a0;
+      CU_TRY(cudaMemcpyAsync(sec->species + f, h.sp + f, k, cudaMemcpyDeviceToHost, cs));
+      CU_TRY(cudaMemcpyAsync(sec->T + f, h.T + f, k * sizeof(real), cudaMemcpyDeviceToHost, cs));
+      CU_TRY(cudaMemcpyAsync(sec->ux + f, h.ux + f, k * sizeof(real), cudaMemcpyDeviceToHost, cs));
+      CU_TRY(cudaMemcpyAsync(sec->uy + f, h.uy + f, k * sizeof(real), cudaMemcpyDeviceToHost, cs));
+      CU_TRY(cudaMemcpyAsync(sec->uz + f, h.uz + f, k * sizeof(real), cudaMemcpyDeviceToHost, cs));
+    }
+    return 0;
+  };
+  g.chunk_hook = [&](int c, long long e0, int nc) -> int {
+    if (c >= kMaxHostChunks) return fail(INC_E_BADARG, "inc_simulate_host: too many chunks (raise the chunk size)");
+    while ((int)h.ev.size() <= c) {
+      cudaEvent_t e;
+      CU_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+      h.ev.push_back(e);
+    }
+    CU_TRY(cudaMemcpyAsync(&h.h_tot[c], &g.d_ctr->total_sec, sizeof(unsigned long long), cudaMemcpyDeviceToHost, g.stream));
+    CU_TRY(cudaEventRecord(h.ev[c], g.stream));
+    if (!pend.empty()) {            // chunk c is enqueued: now wait for chunk c-1 and send its outputs home
+      const Pending q = pend.back();
+      pend.pop_back();
+      if (int rc = copy_chunk(q)) return rc;
+    }
+    pend.push_back(Pending{e0, nc, c});
+    return 0;
+  };
   const int64_t tot = inc_simulate(n, h.E, h.tid, seed, &ds, h.counts, &dr);
-  if (tot < 0 && tot != INC_E_CAPACITY) return tot;
-  const size_t m = (size_t)n;
-  CU_TRY(cudaMemcpyAsync(counts, h.counts, m * 4, cudaMemcpyDeviceToHost, g.stream));
-  CU_TRY(cudaMemcpyAsync(res->A, h.A, m * 4, cudaMemcpyDeviceToHost, g.stream));
-  CU_TRY(cudaMemcpyAsync(res->Z, h.Z, m * 4, cudaMemcpyDeviceToHost, g.stream));
-  CU_TRY(cudaMemcpyAsync(res->Estar, h.Es, m * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
-  CU_TRY(cudaMemcpyAsync(res->px, h.px, m * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
-  CU_TRY(cudaMemcpyAsync(res->py, h.py, m * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
-  CU_TRY(cudaMemcpyAsync(res->pz, h.pz, m * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
-  CU_TRY(cudaMemcpyAsync(res->status, h.status, m * 4, cudaMemcpyDeviceToHost, g.stream));
-  if (tot >= 0) {
-    const size_t k = (size_t)tot;
-    CU_TRY(cudaMemcpyAsync(sec->species, h.sp, k, cudaMemcpyDeviceToHost, g.stream));
-    CU_TRY(cudaMemcpyAsync(sec->T, h.T, k * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
-    CU_TRY(cudaMemcpyAsync(sec->ux, h.ux, k * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
-    CU_TRY(cudaMemcpyAsync(sec->uy, h.uy, k * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
-    CU_TRY(cudaMemcpyAsync(sec->uz, h.uz, k * sizeof(real), cudaMemcpyDeviceToHost, g.stream));
+  g.chunk_hook = nullptr;
+  if (tot < 0 && tot != INC_E_CAPACITY) { cudaStreamSynchronize(h.copy_stream); return tot; }
+  while (!pend.empty()) {
+    const Pending q = pend.back();
+    pend.pop_back();
+    if (int rc = copy_chunk(q)) return rc;
   }
+  CU_TRY(cudaStreamSynchronize(h.copy_stream));
   CU_TRY(cudaStreamSynchronize(g.stream));
   return tot;
 }

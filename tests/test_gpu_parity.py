@@ -430,3 +430,39 @@ def test_neutron_projectiles(gpu, orc, otables, ptables, cfg, n):
     with pytest.raises(gpu.IncError) as ei:
         gpu.simulate(lib32, targets, E, tid, seed, ptables, projectile=bad)
     assert ei.value.code == -1 and "projectile" in str(ei.value)
+
+
+def test_host_path_streams_in_chunks(gpu, ptables):
+    """inc_simulate_host pipelines chunks (copy of chunk c overlaps the compute of chunk c+1): with 4096-event
+    chunks a 20000-event call goes through five of them and must equal the device-buffer call bit for bit,
+    including the case where the secondary capacity is too small (INC_E_CAPACITY, nothing past it written)."""
+    import torch
+    E, tid, targets, seed, _ = _inputs(4, 20000)
+    lib = gpu.load("f32")
+    ref = gpu.simulate(lib, targets, E, tid, seed, ptables)
+    slots = np.asarray([lib.inc_init(a, z, ptables) for a, z in targets], dtype=np.int32)   # same slots again
+    lib.inc_shutdown()
+    slots = np.asarray([lib.inc_init(a, z, ptables) for a, z in targets], dtype=np.int32)
+    lib.inc_set_stream(); lib.inc_set_flags(0)
+    n = len(E)
+    Eh = torch.as_tensor(np.asarray(E, dtype=lib.real)).pin_memory()
+    th = torch.as_tensor(slots[np.asarray(tid)]).pin_memory()
+    try:
+        lib.inc_set_chunk_events(4096)
+        outh = lib.alloc_outputs(n, n * 24, device="cpu")
+        tot = lib.inc_simulate_host(Eh, th, seed, outh)
+        small = lib.alloc_outputs(n, ref["total"] // 2, device="cpu")
+        for k in ("species",):
+            small[k].fill_(255)
+        rc = lib.inc_simulate_host(Eh, th, seed, small, check=False)
+    finally:
+        lib.inc_set_chunk_events(0)
+    assert tot == ref["total"]
+    for k in ("counts", "A", "Z", "Estar", "px", "py", "pz"):
+        assert np.array_equal(outh[k].numpy(), ref[k]), k
+    for k in ("species", "T", "ux", "uy", "uz"):
+        assert np.array_equal(outh[k].numpy()[:tot], ref[k]), k
+    assert rc == -3
+    half = ref["total"] // 2
+    assert np.array_equal(small["counts"].numpy(), ref["counts"])
+    assert np.array_equal(small["T"].numpy()[:half], ref["T"][:half])
