@@ -122,7 +122,7 @@ double orc_lerp_table(const double *y, int n, double plab_max, double plab) {
   return y[k] + f * (y[k + 1] - y[k]);
 }
 
-static double lerp_z(const double *zz, const double *y, int n, double z) {
+double orc_lerp_z(const double *zz, const double *y, int n, double z) {
   /* Dostrovsky parameters vs Z_d: linear, clamped outside the grid (R-T) */
   if (z <= zz[0]) return y[0];
   if (z >= zz[n - 1]) return y[n - 1];
@@ -356,10 +356,10 @@ double orc_evap_widths(int A, int Z, double Estar, const orc_tables *t,
       V[j] = 0.0;
     } else {
       double zd = (double)Zd;
-      double kp = lerp_z(t->ev_Z, t->ev_kp, t->n_evz, zd);
-      double cp = lerp_z(t->ev_Z, t->ev_cp, t->n_evz, zd);
-      double ka = lerp_z(t->ev_Z, t->ev_ka, t->n_evz, zd);
-      double ca = lerp_z(t->ev_Z, t->ev_ca, t->n_evz, zd);
+      double kp = orc_lerp_z(t->ev_Z, t->ev_kp, t->n_evz, zd);
+      double cp = orc_lerp_z(t->ev_Z, t->ev_cp, t->n_evz, zd);
+      double ka = orc_lerp_z(t->ev_Z, t->ev_ka, t->n_evz, zd);
+      double ca = orc_lerp_z(t->ev_Z, t->ev_ca, t->n_evz, zd);
       double k, c, rj;
       switch (j) {
         case 1: k = kp; c = cp; rj = 0.0; break;
@@ -384,6 +384,16 @@ double orc_evap_widths(int A, int Z, double Estar, const orc_tables *t,
     sum += W[j];
   }
   return sum;
+}
+
+/* E3: channel by cumulative sum over j in the E1 order against u_ch * Sum W (R-E3) */
+int orc_evap_choose(const double W[6], double Wsum, double u_ch) {
+  int j = -1;
+  double cum = 0.0, thr = u_ch * Wsum;
+  for (int q = 0; q < 6; ++q) {
+    if (W[q] > 0.0) { cum += W[q]; j = q; if (thr < cum) break; }
+  }
+  return j;
 }
 
 double orc_evap_sample_x(double a, double X, double beta, const uint32_t key[2],
@@ -463,9 +473,14 @@ static int cmp_esc(const void *a, const void *b) {
 #define STACK_MAX 256
 
 /* One cascade attempt (C0-C5).  Returns n_real; fills esc[0..*n_esc). */
+/* trace: optional log of every collision of the attempt (decision inputs and outcomes), filled only for
+ * orc_cascade_trace -- the window through which the pins check the C2/C3 wiring (which table, which species'
+ * E_F, which cutoff, which child codes).  Recording changes nothing of the attempt. */
+typedef struct { orc_coll_rec *rec; int cap, n; } coll_trace;
+
 static int cascade_attempt(const orc_tables *t, const orc_nucleus *nu, const rng_ctx *g,
                            uint32_t attempt, double E_in, int proj, uint32_t flags,
-                           esc_rec *esc, int *n_esc, uint32_t *status, orc_stats *st) {
+                           esc_rec *esc, int *n_esc, uint32_t *status, orc_stats *st, coll_trace *trc) {
   int ns = nu->n_shells;
   int n_real = 0;
   *n_esc = 0;
@@ -534,13 +549,25 @@ static int cascade_attempt(const orc_tables *t, const orc_nucleus *nu, const rng
         double B = orc_lerp_table(same ? t->B_pp : t->B_np, t->n_xs, t->plab_max, plab);
         double ab = same ? 0.0 : orc_lerp_table(t->a_np, t->n_xs, t->plab_max, plab);
         double q1[3], q2[3];
-        orc_collide(tr.p, m1, p2, m2, B, ab, same, u[1], u[2], u[3], q1, q2, NULL);
+        double ct_cm;
+        orc_collide(tr.p, m1, p2, m2, B, ab, same, u[1], u[2], u[3], q1, q2, &ct_cm);
         double T1 = sqrt(dot3(q1, q1) + m1 * m1) - m1;
         double T2 = sqrt(dot3(q2, q2) + m2 * m2) - m2;
         double EF1 = tr.type ? nu->EF_p[i] : nu->EF_n[i];
         double EF2 = t2 ? nu->EF_p[i] : nu->EF_n[i];
+        orc_coll_rec *lg = NULL;
+        if (trc && trc->n < trc->cap) {
+          lg = &trc->rec[trc->n];
+          lg->pi = tr.pi; lg->k = tr.k - 1u; lg->shell = i; lg->type1 = tr.type; lg->type2 = t2;
+          lg->blocked = 0; lg->keep1 = 0; lg->keep2 = 0;
+          lg->T_in = sqrt(dot3(tr.p, tr.p) + m1 * m1) - m1;
+          lg->plab = plab; lg->B = B; lg->a_back = ab; lg->Sp = Sp; lg->Sigma = Sigma;
+          lg->T1 = T1; lg->T2 = T2; lg->costheta = ct_cm;
+        }
+        if (trc) trc->n++;
         if (!(T1 > EF1 && T2 > EF2)) {           /* Pauli, strict > (R-Q12) */
           if (st) st->blocked++;
+          if (lg) lg->blocked = 1;
           continue;                              /* projectile continues unchanged (R-Q13) */
         }
         n_real++;
@@ -565,6 +592,7 @@ static int cascade_attempt(const orc_tables *t, const orc_nucleus *nu, const rng
           double eps = Tc - Vc;
           double cut = ch[c].type ? nu->EC : 0.0;
           if (eps <= cut) { if (st) st->absorbed++; continue; }
+          if (lg) { if (c == 0) lg->keep1 = 1; else lg->keep2 = 1; }
           if (sp < STACK_MAX) stack[sp++] = ch[c];
         }
       } else {
@@ -592,6 +620,36 @@ static int cascade_attempt(const orc_tables *t, const orc_nucleus *nu, const rng
       }
     }
   }
+  return n_real;
+}
+
+/* One cascade attempt (C0-C5) of one event with its collision log and its escaped list in ascending path
+ * code.  For the pins of the decision logic; orc_simulate runs the very same cascade_attempt. */
+int orc_cascade_trace(const orc_tables *t, const orc_nucleus *nu, uint64_t seed, uint64_t event, uint32_t attempt,
+                      double E_in, int proj, uint32_t flags,
+                      int cap_coll, orc_coll_rec *coll, int *n_coll,
+                      uint32_t *esc_pi, int32_t *esc_type, double *esc_T, double *esc_p, int *n_esc_out,
+                      uint32_t *status) {
+  if (!t || !nu || !n_coll || !n_esc_out || (proj != 0 && proj != 1)) return -1;
+  rng_ctx g;
+  g.key[0] = (uint32_t)seed; g.key[1] = (uint32_t)(seed >> 32);
+  g.c2 = (uint32_t)event; g.c3 = (uint32_t)(event >> 32);
+  g.st = NULL;
+  esc_rec esc[ORC_MAX_SEC];
+  int n_esc = 0;
+  uint32_t st_try = 0;
+  coll_trace trc = {coll, coll ? cap_coll : 0, 0};
+  int n_real = cascade_attempt(t, nu, &g, attempt, E_in, proj, flags, esc, &n_esc, &st_try, NULL, &trc);
+  qsort(esc, (size_t)n_esc, sizeof(esc_rec), cmp_esc);
+  for (int k = 0; k < n_esc; ++k) {
+    if (esc_pi) esc_pi[k] = esc[k].pi;
+    if (esc_type) esc_type[k] = esc[k].type;
+    if (esc_T) esc_T[k] = esc[k].T;
+    if (esc_p) { esc_p[3 * k] = esc[k].p[0]; esc_p[3 * k + 1] = esc[k].p[1]; esc_p[3 * k + 2] = esc[k].p[2]; }
+  }
+  *n_coll = trc.n;
+  *n_esc_out = n_esc;
+  if (status) *status = st_try;
   return n_real;
 }
 
@@ -633,7 +691,7 @@ int64_t orc_simulate(const orc_tables *t, const orc_nucleus *nuc, int n_nuc,
     for (attempt = 0; attempt < ORC_MAX_ATTEMPT; ++attempt) {
       if (stats) stats->attempts++;
       uint32_t st_try = 0;
-      int n_real = cascade_attempt(t, nu, &g, attempt, Ein, proj, flags, esc, &n_esc, &st_try, stats);
+      int n_real = cascade_attempt(t, nu, &g, attempt, Ein, proj, flags, esc, &n_esc, &st_try, stats, NULL);
       /* C6: epilogue — sums in ascending path-code order */
       qsort(esc, (size_t)n_esc, sizeof(esc_rec), cmp_esc);
       int n_p = 0;
@@ -692,11 +750,7 @@ int64_t orc_simulate(const orc_tables *t, const orc_nucleus *nuc, int n_nuc,
           if (stats) stats->evap_steps++;
           double u[4];
           draw4(&g, attempt, 0u, k++, u);        /* E3: (u_ch, u_cos, u_phi, -) */
-          int j = -1;                            /* cumulative sum over j in the E1 order */
-          double cum = 0.0, thr = u[0] * Wsum;
-          for (int q = 0; q < 6; ++q) {
-            if (W[q] > 0.0) { cum += W[q]; j = q; if (thr < cum) break; }
-          }
+          int j = orc_evap_choose(W, Wsum, u[0]);
           int trials = 0;
           double x = orc_evap_sample_x(a_d[j], X[j], beta[j], g.key, c1, g.c2, g.c3, &k, &trials);
           if (stats) { stats->evap_trials += (uint64_t)trials; stats->philox_blocks += (uint64_t)trials; }

@@ -96,6 +96,26 @@ int64_t orc_simulate(const orc_tables *t, const orc_nucleus *nuc, int n_nuc,
                      int32_t *casc_count, orc_stats *stats,
                      const uint8_t *projectile /* [n] 0 = neutron, 1 = proton; NULL = all protons (NEXT-3) */);
 
+/* ---- one cascade attempt with its collision log (for the pins of the C2/C3 decision logic) ---- */
+typedef struct orc_coll_rec {     /* one collision (C3), allowed or blocked */
+  uint32_t pi, k;                 /* path code of the projectile track, Philox block of the collision */
+  int32_t shell, type1, type2;    /* collision shell; species of the projectile and of the partner (1 = p) */
+  int32_t blocked, keep1, keep2;  /* Pauli-blocked; scattered projectile / recoil survived the cutoff */
+  double T_in;                    /* kinetic energy of the projectile before the collision */
+  double plab, B, a_back;         /* GeV/c; slope and np backward weight read from the tables */
+  double Sp, Sigma;               /* rho_p sigma_p and the total macroscopic cross section, fm^-1 */
+  double T1, T2, costheta;        /* kinetic energies after the collision; cos(theta_cm) */
+} orc_coll_rec;
+/* Runs attempt `attempt` of global event `event` (R-R2 counters) and returns n_real (allowed collisions), or
+ * -1 on bad arguments.  coll[0..min(*n_coll, cap_coll)) are the collisions in processing order (*n_coll counts
+ * all of them); esc_* (each nullable, capacity ORC_MAX_SEC; esc_p is [3 * ORC_MAX_SEC]) the escaped particles in
+ * ascending path code. */
+int orc_cascade_trace(const orc_tables *t, const orc_nucleus *nu, uint64_t seed, uint64_t event, uint32_t attempt,
+                      double E_in, int proj, uint32_t flags,
+                      int cap_coll, orc_coll_rec *coll, int *n_coll,
+                      uint32_t *esc_pi, int32_t *esc_type, double *esc_T, double *esc_p, int *n_esc,
+                      uint32_t *status);
+
 /* ---- single steps, exported so the pins can test each in isolation ----------- */
 void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 double orc_u01(uint32_t x);                                   /* R-R3 */
@@ -103,6 +123,8 @@ int orc_valid_nucleus(int A, int Z);
 double orc_binding(int A, int Z, const orc_tables *t);        /* MeV; NaN if invalid */
 double orc_mass(int A, int Z, const orc_tables *t);
 double orc_lerp_table(const double *y, int n, double plab_max, double plab);
+/* R-T: Dostrovsky k, c versus daughter charge: linear in Z_d, clamped outside the grid */
+double orc_lerp_z(const double *zz, const double *y, int n, double z);
 /* R-C2 partner: p2 = pF * cbrt(u_mag) * n(u_cos,u_phi) */
 void orc_partner(double pF, double u_mag, double u_cos, double u_phi, double p2[3]);
 /* R-C2: partner-rest-frame momentum (GeV/c) of particle 1 */
@@ -122,6 +144,8 @@ int orc_boundary(const double x[3], double p[3], double m, double V_from, double
 double orc_evap_widths(int A, int Z, double Estar, const orc_tables *t,
                        double W[6], double X[6], double Q[6], double V[6],
                        double beta[6], double a_d[6]);
+/* R-E3: channel chosen by the cumulative sum of W in the E1 order against u_ch * Wsum; -1 if no W > 0 */
+int orc_evap_choose(const double W[6], double Wsum, double u_ch);
 /* R-E4: sample x in [0,X] from (x+beta)exp(2 sqrt(a (X-x))) using Philox stream
  * (key, ctr base c1,c2,c3) starting at block *k; returns x, advances *k, *trials. */
 double orc_evap_sample_x(double a, double X, double beta, const uint32_t key[2],

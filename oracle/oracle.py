@@ -16,8 +16,10 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRC = os.path.join(_HERE, "inc_oracle.c")
-_LIB = os.path.join(_HERE, "libinc_oracle.so")
+# INC_ORACLE_SRC / INC_ORACLE_LIB: tests/test_pins_bite.py points them at a deliberately broken copy of the
+# oracle to prove that the pins notice it
+_SRC = os.environ.get("INC_ORACLE_SRC", os.path.join(_HERE, "inc_oracle.c"))
+_LIB = os.environ.get("INC_ORACLE_LIB", os.path.join(_HERE, "libinc_oracle.so"))
 
 MAX_SHELLS = 32
 MAX_SEC = 64
@@ -47,7 +49,7 @@ def build(force: bool = False) -> str:
             and os.path.getmtime(_LIB) >= max(os.path.getmtime(_SRC), os.path.getmtime(hdr))):
         return _LIB
     cmd = ["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
-           "-o", _LIB, _SRC, "-lm"]
+           "-I", _HERE, "-o", _LIB, _SRC, "-lm"]
     subprocess.check_call(cmd)
     return _LIB
 
@@ -87,6 +89,17 @@ _STAT_FIELDS = ["events", "failed", "attempts", "retry_transparent", "retry_inva
                 "retry_estar", "segments", "boundaries", "reflections", "escapes",
                 "collisions", "blocked", "allowed", "absorbed", "evap_steps", "evap_trials",
                 "evap_emitted", "cap_seg", "cap_depth", "cap_sec", "cap_trial", "philox_blocks"]
+
+
+class OrcCollRec(C.Structure):
+    _fields_ = [("pi", C.c_uint32), ("k", C.c_uint32), ("shell", C.c_int32), ("type1", C.c_int32), ("type2", C.c_int32),
+                ("blocked", C.c_int32), ("keep1", C.c_int32), ("keep2", C.c_int32),
+                ("T_in", C.c_double), ("plab", C.c_double), ("B", C.c_double), ("a_back", C.c_double),
+                ("Sp", C.c_double), ("Sigma", C.c_double), ("T1", C.c_double), ("T2", C.c_double), ("costheta", C.c_double)]
+
+
+COLL_DTYPE = np.dtype([(n, np.uint32 if t is C.c_uint32 else np.int32 if t is C.c_int32 else np.float64)
+                       for n, t in OrcCollRec._fields_], align=True)
 
 
 class OrcStats(C.Structure):
@@ -147,6 +160,15 @@ def lib():
     L.orc_evap_emit.argtypes = [C.c_int, C.c_int, C.c_double, dp, C.c_int, C.c_double, C.c_double,
                                 C.c_double, C.c_double, C.POINTER(OrcTables), dp, dp, dp]
     L.orc_evap_emit.restype = None
+    L.orc_lerp_z.argtypes = [dp, dp, C.c_int, C.c_double]
+    L.orc_lerp_z.restype = C.c_double
+    L.orc_evap_choose.argtypes = [dp, C.c_double, C.c_double]
+    L.orc_evap_choose.restype = C.c_int
+    L.orc_cascade_trace.argtypes = [C.POINTER(OrcTables), C.POINTER(OrcNucleus), C.c_uint64, C.c_uint64, C.c_uint32,
+                                    C.c_double, C.c_int, C.c_uint32, C.c_int, C.c_void_p, C.POINTER(C.c_int),
+                                    C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int),
+                                    C.POINTER(C.c_uint32)]
+    L.orc_cascade_trace.restype = C.c_int
     _lib = L
     return L
 
@@ -154,20 +176,27 @@ def lib():
 # ----------------------------------------------------------------------------------
 # Oracle's own model-input tables (R-T in DESIGN.md).  p in GeV/c, sigma in mb.
 # ----------------------------------------------------------------------------------
+SIGMA_P_FLOOR = 0.1   # GeV/c; the p -> 0 divergence of the lowest branches is cut here (R-T)
+
+
 def cugnon_sigma_pp(p):
     p = np.asarray(p, dtype=np.float64)
-    lo = 23.5 + 1000.0 * (p - 0.7) ** 4
+    pc = np.clip(p, SIGMA_P_FLOOR, None)
+    vlo = 34.0 * (pc / 0.4) ** (-2.104)                       # p < 0.44
+    lo = 23.5 + 1000.0 * (p - 0.7) ** 4                       # 0.44 <= p < 0.8
     mid = 1250.0 / (p + 50.0) - 4.0 * (p - 1.3) ** 2
     hi = 77.0 / (p + 1.5)
-    return np.where(p < 0.8, lo, np.where(p < 2.0, mid, hi))
+    return np.where(p < 0.44, vlo, np.where(p < 0.8, lo, np.where(p < 2.0, mid, hi)))
 
 
 def cugnon_sigma_np(p):
     p = np.asarray(p, dtype=np.float64)
-    lo = 33.0 + 196.0 * np.abs(p - 0.95) ** 2.5
+    pc = np.clip(p, SIGMA_P_FLOOR, None)
+    vlo = 6.3555 * pc ** (-3.2481) * np.exp(-0.377 * np.log(pc) ** 2)   # p < 0.45
+    lo = 33.0 + 196.0 * np.abs(p - 0.95) ** 2.5                         # 0.45 <= p < 0.8
     mid = 31.0 / np.sqrt(np.maximum(p, 0.8))
     hi = 77.0 / (p + 1.5)
-    return np.where(p < 0.8, lo, np.where(p < 2.0, mid, hi))
+    return np.where(p < 0.45, vlo, np.where(p < 0.8, lo, np.where(p < 2.0, mid, hi)))
 
 
 def cugnon_B_pp(p):
@@ -291,6 +320,26 @@ def simulate(tables: Tables, nuclei, E_in, target, seed, e0=0, flags=0, want_sta
                 offsets=offsets, A=rA, Z=rZ, Estar=rE, px=rpx, py=rpy, pz=rpz, status=status,
                 casc_A=cA, casc_Z=cZ, casc_Estar=cE, casc_P=cP, casc_count=cN,
                 stats=st.as_dict() if want_stats else None, total=int(tot))
+
+
+def cascade_trace(tables: Tables, nucleus, seed, event, attempt, E_in, proj=1, flags=0, cap_coll=512):
+    """One cascade attempt of one event with its collision log (numpy structured array, COLL_DTYPE) and its
+    escaped particles in ascending path code.  nucleus: (A, Z) or OrcNucleus."""
+    assert C.sizeof(OrcCollRec) == COLL_DTYPE.itemsize
+    nu = nucleus if isinstance(nucleus, OrcNucleus) else setup_nucleus(nucleus[0], nucleus[1], tables)
+    coll = np.zeros(cap_coll, dtype=COLL_DTYPE)
+    pi = np.zeros(MAX_SEC, dtype=np.uint32); typ = np.zeros(MAX_SEC, dtype=np.int32)
+    T = np.zeros(MAX_SEC); p = np.zeros((MAX_SEC, 3))
+    nc, ne, st = C.c_int(0), C.c_int(0), C.c_uint32(0)
+    vp = lambda a: a.ctypes.data_as(C.c_void_p)
+    n_real = lib().orc_cascade_trace(C.byref(tables.c), C.byref(nu), C.c_uint64(int(seed)), C.c_uint64(int(event)),
+                                     C.c_uint32(int(attempt)), float(E_in), int(proj), C.c_uint32(int(flags)), cap_coll,
+                                     vp(coll), C.byref(nc), vp(pi), vp(typ), vp(T), vp(p), C.byref(ne), C.byref(st))
+    if n_real < 0:
+        raise ValueError("orc_cascade_trace: bad arguments")
+    assert nc.value <= cap_coll, "collision log truncated: raise cap_coll"
+    k = ne.value
+    return dict(n_real=n_real, coll=coll[:nc.value], esc_pi=pi[:k], esc_type=typ[:k], esc_T=T[:k], esc_p=p[:k], status=st.value)
 
 
 def tally_reference(species, T, uz, counts, A_res, Z_res, n_T=50, T_max=250.0, n_cos=20, mult_max=24,

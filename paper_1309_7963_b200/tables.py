@@ -12,6 +12,7 @@ import numpy as np
 
 N_XS = 1025
 PLAB_MAX = 2.048            # GeV/c -> 2 MeV/c grid step
+P_FLOOR = 0.1               # GeV/c: the low-momentum cross sections are held constant below this
 WS_C0, WS_DELTA, WS_RPAD, N_SHELLS = 1.07, 0.545, 2.5, 15
 SEMF = (15.75, 17.8, 0.711, 23.7, 11.18)                       # a_v a_s a_c a_a a_p, MeV
 EVAP_R0, EVAP_RJ, EVAP_A_DIV = 1.5, 1.2, 8.0
@@ -29,13 +30,16 @@ def _piecewise(p, edges, funcs):
 
 def nn_tables(n_xs: int = N_XS, plab_max: float = PLAB_MAX) -> dict:
     """Elastic NN cross sections and angular-distribution parameters on the p_lab grid."""
-    p = np.linspace(0.0, plab_max, n_xs)
     p = np.arange(n_xs, dtype=np.float64) * (plab_max / (n_xs - 1))
-    sig_pp = _piecewise(p, [0.8, 2.0], [
+    # low-momentum branches of ref. [17] below 0.44 (pp) / 0.45 (np) GeV/c, where they meet the next branch to
+    # ~1 %; both diverge for p -> 0, so knots below P_FLOOR carry the value at P_FLOOR (T_lab ~ 5 MeV)
+    sig_pp = _piecewise(p, [0.44, 0.8, 2.0], [
+        lambda q: 34.0 * (np.maximum(q, P_FLOOR) / 0.4) ** -2.104,
         lambda q: 23.5 + 1000.0 * (q - 0.7) ** 4,
         lambda q: 1250.0 / (q + 50.0) - 4.0 * (q - 1.3) ** 2,
         lambda q: 77.0 / (q + 1.5)])
-    sig_np = _piecewise(p, [0.8, 2.0], [
+    sig_np = _piecewise(p, [0.45, 0.8, 2.0], [
+        lambda q: 6.3555 * np.maximum(q, P_FLOOR) ** -3.2481 * np.exp(-0.377 * np.log(np.maximum(q, P_FLOOR)) ** 2),
         lambda q: 33.0 + 196.0 * np.abs(q - 0.95) ** 2.5,
         lambda q: 31.0 / np.sqrt(q),
         lambda q: 77.0 / (q + 1.5)])

@@ -30,9 +30,9 @@ CONFIGS = {
 def make_inputs(config_id: int, n: int | None = None):
     """Return (E_in float64[n], target_id int32[n], targets [(A,Z)], seed, name).
 
-    target_id indexes `targets` (the caller maps it onto inc_init slots).  A prefix of a
-    config (n smaller than the config's) is the prefix of the full arrays, so slices are
-    consistent with full runs.
+    target_id indexes `targets` (the caller maps it onto inc_init slots).  Energies and targets
+    come from two independent streams of the config's seed, so a prefix of a config (n smaller
+    than the config's) is the prefix of the full arrays and slices are consistent with full runs.
     """
     c = CONFIGS[config_id]
     n_full = c["n"]
@@ -47,7 +47,8 @@ def make_inputs(config_id: int, n: int | None = None):
     if len(c["targets"]) > 1:
         w = np.asarray(c["weights"], dtype=np.float64)
         cdf = np.cumsum(w / w.sum())
-        tid = np.minimum(np.searchsorted(cdf, rng.random(m), side="right"), len(w) - 1).astype(np.int32)
+        rng_t = np.random.Generator(np.random.PCG64(np.random.SeedSequence(c["seed"], spawn_key=(1,))))
+        tid = np.minimum(np.searchsorted(cdf, rng_t.random(m), side="right"), len(w) - 1).astype(np.int32)
     else:
         tid = np.zeros(m, dtype=np.int32)
     return E, tid, list(c["targets"]), c["seed"], c["name"]

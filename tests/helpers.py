@@ -162,3 +162,34 @@ def conservation_residuals(r, targets, tid, E_in, mass_fn, species_A, species_Z,
     dE = (sumE + Eres - Etot) / Etot
     dP = np.sqrt((sp[0] + r["px"]) ** 2 + (sp[1] + r["py"]) ** 2 + (sp[2] + r["pz"] - p_in) ** 2) / p_in
     return dA, dZ, dE, dP
+
+
+def blocked_indicator_independent(T1, m1, m2, pF2, EF1, EF2, B, f, ck, phik, ut, phi):
+    """Independent restatement with Lorentz scalars only (no vector boosts/rotations):
+    E1' = gamma (E1cm + beta pcm (cos th cos al + sin th sin al cos phi)), E2' = E - E1'."""
+    p1 = np.sqrt(T1 * (T1 + 2 * m1))
+    E1 = T1 + m1
+    p2 = pF2 * f
+    E2 = np.hypot(p2, m2)
+    sk = np.sqrt(1 - ck * ck)
+    p2v = (p2 * sk * np.cos(phik), p2 * sk * np.sin(phik), p2 * ck)
+    Px, Py, Pz = p2v[0], p2v[1], p2v[2] + p1
+    E = E1 + E2
+    P2 = Px * Px + Py * Py + Pz * Pz
+    s = E * E - P2
+    beta = np.sqrt(P2) / E
+    gamma = E / np.sqrt(s)
+    pcm = np.sqrt((s - (m1 + m2) ** 2) * (s - (m1 - m2) ** 2) / (4 * s))
+    E1cm = (s + m1 * m1 - m2 * m2) / (2 * np.sqrt(s))
+    p1par = p1 * Pz / np.sqrt(P2)                     # component of p1 along the CM velocity
+    cos_al = gamma * (p1par - beta * E1) / pcm
+    cos_al = np.clip(cos_al, -1, 1)
+    sin_al = np.sqrt(1 - cos_al ** 2)
+    pg2 = pcm * pcm * 1e-6
+    tmin = -4 * pg2
+    t = np.log1p(-ut * (1 - np.exp(B * tmin))) / B
+    cth = 1 + t / (2 * pg2)
+    sth = np.sqrt(np.clip(1 - cth * cth, 0, 1))
+    E1o = gamma * (E1cm + beta * pcm * (cth * cos_al + sth * sin_al * np.cos(phi)))
+    E2o = E - E1o
+    return ~((E1o - m1 > EF1) & (E2o - m2 > EF2))

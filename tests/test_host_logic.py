@@ -98,7 +98,10 @@ def test_workloads_match_baseline_configs():
     assert np.all(E5 == 250.0) and targets5 == [(48, 22)]
     # deterministic, and a shorter request is a prefix of a longer one
     Ea, ta, *_ = W.make_inputs(4, 5000)
-    assert np.array_equal(Ea[:100], W.make_inputs(4, 5000)[0][:100])
+    Eb, tb, *_ = W.make_inputs(4, 100)
+    assert np.array_equal(Ea[:100], Eb) and np.array_equal(ta[:100], tb) and len(np.unique(ta[:100])) > 1
+    Ec, tc, *_ = W.make_inputs(4, 5000)
+    assert np.array_equal(Ea, Ec) and np.array_equal(ta, tc)
 
 
 def test_shard_ranges_cover_exactly():

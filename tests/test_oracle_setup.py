@@ -126,7 +126,7 @@ def test_table_lookup_is_numpy_interp(orc, otables):
 def test_cugnon_branch_continuity(orc):
     """The parameterisations join within 3 % at their break points (R-Q10)."""
     e = 1e-9
-    for f, brk in ((orc.cugnon_sigma_pp, (0.8, 2.0)), (orc.cugnon_sigma_np, (0.8, 2.0)),
+    for f, brk in ((orc.cugnon_sigma_pp, (0.44, 0.8, 2.0)), (orc.cugnon_sigma_np, (0.45, 0.8, 2.0)),
                    (orc.cugnon_B_np, (0.225, 0.6, 1.6)), (orc.cugnon_B_pp, (2.0,)), (orc.cugnon_a_np, (0.8,))):
         for b in brk:
             lo, hi = float(f(b - e)), float(f(b + e))
@@ -135,3 +135,13 @@ def test_cugnon_branch_continuity(orc):
     p = np.sqrt(240.0 * (240.0 + 2 * 938.27)) / 1000.0
     sig = 0.5 * (orc.cugnon_sigma_pp(p) + orc.cugnon_sigma_np(p)) * 0.1
     assert 1.5 < 1.0 / (0.14 * sig) < 3.5
+    # low-momentum branches (ref. [17] switches below ~0.44 / 0.45 GeV/c): rising towards p -> 0 with
+    # sigma_np ~ 3 sigma_pp, of the magnitude of free NN scattering at T_lab = 10 MeV (np ~ 0.9 b, pp ~ 0.3 b:
+    # sanity, not parity), and held constant below the 0.1 GeV/c floor so that the p = 0 knot is finite
+    p10 = np.sqrt(10.0 * (10.0 + 2 * 938.27)) / 1000.0
+    assert 700.0 < float(orc.cugnon_sigma_np(p10)) < 1100.0 and 250.0 < float(orc.cugnon_sigma_pp(p10)) < 450.0
+    q = np.linspace(0.1, 0.44, 50)
+    assert np.all(np.diff(orc.cugnon_sigma_pp(q)) < 0) and np.all(np.diff(orc.cugnon_sigma_np(q)) < 0)
+    assert np.all(orc.cugnon_sigma_np(q) > 2.0 * orc.cugnon_sigma_pp(q))
+    for f in (orc.cugnon_sigma_pp, orc.cugnon_sigma_np):
+        assert float(f(0.0)) == float(f(0.05)) == float(f(0.1)) and np.isfinite(float(f(0.0)))
