@@ -162,7 +162,7 @@ def main():
     real_t = lib.torch_real()
     E_d = torch.as_tensor(E.astype(lib.real), device="cuda")
     tid_d = torch.as_tensor(slots[tid], device="cuda")
-    cap = n * 8 if cfg != 5 else n * 10
+    cap = n * 16
     out = lib.alloc_outputs(n, cap)
     lib.inc_set_event_offset(rank * n)      # weak scaling: rank r owns global events [r n, (r+1) n)
 

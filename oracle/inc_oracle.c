@@ -136,7 +136,7 @@ double orc_lerp_z(const double *zz, const double *y, int n, double z) {
 static double ws_shape(double r, double c, double d) { return 1.0 / (1.0 + exp((r - c) / d)); } /* Eq.(1) */
 
 int orc_setup_nucleus(int A, int Z, const orc_tables *t, orc_nucleus *nu) {
-  if (!t || !nu || t->version != 1) return -2;
+  if (!t || !nu || (t->version != 1 && t->version != 2)) return -2;
   if (t->n_shells < 1 || t->n_shells > ORC_MAX_SHELLS) return -2;
   if (A < 2 || Z < 1 || Z >= A) return -1;
   memset(nu, 0, sizeof(*nu));
@@ -374,6 +374,15 @@ double orc_evap_widths(int A, int Z, double Estar, const orc_tables *t,
     }
     X[j] = Estar - Q[j] - V[j];
     if (!(X[j] > 0.0)) { X[j] = -1.0; continue; }           /* E1: closed */
+    if (t->version >= 2 && t->level_density == 1) {         /* NEXT-2: GEM level density (R-G1..G5) */
+      orc_ld ld;
+      if (orc_gem_ld(Ad, Zd, t, &ld) != 0) { X[j] = -1.0; continue; }
+      a_d[j] = ld.a;
+      W[j] = EV_G[j] * Mj * ad13 * ad13 * alpha * orc_gem_integral(&ld, X[j], beta[j]);
+      if (W[j] < 0.0) W[j] = 0.0;
+      sum += W[j];
+      continue;
+    }
     double a = (double)Ad / t->evap_a_div;
     a_d[j] = a;
     double s = 2.0 * sqrt(a * X[j]);
@@ -384,6 +393,108 @@ double orc_evap_widths(int A, int Z, double Estar, const orc_tables *t,
     sum += W[j];
   }
   return sum;
+}
+
+/* ---- NEXT-2: GEM level density ("we adopt the generalized evaporation model (GEM) [18]"; DESIGN R-G1..G6) ---- */
+static double ld_table(const double *y, int n, int i) { return (y && i >= 0 && i < n) ? y[i] : 0.0; }
+
+int orc_gem_ld(int A_d, int Z_d, const orc_tables *t, orc_ld *ld) {
+  int N_d = A_d - Z_d;
+  double S = ld_table(t->shell_Z, t->n_ldZ, Z_d) + ld_table(t->shell_N, t->n_ldN, N_d);
+  ld->a = (double)A_d * (t->gc_a0 + t->gc_a1 * S);                                   /* R-G2 */
+  ld->delta = ld_table(t->pair_Z, t->n_ldZ, Z_d) + ld_table(t->pair_N, t->n_ldN, N_d);   /* R-G3 */
+  ld->Ux = 150.0 / (double)A_d + 2.5;                                                /* R-G4 */
+  ld->Ex = ld->Ux + ld->delta;
+  if (!(ld->a > 0.0)) return -1;
+  double invT = sqrt(ld->a / ld->Ux) - 1.5 / ld->Ux;
+  ld->T = 1.0 / invT;
+  ld->E0 = ld->Ex - ld->T * (log(ld->T) - 0.25 * log(ld->a) - 1.25 * log(ld->Ux) + 2.0 * sqrt(ld->a * ld->Ux));
+  return 0;
+}
+
+double orc_gem_lnrho(const orc_ld *ld, double U) {
+  if (U >= ld->Ex) {                               /* Fermi gas with the pre-exponential factor */
+    double u = U - ld->delta;
+    return 2.0 * sqrt(ld->a * u) - 0.25 * log(ld->a) - 1.25 * log(u);
+  }
+  return (U - ld->E0) / ld->T - log(ld->T);        /* constant temperature */
+}
+
+/* 16-point Gauss-Legendre nodes and weights on [-1, 1], found by Newton iteration on P_16 */
+static void gl16(double x[16], double w[16]) {
+  for (int i = 0; i < 16; ++i) {
+    double z = cos(PI * ((double)i + 0.75) / 16.5), dp = 1.0;
+    for (int it = 0; it < 100; ++it) {
+      double p0 = 1.0, p1 = z;
+      for (int k = 2; k <= 16; ++k) { double p2 = ((2.0 * k - 1.0) * z * p1 - (k - 1.0) * p0) / k; p0 = p1; p1 = p2; }
+      dp = 16.0 * (z * p1 - p0) / (z * z - 1.0);
+      double dz = p1 / dp;
+      z -= dz;
+      if (fabs(dz) < 1e-16) break;
+    }
+    x[i] = z; w[i] = 2.0 / ((1.0 - z * z) * dp * dp);
+  }
+}
+
+static double gem_range(const orc_ld *ld, double X, double beta, double x0, double x1, const double gx[16], const double gw[16]) {
+  /* int_x0^x1 (x + beta) rho(X - x) dx, panels of at most 8 MeV */
+  if (!(x1 > x0)) return 0.0;
+  int np = (int)ceil((x1 - x0) / 8.0);
+  if (np < 1) np = 1;
+  double h = (x1 - x0) / (double)np, sum = 0.0;
+  for (int p = 0; p < np; ++p) {
+    double a = x0 + h * (double)p;
+    for (int q = 0; q < 16; ++q) {
+      double x = a + 0.5 * h * (gx[q] + 1.0);
+      double U = X - x;
+      if (U < 0.0) U = 0.0;
+      sum += 0.5 * h * gw[q] * (x + beta) * exp(orc_gem_lnrho(ld, U));
+    }
+  }
+  return sum;
+}
+
+double orc_gem_integral(const orc_ld *ld, double X, double beta) {
+  double gx[16], gw[16];
+  gl16(gx, gw);
+  double xs = X - ld->Ex;                          /* x below xs: daughter above E_x (Fermi gas) */
+  if (xs <= 0.0) return gem_range(ld, X, beta, 0.0, X, gx, gw);
+  return gem_range(ld, X, beta, 0.0, xs, gx, gw) + gem_range(ld, X, beta, xs, X, gx, gw);
+}
+
+double orc_evap_sample_x_gem(const orc_ld *ld, double X, double beta, const uint32_t key[2],
+                             uint32_t c1, uint32_t c2, uint32_t c3, uint32_t *k, int *trials) {
+  /* R-G6: rejection from the two envelopes of R-E4 with ln rho in place of 2 sqrt(a U).  ln rho(U) rises with a
+   * slope that is 1/T on the constant-temperature branch and falls from there on the Fermi-gas branch, so
+   * ln rho(X - x) <= ln rho(X) - x m with m the smallest slope on [0, X]: envelope (A) is (x + beta) e^(-x m). */
+  double m = 1.0 / ld->T;
+  if (X > ld->Ex) {
+    double u = X - ld->delta;
+    double sfg = sqrt(ld->a / u) - 1.25 / u;
+    if (sfg < m) m = sfg;
+  }
+  double T = 1.0 / m;
+  double l0 = orc_gem_lnrho(ld, X);
+  double areaA = T * (T + beta), areaB = 0.5 * X * X + beta * X;
+  for (int n = 0; n < ORC_MAX_TRIAL; ++n) {
+    uint32_t ctr[4] = {*k, c1, c2, c3}, out[4];
+    orc_philox4x32_10(ctr, key, out);
+    (*k)++;
+    if (trials) (*trials)++;
+    double u_mix = orc_u01(out[0]), u1 = orc_u01(out[1]), u2 = orc_u01(out[2]), u_acc = orc_u01(out[3]);
+    double x;
+    if (areaB < areaA) {
+      x = -beta + sqrt(beta * beta + u1 * (X * X + 2.0 * beta * X));
+      double rem = X - x;
+      if (rem < 0.0) rem = 0.0;
+      if (log(u_acc) < orc_gem_lnrho(ld, rem) - l0) return x < X ? x : X;
+    } else {
+      if (u_mix * (T + beta) < T) x = -T * log(u1 * u2);
+      else x = -T * log(u1);
+      if (x < X && log(u_acc) < orc_gem_lnrho(ld, X - x) - l0 + x / T) return x;
+    }
+  }
+  return -1.0;
 }
 
 /* E3: channel by cumulative sum over j in the E1 order against u_ch * Sum W (R-E3) */
@@ -752,7 +863,14 @@ int64_t orc_simulate(const orc_tables *t, const orc_nucleus *nuc, int n_nuc,
           draw4(&g, attempt, 0u, k++, u);        /* E3: (u_ch, u_cos, u_phi, -) */
           int j = orc_evap_choose(W, Wsum, u[0]);
           int trials = 0;
-          double x = orc_evap_sample_x(a_d[j], X[j], beta[j], g.key, c1, g.c2, g.c3, &k, &trials);
+          double x;
+          if (t->version >= 2 && t->level_density == 1) {
+            orc_ld ld;
+            orc_gem_ld(A_res - EV_A[j], Z_res - EV_Z[j], t, &ld);
+            x = orc_evap_sample_x_gem(&ld, X[j], beta[j], g.key, c1, g.c2, g.c3, &k, &trials);
+          } else {
+            x = orc_evap_sample_x(a_d[j], X[j], beta[j], g.key, c1, g.c2, g.c3, &k, &trials);
+          }
           if (stats) { stats->evap_trials += (uint64_t)trials; stats->philox_blocks += (uint64_t)trials; }
           if (x < 0.0) { st_bits |= ORC_ST_TRIAL_CAP; if (stats) stats->cap_trial++; break; }
           double Tej, pej[3], Pd[3];

@@ -40,7 +40,7 @@ extern "C" {
 #define ORC_F_FIFO 4u              /* debug: process pending tracks first-in-first-out (R-R4 pin)*/
 
 typedef struct orc_tables { /* caller-supplied model inputs ("precalculated ... tables") */
-  int32_t version;          /* 1 */
+  int32_t version;          /* 1: the fields up to evap_a_div; 2: also the level-density block at the end */
   int32_t n_xs;             /* NN grid points; plab_k = k*plab_max/(n_xs-1) GeV/c */
   double plab_max;
   const double *sig_pp, *sig_np;     /* mb */
@@ -51,7 +51,19 @@ typedef struct orc_tables { /* caller-supplied model inputs ("precalculated
   int32_t n_shells;                  /* 15 */
   double semf[5];                    /* a_v a_s a_c a_a a_p */
   double evap_r0, evap_rj, evap_a_div;
+  /* ---- version 2: evaporation level density ("generalized evaporation model (GEM) [18]") */
+  int32_t level_density;    /* 0: rho ~ exp(2 sqrt(a U)), a = A_d / evap_a_div (R-Q19); 1: GEM level density (R-G1..G6) */
+  int32_t n_ldZ, n_ldN;     /* lengths of the arrays below, indexed by Z_d resp. N_d (beyond the end: 0) */
+  const double *pair_Z, *pair_N;     /* pairing energies, MeV: delta = pair_Z[Z_d] + pair_N[N_d] (R-G3) */
+  const double *shell_Z, *shell_N;   /* shell corrections S, MeV: a = A_d (gc_a0 + gc_a1 (S_Z + S_N)) (R-G2) */
+  double gc_a0, gc_a1;      /* 1/8 and 0.00917 MeV^-1 */
 } orc_tables;
+
+typedef struct orc_ld {     /* level-density constants of one daughter nucleus (R-G2..G4) */
+  double a, delta;          /* level-density parameter MeV^-1, pairing energy MeV */
+  double Ux, Ex;            /* matching energy U_x = 150/A_d + 2.5 and E_x = U_x + delta */
+  double T, E0;             /* constant-temperature branch: rho = exp((U - E0)/T)/T below E_x */
+} orc_ld;
 
 typedef struct orc_nucleus {
   int32_t A, Z, n_shells;
@@ -144,6 +156,15 @@ int orc_boundary(const double x[3], double p[3], double m, double V_from, double
 double orc_evap_widths(int A, int Z, double Estar, const orc_tables *t,
                        double W[6], double X[6], double Q[6], double V[6],
                        double beta[6], double a_d[6]);
+/* R-G2..G4: level-density constants of the daughter (A_d, Z_d); returns 0, or -1 if a <= 0 */
+int orc_gem_ld(int A_d, int Z_d, const orc_tables *t, orc_ld *out);
+/* R-G5: ln rho(U) of the GEM level density (common factor pi/12 dropped), U >= 0 */
+double orc_gem_lnrho(const orc_ld *ld, double U);
+/* R-G5: int_0^X (x + beta) rho(X - x) dx by composite 16-point Gauss-Legendre (the definition, written out) */
+double orc_gem_integral(const orc_ld *ld, double X, double beta);
+/* R-G6: like orc_evap_sample_x, for the pdf (x + beta) rho(X - x) */
+double orc_evap_sample_x_gem(const orc_ld *ld, double X, double beta, const uint32_t key[2],
+                             uint32_t c1, uint32_t c2, uint32_t c3, uint32_t *k, int *trials);
 /* R-E3: channel chosen by the cumulative sum of W in the E1 order against u_ch * Wsum; -1 if no W > 0 */
 int orc_evap_choose(const double W[6], double Wsum, double u_ch);
 /* R-E4: sample x in [0,X] from (x+beta)exp(2 sqrt(a (X-x))) using Philox stream

@@ -68,7 +68,15 @@ class OrcTables(C.Structure):
         ("n_shells", C.c_int32),
         ("semf", C.c_double * 5),
         ("evap_r0", C.c_double), ("evap_rj", C.c_double), ("evap_a_div", C.c_double),
+        ("level_density", C.c_int32), ("n_ldZ", C.c_int32), ("n_ldN", C.c_int32),
+        ("pair_Z", C.POINTER(C.c_double)), ("pair_N", C.POINTER(C.c_double)),
+        ("shell_Z", C.POINTER(C.c_double)), ("shell_N", C.POINTER(C.c_double)),
+        ("gc_a0", C.c_double), ("gc_a1", C.c_double),
     ]
+
+
+class OrcLd(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("a", "delta", "Ux", "Ex", "T", "E0")]
 
 
 class OrcNucleus(C.Structure):
@@ -160,6 +168,15 @@ def lib():
     L.orc_evap_emit.argtypes = [C.c_int, C.c_int, C.c_double, dp, C.c_int, C.c_double, C.c_double,
                                 C.c_double, C.c_double, C.POINTER(OrcTables), dp, dp, dp]
     L.orc_evap_emit.restype = None
+    L.orc_gem_ld.argtypes = [C.c_int, C.c_int, C.POINTER(OrcTables), C.POINTER(OrcLd)]
+    L.orc_gem_ld.restype = C.c_int
+    L.orc_gem_lnrho.argtypes = [C.POINTER(OrcLd), C.c_double]
+    L.orc_gem_lnrho.restype = C.c_double
+    L.orc_gem_integral.argtypes = [C.POINTER(OrcLd), C.c_double, C.c_double]
+    L.orc_gem_integral.restype = C.c_double
+    L.orc_evap_sample_x_gem.argtypes = [C.POINTER(OrcLd), C.c_double, C.c_double, C.POINTER(C.c_uint32),
+                                        C.c_uint32, C.c_uint32, C.c_uint32, C.POINTER(C.c_uint32), C.POINTER(C.c_int)]
+    L.orc_evap_sample_x_gem.restype = C.c_double
     L.orc_lerp_z.argtypes = [dp, dp, C.c_int, C.c_double]
     L.orc_lerp_z.restype = C.c_double
     L.orc_evap_choose.argtypes = [dp, C.c_double, C.c_double]
@@ -221,7 +238,8 @@ class Tables:
     """Holds the numpy arrays alive and exposes the ctypes struct."""
 
     def __init__(self, n_xs=1025, plab_max=2.048, n_shells=15, semf=(15.75, 17.8, 0.711, 23.7, 11.18),
-                 ws=(1.07, 0.545, 2.5), evap=(1.5, 1.2, 8.0), sigma_scale=1.0, B_scale=1.0):
+                 ws=(1.07, 0.545, 2.5), evap=(1.5, 1.2, 8.0), sigma_scale=1.0, B_scale=1.0,
+                 level_density=0, pair_Z=None, pair_N=None, shell_Z=None, shell_N=None, gc=(0.125, 0.00917)):
         p = np.arange(n_xs, dtype=np.float64) * (plab_max / (n_xs - 1))
         self.plab = p
         self.sig_pp = np.ascontiguousarray(cugnon_sigma_pp(p) * sigma_scale)
@@ -236,15 +254,23 @@ class Tables:
         self.ev_ca = np.array([0.10, 0.10, 0.10, 0.08, 0.06])
         self.n_xs, self.plab_max, self.n_shells = n_xs, plab_max, n_shells
         self.semf, self.ws, self.evap = tuple(semf), tuple(ws), tuple(evap)
+        # NEXT-2 (version 2 block): level-density mode and the caller-supplied pairing / shell-correction arrays
+        self.level_density, self.gc = int(level_density), tuple(gc)
+        nz = max(len(x) for x in (pair_Z, shell_Z) if x is not None) if (pair_Z is not None or shell_Z is not None) else 1
+        nn = max(len(x) for x in (pair_N, shell_N) if x is not None) if (pair_N is not None or shell_N is not None) else 1
+        pad = lambda x, n: np.concatenate([np.asarray(x, dtype=np.float64), np.zeros(n - len(x))]) if x is not None else np.zeros(n)
+        self.pair_Z, self.shell_Z = pad(pair_Z, nz), pad(shell_Z, nz)
+        self.pair_N, self.shell_N = pad(pair_N, nn), pad(shell_N, nn)
         self.refresh()
 
     def refresh(self):
         dp = C.POINTER(C.c_double)
         s = OrcTables()
-        s.version = 1
+        s.version = 2
         s.n_xs = self.n_xs
         s.plab_max = self.plab_max
-        for name in ("sig_pp", "sig_np", "B_pp", "B_np", "a_np", "ev_Z", "ev_kp", "ev_cp", "ev_ka", "ev_ca"):
+        for name in ("sig_pp", "sig_np", "B_pp", "B_np", "a_np", "ev_Z", "ev_kp", "ev_cp", "ev_ka", "ev_ca",
+                     "pair_Z", "pair_N", "shell_Z", "shell_N"):
             arr = np.ascontiguousarray(getattr(self, name), dtype=np.float64)
             setattr(self, name, arr)
             setattr(s, name, arr.ctypes.data_as(dp))
@@ -254,6 +280,9 @@ class Tables:
         for i in range(5):
             s.semf[i] = self.semf[i]
         s.evap_r0, s.evap_rj, s.evap_a_div = self.evap
+        s.level_density, s.n_ldZ, s.n_ldN = self.level_density, len(self.pair_Z), len(self.pair_N)
+        assert len(self.shell_Z) == len(self.pair_Z) and len(self.shell_N) == len(self.pair_N)
+        s.gc_a0, s.gc_a1 = self.gc
         self.c = s
         return self
 

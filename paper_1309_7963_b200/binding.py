@@ -308,7 +308,7 @@ def load(variant: str = "f32") -> IncLibrary:
 
 
 def simulate(lib: IncLibrary, targets, E_in_np, target_idx_np, seed, tables: dict, flags: int = 0, capacity_per_event: int = 24,
-             chunk_events: int = 1 << 22, projectile=None):
+             chunk_events: int = 1 << 22, projectile=None, event_offset: int = 0):
     """Convenience used by tests/bench: init targets, run on the GPU, return numpy arrays.
     targets: list of (A,Z); target_idx_np indexes that list."""
     import torch
@@ -320,6 +320,7 @@ def simulate(lib: IncLibrary, targets, E_in_np, target_idx_np, seed, tables: dic
     tid = torch.as_tensor(slot_map[np.asarray(target_idx_np)], device="cuda")
     lib.inc_set_stream()
     lib.inc_set_flags(flags)
+    lib.inc_set_event_offset(event_offset)
     lib.inc_set_projectiles(None if projectile is None else torch.as_tensor(np.asarray(projectile, dtype=np.uint8), device="cuda"))
     cap = max(64, n * capacity_per_event)
     out = lib.alloc_outputs(n, cap)
@@ -327,6 +328,7 @@ def simulate(lib: IncLibrary, targets, E_in_np, target_idx_np, seed, tables: dic
         total = lib.inc_simulate(E, tid, seed, out)
     finally:
         lib.inc_set_projectiles(None)
+        lib.inc_set_event_offset(0)
     off = lib.inc_get_offsets(n)
     res = {k: v.cpu().numpy() for k, v in out.items()}
     for k in ("species", "T", "ux", "uy", "uz"):

@@ -109,13 +109,30 @@ def compare_histograms(hg, ho, p_min=1e-3):
     return failures
 
 
-def event_identity(g, o, rel=1e-9):
+T_FLOOR = 1e-2      # MeV: below it the energy bar is absolute, rel * T_FLOOR (see event_identity)
+# Directions and residual momenta: the cascade amplifies rounding (a track that grazes a shell sphere turns an
+# ulp of its position into ~1e5..1e6 ulp of its later direction): a ONE-ulp change of E_in moves the oracle's own
+# outputs by up to 6e-11 relative in T and 1.3e-7 MeV/c in the residual momentum over 2e4 events
+# (test_oracle_conditioning).  The bars are ~10x that.
+DIR_TOL = 1e-8      # unit-vector components, fp64
+P_TOL = 1e-6        # MeV/c absolute on residual momenta (1e-9 of the ~1 GeV/c scale of p_in)
+
+
+def event_identity(g, o, rel=1e-9, detail=None):
     """Criterion (2): per event identical multiplicity, species, residual (A,Z); energies within rel.
-    Returns (fraction identical, max relative energy error among identical events)."""
+    Returns (fraction identical, max relative energy error among identical events, mask).
+
+    Energies: |dT| <= rel * max(|T|, T_FLOOR).  The floor is the oracle's own rounding, not slack for the kernel:
+    the oracle forms T = sqrt(p^2 + M^2) - M (emission, boundary), whose absolute error is a few ulp(M) ~ 1e-13 to
+    5e-13 MeV whatever T is, i.e. 5e-10 relative already at T = 1 keV (the library uses p^2 / (E + M)).  Excitation
+    energies: |dE*| <= rel * max(|E*|, 1 MeV) (E* is a difference of ~1e4 MeV masses).  Directions to DIR_TOL,
+    the final residual momentum to P_TOL absolute.  `detail` (a dict) receives the observed maxima: over the identical
+    events, and ("worst_*") over all events with the same species list, whatever their errors."""
     n = len(o["counts"])
     same = (g["counts"] == o["counts"]) & (g["A"] == o["A"]) & (g["Z"] == o["Z"])
     og, oo = g["offsets"], o["offsets"]
     max_err = 0.0
+    mx = dict(T_rel=0.0, T_rel_floored=0.0, Estar=0.0, dir=0.0, P=0.0, worst_T_rel_floored=0.0, worst_Estar=0.0, worst_dir=0.0, worst_P=0.0)
     ident = np.zeros(n, dtype=bool)
     for e in np.nonzero(same)[0]:
         a, b = og[e], oo[e]
@@ -123,15 +140,23 @@ def event_identity(g, o, rel=1e-9):
         if not np.array_equal(g["species"][a:a + c], o["species"][b:b + c]):
             continue
         tg, to = g["T"][a:a + c], o["T"][b:b + c]
-        err = np.max(np.abs(tg - to) / np.maximum(np.abs(to), 1e-300)) if c else 0.0
+        err = np.max(np.abs(tg - to) / np.maximum(np.abs(to), T_FLOOR)) if c else 0.0
+        raw = np.max(np.abs(tg - to) / np.maximum(np.abs(to), 1e-300)) if c else 0.0
         es_o = o["Estar"][e]
         err_e = abs(g["Estar"][e] - es_o) / max(abs(es_o), 1.0)
         dirs = 0.0
         if c:
             dirs = max(np.max(np.abs(g[k][a:a + c] - o[k][b:b + c])) for k in ("ux", "uy", "uz"))
-        if err <= rel and err_e <= rel and dirs <= 1e-7:
+        dp = max(abs(float(g[k][e]) - float(o[k][e])) for k in ("px", "py", "pz"))
+        mx["worst_T_rel_floored"] = max(mx["worst_T_rel_floored"], err); mx["worst_Estar"] = max(mx["worst_Estar"], err_e)
+        mx["worst_dir"] = max(mx["worst_dir"], dirs); mx["worst_P"] = max(mx["worst_P"], dp)
+        if err <= rel and err_e <= rel and dirs <= DIR_TOL and dp <= P_TOL:
             ident[e] = True
             max_err = max(max_err, err, err_e)
+            mx["T_rel"] = max(mx["T_rel"], raw); mx["T_rel_floored"] = max(mx["T_rel_floored"], err)
+            mx["Estar"] = max(mx["Estar"], err_e); mx["dir"] = max(mx["dir"], dirs); mx["P"] = max(mx["P"], dp)
+    if detail is not None:
+        detail.update(mx, n=n, identical=int(ident.sum()), same_discrete=int(same.sum()))
     return ident.mean() if n else 1.0, max_err, ident
 
 

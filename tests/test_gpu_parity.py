@@ -104,9 +104,62 @@ def test_fp64_event_identity(gpu, orc, otables, ptables, cfg, n):
     same = ident
     assert np.array_equal(g["casc_A"][same], o["casc_A"][same])
     assert np.allclose(g["casc_Estar"][same], o["casc_Estar"][same], rtol=1e-9, atol=1e-9)
-    assert np.allclose(g["casc_P"][same], o["casc_P"][same], rtol=1e-9, atol=1e-6)   # 1e-9 of the ~1 GeV/c scale
+    assert np.allclose(g["casc_P"][same], o["casc_P"][same], rtol=0, atol=H.P_TOL)
     # criterion (1) on the GPU output itself
     _assert_conservation(g, targets, tid, E, orc, otables, 1e-12, 1e-9)
+
+
+@pytest.mark.parametrize("cfg", [2, 5])
+def test_fp64_event_identity_1e5(gpu, orc, otables, ptables, cfg, capsys):
+    """Criterion (2) on the first 1e5 events of the headline config and of the long-chain config: the observed
+    maxima and the number of events that differ are printed (pytest -s) and quoted in DESIGN.md section 9."""
+    n = 100000
+    E, tid, targets, seed, _ = _inputs(cfg, n)
+    g = gpu.simulate(gpu.load("f64"), targets, E, tid, seed, ptables)
+    o = orc.simulate(otables, targets, E, tid, seed)
+    d = {}
+    frac, max_err, ident = H.event_identity(g, o, rel=REL_F64, detail=d)
+    with capsys.disabled():
+        print(f"\n[fp64 1e5 slice] config {cfg}: {d}")
+    assert frac >= FRAC_IDENTICAL and max_err <= REL_F64, d
+    assert np.array_equal(g["status"][ident], o["status"][ident])
+    _assert_conservation(g, targets, tid, E, orc, otables, 1e-12, 1e-9)
+
+
+@pytest.mark.parametrize("variant", ["f64", "f32"])
+def test_event_offset_shards(gpu, orc, otables, ptables, variant):
+    """inc_set_event_offset, the one multi-GPU hook ("one full cascade ... per GPU thread": events are
+    independent): a batch run as two calls with offsets 0 and n/2 is bit-identical to the single
+    call; a batch that straddles global event 2^32 (counter word c3 changes inside it) equals the oracle run with
+    the same first event."""
+    n = 6000
+    E, tid, targets, seed, _ = _inputs(4, n)
+    lib = gpu.load(variant)
+    whole = gpu.simulate(lib, targets, E, tid, seed, ptables)
+    h = n // 2
+    lo = gpu.simulate(lib, targets, E[:h], tid[:h], seed, ptables, event_offset=0)
+    hi = gpu.simulate(lib, targets, E[h:], tid[h:], seed, ptables, event_offset=h)
+    for k in ("species", "T", "ux", "uy", "uz", "counts", "A", "Z", "Estar", "px", "py", "pz", "status"):
+        assert np.array_equal(whole[k], np.concatenate([lo[k], hi[k]])), k
+    assert np.array_equal(whole["offsets"], np.concatenate([lo["offsets"], hi["offsets"][1:] + lo["total"]]))
+    # without the offset the second half is a different sample
+    hi0 = gpu.simulate(lib, targets, E[h:], tid[h:], seed, ptables)
+    assert not np.array_equal(hi0["counts"], hi["counts"])
+    e0 = 2 ** 32 - 1500
+    far = gpu.simulate(lib, targets, E[:h], tid[:h], seed, ptables, event_offset=e0)
+    o = orc.simulate(otables, targets, E[:h], tid[:h], seed, e0=e0)
+    assert not np.array_equal(far["counts"], lo["counts"])
+    if variant == "f64":
+        frac, max_err, ident = H.event_identity(far, o, rel=REL_F64)
+        assert frac == 1.0 and max_err <= REL_F64
+        assert np.array_equal(far["status"], o["status"])
+    else:
+        same = (far["counts"] == o["counts"]) & (far["A"] == o["A"]) & (far["Z"] == o["Z"])
+        assert same.mean() > 0.95 and same[1400:1600].mean() > 0.9       # on both sides of 2^32
+        _assert_conservation(far, targets, tid[:h], E[:h], orc, otables, 2e-6, 2e-4)
+    # the library rejects a negative offset and forgets the offset at shutdown
+    with pytest.raises(gpu.IncError):
+        lib.inc_set_event_offset(-1)
 
 
 def test_fp64_ragged_sizes_and_empty(gpu, orc, otables, ptables):
@@ -119,7 +172,7 @@ def test_fp64_ragged_sizes_and_empty(gpu, orc, otables, ptables):
         if n:
             o = orc.simulate(otables, targets, E, tid, seed)
             frac, _, _ = H.event_identity(g, o)
-            assert frac == 1.0 or frac >= 1 - 1.0 / n
+            assert frac == 1.0
 
 
 def test_fp64_cascade_only_and_flags(gpu, orc, otables, ptables):
@@ -290,13 +343,13 @@ def test_chunk_boundary_determinism(gpu, orc, otables, ptables):
     for bnd in (chunk, 2 * chunk, 3 * chunk):
         lo, hi = bnd - 200, bnd + 200
         o = orc.simulate(otables, [(16, 8)], E[lo:hi], tid[lo:hi], 2, e0=lo)
-        g = {k: out[k][lo:hi].cpu().numpy() for k in ("counts", "A", "Z", "Estar")}
+        g = {k: out[k][lo:hi].cpu().numpy() for k in ("counts", "A", "Z", "Estar", "px", "py", "pz")}
         a, b = off[lo], off[hi]
         for k in ("species", "T", "ux", "uy", "uz"):
             g[k] = out[k][a:b].cpu().numpy()
         g["offsets"] = off[lo:hi + 1] - off[lo]
         frac, err, _ = H.event_identity(g, o)
-        assert frac >= 0.995 and err <= REL_F64
+        assert frac == 1.0 and err <= REL_F64
 
 
 # ------------------------------------------------------------------------------- criteria (1), (3)
