@@ -79,6 +79,18 @@ MUTATIONS = [
     ("dostrovsky_row_search_stuck_on_the_first_interval",
      "while (k < n - 2 && z > zz[k + 1]) ++k;", "",
      DEC + "test_dostrovsky_interpolation_interior"),
+    ("gem_pre_exponential_power",
+     "- 0.25 * log(ld->a) - 1.25 * log(u);", "- 0.25 * log(ld->a) - 1.5 * log(u);",
+     "tests/test_oracle_gem.py::test_level_density_constants_and_matching"),
+    ("gem_matching_energy",
+     "ld->Ux = 150.0 / (double)A_d + 2.5;", "ld->Ux = 150.0 / (double)A_d + 2.0;",
+     "tests/test_oracle_gem.py::test_gem_widths_vs_numerical_integration"),
+    ("gem_pairing_not_subtracted_in_the_fermi_gas_branch",
+     "double u = U - ld->delta;\n    return 2.0", "double u = U;\n    return 2.0",
+     "tests/test_oracle_gem.py::test_gem_widths_vs_numerical_integration"),
+    ("gem_envelope_uses_the_constant_temperature_slope_only",
+     "if (sfg < m) m = sfg;", "",
+     "tests/test_oracle_gem.py::test_gem_sampler_matches_pdf"),
     ("dostrovsky_fraction_over_the_whole_grid",
      "double f = (z - zz[k]) / (zz[k + 1] - zz[k]);", "double f = (z - zz[k]) / (zz[n - 1] - zz[0]);",
      DEC + "test_dostrovsky_interpolation_interior"),
