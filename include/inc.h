@@ -205,6 +205,13 @@ int inc_get_stage_times(float ms[4] /*HOST*/, int32_t launches[4] /*HOST*/);
  * kernel only, zeros otherwise. */
 int inc_get_drain_timeline(double ms[4] /*HOST*/);
 
+/* Per-warp drain trace of the cascade kernel of the last inc_simulate (last chunk; needs INC_F_TIMING; wavefront
+ * kernel only): 8 words per warp -- [0] %globaltimer ns (low 32 bits) when the event counter ran out for the warp,
+ * [1] ns when its own work was finished, [2] passes of its drain phase, [3] segment passes among them, [4] active
+ * lanes summed over those, [5] highest attempt number started in the drain, [6] tracks handed to drain helpers,
+ * [7] ns at kernel entry.  Returns the number of warps written (<= max_warps), 0 if none was recorded.  Diagnostic. */
+int inc_get_warp_trace(uint32_t *out /*HOST [8 * max_warps]*/, int32_t max_warps);
+
 /* Nuclear-setup record of a target, for tests of inc_init (all HOST, fp64, length n_shells
  * except r, V_p, V_n which have n_shells+1; pointers may be NULL). */
 int inc_get_nucleus(int target_id, int32_t *A, int32_t *Z, int32_t *n_shells, double *R,

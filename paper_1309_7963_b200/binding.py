@@ -77,7 +77,7 @@ def make_tables_struct(t: dict):
 
 
 EXPORTS = ["inc_init", "inc_free_target", "inc_shutdown", "inc_set_stream", "inc_set_flags", "inc_set_event_offset",
-           "inc_get_stage_times", "inc_get_drain_timeline", "inc_set_vote_thresholds", "inc_set_long_track_threshold", "inc_set_chunk_events", "inc_set_projectiles", "inc_simulate",
+           "inc_get_stage_times", "inc_get_drain_timeline", "inc_get_warp_trace", "inc_set_vote_thresholds", "inc_set_long_track_threshold", "inc_set_chunk_events", "inc_set_projectiles", "inc_simulate",
            "inc_simulate_host", "inc_get_offsets", "inc_get_cascade_stage", "inc_get_stats", "inc_get_nucleus",
            "inc_measure_issue_peak", "inc_philox_blocks", "inc_tally", "inc_last_error", "inc_build_info"]
 
@@ -184,6 +184,11 @@ class IncLibrary:
         ms = (C.c_double * 4)()
         self._check(self.lib.inc_get_drain_timeline(ms))
         return dict(zip(("exhausted_mean", "exit_mean", "exit_last", "exit_first"), [float(x) for x in ms]))
+
+    def inc_get_warp_trace(self, max_warps: int = 8192):
+        buf = np.zeros((max_warps, 8), dtype=np.uint32)
+        n = self._check(self.lib.inc_get_warp_trace(buf.ctypes.data_as(C.c_void_p), int(max_warps)))
+        return buf[:n]
 
     def inc_set_vote_thresholds(self, coll: int, epi: int):
         self._check(self.lib.inc_set_vote_thresholds(int(coll), int(epi)))

@@ -632,7 +632,11 @@ template <typename R> struct CascadeParams {
   int vote_coll, vote_epi;  // lane kernel: phase-vote thresholds
   int long_seg;             // wavefront kernel: tracks with this many segments behind them may go to a drain helper
   int n_stage;              // nuclei slots staged into shared memory (target_id must be < n_stage)
+  uint32_t *wtrace;         // INC_F_TIMING: kWTrace words per warp of the wavefront kernel (inc_get_warp_trace), or nullptr
 };
+constexpr int kWTrace = 8;  // [0] ns (low 32 bits) when the event counter ran out for the warp, [1] ns at exit of its own work,
+                            // [2] passes of the drain phase, [3] segment passes among them, [4] lanes summed over those,
+                            // [5] highest attempt number started in the drain, [6] tracks handed to helpers, [7] ns at kernel entry
 
 // shared-memory staging of the model: [NucDev x n_stage] [tabS n_xs*4]   (n_stage = highest live slot + 1)
 template <typename R> __host__ __device__ inline size_t model_smem_bytes(int n_xs, int n_stage) {
@@ -1060,6 +1064,10 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   __syncwarp();
   const bool timeline = (P.flags & INC_F_TIMING) != 0;
   if (timeline && lane == 0) { atomicMax(&P.ctr->tl[0], ~global_ns()); atomicAdd(&P.ctr->tl[4], 1ull); }
+  // per-warp drain trace (diagnostic, INC_F_TIMING only)
+  uint32_t *wt = (timeline && P.wtrace) ? P.wtrace + (size_t)kWTrace * (blockIdx.x * C::WARPS + (threadIdx.x >> 5)) : nullptr;
+  uint32_t tr_pass = 0, tr_seg = 0, tr_lanes = 0, tr_att = 0, tr_out = 0;
+  if (wt && lane == 0) wt[7] = (uint32_t)global_ns();
 
   auto load_key = [&](int slot, RngKey &g, uint32_t &attempt, int &tgt, int &ev) {
     ev = w.ev[slot];
@@ -1168,6 +1176,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
         nSeg -= take; nRes += take;
       }
       if (lane == 0) { st.add(S_WI_SEG); st.add(S_LS_SEG, nRes); }
+      if (DRAIN && wt) { tr_seg++; tr_lanes += (uint32_t)nRes; }
       int out = -1;
       CollCarry<R> cc;
       Escape<R> esc;
@@ -1206,6 +1215,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
           const unsigned mm = __ballot_sync(kFull, moved);
           if (moved) rhas = false;
           nRes -= __popc(mm); n_out += __popc(mm);
+          if (wt) tr_out += (uint32_t)__popc(mm);
         }
       }
       const unsigned left = __ballot_sync(kFull, out > SEG_CONT);     // tracks that leave the segment state
@@ -1368,7 +1378,8 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
         }
       }
       const bool ran_out = __ballot_sync(kFull, got_none) != 0u;
-      if (timeline && ran_out && !exhausted && lane == 0) atomicAdd(&P.ctr->tl[1], global_ns());
+      if (timeline && ran_out && !exhausted && lane == 0) { atomicAdd(&P.ctr->tl[1], global_ns()); if (wt) wt[0] = (uint32_t)global_ns(); }
+      if (DRAIN && wt) { const uint32_t am = __reduce_max_sync(kFull, do_entry ? attempt : 0u); tr_att = am > tr_att ? am : tr_att; }
       if (ran_out) exhausted = true;
       // slots that did not get work go back to the free list
       {
@@ -1395,7 +1406,25 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   };
   bool done = false;
   while (!exhausted && !done) done = pass(std::false_type());
-  while (!done) done = pass(std::true_type());
+  // watchdog: a drain phase is a few hundred passes (thousands with waits for helpers); 2^24 means a scheduling bug:
+  // fail loudly (error bit 16 -> INC_E_STATE) instead of hanging the device
+  while (!done) {
+    done = pass(std::true_type());
+    if (++tr_pass > (1u << 24)) {
+      if (wt) {   // (debug dump of the stuck state)
+        const unsigned mh = __ballot_sync(kFull, rhas);
+        const int fl = mh ? __ffs(mh) - 1 : 0;
+        const uint32_t ns = (uint32_t)__shfl_sync(kFull, rt.nseg, fl), sl = (uint32_t)__shfl_sync(kFull, rslot, fl), kk = __shfl_sync(kFull, rt.k, fl), pp = __shfl_sync(kFull, rt.pi, fl);
+        if (lane == 0) { wt[0] = mh; wt[1] = ns | (kk << 16); wt[6] = w.status[sl]; wt[7] = tr_seg; wt[3] = (uint32_t)nSeg | ((uint32_t)nRes << 16); }
+      }
+      if (lane == 0) {
+        atomicOr(&P.ctr->error_word, 16u);
+        if (wt) { wt[2] = tr_pass; wt[4] = (uint32_t)nColl | ((uint32_t)nEpi << 16); wt[5] = (uint32_t)nFree | ((uint32_t)n_out << 16); }
+      }
+      break;
+    }
+  }
+  if (wt && lane == 0 && tr_pass <= (1u << 24)) { wt[1] = (uint32_t)global_ns(); wt[2] = tr_pass; wt[3] = tr_seg; wt[4] = tr_lanes; wt[5] = tr_att; wt[6] = tr_out; }
   if (timeline && lane == 0) {
     const unsigned long long t = global_ns();
     atomicAdd(&P.ctr->tl[2], t); atomicMax(&P.ctr->tl[3], t); atomicMax(&P.ctr->tl[5], ~t);

@@ -52,6 +52,7 @@ struct State {
   EvChan<real> *d_evch = nullptr;
   NucDev<real> *d_nuc = nullptr;
   DevCounters *d_ctr = nullptr;
+  uint32_t *d_wtrace = nullptr; int wtrace_warps = 0;   // inc_get_warp_trace (INC_F_TIMING)
   // workspace
   size_t ws_chunk = 0;
   Workspace<real> ws{};
@@ -400,6 +401,7 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   const bool naive = (g.flags & INC_F_LANE_PER_EVENT) != 0;
   cp.vote_coll = naive ? 1 : g.vote_coll; cp.vote_epi = naive ? 1 : g.vote_epi;
   cp.long_seg = g.long_seg;
+  cp.wtrace = nullptr;
   int n_stage = 0;
   for (int i = 0; i < INC_MAX_TARGETS; ++i) if (g.nuc[i].live) n_stage = i + 1;
   cp.n_stage = n_stage;
@@ -433,6 +435,12 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
     int blocks = occ * g.sm_count;
     const int wneed = (n_chunk + threads - 1) / threads;
     if (blocks > wneed) blocks = wneed;
+    cp.wtrace = nullptr;
+    if (timing) {
+      const int nw = blocks * WaveCfg<real>::WARPS;
+      if (!g.d_wtrace) CU_TRY(cudaMalloc((void **)&g.d_wtrace, sizeof(uint32_t) * kWTrace * 8192));
+      if (nw <= 8192) { CU_TRY(cudaMemsetAsync(g.d_wtrace, 0, sizeof(uint32_t) * kWTrace * nw, g.stream)); cp.wtrace = g.d_wtrace; g.wtrace_warps = nw; }
+    }
     kern<<<blocks, threads, wsmem, g.stream>>>(cp);
   }
   CU_TRY(cudaGetLastError());
@@ -529,7 +537,7 @@ int inc_free_target(int id) {
 void inc_shutdown(void) {
   free_ws();
   void **p[] = {(void **)&g.d_tabS, (void **)&g.d_tabC, (void **)&g.d_bind, (void **)&g.d_evch, (void **)&g.d_nuc,
-                (void **)&g.d_ctr, (void **)&g.d_offsets, (void **)&g.d_tiles,
+                (void **)&g.d_ctr, (void **)&g.d_wtrace, (void **)&g.d_offsets, (void **)&g.d_tiles,
                 (void **)&g.hp.E, (void **)&g.hp.tid, (void **)&g.hp.counts, (void **)&g.hp.A, (void **)&g.hp.Z,
                 (void **)&g.hp.Es, (void **)&g.hp.px, (void **)&g.hp.py, (void **)&g.hp.pz, (void **)&g.hp.status,
                 (void **)&g.hp.sp, (void **)&g.hp.T, (void **)&g.hp.ux, (void **)&g.hp.uy, (void **)&g.hp.uz};
@@ -591,6 +599,7 @@ int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64
   for (auto e : g.pending_events) cudaEventDestroy(e);
   g.pending_events.clear();
   g.last_n = n; g.last_total = (long long)tail.total;
+  if (tail.err & 16u) return fail(INC_E_STATE, "watchdog: a warp of the wavefront cascade kernel made no progress (results invalid)");
   if (tail.err & 4u) return fail(INC_E_STATE, "internal track-queue overflow in the wavefront cascade kernel (results invalid)");
   if (tail.err) {
     return fail(INC_E_BADARG, std::string("device-side input check failed:") + ((tail.err & 1u) ? " E_in outside [20,250] MeV" : "") +
@@ -659,6 +668,14 @@ int inc_get_drain_timeline(double ms[4]) {
   ms[2] = ((double)c.tl[3] - t0) * 1e-6;
   ms[3] = ((double)(~c.tl[5]) - t0) * 1e-6;
   return 0;
+}
+
+int inc_get_warp_trace(uint32_t *out, int32_t max_warps) {
+  if (!out || max_warps < 0) return fail(INC_E_BADARG, "null pointer");
+  if (g.last_n < 0 || !g.d_wtrace) return 0;
+  const int n = g.wtrace_warps < max_warps ? g.wtrace_warps : max_warps;
+  CU_TRY(cudaMemcpy(out, g.d_wtrace, sizeof(uint32_t) * kWTrace * (size_t)n, cudaMemcpyDeviceToHost));
+  return n;
 }
 
 int inc_get_stage_times(float ms[4], int32_t launches[4]) {
