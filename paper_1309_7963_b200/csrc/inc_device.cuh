@@ -925,9 +925,16 @@ template <typename R, int NS, int QS, int QC> struct WarpMem {
   uint32_t rqi[3][kRetQ];
 };
 
+// Defaults per build; -DINC_WNS= -DINC_WQS= -DINC_WQC= -DINC_WWARPS= (all four) override them for the build's real type:
+// tuning experiments and the small-queue test build, which exercises the capacity guards.  Needs QS >= 64, QC >= 33.
+#ifdef INC_WNS
+static_assert(INC_WQS >= 64 && INC_WQC >= 33 && INC_WNS <= 128 && INC_WNS >= 32, "wavefront queue sizes");
+template <typename R> struct WaveCfg { static constexpr int NS = INC_WNS, QS = INC_WQS, QC = INC_WQC, WARPS = INC_WWARPS; };
+#else
 template <typename R> struct WaveCfg;
 template <> struct WaveCfg<float> { static constexpr int NS = 80, QS = 128, QC = 64, WARPS = 16; };
 template <> struct WaveCfg<double> { static constexpr int NS = 64, QS = 128, QC = 64, WARPS = 8; };
+#endif
 
 template <typename R> __host__ __device__ inline size_t wave_smem_bytes(int n_xs, int n_stage) {
   typedef WaveCfg<R> C;
@@ -1128,11 +1135,17 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       }
     }
     // ---- choose the kind of step of this pass (warp-uniform) ----
+    // Queue invariants: a segment pass adds at most one collision item per running lane, a collision pass at most two
+    // segment tracks per item, an entry pass one per item.  kCollTrig: from this many waiting collisions on a full
+    // segment pass might not fit into the collision queue, so a collision pass runs first.
+    constexpr int kCollTrig = C::QC - 31 < 32 ? C::QC - 31 : 32;
+    constexpr int kAdmit = (C::QS + C::QC) / 3;       // admission control: no new attempts while more tracks wait
     const int nSegT = nSeg + nRes;
     const int availE = nEpi + (exhausted ? 0 : nFree);
     int phase = ST_SEG;
-    if (!(nColl < 32 && nSegT >= 32)) {        // (the common case needs none of what follows)
-      if (nColl >= 32) phase = ST_COLL;
+    int capS = 32;                                // lanes the segment pass may run
+    if (!(nColl < kCollTrig && nSegT >= 32)) {        // (the common case needs none of what follows)
+      if (nColl >= kCollTrig) phase = ST_COLL;
       else if (availE >= 32) phase = ST_EPI;
       else {
         // nothing fills a whole pass: take the fullest queue (ties: entry first, it creates work)
@@ -1142,20 +1155,36 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
         else if (DRAIN && n_out > 0) { __nanosleep(100); return false; }      // our last tracks are with helpers
         else return true;
       }
-      // capacity guards: a collision pass can add 2 tracks per item, an entry pass 1 track per item.  While a full
-      // collision pass does not fit, segment passes make room first -- unless the collision queue could then
-      // overflow (a segment pass adds up to one item per lane): then a partial collision pass runs.
-      if (phase == ST_COLL && nSegT + 2 * (nColl < 32 ? nColl : 32) > C::QS && nColl <= C::QC - 32) phase = ST_SEG;
-      if (phase == ST_EPI && nSegT + nColl > 64) phase = nSegT > 0 ? ST_SEG : ST_COLL;   // admission control
+      if (phase == ST_EPI && nSegT + nColl > kAdmit) phase = nSegT > 0 ? ST_SEG : ST_COLL;   // admission control
+      // While a full collision pass does not fit into the segment queue, segment passes make room first (nSegT > 0
+      // then, because QS >= 64); as long as the collision queue can take a full segment pass they are ordinary ones,
+      // beyond that a partial collision pass runs if it can (m >= 1), else a segment pass of at most QC - nColl lanes.
+      // So some pass can always run unless both queues are full (error bit 4: inc_simulate reruns the call with the
+      // lane kernel).
+      if (phase == ST_COLL && nSegT + 2 * (nColl < 32 ? nColl : 32) > C::QS) {
+        if (nColl <= C::QC - 32) phase = ST_SEG;
+        else if (C::QS - nSegT < 2 && nColl < C::QC) { phase = ST_SEG; capS = C::QC - nColl; }
+      }
     }
 
     if (phase == ST_SEG) {
+      int lim = nSeg;               // tracks the refill may take from the queue
+      if (__builtin_expect(capS < 32, 0)) {
+        // (rare) the collision queue has room for fewer than 32 new items: at most capS lanes may run.  Resident
+        // tracks beyond that go back to the queue, and the refill takes no more than the pass may run.
+        const bool over = rhas && __popc(__ballot_sync(kFull, rhas) & lt) >= capS;
+        const int nOver = __popc(__ballot_sync(kFull, over));
+        push_seg(over, rt, rslot);
+        if (over) rhas = false;
+        nRes -= nOver;
+        lim = capS - nRes;
+      }
       // refill lanes without a resident track from the top of the segment queue
       {
         const bool need = !rhas;
         const unsigned mk = __ballot_sync(kFull, need);
         int take = __popc(mk);
-        take = take < nSeg ? take : nSeg;
+        take = take < lim ? take : lim;
         const int r = __popc(mk & lt);
         if (need && r < take) {
           const int i = nSeg - 1 - r;
