@@ -80,6 +80,8 @@ extern "C" {
                                       warp-voted phases instead of the default per-warp
                                       wavefront queues.  Results never depend on the variant. */
 
+#define INC_F_NO_OVERLAP 512u       /* scheduling variant: the evaporation kernel starts only after the cascade kernel
+                                      has finished (no programmatic dependent launch).  Results never depend on it. */
 #define INC_F_NO_DRAIN_HELPERS 256u /* scheduling variant: every track stays with the warp that owns its
                                       event (no drain helpers).  Results never depend on it.   */
 
@@ -180,7 +182,9 @@ int64_t inc_simulate_host(int64_t n_events, const INC_REAL *E_in /*HOST*/,
 int inc_get_offsets(int64_t *dev_offsets /*DEVICE [n_events+1]*/);
 
 /* Post-cascade nuclei of the last inc_simulate (the paper's "SoA of excited nuclei", P:69,
- * P:83), for stage-level tests: any pointer may be NULL. */
+ * P:83), for stage-level tests: any pointer may be NULL; n_cascade_secondaries[e] is the number of
+ * cascade nucleons of event e.  Only after a call that ran as ONE chunk (n_events <= the chunk size):
+ * the records are per chunk, so after a multi-chunk call this returns INC_E_STATE. */
 int inc_get_cascade_stage(int32_t *A /*DEVICE [n]*/, int32_t *Z, INC_REAL *Estar,
                           INC_REAL *px, INC_REAL *py, INC_REAL *pz, int32_t *n_cascade_secondaries);
 

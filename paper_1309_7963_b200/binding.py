@@ -17,6 +17,7 @@ INC_E_BADARG, INC_E_TABLES, INC_E_CAPACITY, INC_E_CUDA, INC_E_STATE = -1, -2, -3
 ST_FAILED, ST_SEC_TRUNC, ST_DEPTH_CAP, ST_SEG_CAP, ST_TRIAL_CAP, ST_QUEUE_OVF = (1 << 8, 1 << 9, 1 << 10, 1 << 11, 1 << 12, 1 << 13)
 F_CASCADE_ONLY, F_KEEP_TRANSPARENT, F_SAME_STREAM, F_STATS, F_LANE_PER_EVENT, F_TIMING, F_LANE_STATE_MACHINE = 1, 2, 4, 8, 16, 32, 64
 F_NO_DRAIN_HELPERS = 256
+F_NO_OVERLAP = 512
 MAX_SEC = 64
 
 _DP = C.POINTER(C.c_double)

@@ -92,13 +92,47 @@ template <typename R> struct __align__(16) StageRec {
   uint32_t pad[3];
 };
 
+// One nucleus record per event: 32 bytes in the f32 build (one DRAM sector), 48 in f64.  Events finish, and are
+// evaporated, in an order unrelated to their index, so a record that is one sector costs one sector of traffic
+// where eight parallel arrays cost eight.  crec: post-cascade nucleus (the paper's "SoA of excited nuclei"),
+// meta = n_casc | attempt << 8 | failed << 16.  frec: final residual, meta = number of secondaries of the event; the
+// compaction kernel, which walks the events in index order, transposes it into the caller's arrays.
+template <typename R> struct __align__(16) NucRec {
+  R E, Px, Py, Pz;
+  int32_t A, Z;
+  uint32_t meta, status;
+};
+
 template <typename R> struct Workspace {   // per-chunk internal buffers (DEVICE)
   StageRec<R> *st;        // [chunk][kMaxSec] staged secondaries, one record per secondary
-  int32_t *cA, *cZ;       // post-cascade nucleus ("SoA of excited nuclei")
-  R *cE, *cPx, *cPy, *cPz;
-  uint32_t *cmeta;        // n_casc | attempt << 8 | failed << 16
-  uint32_t *cstatus;
+  NucRec<R> *crec;        // [chunk] post-cascade nuclei
+  NucRec<R> *frec;        // [chunk] final residuals
+  // Completion list: the cascade kernel appends the chunk-local index of every event whose post-cascade record is
+  // complete; the evaporation kernel, which may start while the cascade kernel's last CTAs are still draining
+  // (programmatic dependent launch), consumes the entries in order.  kNotDone = not written yet.
+  uint32_t *done_list;    // [chunk]
 };
+constexpr uint32_t kNotDone = 0xFFFFFFFFu;
+
+// release / acquire pair of the completion list (gpu scope)
+__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t *p) {
+  uint32_t v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+// Warp-collective: publishes the events of the lanes with `pub` set.  Every lane's earlier global writes (post-cascade
+// record; staged escapes, written by lanes of this warp in earlier passes and ordered by the __syncwarp()s since) are
+// made visible before the entry (fence + release store).
+__device__ __forceinline__ void publish_done(bool pub, int ev, unsigned long long *n_done, uint32_t *done_list, int lane) {
+  const unsigned mp = __ballot_sync(kFull, pub);
+  if (mp == 0u) return;
+  const int leader = __ffs(mp) - 1;
+  unsigned long long base = 0;
+  if (lane == leader) base = atomicAdd(n_done, (unsigned long long)__popc(mp));
+  base = __shfl_sync(kFull, base, leader);
+  __threadfence();
+  if (pub) *(volatile uint32_t *)(done_list + base + (unsigned long long)__popc(mp & ((1u << lane) - 1u))) = (uint32_t)ev;
+}
 
 template <typename R>
 __device__ __forceinline__ void stage_write(StageRec<R> *dst, R T, R ux, R uy, R uz, uint32_t code) {
@@ -109,6 +143,7 @@ __device__ __forceinline__ void stage_write(StageRec<R> *dst, R T, R ux, R uy, R
 
 struct DevCounters {       // device scalars
   unsigned long long next_event_casc, next_event_evap;
+  unsigned long long n_done;          // entries of the completion list handed out (cascade -> evaporation)
   unsigned long long total_sec;
   unsigned int error_word;   // bit0: E_in out of range, bit1: bad target id
   unsigned int pad;
@@ -667,18 +702,18 @@ __device__ __forceinline__ bool check_inputs(const CascadeParams<R> &P, const Nu
   else if (!s_nuc[tgt].live) err |= 2u;
   if (!err) return true;
   atomicOr(&P.ctr->error_word, err);
-  P.ws.cA[ev] = 0; P.ws.cZ[ev] = 0; P.ws.cE[ev] = R(0);
-  P.ws.cPx[ev] = R(0); P.ws.cPy[ev] = R(0); P.ws.cPz[ev] = R(0);
-  P.ws.cmeta[ev] = (1u << 16); P.ws.cstatus[ev] = INC_ST_FAILED;
+  NucRec<R> r;
+  r.E = R(0); r.Px = R(0); r.Py = R(0); r.Pz = R(0); r.A = 0; r.Z = 0; r.meta = (1u << 16); r.status = INC_ST_FAILED;
+  P.ws.crec[ev] = r;
   return false;
 }
 
 template <typename R>
 __device__ __forceinline__ void write_cascade_result(const Workspace<R> &ws, int ev, int A, int Z, R Es, R Px, R Py, R Pz,
                                                      uint32_t meta, uint32_t status) {
-  ws.cA[ev] = A; ws.cZ[ev] = Z; ws.cE[ev] = Es;
-  ws.cPx[ev] = Px; ws.cPy[ev] = Py; ws.cPz[ev] = Pz;
-  ws.cmeta[ev] = meta; ws.cstatus[ev] = status;
+  NucRec<R> r;
+  r.E = Es; r.Px = Px; r.Py = Py; r.Pz = Pz; r.A = A; r.Z = Z; r.meta = meta; r.status = status;
+  ws.crec[ev] = r;          // 16-byte vector stores
 }
 
 // Order-independent sums (escaped energy and momentum): fixed point, so that any processing order of
@@ -713,6 +748,9 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
   NucDev<R> *s_nuc = reinterpret_cast<NucDev<R> *>(smem_raw);
   R *s_tabS = reinterpret_cast<R *>(smem_raw + sizeof(NucDev<R>) * P.n_stage);
   stage_model<R>(P.model, P.n_stage, s_nuc, s_tabS);
+  // programmatic dependent launch: the evaporation kernel may be scheduled as soon as every CTA of this grid is
+  // resident; it takes its events from the completion list, never from stream order
+  asm volatile("griddepcontrol.launch_dependents;");
 
   const int lane = threadIdx.x & 31;
   const int n_xs = P.model.n_xs;
@@ -809,6 +847,8 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
     } else {  // EPI phase: epilogue of the finished attempt, then entry of the next attempt / event
       if (lane == 0) { st.add(S_WI_EPI); st.add(S_LS_EPI, nE); }
       bool want_event = false;
+      bool done_now = false;
+      int ev_done = ev;
       if (state == ST_EPI) {
         if (ev >= 0) {
           const NucDev<R> &nu = s_nuc[tgt];
@@ -820,19 +860,24 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
             const uint32_t used = attempt + 1u > 255u ? 255u : attempt + 1u;
             write_cascade_result<R>(P.ws, ev, A_res, Z_res, Estar, Prx, Pry, Prz, (uint32_t)n_esc | (attempt << 8), st_try | used);
             ev = -1;
+            done_now = true;
           } else {
             attempt++;
             if (attempt >= (uint32_t)kMaxAttempt) {          // FAILED: count 0, target at rest
               write_cascade_result<R>(P.ws, ev, nu.A, nu.Z, R(0), R(0), R(0), R(0), (1u << 16), INC_ST_FAILED | 0xFFu);
               st.add(S_FAILED);
               ev = -1;
+              done_now = true;
             }
           }
         }
         want_event = (ev < 0);
       }
+      publish_done(done_now, ev_done, &P.ctr->n_done, P.ws.done_list, lane);
       const unsigned need = __ballot_sync(kFull, want_event);
       if (need) {
+        bool rejected = false;
+        int ev_rej = 0;
         const int leader = __ffs(need) - 1;
         unsigned long long base = 0;
         if (lane == leader) base = atomicAdd(&P.ctr->next_event_casc, (unsigned long long)__popc(need));
@@ -845,7 +890,7 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
             E_in = P.E_in[ev];
             tgt = P.target_id[ev];
             ptype = P.projectile ? (int)P.projectile[ev] : 1;
-            if (!check_inputs<R>(P, s_nuc, ev, E_in, tgt, ptype)) { ev = -1; tgt = 0; }
+            if (!check_inputs<R>(P, s_nuc, ev, E_in, tgt, ptype)) { rejected = true; ev_rej = ev; ev = -1; tgt = 0; }
             else {
               const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
               g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
@@ -855,6 +900,7 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
             state = ST_DONE;
           }
         }
+        publish_done(rejected, ev_rej, &P.ctr->n_done, P.ws.done_list, lane);   // (neutral outputs are complete results too)
       }
       if (state == ST_EPI && ev >= 0) {
         st.add(S_ATTEMPTS);
@@ -918,6 +964,8 @@ template <typename R, int NS, int QS, int QC> struct WarpMem {
   R cf[QC], cnx[QC], cny[QC], cnz[QC], cSp[QC], cSig[QC];
   // slot lists
   uint8_t epi_q[NS], free_q[NS];
+  // finished events waiting to be published in the completion list (a batch costs one fence and one global atomic)
+  uint32_t pub_q[96];
   // tracks coming back from the drain helpers
   uint32_t r_tail;
   uint32_t r_valid[kRetQ];
@@ -1049,6 +1097,9 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   if (threadIdx.x < kCtaLongQ) cq.valid[threadIdx.x] = 0u;
   if (threadIdx.x == 0) { cq.credits = kCtaLongQ; cq.avail = 0; cq.tail = 0u; cq.head = 0u; cq.n_helpers = 0u; cq.lock = 0u; cq.idle = 0; }
   stage_model<R>(P.model, P.n_stage, s_nuc, s_tabS);      // ends with __syncthreads()
+  // programmatic dependent launch: the evaporation kernel may be scheduled as soon as every CTA of this grid is
+  // resident (it then fills the SMs whose CTA has finished); it takes its events from the completion list
+  asm volatile("griddepcontrol.launch_dependents;");
 
   const unsigned lt = (1u << lane) - 1u;
   const int n_xs = P.model.n_xs;
@@ -1092,6 +1143,23 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       w.qmeta[i] = (uint32_t)t.type | ((uint32_t)t.shell << 1) | ((uint32_t)slot << 8);
     }
     nSeg += __popc(m);
+  };
+  // Completion list: finished events are collected per warp and published in batches.
+  int nPub = 0;
+  auto push_pub = [&](bool pred, int ev) {
+    const unsigned m = __ballot_sync(kFull, pred);
+    if (pred) w.pub_q[nPub + __popc(m & lt)] = (uint32_t)ev;
+    nPub += __popc(m);
+  };
+  auto flush_pub = [&]() {
+    if (nPub == 0) return;
+    unsigned long long base = 0;
+    if (lane == 0) base = atomicAdd(&P.ctr->n_done, (unsigned long long)nPub);
+    base = __shfl_sync(kFull, base, 0);
+    __syncwarp();
+    __threadfence();          // every lane: its records (and, through the __syncwarp()s since, the warp's) before the entries
+    for (int i = lane; i < nPub; i += 32) *(volatile uint32_t *)(P.ws.done_list + base + i) = w.pub_q[i];
+    nPub = 0;
   };
   auto push_epi = [&](bool pred, int slot) {
     const unsigned m = __ballot_sync(kFull, pred);
@@ -1143,7 +1211,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
     const int nSegT = nSeg + nRes;
     const int availE = nEpi + (exhausted ? 0 : nFree);
     int phase = ST_SEG;
-    int capS = 32;                                // lanes the segment pass may run
+    int lim = 32;                                 // tracks the refill of a segment pass may take
     if (!(nColl < kCollTrig && nSegT >= 32)) {        // (the common case needs none of what follows)
       if (nColl >= kCollTrig) phase = ST_COLL;
       else if (availE >= 32) phase = ST_EPI;
@@ -1158,32 +1226,26 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       if (phase == ST_EPI && nSegT + nColl > kAdmit) phase = nSegT > 0 ? ST_SEG : ST_COLL;   // admission control
       // While a full collision pass does not fit into the segment queue, segment passes make room first (nSegT > 0
       // then, because QS >= 64); as long as the collision queue can take a full segment pass they are ordinary ones,
-      // beyond that a partial collision pass runs if it can (m >= 1), else a segment pass of at most QC - nColl lanes.
-      // So some pass can always run unless both queues are full (error bit 4: inc_simulate reruns the call with the
-      // lane kernel).
+      // beyond that a partial collision pass runs if it can (m >= 1), else a segment pass of at most QC - nColl lanes:
+      // the resident tracks go back to the queue and the refill takes no more than that.  So some pass can always run
+      // unless both queues are full (error bit 4: inc_simulate reruns the call with the lane kernel).
       if (phase == ST_COLL && nSegT + 2 * (nColl < 32 ? nColl : 32) > C::QS) {
         if (nColl <= C::QC - 32) phase = ST_SEG;
-        else if (C::QS - nSegT < 2 && nColl < C::QC) { phase = ST_SEG; capS = C::QC - nColl; }
+        else if (C::QS - nSegT < 2 && nColl < C::QC) {
+          push_seg(rhas, rt, rslot);
+          rhas = false; nRes = 0;
+          phase = ST_SEG; lim = C::QC - nColl;
+        }
       }
     }
 
     if (phase == ST_SEG) {
-      int lim = nSeg;               // tracks the refill may take from the queue
-      if (__builtin_expect(capS < 32, 0)) {
-        // (rare) the collision queue has room for fewer than 32 new items: at most capS lanes may run.  Resident
-        // tracks beyond that go back to the queue, and the refill takes no more than the pass may run.
-        const bool over = rhas && __popc(__ballot_sync(kFull, rhas) & lt) >= capS;
-        const int nOver = __popc(__ballot_sync(kFull, over));
-        push_seg(over, rt, rslot);
-        if (over) rhas = false;
-        nRes -= nOver;
-        lim = capS - nRes;
-      }
       // refill lanes without a resident track from the top of the segment queue
       {
         const bool need = !rhas;
         const unsigned mk = __ballot_sync(kFull, need);
         int take = __popc(mk);
+        take = take < nSeg ? take : nSeg;
         take = take < lim ? take : lim;
         const int r = __popc(mk & lt);
         if (need && r < take) {
@@ -1356,6 +1418,8 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       __syncwarp();
       bool want_event = has && lane >= mE;
       bool do_entry = false;
+      bool done_now = false;
+      int ev_done = 0;
       int ev = -1, tgt = 0, ptype = 1;
       uint32_t attempt = 0;
       R E_in = R(0);
@@ -1374,20 +1438,23 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
         if (ok) {
           const uint32_t used = attempt + 1u > 255u ? 255u : attempt + 1u;
           write_cascade_result<R>(P.ws, ev, A_res, Z_res, Estar, Prx, Pry, Prz, (uint32_t)n_esc | (attempt << 8), w.status[slot] | used);
-          want_event = true;
+          want_event = true; done_now = true; ev_done = ev;
         } else if (attempt + 1u >= (uint32_t)kMaxAttempt) {    // FAILED: count 0, target at rest
           write_cascade_result<R>(P.ws, ev, nu.A, nu.Z, R(0), R(0), R(0), R(0), (1u << 16), INC_ST_FAILED | 0xFFu);
           st.add(S_FAILED);
-          want_event = true;
+          want_event = true; done_now = true; ev_done = ev;
         } else {
           attempt++;
           do_entry = true;
         }
       }
+      push_pub(done_now, ev_done);                 // finished events -> evaporation kernel
       // ---- warp-aggregated event fetch ----
       const unsigned need = __ballot_sync(kFull, want_event && !exhausted);
       bool got_none = false;
       if (need) {
+        bool rejected = false;
+        int ev_rej = 0;
         const int leader = __ffs(need) - 1;
         unsigned long long base = 0;
         if (lane == leader) base = atomicAdd(&P.ctr->next_event_casc, (unsigned long long)__popc(need));
@@ -1401,11 +1468,16 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
             tgt = P.target_id[ev];
             ptype = P.projectile ? (int)P.projectile[ev] : 1;
             if (check_inputs<R>(P, s_nuc, ev, E_in, tgt, ptype)) { do_entry = true; st.add(S_EVENTS); }
+            else { rejected = true; ev_rej = ev; }
           } else {
             got_none = true;
           }
         }
+        push_pub(rejected, ev_rej);               // (neutral outputs are complete results too)
       }
+      // a batch is more than a pass's worth (one fence + one global atomic round trip each); the rest goes out when
+      // the warp has finished its own events
+      if (nPub > 32) flush_pub();
       const bool ran_out = __ballot_sync(kFull, got_none) != 0u;
       if (timeline && ran_out && !exhausted && lane == 0) { atomicAdd(&P.ctr->tl[1], global_ns()); if (wt) wt[0] = (uint32_t)global_ns(); }
       if (DRAIN && wt) { const uint32_t am = __reduce_max_sync(kFull, do_entry ? attempt : 0u); tr_att = am > tr_att ? am : tr_att; }
@@ -1458,6 +1530,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
     const unsigned long long t = global_ns();
     atomicAdd(&P.ctr->tl[2], t); atomicMax(&P.ctr->tl[3], t); atomicMax(&P.ctr->tl[5], ~t);
   }
+  flush_pub();
   st.flush(P.ctr, lane);
   if (helpers_on) {
     if (lane == 0) { __threadfence_block(); atomicAdd(&cq.n_helpers, 1u); }
@@ -1480,11 +1553,7 @@ template <typename R> struct EvapParams {
   int n_chunk;
   uint32_t seed_lo, seed_hi;
   uint32_t flags;
-  // final outputs (caller arrays, chunk base)
-  int32_t *out_counts;
-  int32_t *rA, *rZ;
-  R *rE, *rPx, *rPy, *rPz;
-  uint32_t *rstatus;
+  int32_t *out_counts;      // caller array, chunk base (the residual goes to ws.frec, see compact_kernel)
 };
 
 // G_n(s) e^{-s_ref} with G_n(s) = int_0^s t^n e^t dt, n = 1 or 3 (closed forms of R-E2)
@@ -1515,6 +1584,9 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
   const bool cascade_only = (P.flags & INC_F_CASCADE_ONLY) != 0;
   const bool same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
   int ev = -1;
+  unsigned long long pbase = 0;      // the warp's pool of completion-list entries: [pbase + ph, pbase + pn) not handed out yet
+  int pn = 0, ph = 0;
+  uint32_t pent = kNotDone;
   int A = 0, Z = 0, count = 0;
   R Es = 0, Px = 0, Py = 0, Pz = 0;
   uint32_t status = 0, attempt = 0, kblk = 0;
@@ -1534,32 +1606,53 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
   R u1 = R(0), u2 = R(0);
   for (;;) {
     __syncwarp();
-    // ---- refill idle lanes ----
-    const unsigned need = __ballot_sync(kFull, ev < 0 && !exhausted);
+    // ---- refill idle lanes from the warp's pool of 32 consecutive entries of the cascade kernel's completion list
+    // (one global atomic and one coalesced load per 32 events; lane i holds entry pbase + i) ----
+    const bool want = ev < 0;
+    const unsigned need = __ballot_sync(kFull, want);
     if (need) {
-      const int leader = __ffs(need) - 1;
-      unsigned long long base = 0;
-      if (lane == leader) base = atomicAdd(&P.ctr->next_event_evap, (unsigned long long)__popc(need));
-      base = __shfl_sync(kFull, base, leader);
-      if (ev < 0 && !exhausted) {
-        const unsigned long long mine = base + (unsigned long long)__popc(need & ((1u << lane) - 1u));
-        if (mine < (unsigned long long)P.n_chunk) {
-          ev = (int)mine;
-          A = P.ws.cA[ev]; Z = P.ws.cZ[ev]; Es = P.ws.cE[ev];
-          Px = P.ws.cPx[ev]; Py = P.ws.cPy[ev]; Pz = P.ws.cPz[ev];
-          const uint32_t meta = P.ws.cmeta[ev];
+      if (ph == pn && !exhausted) {
+        unsigned long long base = 0;
+        if (lane == 0) base = atomicAdd(&P.ctr->next_event_evap, 32ull);
+        base = __shfl_sync(kFull, base, 0);
+        if (base >= (unsigned long long)P.n_chunk) exhausted = true;
+        else {
+          pbase = base; ph = 0; pent = kNotDone;
+          const unsigned long long left = (unsigned long long)P.n_chunk - base;
+          pn = left < 32ull ? (int)left : 32;
+        }
+      }
+      if (ph < pn) {
+        // (the cascade kernel may still be running: poll the entries not seen yet; acquire = their events' records)
+        const bool mine = lane >= ph && lane < pn;
+        if (mine && pent == kNotDone) pent = ld_acquire_u32(P.ws.done_list + pbase + lane);
+        const unsigned rdy = __ballot_sync(kFull, mine && pent != kNotDone);
+        const unsigned gap = ~rdy & (kFull << ph);                    // first entry from ph on that is not there yet
+        const int nready = (gap ? __ffs(gap) - 1 : 32) - ph;
+        const int r = __popc(need & ((1u << lane) - 1u));
+        int give = __popc(need);
+        give = give < nready ? give : nready;
+        const uint32_t d = __shfl_sync(kFull, pent, (ph + r) & 31);
+        if (want && r < give) {
+          ev = (int)d;
+          const NucRec<R> rec = P.ws.crec[ev];
+          A = rec.A; Z = rec.Z; Es = rec.E; Px = rec.Px; Py = rec.Py; Pz = rec.Pz;
+          const uint32_t meta = rec.meta;
           count = (int)(meta & 0xFFu); attempt = (meta >> 8) & 0xFFu;
-          status = P.ws.cstatus[ev];
+          status = rec.status;
           kblk = 0;
           const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
           g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
           if ((meta >> 16) & 1u) count = 0;   // FAILED or rejected input
-        } else {
-          exhausted = true;
         }
+        ph += give;
       }
     }
-    if (__ballot_sync(kFull, ev >= 0) == 0) break;
+    if (__ballot_sync(kFull, ev >= 0) == 0) {
+      if (exhausted && ph == pn) break;
+      __nanosleep(200);                     // every lane waits for the cascade kernel
+      continue;
+    }
     // The step is written as stages that every lane of the warp walks through, each under its own predicate, with
     // the rejection loop ended by a vote: the warp is converged again before the two-body kinematics.  (With the
     // loop left by `break`, the compiler ran everything behind it once per group of lanes that left the loop
@@ -1706,9 +1799,9 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
     }
     if (finish) {
       P.out_counts[ev] = count;
-      P.rA[ev] = A; P.rZ[ev] = Z; P.rE[ev] = Es;
-      P.rPx[ev] = Px; P.rPy[ev] = Py; P.rPz[ev] = Pz;
-      P.rstatus[ev] = status;
+      NucRec<R> r;
+      r.E = Es; r.Px = Px; r.Py = Py; r.Pz = Pz; r.A = A; r.Z = Z; r.meta = (uint32_t)count; r.status = status;
+      P.ws.frec[ev] = r;
       ev = -1;
     }
   }
@@ -1816,6 +1909,10 @@ template <typename R> struct CompactParams {
   uint8_t *species;
   R *T, *ux, *uy, *uz;
   long long capacity;
+  // residual of the caller (chunk base): transposed from ws.frec
+  int32_t *rA, *rZ;
+  R *rE, *rPx, *rPy, *rPz;
+  uint32_t *rstatus;
 };
 
 // One warp per group of 32 events; lanes sweep the records of each event so that the stores of a
@@ -1830,7 +1927,11 @@ __global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) 
   const int e = e0 + lane;
   long long off = 0;
   int cnt = 0;
-  if (e < P.n_chunk) { off = P.offsets[e]; cnt = P.counts[e]; }
+  if (e < P.n_chunk) {
+    off = P.offsets[e]; cnt = P.counts[e];
+    const NucRec<R> r = P.ws.frec[e];
+    P.rA[e] = r.A; P.rZ[e] = r.Z; P.rE[e] = r.E; P.rPx[e] = r.Px; P.rPy[e] = r.Py; P.rPz[e] = r.Pz; P.rstatus[e] = r.status;
+  }
   // flatten (event, record) pairs of the 32 events over the lanes
   int incl = cnt;
 #pragma unroll
@@ -1866,7 +1967,7 @@ __global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) 
       } else {
         sp = (uint8_t)((code >> 24) & 1u);
         const uint32_t key = code & 0xFFFFFFu;
-        const int n_casc = (int)(P.ws.cmeta[el] & 0xFFu);
+        const int n_casc = (int)(P.ws.crec[el].meta & 0xFFu);
         rank = 0;
         for (int l = 0; l < n_casc; ++l) rank += ((row[l].code & 0xFFFFFFu) < key) ? 1 : 0;
       }
@@ -1949,6 +2050,21 @@ __global__ void __launch_bounds__(256) tally_kernel(const TallyParams<R> P) {
       }
     }
   }
+}
+
+// post-cascade records -> parallel arrays (inc_get_cascade_stage); any pointer may be null
+template <typename R>
+__global__ void unpack_cascade_kernel(const NucRec<R> *rec, long long n, int32_t *A, int32_t *Z, R *E, R *px, R *py, R *pz, int32_t *ncs) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const NucRec<R> r = rec[i];
+  if (A) A[i] = r.A;
+  if (Z) Z[i] = r.Z;
+  if (E) E[i] = r.E;
+  if (px) px[i] = r.Px;
+  if (py) py[i] = r.Py;
+  if (pz) pz[i] = r.Pz;
+  if (ncs) ncs[i] = (int32_t)(r.meta & 0xFFu);
 }
 
 // ---- issue-peak microbenchmark: 8 independent FMA chains per thread ------------------------------

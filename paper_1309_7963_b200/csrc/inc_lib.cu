@@ -74,6 +74,7 @@ struct State {
   std::function<int(int, long long, int)> chunk_hook;
   // last call
   long long last_n = -1;
+  int last_chunks = 0;              // chunks of the last inc_simulate (the cascade stage survives single-chunk calls only)
   long long last_total = 0;
   long long event_offset = 0;
   // stage timing (INC_F_TIMING)
@@ -334,8 +335,7 @@ ModelDev<real> model_dev() {
 }
 
 void free_ws() {
-  void **p[] = {(void **)&g.ws.st, (void **)&g.ws.cA, (void **)&g.ws.cZ, (void **)&g.ws.cE, (void **)&g.ws.cPx,
-                (void **)&g.ws.cPy, (void **)&g.ws.cPz, (void **)&g.ws.cmeta, (void **)&g.ws.cstatus};
+  void **p[] = {(void **)&g.ws.st, (void **)&g.ws.crec, (void **)&g.ws.frec, (void **)&g.ws.done_list};
   for (auto q : p) { if (*q) cudaFree(*q); *q = nullptr; }
   g.ws_chunk = 0;
 }
@@ -345,14 +345,9 @@ int ensure_ws(size_t chunk, size_t n_total) {
     free_ws();
     const size_t ns = chunk * kMaxSec;
     CU_TRY(cudaMalloc((void **)&g.ws.st, ns * sizeof(StageRec<real>)));
-    CU_TRY(cudaMalloc((void **)&g.ws.cA, chunk * sizeof(int32_t)));
-    CU_TRY(cudaMalloc((void **)&g.ws.cZ, chunk * sizeof(int32_t)));
-    CU_TRY(cudaMalloc((void **)&g.ws.cE, chunk * sizeof(real)));
-    CU_TRY(cudaMalloc((void **)&g.ws.cPx, chunk * sizeof(real)));
-    CU_TRY(cudaMalloc((void **)&g.ws.cPy, chunk * sizeof(real)));
-    CU_TRY(cudaMalloc((void **)&g.ws.cPz, chunk * sizeof(real)));
-    CU_TRY(cudaMalloc((void **)&g.ws.cmeta, chunk * sizeof(uint32_t)));
-    CU_TRY(cudaMalloc((void **)&g.ws.cstatus, chunk * sizeof(uint32_t)));
+    CU_TRY(cudaMalloc((void **)&g.ws.crec, chunk * sizeof(NucRec<real>)));
+    CU_TRY(cudaMalloc((void **)&g.ws.frec, chunk * sizeof(NucRec<real>)));
+    CU_TRY(cudaMalloc((void **)&g.ws.done_list, chunk * sizeof(uint32_t)));
     g.ws_chunk = chunk;
   }
   if (n_total + 1 > g.offsets_cap) {
@@ -412,7 +407,8 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   CU_TRY(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
   const size_t wsmem = wave_smem_bytes<real>(model.n_xs, n_stage);
   const bool lane_kernel = naive || (g.flags & INC_F_LANE_STATE_MACHINE) != 0 || wsmem > (size_t)smem_max;
-  CU_TRY(cudaMemsetAsync(&g.d_ctr->next_event_casc, 0, 2 * sizeof(unsigned long long), g.stream));
+  CU_TRY(cudaMemsetAsync(&g.d_ctr->next_event_casc, 0, 3 * sizeof(unsigned long long), g.stream));   // + next_event_evap, n_done
+  CU_TRY(cudaMemsetAsync(g.ws.done_list, 0xFF, (size_t)n_chunk * sizeof(uint32_t), g.stream));      // kNotDone
   if (mark(timing)) return INC_E_CUDA;
   if (lane_kernel) {
     const size_t smem = model_smem_bytes<real>(model.n_xs, n_stage);
@@ -449,15 +445,25 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   EvapParams<real> ep;
   ep.model = model; ep.ws = g.ws; ep.ctr = g.d_ctr; ep.e_base = e_base + g.event_offset; ep.n_chunk = n_chunk;
   ep.seed_lo = cp.seed_lo; ep.seed_hi = cp.seed_hi; ep.flags = g.flags;
-  ep.out_counts = counts; ep.rA = res->A; ep.rZ = res->Z; ep.rE = res->Estar;
-  ep.rPx = res->px; ep.rPy = res->py; ep.rPz = res->pz; ep.rstatus = res->status;
+  ep.out_counts = counts;
   auto ekern = evap_kernel<real, STATS>;
   int eocc = 0;
   CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&eocc, ekern, 256, 0));
   if (eocc < 1) return fail(INC_E_CUDA, "evaporation kernel does not fit on an SM");
   int eblocks = eocc * g.sm_count;
   if (eblocks > need) eblocks = need;
-  ekern<<<eblocks, 256, 0, g.stream>>>(ep);
+  {
+    // Programmatic dependent launch: the evaporation CTAs may be scheduled while the cascade kernel's last CTAs are
+    // still draining; they consume the completion list, so they never run ahead of the data.  With INC_F_TIMING the
+    // stages are separated by events and run one after the other, so that each has a duration of its own.
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)eblocks); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = g.stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = (timing || (g.flags & INC_F_NO_OVERLAP)) ? 0 : 1;
+    CU_TRY(cudaLaunchKernelEx(&cfg, ekern, ep));
+  }
   CU_TRY(cudaGetLastError());
   if (mark(timing)) return INC_E_CUDA;
   // --- prefix sum of counts (running base carried across chunks in ctr->total_sec) ---
@@ -472,6 +478,7 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   kp.ws = g.ws; kp.offsets = offsets; kp.counts = counts; kp.n_chunk = n_chunk;
   kp.species = sec->species; kp.T = sec->T; kp.ux = sec->ux; kp.uy = sec->uy; kp.uz = sec->uz;
   kp.capacity = sec->capacity;
+  kp.rA = res->A; kp.rZ = res->Z; kp.rE = res->Estar; kp.rPx = res->px; kp.rPy = res->py; kp.rPz = res->pz; kp.rstatus = res->status;
   const int cwarps = (n_chunk + 31) / 32;
   const int cblocks = (cwarps + 7) / 8;
   compact_kernel<real><<<cblocks, 256, 0, g.stream>>>(kp);
@@ -599,6 +606,7 @@ int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64
   for (auto e : g.pending_events) cudaEventDestroy(e);
   g.pending_events.clear();
   g.last_n = n; g.last_total = (long long)tail.total;
+  g.last_chunks = (int)((n + (long long)chunk - 1) / (long long)chunk);
   if (tail.err & 16u) return fail(INC_E_STATE, "watchdog: a warp of the wavefront cascade kernel made no progress (results invalid)");
   if (tail.err & 4u) return fail(INC_E_STATE, "internal track-queue overflow in the wavefront cascade kernel (results invalid)");
   if (tail.err) {
@@ -624,17 +632,11 @@ int inc_get_offsets(int64_t *dev_offsets) {
 
 int inc_get_cascade_stage(int32_t *A, int32_t *Z, INC_REAL *Es, INC_REAL *px, INC_REAL *py, INC_REAL *pz, int32_t *ncs) {
   if (g.last_n < 0) return fail(INC_E_STATE, "no previous inc_simulate");
-  if ((size_t)g.last_n > g.ws_chunk) return fail(INC_E_STATE, "cascade stage is only kept for single-chunk calls (n <= the chunk size, inc_set_chunk_events)");
-  const size_t n = (size_t)g.last_n;
-  if (A) CU_TRY(cudaMemcpyAsync(A, g.ws.cA, n * 4, cudaMemcpyDeviceToDevice, g.stream));
-  if (Z) CU_TRY(cudaMemcpyAsync(Z, g.ws.cZ, n * 4, cudaMemcpyDeviceToDevice, g.stream));
-  if (Es) CU_TRY(cudaMemcpyAsync(Es, g.ws.cE, n * sizeof(real), cudaMemcpyDeviceToDevice, g.stream));
-  if (px) CU_TRY(cudaMemcpyAsync(px, g.ws.cPx, n * sizeof(real), cudaMemcpyDeviceToDevice, g.stream));
-  if (py) CU_TRY(cudaMemcpyAsync(py, g.ws.cPy, n * sizeof(real), cudaMemcpyDeviceToDevice, g.stream));
-  if (pz) CU_TRY(cudaMemcpyAsync(pz, g.ws.cPz, n * sizeof(real), cudaMemcpyDeviceToDevice, g.stream));
-  if (ncs) {
-    // low byte of cmeta
-    CU_TRY(cudaMemcpyAsync(ncs, g.ws.cmeta, n * 4, cudaMemcpyDeviceToDevice, g.stream));
+  if (g.last_chunks > 1) return fail(INC_E_STATE, "cascade stage is only kept for single-chunk calls (n <= the chunk size, inc_set_chunk_events)");
+  const long long n = g.last_n;
+  if (n > 0) {
+    unpack_cascade_kernel<real><<<(unsigned)((n + 255) / 256), 256, 0, g.stream>>>(g.ws.crec, n, A, Z, Es, px, py, pz, ncs);
+    CU_TRY(cudaGetLastError());
   }
   CU_TRY(cudaStreamSynchronize(g.stream));
   return 0;
