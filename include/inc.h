@@ -10,7 +10,10 @@
  * Conventions
  *  - Every function returns 0 (or a non-negative value where stated) on success and a
  *    negative INC_E_* code on failure.  Nothing throws or aborts; inc_last_error() gives
- *    a human-readable message for the last failure on the calling thread's library state.
+ *    a human-readable message for the last failure.
+ *  - The library has ONE process-wide state (targets, tables, workspace, stream, flags) bound to the CUDA
+ *    device that was current at the first inc_init: it is not thread-safe, and concurrent callers must
+ *    serialise their calls.  One process drives one GPU (one process per GPU).
  *  - "DEVICE" pointers are CUDA device pointers owned by the caller (e.g. torch tensors);
  *    the library never frees or reallocates them.  "HOST" pointers are ordinary host
  *    memory.  The library owns only its internal workspace and the device copies of the
@@ -82,6 +85,8 @@ extern "C" {
 
 #define INC_F_NO_OVERLAP 512u       /* scheduling variant: the evaporation kernel starts only after the cascade kernel
                                       has finished (no programmatic dependent launch).  Results never depend on it. */
+#define INC_F_TEST_QUEUE_OVF 1024u  /* test hook: the wavefront kernel reports a track-queue overflow although there is
+                                      none, which exercises the library's rerun of the call with the lane kernel     */
 #define INC_F_NO_DRAIN_HELPERS 256u /* scheduling variant: every track stays with the warp that owns its
                                       event (no drain helpers).  Results never depend on it.   */
 
@@ -103,7 +108,8 @@ typedef struct inc_tables {   /* HOST memory, caller-owned, copied during inc_in
 /* inc_init — nuclear setup for one target (Woods-Saxon -> n_shells constant-density
  * shells, Fermi momenta/energies, V = E_F + E_B, Coulomb barrier) done in fp64 on the host,
  * uploaded once.  The first call also captures the NN / evaporation tables.
- * Supported: 6 <= A <= 64, 2 <= Z <= A-2 (the separation energies need valid A-1 nuclei).  Returns target_id >= 0 (slot, < INC_MAX_TARGETS). */
+ * Supported: 6 <= A <= 64, 2 <= Z <= A-2 (the separation energies need valid A-1 nuclei; the library's binding-energy
+ * and evaporation-channel tables cover every nucleus a cascade on such a target can leave).  Returns target_id >= 0 (slot, < INC_MAX_TARGETS). */
 int inc_init(int A, int Z, const inc_tables *tables /*HOST*/);
 int inc_free_target(int target_id);
 void inc_shutdown(void);       /* frees every target, the tables and the workspace          */
@@ -115,9 +121,9 @@ int inc_set_flags(uint32_t flags);
  * Results never depend on it. */
 int inc_set_vote_thresholds(int coll, int epi);
 /* Incident nucleon species (the paper's model is a "nucleon-nucleus" one, and is
- * applied to protons, P:9): projectile[i] = 1 proton, 0 neutron for event i of the following inc_simulate /
- * inc_simulate_host calls.  DEVICE array, caller-owned, at least as long as the calls' n_events; it must stay
- * valid until those calls have returned.  NULL (the default) = all protons.  A neutron enters with its own mass
+ * applied to protons, P:9): projectile[i] = 1 proton, 0 neutron for event i of the NEXT inc_simulate /
+ * inc_simulate_host call only (the pointer is dropped when that call returns, so a stale pointer is never read).
+ * DEVICE array, caller-owned, at least as long as that call's n_events.  NULL (the default) = all protons.  A neutron enters with its own mass
  * and feels the neutron potential; the residual then has charge Z - n_p instead of Z + 1 - n_p.  Any other
  * value is an input error (INC_E_BADARG, found on the device like E_in out of range). */
 int inc_set_projectiles(const uint8_t *projectile /*DEVICE [n] or NULL*/);
@@ -131,6 +137,11 @@ int inc_set_chunk_events(int64_t n);
  * segments of the one track per pass along its collision-free path (drain helpers, DESIGN.md
  * section 6).  0 restores the default (48).  Results never depend on it. */
 int inc_set_long_track_threshold(int n_segments);
+/* Scheduling knob of the default (wavefront) cascade kernel: a segment pass advances its 32 resident tracks by up to
+ * `n` segments (1..8) before the tracks that collided, escaped or were absorbed are handed over and the lanes are
+ * refilled.  0 (the default) lets the library choose: 3 while every live target has A <= 20 (a track then continues
+ * in ~87 % of its segments), otherwise 2.  Results never depend on it. */
+int inc_set_segments_per_pass(int n);
 /* Global index of the first event of the following inc_simulate calls (default 0): event i of a
  * call uses the random stream of global event e = offset + i.  This is how a job is sharded over
  * several GPUs or calls with bit-identical per-event results (R-R4). */
@@ -215,6 +226,11 @@ int inc_get_drain_timeline(double ms[4] /*HOST*/);
  * lanes summed over those, [5] highest attempt number started in the drain, [6] tracks handed to drain helpers,
  * [7] ns at kernel entry.  Returns the number of warps written (<= max_warps), 0 if none was recorded.  Diagnostic. */
 int inc_get_warp_trace(uint32_t *out /*HOST [8 * max_warps]*/, int32_t max_warps);
+
+/* How many inc_simulate calls so far were run a second time with the lane-per-event cascade kernel because the
+ * wavefront kernel's per-warp track queues overflowed (an implementation limit of the default kernel, never a
+ * property of the result: both kernels give the same events).  Diagnostic; expected to stay 0. */
+int64_t inc_get_rerun_count(void);
 
 /* Nuclear-setup record of a target, for tests of inc_init (all HOST, fp64, length n_shells
  * except r, V_p, V_n which have n_shells+1; pointers may be NULL). */

@@ -18,6 +18,7 @@ ST_FAILED, ST_SEC_TRUNC, ST_DEPTH_CAP, ST_SEG_CAP, ST_TRIAL_CAP, ST_QUEUE_OVF = 
 F_CASCADE_ONLY, F_KEEP_TRANSPARENT, F_SAME_STREAM, F_STATS, F_LANE_PER_EVENT, F_TIMING, F_LANE_STATE_MACHINE = 1, 2, 4, 8, 16, 32, 64
 F_NO_DRAIN_HELPERS = 256
 F_NO_OVERLAP = 512
+F_TEST_QUEUE_OVF = 1024
 MAX_SEC = 64
 
 _DP = C.POINTER(C.c_double)
@@ -78,7 +79,7 @@ def make_tables_struct(t: dict):
 
 
 EXPORTS = ["inc_init", "inc_free_target", "inc_shutdown", "inc_set_stream", "inc_set_flags", "inc_set_event_offset",
-           "inc_get_stage_times", "inc_get_drain_timeline", "inc_get_warp_trace", "inc_set_vote_thresholds", "inc_set_long_track_threshold", "inc_set_chunk_events", "inc_set_projectiles", "inc_simulate",
+           "inc_get_stage_times", "inc_get_drain_timeline", "inc_get_warp_trace", "inc_get_rerun_count", "inc_set_vote_thresholds", "inc_set_long_track_threshold", "inc_set_segments_per_pass", "inc_set_chunk_events", "inc_set_projectiles", "inc_simulate",
            "inc_simulate_host", "inc_get_offsets", "inc_get_cascade_stage", "inc_get_stats", "inc_get_nucleus",
            "inc_measure_issue_peak", "inc_philox_blocks", "inc_tally", "inc_last_error", "inc_build_info"]
 
@@ -96,7 +97,7 @@ class IncLibrary:
     """One loaded variant ('f32' production, 'f64' parity) of the C-ABI library."""
 
     def __init__(self, variant: str = "f32", build_if_missing: bool = True):
-        if variant not in ("f32", "f64"):
+        if variant not in ("f32", "f64", "f64q"):
             raise ValueError(variant)
         self.variant = variant
         path = _build.lib_path(variant)
@@ -106,7 +107,7 @@ class IncLibrary:
             _build.build()
         self.path = path
         self.lib = L = C.CDLL(path, mode=C.RTLD_LOCAL)
-        self.real = np.float32 if variant == "f32" else np.float64
+        self.real = np.float32 if variant == "f32" else np.float64        # ("f64q": the small-queue test build of f64)
         vp = C.c_void_p
         L.inc_init.argtypes = [C.c_int, C.c_int, C.POINTER(IncTables)]
         L.inc_init.restype = C.c_int
@@ -128,6 +129,7 @@ class IncLibrary:
         L.inc_last_error.restype = C.c_char_p
         L.inc_build_info.restype = C.c_char_p
         L.inc_set_vote_thresholds.argtypes = [C.c_int, C.c_int]
+        L.inc_get_rerun_count.restype = C.c_int64
         self._tables_keep = None
 
     # ---- helpers ----
@@ -178,6 +180,9 @@ class IncLibrary:
     def inc_set_chunk_events(self, n: int):
         self._check(self.lib.inc_set_chunk_events(C.c_int64(int(n))))
 
+    def inc_set_segments_per_pass(self, n: int):
+        self._check(self.lib.inc_set_segments_per_pass(int(n)))
+
     def inc_set_long_track_threshold(self, n_segments: int):
         self._check(self.lib.inc_set_long_track_threshold(int(n_segments)))
 
@@ -190,6 +195,9 @@ class IncLibrary:
         buf = np.zeros((max_warps, 8), dtype=np.uint32)
         n = self._check(self.lib.inc_get_warp_trace(buf.ctypes.data_as(C.c_void_p), int(max_warps)))
         return buf[:n]
+
+    def inc_get_rerun_count(self) -> int:
+        return int(self.lib.inc_get_rerun_count())
 
     def inc_set_vote_thresholds(self, coll: int, epi: int):
         self._check(self.lib.inc_set_vote_thresholds(int(coll), int(epi)))

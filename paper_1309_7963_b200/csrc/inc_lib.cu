@@ -74,7 +74,8 @@ struct State {
   std::function<int(int, long long, int)> chunk_hook;
   // last call
   long long last_n = -1;
-  int last_chunks = 0;              // chunks of the last inc_simulate (the cascade stage survives single-chunk calls only)
+  int last_chunks = 0;
+  long long reruns = 0;             // calls run again with the lane kernel after a queue overflow of the wavefront kernel              // chunks of the last inc_simulate (the cascade stage survives single-chunk calls only)
   long long last_total = 0;
   long long event_offset = 0;
   // stage timing (INC_F_TIMING)
@@ -84,6 +85,7 @@ struct State {
   std::vector<cudaEvent_t> pending_events;   // 5 per chunk, resolved after the stream sync
   int vote_coll = 8, vote_epi = 8;
   int long_seg = kLongSegDefault;
+  int seg_per_pass = 0;             // 0 = chosen from the targets
   size_t chunk_events = (size_t)1 << 22;
   const uint8_t *projectile = nullptr;   // DEVICE, caller-owned; nullptr = protons
   int sm_count = 0;
@@ -396,6 +398,12 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   const bool naive = (g.flags & INC_F_LANE_PER_EVENT) != 0;
   cp.vote_coll = naive ? 1 : g.vote_coll; cp.vote_epi = naive ? 1 : g.vote_epi;
   cp.long_seg = g.long_seg;
+  {
+    // segment steps per pass of the wavefront kernel: three pay while collisions are rare (light targets), two otherwise
+    int a_max = 0;
+    for (int i = 0; i < INC_MAX_TARGETS; ++i) if (g.nuc[i].live && g.nuc[i].A > a_max) a_max = g.nuc[i].A;
+    cp.seg_per_pass = g.seg_per_pass > 0 ? g.seg_per_pass : (a_max <= 20 ? 3 : 2);
+  }
   cp.wtrace = nullptr;
   int n_stage = 0;
   for (int i = 0; i < INC_MAX_TARGETS; ++i) if (g.nuc[i].live) n_stage = i + 1;
@@ -560,8 +568,43 @@ void inc_shutdown(void) {
   g.event_offset = 0;
 }
 
+}  // extern "C"
+
+namespace {
+constexpr int64_t kQueueOverflow = -1000;   // internal: the wavefront kernel's track queues overflowed
+
+int64_t simulate_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
+                      int32_t *counts, inc_residual *res);
+}  // namespace
+
+extern "C" {
+
 int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
                      int32_t *counts, inc_residual *res) {
+  int64_t rc = simulate_once(n, E_in, tid, seed, sec, counts, res);
+  if (rc == kQueueOverflow) {
+    // The default cascade kernel keeps its tracks in fixed per-warp queues; a batch that overflows them (never seen:
+    // it takes ~190 simultaneous tracks in one warp's ~80 events) is run again with the lane-per-event kernel, which
+    // has no such limit and gives the same events (R-R4: a track's fate depends only on its own draws).
+    const uint32_t f = g.flags;
+    g.flags = (f | INC_F_LANE_STATE_MACHINE) & ~INC_F_TEST_QUEUE_OVF;
+    g.reruns++;
+    rc = simulate_once(n, E_in, tid, seed, sec, counts, res);
+    g.flags = f;
+    if (rc == kQueueOverflow) rc = fail(INC_E_STATE, "internal track-queue overflow (results invalid)");
+  }
+  g.projectile = nullptr;       // inc_set_projectiles applies to one call
+  return rc;
+}
+
+int64_t inc_get_rerun_count(void) { return g.reruns; }
+
+}  // extern "C"
+
+namespace {
+
+int64_t simulate_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
+                      int32_t *counts, inc_residual *res) {
   if (!g.tab.captured) return fail(INC_E_STATE, "inc_simulate before inc_init");
   if (n < 0 || !sec || !res || (n > 0 && (!E_in || !tid || !counts))) return fail(INC_E_BADARG, "null argument or n < 0");
   if (n > 0 && (!res->A || !res->Z || !res->Estar || !res->px || !res->py || !res->pz || !res->status))
@@ -577,6 +620,7 @@ int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64
   if (rc) return rc;
   CU_TRY(cudaMemsetAsync(g.d_ctr, 0, sizeof(DevCounters), g.stream));
   if (int rk_rc = set_round_keys(seed)) return rk_rc;
+  if (g.chunk_hook) { rc = g.chunk_hook(-1, 0, 0); if (rc) return rc; }     // (a rerun starts its pipeline afresh)
   for (auto e : g.pending_events) cudaEventDestroy(e);
   g.pending_events.clear();
   for (int i = 0; i < 4; ++i) { g.stage_ms[i] = 0; g.stage_launches[i] = 0; }
@@ -608,7 +652,7 @@ int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64
   g.last_n = n; g.last_total = (long long)tail.total;
   g.last_chunks = (int)((n + (long long)chunk - 1) / (long long)chunk);
   if (tail.err & 16u) return fail(INC_E_STATE, "watchdog: a warp of the wavefront cascade kernel made no progress (results invalid)");
-  if (tail.err & 4u) return fail(INC_E_STATE, "internal track-queue overflow in the wavefront cascade kernel (results invalid)");
+  if (tail.err & 4u) return kQueueOverflow;
   if (tail.err) {
     return fail(INC_E_BADARG, std::string("device-side input check failed:") + ((tail.err & 1u) ? " E_in outside [20,250] MeV" : "") +
                                   ((tail.err & 2u) ? " target_id not initialised" : "") +
@@ -621,6 +665,10 @@ int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64
   }
   return (int64_t)tail.total;
 }
+
+}  // namespace
+
+extern "C" {
 
 int inc_get_offsets(int64_t *dev_offsets) {
   if (g.last_n < 0) return fail(INC_E_STATE, "no previous inc_simulate");
@@ -713,6 +761,12 @@ int inc_set_projectiles(const uint8_t *projectile) {
 int inc_set_chunk_events(int64_t n) {
   if (n < 0 || (n > 0 && n < 1024) || n > ((int64_t)1 << 24)) return fail(INC_E_BADARG, "chunk size must be 0 (default) or 1024 .. 2^24");
   g.chunk_events = n == 0 ? ((size_t)1 << 22) : (size_t)n;
+  return 0;
+}
+
+int inc_set_segments_per_pass(int n) {
+  if (n < 0 || n > 8) return fail(INC_E_BADARG, "segments per pass must be 0 (automatic) or 1..8");
+  g.seg_per_pass = n;
   return 0;
 }
 
@@ -853,6 +907,11 @@ int64_t inc_simulate_host(int64_t n, const INC_REAL *E_in, const int32_t *tid, u
     return 0;
   };
   g.chunk_hook = [&](int c, long long e0, int nc) -> int {
+    if (c < 0) {                    // start of a run
+      CU_TRY(cudaStreamSynchronize(h.copy_stream));
+      pend.clear();
+      return 0;
+    }
     if (c >= kMaxHostChunks) return fail(INC_E_BADARG, "inc_simulate_host: too many chunks (raise the chunk size)");
     while ((int)h.ev.size() <= c) {
       cudaEvent_t e;

@@ -214,11 +214,17 @@ def test_drain_helpers_change_nothing(gpu, orc, otables, ptables, variant, cfg, 
     lib = gpu.load(variant)
     runs = []
     try:
-        for thr, flags in ((2, 0), (0, 0), (0, gpu.F_NO_DRAIN_HELPERS), (16, 0)):
+        # (F_NO_OVERLAP: the evaporation kernel starts after the cascade kernel instead of consuming its completion
+        # list while the last cascade CTAs drain)
+        for thr, flags in ((2, 0), (0, 0), (0, gpu.F_NO_DRAIN_HELPERS), (16, 0), (0, gpu.F_NO_OVERLAP), (2, gpu.F_NO_OVERLAP | gpu.F_TIMING)):
             lib.inc_set_long_track_threshold(thr)
             runs.append(gpu.simulate(lib, targets, E, tid, seed, ptables, flags=flags))
+        for spp in (1, 2, 5):           # segment steps per pass of the wavefront kernel
+            lib.inc_set_segments_per_pass(spp)
+            runs.append(gpu.simulate(lib, targets, E, tid, seed, ptables))
     finally:
         lib.inc_set_long_track_threshold(0)
+        lib.inc_set_segments_per_pass(0)
     for other in runs[1:]:
         for k in ("species", "T", "ux", "uy", "uz", "counts", "A", "Z", "Estar", "px", "py", "pz", "status", "offsets"):
             assert np.array_equal(runs[0][k], other[k]), k
@@ -226,6 +232,30 @@ def test_drain_helpers_change_nothing(gpu, orc, otables, ptables, variant, cfg, 
         o = orc.simulate(otables, targets, E, tid, seed)
         frac, max_err, _ = H.event_identity(runs[0], o, rel=REL_F64)
         assert frac >= FRAC_IDENTICAL and max_err <= REL_F64
+
+
+@pytest.mark.parametrize("cfg,n", [(5, 20000), (4, 20000)])
+def test_small_queue_build_and_overflow_rerun(gpu, ptables, cfg, n):
+    """Capacity guards of the wavefront scheduler (a full segment queue with more than QC - 32 waiting
+    collisions had no pass it could run).  `f64q` is the f64 library built with 64-entry segment and 33-entry
+    collision queues, where partial collision passes and lane-capped segment passes happen all the time; its
+    events must be those of the normal build, bit for bit.  If its queues really overflow, or when the test hook
+    reports an overflow, inc_simulate runs the call again with the lane kernel: same events again."""
+    E, tid, targets, seed, _ = _inputs(cfg, n)
+    ref = gpu.simulate(gpu.load("f64"), targets, E, tid, seed, ptables)
+    keys = ("species", "T", "ux", "uy", "uz", "counts", "A", "Z", "Estar", "px", "py", "pz", "status", "offsets")
+    small = gpu.load("f64q")
+    r0 = small.inc_get_rerun_count()
+    got = gpu.simulate(small, targets, E, tid, seed, ptables)
+    for k in keys:
+        assert np.array_equal(ref[k], got[k]), k
+    print(f"[small queues] config {cfg}: reruns with the lane kernel: {small.inc_get_rerun_count() - r0}")
+    lib = gpu.load("f64")
+    r1 = lib.inc_get_rerun_count()
+    forced = gpu.simulate(lib, targets, E, tid, seed, ptables, flags=gpu.F_TEST_QUEUE_OVF)
+    assert lib.inc_get_rerun_count() == r1 + 1
+    for k in keys:
+        assert np.array_equal(ref[k], forced[k]), k
 
 
 def test_fp64_transparent_and_failed(gpu, orc, ptables):
@@ -285,6 +315,19 @@ def test_error_paths(gpu, ptables):
     assert str(total) in lib.last_error()
     assert torch.equal(small["counts"], big["counts"])
     assert torch.equal(small["T"][:100], big["T"][:100])
+    # the post-cascade records are per chunk: after a multi-chunk call the stage is gone, however large an earlier
+    # call's workspace was; and the last argument is the count, not the packed word
+    lib.inc_simulate(E, tid, 3, big)
+    st = lib.inc_get_cascade_stage(n)
+    assert int(st["meta"].max()) < 64 and int(st["meta"].min()) >= 0
+    lib.inc_set_chunk_events(1024)
+    try:
+        lib.inc_simulate(E, tid, 3, big)
+        with pytest.raises(gpu.IncError) as ei:
+            lib.inc_get_cascade_stage(n)
+        assert ei.value.code == gpu.INC_E_STATE
+    finally:
+        lib.inc_set_chunk_events(0)
     lib.inc_free_target(t0)
     assert lib.inc_simulate(E, tid, 3, big, check=False) == gpu.INC_E_BADARG
 
@@ -483,6 +526,20 @@ def test_neutron_projectiles(gpu, orc, otables, ptables, cfg, n):
     with pytest.raises(gpu.IncError) as ei:
         gpu.simulate(lib32, targets, E, tid, seed, ptables, projectile=bad)
     assert ei.value.code == -1 and "projectile" in str(ei.value)
+    # inc_set_projectiles holds for ONE call: the next one is all protons again, whatever became of the array
+    m = 2000
+    ref_p = gpu.simulate(lib32, targets, E[:m], tid[:m], seed, ptables)                       # leaves the targets initialised
+    Ed = torch.as_tensor(np.asarray(E[:m], dtype=np.float32), device="cuda")
+    td = torch.as_tensor(np.asarray(tid[:m], dtype=np.int32), device="cuda")                  # (slots are 0..k-1 in order)
+    out = lib32.alloc_outputs(m, m * 24)
+    pj = torch.zeros(m, dtype=torch.uint8, device="cuda")
+    lib32.inc_set_projectiles(pj)
+    lib32.inc_simulate(Ed, td, seed, out)
+    assert not np.array_equal(out["Z"].cpu().numpy(), ref_p["Z"])                              # neutrons went in
+    del pj
+    lib32._projectile = None
+    lib32.inc_simulate(Ed, td, seed, out)
+    assert np.array_equal(out["Z"].cpu().numpy(), ref_p["Z"]) and np.array_equal(out["counts"].cpu().numpy(), ref_p["counts"])
 
 
 def test_host_path_streams_in_chunks(gpu, ptables):

@@ -22,11 +22,11 @@ def test_library_exports_every_declared_symbol():
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
     declared = set(re.findall(r"\b(inc_[a-z_0-9]+)\s*\(", hdr))
     assert {"inc_init", "inc_simulate", "inc_simulate_host", "inc_get_offsets"} <= declared
-    for variant in ("f32", "f64"):
+    for variant in ("f32", "f64", "f64q"):
         lib = B.load(variant)
         for name in sorted(declared):
             assert hasattr(lib.lib, name), (variant, name)
-        assert variant in lib.build_info()
+        assert variant[:3] in lib.build_info()
     assert declared == set(B.EXPORTS)
 
 
