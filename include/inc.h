@@ -92,7 +92,7 @@ extern "C" {
 
 /* ---- model inputs ("precalculated ... tables and other read-only input data") ----- */
 typedef struct inc_tables {   /* HOST memory, caller-owned, copied during inc_init           */
-  int32_t version;            /* = 1                                                         */
+  int32_t version;            /* 1: the fields up to evap_a_div; 2: also the level-density block at the end */
   int32_t n_xs;               /* NN grid points (<= 4096); plab_k = k*plab_max/(n_xs-1) GeV/c */
   double plab_max;
   const double *sig_pp, *sig_np;    /* [n_xs] elastic NN cross sections, mb (pp also for nn) */
@@ -103,6 +103,21 @@ typedef struct inc_tables {   /* HOST memory, caller-owned, copied during inc_in
   int32_t n_shells;                 /* 15; 1..32                                      */
   double semf[5];                   /* a_v a_s a_c a_a a_p, MeV ("semi-empirical mass formula") */
   double evap_r0, evap_rj, evap_a_div; /* 1.5 fm, 1.2 fm, 8 (R-E1)                           */
+  /* ---- version 2: level density of the evaporation stage ("we adopt the generalized
+   * evaporation model (GEM) [18]").  level_density = 0 is the frozen Weisskopf-Ewing model rho ~ exp(2 sqrt(a U)),
+   * a = A_d / evap_a_div (R-Q19); level_density = 1 is the GEM level density (DESIGN.md R-G1..G6): Fermi gas with
+   * the pre-exponential factor, rho(U) = exp(2 sqrt(a (U - delta))) / (a^(1/4) (U - delta)^(5/4)), above the
+   * Gilbert-Cameron matching energy E_x = U_x + delta, U_x = 150/A_d + 2.5 MeV, and the constant-temperature form
+   * exp((U - E_0)/T)/T below it, with T, E_0 from continuity of value and slope convention of [18]
+   * (1/T = sqrt(a/U_x) - 1.5/U_x).  Pairing energies and shell corrections are CALLER INPUTS like the NN tables
+   * (the paper prints none): delta = pair_Z[Z_d] + pair_N[N_d]; a = A_d (gc_a0 + gc_a1 (shell_Z[Z_d] + shell_N[N_d]));
+   * indices beyond the arrays count as 0; a <= 0 closes the channel.  It changes the emission widths (E2) and the
+   * energy sampler (E4) only. */
+  int32_t level_density;
+  int32_t n_ldZ, n_ldN;              /* lengths of the arrays below (may be 0 with NULL pointers)            */
+  const double *pair_Z, *pair_N;     /* [n_ldZ], [n_ldN] pairing energies, MeV                               */
+  const double *shell_Z, *shell_N;   /* [n_ldZ], [n_ldN] shell corrections, MeV                              */
+  double gc_a0, gc_a1;               /* 1/8 MeV^-1 and 0.00917 MeV^-2 in [18]                                */
 } inc_tables;
 
 /* inc_init — nuclear setup for one target (Woods-Saxon -> n_shells constant-density

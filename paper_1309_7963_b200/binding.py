@@ -37,6 +37,8 @@ class IncTables(C.Structure):
         ("n_evz", C.c_int32), ("ev_Z", _DP), ("ev_kp", _DP), ("ev_cp", _DP), ("ev_ka", _DP), ("ev_ca", _DP),
         ("ws_c0", C.c_double), ("ws_delta", C.c_double), ("ws_rpad", C.c_double), ("n_shells", C.c_int32),
         ("semf", C.c_double * 5), ("evap_r0", C.c_double), ("evap_rj", C.c_double), ("evap_a_div", C.c_double),
+        ("level_density", C.c_int32), ("n_ldZ", C.c_int32), ("n_ldN", C.c_int32),
+        ("pair_Z", _DP), ("pair_N", _DP), ("shell_Z", _DP), ("shell_N", _DP), ("gc_a0", C.c_double), ("gc_a1", C.c_double),
     ]
 
 
@@ -75,6 +77,19 @@ def make_tables_struct(t: dict):
     for i in range(5):
         s.semf[i] = float(t["semf"][i])
     s.evap_r0, s.evap_rj, s.evap_a_div = float(t["evap_r0"]), float(t["evap_rj"]), float(t["evap_a_div"])
+    # version 2 block (level density); a version 1 dict leaves it zeroed and the library never reads it
+    s.level_density = int(t.get("level_density", 0))
+    s.gc_a0, s.gc_a1 = float(t.get("gc_a0", 0.125)), float(t.get("gc_a1", 0.00917))
+    for cnt, names in (("n_ldZ", ("pair_Z", "shell_Z")), ("n_ldN", ("pair_N", "shell_N"))):
+        arrs = [np.ascontiguousarray(t[k], dtype=np.float64) for k in names if t.get(k) is not None]
+        n = max([len(a) for a in arrs], default=0)
+        setattr(s, cnt, n)
+        for k in names:
+            a = np.zeros(max(n, 1))
+            if t.get(k) is not None:
+                a[:len(t[k])] = np.asarray(t[k], dtype=np.float64)
+            keep.append(a)
+            setattr(s, k, a.ctypes.data_as(_DP))
     return s, keep
 
 

@@ -72,11 +72,22 @@ template <typename R> struct __align__(16) EvChan {        // per (A_d, Z_d, cha
   R BdBj;     // B(A_d,Z_d) + B_j, so that X = E* - B(parent) + BdBj - V
 };
 
+// NEXT-2 (GEM level density, R-G2..G4): constants of one daughter nucleus; a = 0 => no level density (channel closed)
+template <typename R> struct __align__(16) LdDev {
+  R a, delta;     // level-density parameter MeV^-1, pairing energy MeV
+  R Ux, Ex;       // matching energy U_x = 150/A_d + 2.5 and E_x = U_x + delta
+  R T, E0;        // constant-temperature branch below E_x: rho = exp((U - E0)/T)/T
+  R lnT, lna4;    // ln T, (1/4) ln a
+};
+template <typename R> struct GaussNodes { R x[16], w[16]; };
+__constant__ GaussNodes<INC_REAL> c_gl;     // 16-point Gauss-Legendre on [-1, 1] (width integral of the GEM mode)
+
 template <typename R> struct ModelDev {
   const R *tabS;          // [n_xs][4]  {sig_pp, dsig_pp, sig_np, dsig_np} in fm^2 (mb * 0.1)
   const R *tabC;          // [n_xs][8]  {B_pp, dB_pp, B_np, dB_np, a_np, da_np, 0, 0}
   const R *bind;          // [kAmax][kZmax] binding energy, MeV; < -1e29 => no such nucleus
   const EvChan<R> *evch;  // [kAmax][kZmax][6]
+  const LdDev<R> *ld;     // [kAmax][kZmax]  (level_density = 1 only)
   const NucDev<R> *nuc;   // [INC_MAX_TARGETS]
   int32_t n_xs;
   R inv_dp;               // 1 / (grid step in MeV/c)
@@ -1572,7 +1583,48 @@ __device__ __forceinline__ void G13_scaled(R s, R s_ref, R &g1, R &g3) {
   }
 }
 
-template <typename R, bool STATS>
+// ---- NEXT-2: GEM level density (DESIGN.md R-G1..G6) ----
+// ln rho(U): Fermi gas with the pre-exponential factor above E_x, constant temperature below (R-G1, R-G5)
+template <typename R>
+__device__ __forceinline__ R gem_lnrho(const LdDev<R> &ld, R U) {
+  if (U >= ld.Ex) {
+    const R u = U - ld.delta;
+    return R(2) * M<R>::sqrt_(ld.a * u) - ld.lna4 - R(1.25) * M<R>::log_(u);
+  }
+  return M<R>::div_(U - ld.E0, ld.T) - ld.lnT;
+}
+
+// int_x0^x1 (x + beta) rho(X - x) e^(-lref) dx: panels of at most 8 MeV, 16 Gauss-Legendre nodes each (R-G5: the
+// definition, evaluated by quadrature)
+template <typename R>
+__device__ __forceinline__ R gem_range(const LdDev<R> &ld, R X, R beta, R x0, R x1, R lref) {
+  if (!(x1 > x0)) return R(0);
+  int np = (int)ceil((double)((x1 - x0) * R(0.125)));
+  np = np < 1 ? 1 : np;
+  const R h = M<R>::div_(x1 - x0, R(np));
+  R sum = R(0);
+#pragma unroll 1
+  for (int p = 0; p < np; ++p) {
+    const R a0 = x0 + h * R(p);
+#pragma unroll 1
+    for (int q = 0; q < 16; ++q) {
+      const R x = a0 + R(0.5) * h * (c_gl.x[q] + R(1));
+      R U = X - x;
+      U = U < R(0) ? R(0) : U;
+      sum += R(0.5) * h * c_gl.w[q] * (x + beta) * M<R>::exp_(gem_lnrho<R>(ld, U) - lref);
+    }
+  }
+  return sum;
+}
+
+template <typename R>
+__device__ __forceinline__ R gem_integral(const LdDev<R> &ld, R X, R beta, R lref) {
+  const R xs = X - ld.Ex;                         // x below xs: daughter above E_x (Fermi gas)
+  if (xs <= R(0)) return gem_range<R>(ld, X, beta, R(0), X, lref);
+  return gem_range<R>(ld, X, beta, R(0), xs, lref) + gem_range<R>(ld, X, beta, xs, X, lref);
+}
+
+template <typename R, bool STATS, bool GEM>
 __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const EvapParams<R> P) {
   const int lane = threadIdx.x & 31;
   const bool cascade_only = (P.flags & INC_F_CASCADE_ONLY) != 0;
@@ -1598,6 +1650,8 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
   int jsel = -1, ntrial = 0;
   R Bpar = R(0), X = R(0), a = R(1), beta = R(0), V = R(0), BdBj = R(0), s = R(0), T = R(1), areaA = R(0), areaB = R(0);
   R u1 = R(0), u2 = R(0);
+  LdDev<R> ldsel;           // GEM mode: level density of the chosen channel's daughter
+  ldsel.a = ldsel.delta = ldsel.Ux = ldsel.Ex = ldsel.T = ldsel.E0 = ldsel.lnT = ldsel.lna4 = R(0);
   for (;;) {
     __syncwarp();
     // ---- refill idle lanes from the warp's pool of 32 consecutive entries of the cascade kernel's completion list
@@ -1671,7 +1725,20 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
           const EvChan<R> c = P.model.evch[(Ad * kZmax + Zd) * 6 + j];
           if (c.pref > R(0)) {
             const R Xc = Es - Bpar + c.BdBj - c.V;
-            if (Xc > R(0)) {
+            if (GEM) {
+              // (GEM mode: sj = ln rho(X) of the daughter, the largest value of the integrand's density; s_ref, their
+              // maximum, scales the f32 integrals like e^{-s_max} does in the Weisskopf-Ewing mode)
+              if (Xc > R(0)) {
+                const LdDev<R> ld = P.model.ld[Ad * kZmax + Zd];
+                if (ld.a > R(0)) {
+                  ch[j] = c;
+                  Xj[j] = Xc;
+                  sj[j] = gem_lnrho<R>(ld, Xc);
+                  s_ref = (!any || sj[j] > s_ref) ? sj[j] : s_ref;
+                  any = true;
+                }
+              }
+            } else if (Xc > R(0)) {
               ch[j] = c;
               Xj[j] = Xc;
               aj[j] = M<R>::div_(R(Ad), P.model.a_div);
@@ -1691,7 +1758,16 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
 #pragma unroll
         for (int j = 0; j < 6; ++j) {
           W[j] = R(0);
-          if (Xj[j] > R(0)) {
+          if (GEM) {
+            if (Xj[j] > R(0)) {
+              // R-G5: W_j = g_j M_j A_d^(2/3) alpha_j int_0^X (x + beta) rho(X - x) dx by quadrature (the f64 build
+              // leaves the integrand unscaled, like the oracle)
+              const LdDev<R> ld = P.model.ld[((A - c_evA[j]) * kZmax + (Z - c_evZ[j]))];
+              const R w = ch[j].pref * gem_integral<R>(ld, Xj[j], ch[j].beta, sizeof(R) == 4 ? s_ref : R(0));
+              W[j] = w > R(0) ? w : R(0);
+              Wsum += W[j];
+            }
+          } else if (Xj[j] > R(0)) {
             R g1, g3;
             G13_scaled<R>(sj[j], s_ref, g1, g3);
             const R I0 = M<R>::div_(g1, R(2) * aj[j]);
@@ -1716,8 +1792,22 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
           }
 #pragma unroll
           for (int j = 0; j < 6; ++j) if (j == jsel) { X = Xj[j]; a = aj[j]; beta = ch[j].beta; V = ch[j].V; BdBj = ch[j].BdBj; }
-          s = R(2) * M<R>::sqrt_(a * X);
-          T = M<R>::sqrt_(M<R>::div_(X, a));
+          if (GEM) {
+            // R-G6: envelope slope = the smallest slope of ln rho on [0, X]: 1/T of the constant-temperature branch,
+            // or the Fermi-gas slope at X if that is smaller; s holds ln rho(X)
+            ldsel = P.model.ld[((A - c_evA[jsel]) * kZmax + (Z - c_evZ[jsel]))];
+            R mm = M<R>::div_(R(1), ldsel.T);
+            if (X > ldsel.Ex) {
+              const R uu = X - ldsel.delta;
+              const R sfg = M<R>::sqrt_(M<R>::div_(ldsel.a, uu)) - M<R>::div_(R(1.25), uu);
+              mm = sfg < mm ? sfg : mm;
+            }
+            T = M<R>::div_(R(1), mm);
+            s = gem_lnrho<R>(ldsel, X);
+          } else {
+            s = R(2) * M<R>::sqrt_(a * X);
+            T = M<R>::sqrt_(M<R>::div_(X, a));
+          }
           areaA = T * (T + beta); areaB = R(0.5) * X * X + beta * X;
           sampling = true; ntrial = 0;
         }
@@ -1740,11 +1830,15 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
           xx = -beta + M<R>::sqrt_(beta * beta + v[1] * (X * X + R(2) * beta * X));
           R rem = X - xx;
           rem = rem > R(0) ? rem : R(0);
-          if (M<R>::log_(v[3]) < R(2) * M<R>::sqrt_(a * rem) - s) { xs = xx < X ? xx : X; pending = false; }
+          const R lr = GEM ? gem_lnrho<R>(ldsel, rem) : R(2) * M<R>::sqrt_(a * rem);
+          if (M<R>::log_(v[3]) < lr - s) { xs = xx < X ? xx : X; pending = false; }
         } else {
           if (v[0] * (T + beta) < T) xx = -T * M<R>::log_(v[1] * v[2]);
           else xx = -T * M<R>::log_(v[1]);
-          if (xx < X && M<R>::log_(v[3]) < R(2) * M<R>::sqrt_(a * (X - xx)) - s + M<R>::div_(xx, T)) { xs = xx; pending = false; }
+          if (xx < X) {
+            const R lr = GEM ? gem_lnrho<R>(ldsel, X - xx) : R(2) * M<R>::sqrt_(a * (X - xx));
+            if (M<R>::log_(v[3]) < lr - s + M<R>::div_(xx, T)) { xs = xx; pending = false; }
+          }
         }
       }
     }

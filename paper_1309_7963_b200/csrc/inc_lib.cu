@@ -40,6 +40,10 @@ struct TablesHost {
   double plab_max = 0, ws_c0 = 0, ws_delta = 0, ws_rpad = 0, semf[5] = {0, 0, 0, 0, 0};
   double evap_r0 = 0, evap_rj = 0, evap_a_div = 0;
   std::vector<double> sig_pp, sig_np, B_pp, B_np, a_np, ev_Z, ev_kp, ev_cp, ev_ka, ev_ca;
+  // version 2 block: level density of the evaporation stage (NEXT-2)
+  int level_density = 0;
+  double gc_a0 = 0.125, gc_a1 = 0.00917;
+  std::vector<double> pair_Z, pair_N, shell_Z, shell_N;
 };
 
 struct State {
@@ -50,6 +54,7 @@ struct State {
   // device model
   real *d_tabS = nullptr, *d_tabC = nullptr, *d_bind = nullptr;
   EvChan<real> *d_evch = nullptr;
+  LdDev<real> *d_ld = nullptr;
   NucDev<real> *d_nuc = nullptr;
   DevCounters *d_ctr = nullptr;
   uint32_t *d_wtrace = nullptr; int wtrace_warps = 0;   // inc_get_warp_trace (INC_F_TIMING)
@@ -219,7 +224,16 @@ void fill_nucdev(const HostNucleus &h, NucDev<real> &d) {
 
 int check_tables(const inc_tables *t) {
   if (!t) return fail(INC_E_BADARG, "tables is NULL");
-  if (t->version != 1) return fail(INC_E_TABLES, "tables.version != 1");
+  if (t->version != 1 && t->version != 2) return fail(INC_E_TABLES, "tables.version must be 1 or 2");
+  if (t->version >= 2) {
+    if (t->level_density != 0 && t->level_density != 1) return fail(INC_E_TABLES, "level_density must be 0 or 1");
+    if (t->n_ldZ < 0 || t->n_ldN < 0 || t->n_ldZ > 4096 || t->n_ldN > 4096) return fail(INC_E_TABLES, "bad level-density array length");
+    if ((t->n_ldZ > 0 && (!t->pair_Z || !t->shell_Z)) || (t->n_ldN > 0 && (!t->pair_N || !t->shell_N)))
+      return fail(INC_E_TABLES, "NULL level-density array");
+    for (int i = 0; i < t->n_ldZ; ++i) if (!std::isfinite(t->pair_Z[i]) || !std::isfinite(t->shell_Z[i])) return fail(INC_E_TABLES, "NaN in pair_Z / shell_Z");
+    for (int i = 0; i < t->n_ldN; ++i) if (!std::isfinite(t->pair_N[i]) || !std::isfinite(t->shell_N[i])) return fail(INC_E_TABLES, "NaN in pair_N / shell_N");
+    if (t->level_density == 1 && !(t->gc_a0 > 0)) return fail(INC_E_TABLES, "gc_a0 must be positive");
+  }
   if (t->n_xs < 2 || t->n_xs > 4096 || !(t->plab_max > 0)) return fail(INC_E_TABLES, "bad NN grid");
   if (!t->sig_pp || !t->sig_np || !t->B_pp || !t->B_np || !t->a_np) return fail(INC_E_TABLES, "NULL NN table");
   if (t->n_evz < 1 || t->n_evz > 16 || !t->ev_Z || !t->ev_kp || !t->ev_cp || !t->ev_ka || !t->ev_ca)
@@ -245,6 +259,13 @@ void copy_tables(const inc_tables *t, TablesHost &h) {
   cp(h.B_np, t->B_np, t->n_xs); cp(h.a_np, t->a_np, t->n_xs);
   cp(h.ev_Z, t->ev_Z, t->n_evz); cp(h.ev_kp, t->ev_kp, t->n_evz); cp(h.ev_cp, t->ev_cp, t->n_evz);
   cp(h.ev_ka, t->ev_ka, t->n_evz); cp(h.ev_ca, t->ev_ca, t->n_evz);
+  h.level_density = 0; h.gc_a0 = 0.125; h.gc_a1 = 0.00917;
+  h.pair_Z.clear(); h.pair_N.clear(); h.shell_Z.clear(); h.shell_N.clear();
+  if (t->version >= 2) {
+    h.level_density = t->level_density; h.gc_a0 = t->gc_a0; h.gc_a1 = t->gc_a1;
+    cp(h.pair_Z, t->pair_Z, t->n_ldZ); cp(h.shell_Z, t->shell_Z, t->n_ldZ);
+    cp(h.pair_N, t->pair_N, t->n_ldN); cp(h.shell_N, t->shell_N, t->n_ldN);
+  }
   h.captured = true;
 }
 
@@ -253,7 +274,17 @@ bool same_tables(const inc_tables *t, const TablesHost &h) {
   if (t->ws_c0 != h.ws_c0 || t->ws_delta != h.ws_delta || t->ws_rpad != h.ws_rpad) return false;
   if (t->evap_r0 != h.evap_r0 || t->evap_rj != h.evap_rj || t->evap_a_div != h.evap_a_div) return false;
   for (int i = 0; i < 5; ++i) if (t->semf[i] != h.semf[i]) return false;
-  auto eq = [](const std::vector<double> &v, const double *p) { return std::memcmp(v.data(), p, v.size() * sizeof(double)) == 0; };
+  auto eq = [](const std::vector<double> &v, const double *p) { return v.empty() || std::memcmp(v.data(), p, v.size() * sizeof(double)) == 0; };
+  {
+    // version 2 block (a version 1 struct means: level_density 0, no arrays)
+    const int ld = t->version >= 2 ? t->level_density : 0;
+    if (ld != h.level_density) return false;
+    if (t->version >= 2) {
+      if (t->gc_a0 != h.gc_a0 || t->gc_a1 != h.gc_a1) return false;
+      if ((size_t)t->n_ldZ != h.pair_Z.size() || (size_t)t->n_ldN != h.pair_N.size()) return false;
+      if (!eq(h.pair_Z, t->pair_Z) || !eq(h.shell_Z, t->shell_Z) || !eq(h.pair_N, t->pair_N) || !eq(h.shell_N, t->shell_N)) return false;
+    } else if (!h.pair_Z.empty() || !h.pair_N.empty()) return false;
+  }
   return eq(h.sig_pp, t->sig_pp) && eq(h.sig_np, t->sig_np) && eq(h.B_pp, t->B_pp) && eq(h.B_np, t->B_np) &&
          eq(h.a_np, t->a_np) && eq(h.ev_Z, t->ev_Z) && eq(h.ev_kp, t->ev_kp) && eq(h.ev_cp, t->ev_cp) &&
          eq(h.ev_ka, t->ev_ka) && eq(h.ev_ca, t->ev_ca);
@@ -306,6 +337,35 @@ int upload_model() {
         e.V = (real)V; e.pref = (real)(kEvG[j] * Mj * ad13 * ad13 * alpha); e.beta = (real)beta; e.BdBj = (real)(Bd + Bj);
       }
     }
+  // NEXT-2: level-density constants per daughter nucleus (R-G2..G4) and the 16 Gauss-Legendre nodes of the width integral
+  std::vector<LdDev<real>> ldv((size_t)kAmax * kZmax);
+  std::memset(ldv.data(), 0, ldv.size() * sizeof(LdDev<real>));
+  if (t.level_density == 1) {
+    auto tab = [](const std::vector<double> &y, int i) { return (i >= 0 && i < (int)y.size()) ? y[i] : 0.0; };
+    for (int Ad = 1; Ad < kAmax; ++Ad)
+      for (int Zd = 0; Zd < kZmax && Zd <= Ad; ++Zd) {
+        if (!valid_nucleus(Ad, Zd)) continue;
+        const int Nd = Ad - Zd;
+        const double S = tab(t.shell_Z, Zd) + tab(t.shell_N, Nd);
+        const double a = (double)Ad * (t.gc_a0 + t.gc_a1 * S);                      // R-G2
+        const double delta = tab(t.pair_Z, Zd) + tab(t.pair_N, Nd);                 // R-G3
+        const double Ux = 150.0 / (double)Ad + 2.5;                                 // R-G4
+        LdDev<real> &d = ldv[(size_t)Ad * kZmax + Zd];
+        if (!(a > 0.0)) continue;                                                   // a = 0 in the table: channel closed
+        const double Ex = Ux + delta;
+        const double invT = std::sqrt(a / Ux) - 1.5 / Ux;
+        const double T = 1.0 / invT;
+        const double E0 = Ex - T * (std::log(T) - 0.25 * std::log(a) - 1.25 * std::log(Ux) + 2.0 * std::sqrt(a * Ux));
+        d.a = (real)a; d.delta = (real)delta; d.Ux = (real)Ux; d.Ex = (real)Ex; d.T = (real)T; d.E0 = (real)E0;
+        d.lnT = (real)std::log(T); d.lna4 = (real)(0.25 * std::log(a));
+      }
+    std::vector<double> gx, gw;
+    gauss_legendre(16, gx, gw);
+    // (nodes in the order of the Newton start values cos(pi (i + 3/4) / 16.5), i = 0..15, so that a panel sum runs in one fixed order)
+    GaussNodes<real> gn;
+    for (int i = 0; i < 16; ++i) { gn.x[i] = (real)gx[i]; gn.w[i] = (real)gw[i]; }
+    CU_TRY(cudaMemcpyToSymbol(c_gl, &gn, sizeof(gn)));
+  }
   auto up = [&](void **dst, const void *src, size_t bytes) -> cudaError_t {
     if (*dst) cudaFree(*dst);
     cudaError_t e = cudaMalloc(dst, bytes);
@@ -316,6 +376,7 @@ int upload_model() {
   CU_TRY(up((void **)&g.d_tabC, Cc.data(), Cc.size() * sizeof(real)));
   CU_TRY(up((void **)&g.d_bind, bind.data(), bind.size() * sizeof(real)));
   CU_TRY(up((void **)&g.d_evch, ev.data(), ev.size() * sizeof(EvChan<real>)));
+  CU_TRY(up((void **)&g.d_ld, ldv.data(), ldv.size() * sizeof(LdDev<real>)));
   if (!g.d_nuc) {
     CU_TRY(cudaMalloc((void **)&g.d_nuc, sizeof(NucDev<real>) * INC_MAX_TARGETS));
     CU_TRY(cudaMemset(g.d_nuc, 0, sizeof(NucDev<real>) * INC_MAX_TARGETS));
@@ -329,7 +390,7 @@ int upload_model() {
 
 ModelDev<real> model_dev() {
   ModelDev<real> m;
-  m.tabS = g.d_tabS; m.tabC = g.d_tabC; m.bind = g.d_bind; m.evch = g.d_evch; m.nuc = g.d_nuc;
+  m.tabS = g.d_tabS; m.tabC = g.d_tabC; m.bind = g.d_bind; m.evch = g.d_evch; m.nuc = g.d_nuc; m.ld = g.d_ld;
   m.n_xs = g.tab.n_xs;
   m.inv_dp = (real)(1.0 / (g.tab.plab_max / (g.tab.n_xs - 1) * 1000.0));
   m.a_div = (real)g.tab.evap_a_div;
@@ -454,7 +515,7 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   ep.model = model; ep.ws = g.ws; ep.ctr = g.d_ctr; ep.e_base = e_base + g.event_offset; ep.n_chunk = n_chunk;
   ep.seed_lo = cp.seed_lo; ep.seed_hi = cp.seed_hi; ep.flags = g.flags;
   ep.out_counts = counts;
-  auto ekern = evap_kernel<real, STATS>;
+  auto ekern = g.tab.level_density == 1 ? evap_kernel<real, STATS, true> : evap_kernel<real, STATS, false>;
   int eocc = 0;
   CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&eocc, ekern, 256, 0));
   if (eocc < 1) return fail(INC_E_CUDA, "evaporation kernel does not fit on an SM");
@@ -551,7 +612,7 @@ int inc_free_target(int id) {
 
 void inc_shutdown(void) {
   free_ws();
-  void **p[] = {(void **)&g.d_tabS, (void **)&g.d_tabC, (void **)&g.d_bind, (void **)&g.d_evch, (void **)&g.d_nuc,
+  void **p[] = {(void **)&g.d_tabS, (void **)&g.d_tabC, (void **)&g.d_bind, (void **)&g.d_evch, (void **)&g.d_ld, (void **)&g.d_nuc,
                 (void **)&g.d_ctr, (void **)&g.d_wtrace, (void **)&g.d_offsets, (void **)&g.d_tiles,
                 (void **)&g.hp.E, (void **)&g.hp.tid, (void **)&g.hp.counts, (void **)&g.hp.A, (void **)&g.hp.Z,
                 (void **)&g.hp.Es, (void **)&g.hp.px, (void **)&g.hp.py, (void **)&g.hp.pz, (void **)&g.hp.status,

@@ -66,9 +66,12 @@ def evap_tables() -> dict:
 
 def default_tables(**overrides) -> dict:
     """Everything inc_init needs, as a plain dict (see binding.IncTables)."""
-    t = dict(version=1, n_xs=N_XS, plab_max=PLAB_MAX, n_shells=N_SHELLS,
+    t = dict(version=2, n_xs=N_XS, plab_max=PLAB_MAX, n_shells=N_SHELLS,
              ws_c0=WS_C0, ws_delta=WS_DELTA, ws_rpad=WS_RPAD, semf=SEMF,
-             evap_r0=EVAP_R0, evap_rj=EVAP_RJ, evap_a_div=EVAP_A_DIV)
+             evap_r0=EVAP_R0, evap_rj=EVAP_RJ, evap_a_div=EVAP_A_DIV,
+             # level density of the evaporation stage (inc.h, version 2 block): 0 = the frozen Weisskopf-Ewing model;
+             # 1 = GEM level density with the caller's pairing energies and shell corrections (none by default)
+             level_density=0, pair_Z=None, pair_N=None, shell_Z=None, shell_N=None, gc_a0=0.125, gc_a1=0.00917)
     t.update(nn_tables(t["n_xs"], t["plab_max"]))
     t.update(evap_tables())
     t.update(overrides)

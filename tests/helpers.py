@@ -43,21 +43,30 @@ def add_hist(a, b):
     return {k: a[k] + b[k] for k in a}
 
 
+def gem_inputs():
+    """Caller inputs of the GEM level density (NEXT-2) used by the tests on both sides: the paper prints no pairing
+    or shell-correction table, any values will do.  Even Z / N: 1.2 / 1.1 MeV pairing, odd: 0; smooth shell corrections."""
+    i = np.arange(40)
+    return dict(level_density=1, pair_Z=np.where(i % 2 == 0, 1.2, 0.0), pair_N=np.where(i % 2 == 0, 1.1, 0.0),
+                shell_Z=3.0 * np.sin(i / 4.0), shell_N=-2.0 * np.cos(i / 5.0))
+
+
 def _oracle_shard(args):
-    config_id, n_total, e0, e1 = args
+    config_id, n_total, e0, e1 = args[:4]
+    tables_kw = args[4] if len(args) > 4 else {}
     from oracle import oracle as O
     import paper_1309_7963_b200.workloads as W
     E, tid, targets, seed, _ = W.make_inputs(config_id, n_total)
-    t = O.Tables()
+    t = O.Tables(**tables_kw)
     r = O.simulate(t, targets, E[e0:e1], tid[e0:e1], seed, e0=e0, want_stats=True)
     return histograms(r["species"], r["T"], r["uz"], r["counts"], r["A"]), r["stats"]
 
 
-def oracle_histograms(config_id, n_total, nproc=None, shard=50000):
+def oracle_histograms(config_id, n_total, nproc=None, shard=50000, tables_kw=None):
     """Oracle histograms over the first n_total events of a config, sharded over processes
-    (counter-keyed RNG makes shards exact)."""
+    (counter-keyed RNG makes shards exact).  tables_kw: keyword arguments of oracle.Tables (e.g. gem_inputs())."""
     nproc = nproc or min(os.cpu_count() or 1, 32)
-    jobs = [(config_id, n_total, a, min(a + shard, n_total)) for a in range(0, n_total, shard)]
+    jobs = [(config_id, n_total, a, min(a + shard, n_total), tables_kw or {}) for a in range(0, n_total, shard)]
     if nproc == 1 or len(jobs) == 1:
         outs = [_oracle_shard(j) for j in jobs]
     else:

@@ -289,7 +289,7 @@ def test_error_paths(gpu, ptables):
         lib.inc_init(300, 8, ptables)
     with pytest.raises(gpu.IncError):
         lib.inc_init(4, 2, ptables)
-    bad = dict(ptables); bad["version"] = 2
+    bad = dict(ptables); bad["version"] = 3
     with pytest.raises(gpu.IncError):
         lib.inc_init(16, 8, bad)
     t0 = lib.inc_init(16, 8, ptables)
@@ -489,6 +489,58 @@ def test_tallies(gpu, orc, otables, ptables, variant, cfg, n):
         lib.inc_tally(out, off, spec, tl)
         torch.cuda.synchronize()
         assert np.array_equal(tl["dd"].cpu().numpy(), 2 * g["dd"]) and np.array_equal(tl["nuclide"].cpu().numpy(), 2 * g["nuclide"])
+
+
+# ------------------------------------------------------------------------------- NEXT-2: GEM level density
+@pytest.mark.parametrize("cfg,n", [(1, 10000), (5, 4000)])
+def test_gem_fp64_identity(gpu, orc, ptables, cfg, n):
+    """inc_tables.level_density = 1 ("we adopt the generalized evaporation model (GEM) [18]"; DESIGN.md R-G1..G6) with
+    caller-supplied pairing energies and shell corrections: the fp64 build equals the oracle event by event; with the
+    corrections switched off the mode still differs from the frozen Weisskopf-Ewing model (pre-exponential factor,
+    constant-temperature branch); a version 1 struct means level_density = 0."""
+    import paper_1309_7963_b200.tables as T
+    E, tid, targets, seed, _ = _inputs(cfg, n)
+    lib = gpu.load("f64")
+    kw = H.gem_inputs()
+    g = gpu.simulate(lib, targets, E, tid, seed, T.default_tables(**kw))
+    o = orc.simulate(orc.Tables(**kw), targets, E, tid, seed)
+    frac, max_err, ident = H.event_identity(g, o, rel=REL_F64)
+    print(f"[GEM fp64] config {cfg}: identical {frac:.5f}, max rel err {max_err:.2e}")
+    assert frac >= FRAC_IDENTICAL and max_err <= REL_F64
+    assert np.array_equal(g["status"][ident], o["status"][ident])
+    _assert_conservation(g, targets, tid, E, orc, orc.Tables(**kw), 1e-12, 1e-9)
+    # the cascade is untouched by the mode; the evaporation is not
+    base = gpu.simulate(lib, targets, E, tid, seed, ptables)
+    assert np.array_equal(base["casc_A"], g["casc_A"]) and np.array_equal(base["casc_Estar"], g["casc_Estar"])
+    assert not np.array_equal(base["counts"], g["counts"])
+    v1 = dict(ptables); v1["version"] = 1
+    old = gpu.simulate(lib, targets, E, tid, seed, v1)
+    for k in ("species", "T", "counts", "A", "Z", "Estar", "status"):
+        assert np.array_equal(base[k], old[k]), k
+
+
+@pytest.mark.parametrize("cfg", [2, 5])
+def test_gem_fp32_histograms(gpu, orc, cfg):
+    """GEM mode, production build, full-size batch against a 2e5-event oracle sample (criterion (3)), plus exact
+    conservation of A and Z and 4-momentum to fp32 accuracy."""
+    import torch
+    import paper_1309_7963_b200.tables as T
+    import paper_1309_7963_b200.workloads as W
+    n = W.CONFIGS[cfg]["n"]
+    E, tid, targets, seed, _ = _inputs(cfg, n)
+    kw = H.gem_inputs()
+    g = gpu.simulate(gpu.load("f32"), targets, E, tid, seed, T.default_tables(**kw), capacity_per_event=12)
+    assert not np.any(g["status"] & (gpu.ST_FAILED | gpu.ST_QUEUE_OVF))
+    hg = H.histograms(g["species"], g["T"].astype(np.float64), g["uz"].astype(np.float64), g["counts"], g["A"])
+    ho, _ = H.oracle_histograms(cfg, 200000, tables_kw=kw)
+    fails = H.compare_histograms(hg, ho)
+    assert not fails, fails
+    m = 100000
+    sl = {k: g[k][:m] for k in ("counts", "A", "Z", "Estar", "px", "py", "pz", "status")}
+    k_end = int(np.sum(g["counts"][:m]))
+    for k in ("species", "T", "ux", "uy", "uz"):
+        sl[k] = g[k][:k_end]
+    _assert_conservation(sl, targets, tid[:m], E[:m], orc, orc.Tables(**kw), 2e-6, 2e-4)
 
 
 # ------------------------------------------------------------------------------- NEXT-3: incident neutrons
