@@ -27,6 +27,15 @@
 
 #include "../../include/inc.h"
 
+// -DINC_CHECKED: every index into the wavefront kernel's shared-memory queues, rings and slot lists is checked and a
+// violation raises error bit 32 (inc_simulate -> INC_E_STATE).  compute-sanitizer is closed on the GPU pool this was
+// developed on, so the checked small-queue build (libinc_f64q.so) is the memory check of the queue code.
+#ifdef INC_CHECKED
+#define INC_CHECK(cond) do { if (!(cond)) atomicOr(&P.ctr->error_word, 32u); } while (0)
+#else
+#define INC_CHECK(cond) do { } while (0)
+#endif
+
 namespace inc {
 
 constexpr int kMaxShells = 32;
@@ -1116,7 +1125,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   if (timeline && lane == 0) { atomicMax(&P.ctr->tl[0], ~global_ns()); atomicAdd(&P.ctr->tl[4], 1ull); }
   // per-warp drain trace (diagnostic, INC_F_TIMING only)
   uint32_t *wt = (timeline && P.wtrace) ? P.wtrace + (size_t)kWTrace * (blockIdx.x * C::WARPS + (threadIdx.x >> 5)) : nullptr;
-  uint32_t tr_pass = 0, tr_seg = 0, tr_lanes = 0, tr_att = 0, tr_out = 0;
+  uint32_t tr_pass = 0, tr_seg = 0, tr_lanes = 0, tr_att = 0, tr_out = 0, tr_wait = 0;
   if (wt && lane == 0) wt[7] = (uint32_t)global_ns();
 
   auto load_key = [&](int slot, RngKey &g, uint32_t &attempt, int &tgt, int &ev) {
@@ -1130,6 +1139,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
     const unsigned m = __ballot_sync(kFull, pred);
     if (pred) {
       const int i = nSeg + __popc(m & lt);
+      INC_CHECK(i >= 0 && i < C::QS && slot >= 0 && slot < C::NS);
       w.qx[i] = t.x; w.qy[i] = t.y; w.qz[i] = t.z; w.qpx[i] = t.px; w.qpy[i] = t.py; w.qpz[i] = t.pz; w.qT[i] = t.T;
       w.qpi[i] = t.pi; w.qkn[i] = t.k | ((uint32_t)t.nseg << 16);
       w.qmeta[i] = (uint32_t)t.type | ((uint32_t)t.shell << 1) | ((uint32_t)slot << 8);
@@ -1140,6 +1150,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   int nPub = 0;
   auto push_pub = [&](bool pred, int ev) {
     const unsigned m = __ballot_sync(kFull, pred);
+    INC_CHECK(!pred || (nPub + __popc(m & lt) < 96 && ev >= 0 && ev < P.n_chunk));
     if (pred) w.pub_q[nPub + __popc(m & lt)] = (uint32_t)ev;
     nPub += __popc(m);
   };
@@ -1155,6 +1166,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   };
   auto push_epi = [&](bool pred, int slot) {
     const unsigned m = __ballot_sync(kFull, pred);
+    INC_CHECK(!pred || (nEpi + __popc(m & lt) < C::NS && slot >= 0 && slot < C::NS));
     if (pred) w.epi_q[nEpi + __popc(m & lt)] = (uint8_t)slot;
     nEpi += __popc(m);
   };
@@ -1212,7 +1224,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
         if (availE > 0 && availE >= nSegT && availE >= nColl) phase = ST_EPI;
         else if (nColl > 0 && nColl >= nSegT) phase = ST_COLL;
         else if (nSegT > 0) phase = ST_SEG;
-        else if (DRAIN && n_out > 0) { __nanosleep(100); return false; }      // our last tracks are with helpers
+        else if (DRAIN && n_out > 0) { __nanosleep(100); tr_wait++; return false; }      // our last tracks are with helpers
         else return true;
       }
       if (phase == ST_EPI && nSegT + nColl > kAdmit) phase = nSegT > 0 ? ST_SEG : ST_COLL;   // admission control
@@ -1242,6 +1254,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
         const int r = __popc(mk & lt);
         if (need && r < take) {
           const int i = nSeg - 1 - r;
+          INC_CHECK(i >= 0 && i < C::QS);
           rt.x = w.qx[i]; rt.y = w.qy[i]; rt.z = w.qz[i]; rt.px = w.qpx[i]; rt.py = w.qpy[i]; rt.pz = w.qpz[i]; rt.T = w.qT[i];
           rt.pi = w.qpi[i];
           const uint32_t kn = w.qkn[i], mt = w.qmeta[i];
@@ -1321,6 +1334,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
           const unsigned mk = __ballot_sync(kFull, pc);
           if (pc) {
             const int i = nColl + __popc(mk & lt);
+            INC_CHECK(i >= 0 && i < C::QC && rslot >= 0 && rslot < C::NS);
             w.cx[i] = rt.x; w.cy[i] = rt.y; w.cz[i] = rt.z; w.cpx[i] = rt.px; w.cpy[i] = rt.py; w.cpz[i] = rt.pz; w.cT[i] = rt.T;
             w.cpi[i] = rt.pi; w.ckn[i] = rt.k | ((uint32_t)rt.nseg << 16);
             w.cmeta[i] = (uint32_t)rt.type | ((uint32_t)rt.shell << 1) | ((uint32_t)rslot << 8);
@@ -1335,6 +1349,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
             const int idx = (int)(old & 0xFFu);
             if (idx < kMaxSec) {
               const size_t o = (size_t)rev * kMaxSec + idx;
+              INC_CHECK(rev >= 0 && rev < P.n_chunk && rslot >= 0 && rslot < C::NS && w.ev[rslot] == rev);
               stage_write<R>(P.ws.st + o, esc.T, esc.ux, esc.uy, esc.uz, rt.pi | ((uint32_t)rt.type << 24));
               typedef typename Fx<R>::U FU;
               atomicAdd((FU *)&w.acc[0][rslot], (FU)(-Fx<R>::to(esc.T)));
@@ -1377,6 +1392,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       int slot = 0;
       if (has) {
         const int i = nColl - 1 - lane;
+        INC_CHECK(i >= 0 && i < C::QC);
         t.x = w.cx[i]; t.y = w.cy[i]; t.z = w.cz[i]; t.px = w.cpx[i]; t.py = w.cpy[i]; t.pz = w.cpz[i]; t.T = w.cT[i];
         t.pi = w.cpi[i];
         const uint32_t kn = w.ckn[i], mt = w.cmeta[i];
@@ -1418,7 +1434,9 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       if (lane == 0) { st.add(S_WI_EPI); st.add(S_LS_EPI, m); }
       const bool has = lane < m;
       int slot = 0;
+      INC_CHECK(!has || (lane < mE ? (nEpi - 1 - lane >= 0 && nEpi - 1 - lane < C::NS) : (nFree - 1 - (lane - mE) >= 0 && nFree - 1 - (lane - mE) < C::NS)));
       if (has) slot = lane < mE ? w.epi_q[nEpi - 1 - lane] : w.free_q[nFree - 1 - (lane - mE)];
+      INC_CHECK(slot >= 0 && slot < C::NS);
       nEpi -= mE; nFree -= mF;
       __syncwarp();
       bool want_event = has && lane >= mE;
@@ -1491,6 +1509,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       {
         const bool fr = has && !do_entry;
         const unsigned mk = __ballot_sync(kFull, fr);
+        INC_CHECK(!fr || nFree + __popc(mk & lt) < C::NS);
         if (fr) { w.free_q[nFree + __popc(mk & lt)] = (uint8_t)slot; w.ev[slot] = -1; }
         nFree += __popc(mk);
       }
@@ -1530,11 +1549,12 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
       break;
     }
   }
-  if (wt && lane == 0 && tr_pass <= (1u << 24)) { wt[1] = (uint32_t)global_ns(); wt[2] = tr_pass; wt[3] = tr_seg; wt[4] = tr_lanes; wt[5] = tr_att; wt[6] = tr_out; }
+  if (wt && lane == 0 && tr_pass <= (1u << 24)) { wt[1] = (uint32_t)global_ns(); wt[2] = tr_pass; wt[3] = tr_seg; wt[4] = tr_lanes; wt[5] = tr_att | (tr_wait << 8); wt[6] = tr_out; }
   if (timeline && lane == 0) {
     const unsigned long long t = global_ns();
     atomicAdd(&P.ctr->tl[2], t); atomicMax(&P.ctr->tl[3], t); atomicMax(&P.ctr->tl[5], ~t);
   }
+  INC_CHECK(nSeg == 0 && nColl == 0 && nEpi == 0 && nRes == 0 && n_out == 0 && nFree == C::NS);   // every slot came back
   flush_pub();
   st.flush(P.ctr, lane);
   if (helpers_on) {

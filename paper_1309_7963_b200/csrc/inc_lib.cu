@@ -712,6 +712,7 @@ int64_t simulate_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint6
   g.pending_events.clear();
   g.last_n = n; g.last_total = (long long)tail.total;
   g.last_chunks = (int)((n + (long long)chunk - 1) / (long long)chunk);
+  if (tail.err & 32u) return fail(INC_E_STATE, "checked build: an index of the wavefront kernel's queues was out of range (results invalid)");
   if (tail.err & 16u) return fail(INC_E_STATE, "watchdog: a warp of the wavefront cascade kernel made no progress (results invalid)");
   if (tail.err & 4u) return kQueueOverflow;
   if (tail.err) {

@@ -249,6 +249,15 @@ def test_small_queue_build_and_overflow_rerun(gpu, ptables, cfg, n):
     got = gpu.simulate(small, targets, E, tid, seed, ptables)
     for k in keys:
         assert np.array_equal(ref[k], got[k]), k
+    # f64q is also the CHECKED build (every queue / ring / slot index verified on the device; a violation fails the
+    # call): with the long-track threshold at 2 nearly every drain-phase track goes through the helpers' rings
+    small.inc_set_long_track_threshold(2)
+    try:
+        got = gpu.simulate(small, targets, E, tid, seed, ptables)
+    finally:
+        small.inc_set_long_track_threshold(0)
+    for k in keys:
+        assert np.array_equal(ref[k], got[k]), k
     print(f"[small queues] config {cfg}: reruns with the lane kernel: {small.inc_get_rerun_count() - r0}")
     lib = gpu.load("f64")
     r1 = lib.inc_get_rerun_count()
