@@ -191,13 +191,14 @@ int64_t inc_simulate(int64_t n_events, const INC_REAL *E_in /*DEVICE, MeV*/,
                      inc_residual *out_residual /*HOST struct of DEVICE ptrs*/);
 
 /* inc_simulate_host — same computation with HOST buffers (every pointer, including those
- * inside the two structs, is host memory).  The library stages inputs to the device,
- * runs inc_simulate and copies the results back, all inside this call (used for the
- * end-to-end number of bench.py).  It streams: the call runs in chunks of at
- * most 2^19 events (2^20 for calls above 2^21 events; or inc_set_chunk_events, if smaller), and while one chunk computes on the
- * caller's stream the outputs of the previous one travel to the host on a second stream, so a
- * long call costs about max(compute, copy) instead of their sum.  Pinned host memory is what
- * makes the copies asynchronous; pageable memory works, without the overlap. */
+ * inside the two structs, is host memory).  It streams: the call runs in chunks of at most
+ * 2^19 events (2^20 for calls above 2^21 events; or inc_set_chunk_events, if smaller); chunk c lives in slot c mod 3
+ * of a ring of chunk-sized device buffers (inputs, per-event outputs, room for INC_MAX_SEC secondaries per event), so
+ * device memory is O(chunk) whatever n_events is; while chunks compute on the caller's stream the outputs of the
+ * previous one travel to the host on a second stream, so a long call costs about max(compute, copy) instead of
+ * their sum.  Pinned host memory is what makes the copies asynchronous; pageable memory works, without the overlap.
+ * After a call of more than one chunk inc_get_offsets and inc_get_cascade_stage return INC_E_STATE (the device holds
+ * per-chunk data only; the offsets are the prefix sum of out_counts). */
 int64_t inc_simulate_host(int64_t n_events, const INC_REAL *E_in /*HOST*/,
                           const int32_t *target_id /*HOST*/, uint64_t seed,
                           inc_secondaries *out_secondaries /*HOST ptrs*/,

@@ -58,28 +58,43 @@ struct State {
   NucDev<real> *d_nuc = nullptr;
   DevCounters *d_ctr = nullptr;
   uint32_t *d_wtrace = nullptr; int wtrace_warps = 0;   // inc_get_warp_trace (INC_F_TIMING)
-  // workspace
+  // workspace.  A lane is what launch_chunk enqueues on: a stream with its workspace, counters and scan buffers.  There
+  // is one (the members below on the caller's stream).  A second lane for inc_simulate_host, alternating chunks so that
+  // one chunk's cascade kernel would start on the SMs the previous chunk's cascade CTAs have left, was measured and
+  // dropped: the evaporation CTAs of the older chunk take those SMs first, and config 2's e2e fell from 2.8e8 to 2.3e8.
+  struct Lane {
+    cudaStream_t stream = nullptr;
+    Workspace<real> ws{};
+    DevCounters *ctr = nullptr;
+    long long *tiles = nullptr;
+    long long *offsets = nullptr;
+  };
+  Lane *cur = nullptr;              // the lane launch_chunk enqueues on
   size_t ws_chunk = 0;
   Workspace<real> ws{};
   long long *d_offsets = nullptr; size_t offsets_cap = 0;
   long long *d_tiles = nullptr; size_t tiles_cap = 0;
-  // host-buffer path
-  struct HostPath {
-    size_t n_cap = 0, sec_cap = 0;
+  // host-buffer path (inc_simulate_host): a ring of kRing chunk-sized sets of device buffers, so that device memory
+  // is O(chunk) whatever the call's n
+  struct HostSlot {
     real *E = nullptr; int32_t *tid = nullptr, *counts = nullptr, *A = nullptr, *Z = nullptr;
     real *Es = nullptr, *px = nullptr, *py = nullptr, *pz = nullptr; uint32_t *status = nullptr;
     uint8_t *sp = nullptr; real *T = nullptr, *ux = nullptr, *uy = nullptr, *uz = nullptr;
-    // pipelined copies (inc_simulate_host): copy stream, per-chunk events, running totals in pinned host memory
+    cudaEvent_t computed = nullptr, copied = nullptr;
+  };
+  static constexpr int kRing = 3;
+  struct HostPath {
+    size_t chunk_cap = 0;                     // events per slot; a slot holds kMaxSec secondaries per event
+    HostSlot slot[kRing];
     cudaStream_t copy_stream = nullptr;
-    unsigned long long *h_tot = nullptr;      // pinned, [kMaxHostChunks]
-    std::vector<cudaEvent_t> ev;
+    unsigned long long *h_tot = nullptr;      // pinned, [kRing]: secondaries of the chunk in the slot
+    unsigned int *h_err = nullptr;            // pinned: the call's device error word
   } hp;
   size_t host_chunk_events = (size_t)1 << 19;
-  // per-chunk hook of the running call (inc_simulate_host): called after chunk c has been enqueued
-  std::function<int(int, long long, int)> chunk_hook;
   // last call
   long long last_n = -1;
   int last_chunks = 0;
+  bool last_offsets_valid = false;  // inc_get_offsets: the last call left the offsets of the whole call on the device
   long long reruns = 0;             // calls run again with the lane kernel after a queue overflow of the wavefront kernel              // chunks of the last inc_simulate (the cascade stage survives single-chunk calls only)
   long long last_total = 0;
   long long event_offset = 0;
@@ -98,6 +113,8 @@ struct State {
 };
 
 State g;
+
+void free_host_ring();
 
 int fail(int code, const std::string &msg) { g.err = msg; return code; }
 
@@ -429,11 +446,18 @@ int ensure_ws(size_t chunk, size_t n_total) {
   return 0;
 }
 
+// lane 0 = the library's main workspace on the caller's stream
+State::Lane lane0() {
+  State::Lane l;
+  l.stream = g.stream; l.ws = g.ws; l.ctr = g.d_ctr; l.tiles = g.d_tiles; l.offsets = g.d_offsets;
+  return l;
+}
+
 int mark(bool timing) {
   if (!timing) return 0;
   cudaEvent_t e;
   CU_TRY(cudaEventCreate(&e));
-  CU_TRY(cudaEventRecord(e, g.stream));
+  CU_TRY(cudaEventRecord(e, g.cur->stream));
   g.pending_events.push_back(e);
   return 0;
 }
@@ -451,9 +475,10 @@ template <bool STATS>
 int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t *tid, const uint8_t *proj, uint64_t seed,
                  inc_secondaries *sec, int32_t *counts, inc_residual *res, long long *offsets) {
   const ModelDev<real> model = model_dev();
+  State::Lane &L = *g.cur;
   // --- cascade ---
   CascadeParams<real> cp;
-  cp.model = model; cp.ws = g.ws; cp.ctr = g.d_ctr; cp.E_in = E_in; cp.target_id = tid; cp.projectile = proj;
+  cp.model = model; cp.ws = L.ws; cp.ctr = L.ctr; cp.E_in = E_in; cp.target_id = tid; cp.projectile = proj;
   cp.e_base = e_base + g.event_offset; cp.n_chunk = n_chunk; cp.seed_lo = (uint32_t)seed; cp.seed_hi = (uint32_t)(seed >> 32);
   cp.flags = g.flags;
   const bool naive = (g.flags & INC_F_LANE_PER_EVENT) != 0;
@@ -476,8 +501,8 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   CU_TRY(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
   const size_t wsmem = wave_smem_bytes<real>(model.n_xs, n_stage);
   const bool lane_kernel = naive || (g.flags & INC_F_LANE_STATE_MACHINE) != 0 || wsmem > (size_t)smem_max;
-  CU_TRY(cudaMemsetAsync(&g.d_ctr->next_event_casc, 0, 3 * sizeof(unsigned long long), g.stream));   // + next_event_evap, n_done
-  CU_TRY(cudaMemsetAsync(g.ws.done_list, 0xFF, (size_t)n_chunk * sizeof(uint32_t), g.stream));      // kNotDone
+  CU_TRY(cudaMemsetAsync(&L.ctr->next_event_casc, 0, 3 * sizeof(unsigned long long), L.stream));   // + next_event_evap, n_done
+  CU_TRY(cudaMemsetAsync(L.ws.done_list, 0xFF, (size_t)n_chunk * sizeof(uint32_t), L.stream));      // kNotDone
   if (mark(timing)) return INC_E_CUDA;
   if (lane_kernel) {
     const size_t smem = model_smem_bytes<real>(model.n_xs, n_stage);
@@ -488,7 +513,7 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
     if (occ < 1) return fail(INC_E_CUDA, "cascade kernel does not fit on an SM");
     int blocks = occ * g.sm_count;
     if (blocks > need) blocks = need;
-    kern<<<blocks, 256, smem, g.stream>>>(cp);
+    kern<<<blocks, 256, smem, L.stream>>>(cp);
   } else {
     // one persistent CTA per SM; each warp keeps WaveCfg::NS events in flight in its shared-memory queues
     auto kern = cascade_wavefront_kernel<real, STATS>;
@@ -504,15 +529,15 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
     if (timing) {
       const int nw = blocks * WaveCfg<real>::WARPS;
       if (!g.d_wtrace) CU_TRY(cudaMalloc((void **)&g.d_wtrace, sizeof(uint32_t) * kWTrace * 8192));
-      if (nw <= 8192) { CU_TRY(cudaMemsetAsync(g.d_wtrace, 0, sizeof(uint32_t) * kWTrace * nw, g.stream)); cp.wtrace = g.d_wtrace; g.wtrace_warps = nw; }
+      if (nw <= 8192) { CU_TRY(cudaMemsetAsync(g.d_wtrace, 0, sizeof(uint32_t) * kWTrace * nw, L.stream)); cp.wtrace = g.d_wtrace; g.wtrace_warps = nw; }
     }
-    kern<<<blocks, threads, wsmem, g.stream>>>(cp);
+    kern<<<blocks, threads, wsmem, L.stream>>>(cp);
   }
   CU_TRY(cudaGetLastError());
   if (mark(timing)) return INC_E_CUDA;
   // --- evaporation ---
   EvapParams<real> ep;
-  ep.model = model; ep.ws = g.ws; ep.ctr = g.d_ctr; ep.e_base = e_base + g.event_offset; ep.n_chunk = n_chunk;
+  ep.model = model; ep.ws = L.ws; ep.ctr = L.ctr; ep.e_base = e_base + g.event_offset; ep.n_chunk = n_chunk;
   ep.seed_lo = cp.seed_lo; ep.seed_hi = cp.seed_hi; ep.flags = g.flags;
   ep.out_counts = counts;
   auto ekern = g.tab.level_density == 1 ? evap_kernel<real, STATS, true> : evap_kernel<real, STATS, false>;
@@ -526,7 +551,7 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
     // still draining; they consume the completion list, so they never run ahead of the data.  With INC_F_TIMING the
     // stages are separated by events and run one after the other, so that each has a duration of its own.
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)eblocks); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = g.stream;
+    cfg.gridDim = dim3((unsigned)eblocks); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = L.stream;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
@@ -537,20 +562,20 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   if (mark(timing)) return INC_E_CUDA;
   // --- prefix sum of counts (running base carried across chunks in ctr->total_sec) ---
   const int tiles = (n_chunk + kScanTile - 1) / kScanTile;
-  scan_tile_sums<<<tiles, kScanBlock, 0, g.stream>>>(counts, n_chunk, g.d_tiles);
-  scan_tiles<<<1, kScanBlock, 0, g.stream>>>(g.d_tiles, tiles, &g.d_ctr->total_sec);
-  scan_write_offsets<<<tiles, kScanBlock, 0, g.stream>>>(counts, n_chunk, g.d_tiles, offsets);
+  scan_tile_sums<<<tiles, kScanBlock, 0, L.stream>>>(counts, n_chunk, L.tiles);
+  scan_tiles<<<1, kScanBlock, 0, L.stream>>>(L.tiles, tiles, &L.ctr->total_sec);
+  scan_write_offsets<<<tiles, kScanBlock, 0, L.stream>>>(counts, n_chunk, L.tiles, offsets);
   CU_TRY(cudaGetLastError());
   if (mark(timing)) return INC_E_CUDA;
   // --- compaction into the caller's SoA ---
   CompactParams<real> kp;
-  kp.ws = g.ws; kp.offsets = offsets; kp.counts = counts; kp.n_chunk = n_chunk;
+  kp.ws = L.ws; kp.offsets = offsets; kp.counts = counts; kp.n_chunk = n_chunk;
   kp.species = sec->species; kp.T = sec->T; kp.ux = sec->ux; kp.uy = sec->uy; kp.uz = sec->uz;
   kp.capacity = sec->capacity;
   kp.rA = res->A; kp.rZ = res->Z; kp.rE = res->Estar; kp.rPx = res->px; kp.rPy = res->py; kp.rPz = res->pz; kp.rstatus = res->status;
   const int cwarps = (n_chunk + 31) / 32;
   const int cblocks = (cwarps + 7) / 8;
-  compact_kernel<real><<<cblocks, 256, 0, g.stream>>>(kp);
+  compact_kernel<real><<<cblocks, 256, 0, L.stream>>>(kp);
   CU_TRY(cudaGetLastError());
   if (mark(timing)) return INC_E_CUDA;
   return 0;
@@ -613,16 +638,13 @@ int inc_free_target(int id) {
 void inc_shutdown(void) {
   free_ws();
   void **p[] = {(void **)&g.d_tabS, (void **)&g.d_tabC, (void **)&g.d_bind, (void **)&g.d_evch, (void **)&g.d_ld, (void **)&g.d_nuc,
-                (void **)&g.d_ctr, (void **)&g.d_wtrace, (void **)&g.d_offsets, (void **)&g.d_tiles,
-                (void **)&g.hp.E, (void **)&g.hp.tid, (void **)&g.hp.counts, (void **)&g.hp.A, (void **)&g.hp.Z,
-                (void **)&g.hp.Es, (void **)&g.hp.px, (void **)&g.hp.py, (void **)&g.hp.pz, (void **)&g.hp.status,
-                (void **)&g.hp.sp, (void **)&g.hp.T, (void **)&g.hp.ux, (void **)&g.hp.uy, (void **)&g.hp.uz};
+                (void **)&g.d_ctr, (void **)&g.d_wtrace, (void **)&g.d_offsets, (void **)&g.d_tiles};
   for (auto q : p) { if (*q) cudaFree(*q); *q = nullptr; }
-  g.offsets_cap = g.tiles_cap = 0; g.hp.n_cap = g.hp.sec_cap = 0;
-  for (auto e : g.hp.ev) cudaEventDestroy(e);
-  g.hp.ev.clear();
+  g.offsets_cap = g.tiles_cap = 0;
+  free_host_ring();
   if (g.hp.copy_stream) { cudaStreamDestroy(g.hp.copy_stream); g.hp.copy_stream = nullptr; }
   if (g.hp.h_tot) { cudaFreeHost(g.hp.h_tot); g.hp.h_tot = nullptr; }
+  if (g.hp.h_err) { cudaFreeHost(g.hp.h_err); g.hp.h_err = nullptr; }
   for (auto &n : g.nuc) n.live = false;
   g.tab.captured = false;
   g.last_n = -1;
@@ -636,6 +658,10 @@ constexpr int64_t kQueueOverflow = -1000;   // internal: the wavefront kernel's 
 
 int64_t simulate_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
                       int32_t *counts, inc_residual *res);
+int64_t simulate_host_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
+                           int32_t *counts, inc_residual *res);
+int resolve_stage_times();
+int64_t device_error(unsigned int err);
 }  // namespace
 
 extern "C" {
@@ -664,42 +690,8 @@ int64_t inc_get_rerun_count(void) { return g.reruns; }
 
 namespace {
 
-int64_t simulate_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
-                      int32_t *counts, inc_residual *res) {
-  if (!g.tab.captured) return fail(INC_E_STATE, "inc_simulate before inc_init");
-  if (n < 0 || !sec || !res || (n > 0 && (!E_in || !tid || !counts))) return fail(INC_E_BADARG, "null argument or n < 0");
-  if (n > 0 && (!res->A || !res->Z || !res->Estar || !res->px || !res->py || !res->pz || !res->status))
-    return fail(INC_E_BADARG, "null residual array");
-  if (sec->capacity < 0 || (sec->capacity > 0 && (!sec->species || !sec->T || !sec->ux || !sec->uy || !sec->uz)))
-    return fail(INC_E_BADARG, "null secondary array");
-  // inc_simulate_host pipelines chunks against their copies: 2^19 events per chunk, 2^20 for long calls (a chunk
-  // costs one drain phase of the cascade kernel, so they should not be smaller than the copies need)
-  const size_t host_chunk = (size_t)n > ((size_t)1 << 21) ? 2 * g.host_chunk_events : g.host_chunk_events;
-  const size_t chunk_max = g.chunk_hook ? (host_chunk < g.chunk_events ? host_chunk : g.chunk_events) : g.chunk_events;
-  const size_t chunk = (size_t)n < chunk_max ? (size_t)(n > 0 ? n : 1) : chunk_max;
-  int rc = ensure_ws(chunk, (size_t)n);
-  if (rc) return rc;
-  CU_TRY(cudaMemsetAsync(g.d_ctr, 0, sizeof(DevCounters), g.stream));
-  if (int rk_rc = set_round_keys(seed)) return rk_rc;
-  if (g.chunk_hook) { rc = g.chunk_hook(-1, 0, 0); if (rc) return rc; }     // (a rerun starts its pipeline afresh)
-  for (auto e : g.pending_events) cudaEventDestroy(e);
-  g.pending_events.clear();
-  for (int i = 0; i < 4; ++i) { g.stage_ms[i] = 0; g.stage_launches[i] = 0; }
-  const bool stats = (g.flags & INC_F_STATS) != 0;
-  for (long long e0 = 0; e0 < n; e0 += (long long)chunk) {
-    const int nc = (int)((n - e0) < (long long)chunk ? (n - e0) : (long long)chunk);
-    inc_residual r = *res;
-    r.A += e0; r.Z += e0; r.Estar += e0; r.px += e0; r.py += e0; r.pz += e0; r.status += e0;
-    const uint8_t *pj = g.projectile ? g.projectile + e0 : nullptr;
-    rc = stats ? launch_chunk<true>(e0, nc, E_in + e0, tid + e0, pj, seed, sec, counts + e0, &r, g.d_offsets + e0)
-               : launch_chunk<false>(e0, nc, E_in + e0, tid + e0, pj, seed, sec, counts + e0, &r, g.d_offsets + e0);
-    if (rc) return rc;
-    if (g.chunk_hook) { rc = g.chunk_hook((int)(e0 / (long long)chunk), e0, nc); if (rc) return rc; }
-  }
-  CU_TRY(cudaMemcpyAsync(g.d_offsets + n, &g.d_ctr->total_sec, sizeof(long long), cudaMemcpyDeviceToDevice, g.stream));
-  struct { unsigned long long total; unsigned int err, pad; } tail;
-  CU_TRY(cudaMemcpyAsync(&tail, &g.d_ctr->total_sec, 16, cudaMemcpyDeviceToHost, g.stream));
-  CU_TRY(cudaStreamSynchronize(g.stream));
+// stage times of the call from the events recorded around the kernels (INC_F_TIMING); the stream has been synchronised
+int resolve_stage_times() {
   for (size_t c = 0; c + 4 < g.pending_events.size(); c += 5) {
     const int nl[4] = {1, 1, 3, 1};
     for (int i = 0; i < 4; ++i) {
@@ -710,16 +702,59 @@ int64_t simulate_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint6
   }
   for (auto e : g.pending_events) cudaEventDestroy(e);
   g.pending_events.clear();
+  return 0;
+}
+
+// the device error word of a finished call -> 0, kQueueOverflow, or a negative INC_E_* code with its message
+int64_t device_error(unsigned int err) {
+  if (err & 32u) return fail(INC_E_STATE, "checked build: an index of the wavefront kernel's queues was out of range (results invalid)");
+  if (err & 16u) return fail(INC_E_STATE, "watchdog: a warp of the wavefront cascade kernel made no progress (results invalid)");
+  if (err & 4u) return kQueueOverflow;
+  if (err) {
+    return fail(INC_E_BADARG, std::string("device-side input check failed:") + ((err & 1u) ? " E_in outside [20,250] MeV" : "") +
+                                  ((err & 2u) ? " target_id not initialised" : "") + ((err & 8u) ? " projectile not 0 or 1" : ""));
+  }
+  return 0;
+}
+
+int64_t simulate_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
+                      int32_t *counts, inc_residual *res) {
+  if (!g.tab.captured) return fail(INC_E_STATE, "inc_simulate before inc_init");
+  if (n < 0 || !sec || !res || (n > 0 && (!E_in || !tid || !counts))) return fail(INC_E_BADARG, "null argument or n < 0");
+  if (n > 0 && (!res->A || !res->Z || !res->Estar || !res->px || !res->py || !res->pz || !res->status))
+    return fail(INC_E_BADARG, "null residual array");
+  if (sec->capacity < 0 || (sec->capacity > 0 && (!sec->species || !sec->T || !sec->ux || !sec->uy || !sec->uz)))
+    return fail(INC_E_BADARG, "null secondary array");
+  const size_t chunk_max = g.chunk_events;
+  const size_t chunk = (size_t)n < chunk_max ? (size_t)(n > 0 ? n : 1) : chunk_max;
+  int rc = ensure_ws(chunk, (size_t)n);
+  if (rc) return rc;
+  CU_TRY(cudaMemsetAsync(g.d_ctr, 0, sizeof(DevCounters), g.stream));
+  if (int rk_rc = set_round_keys(seed)) return rk_rc;
+  for (auto e : g.pending_events) cudaEventDestroy(e);
+  g.pending_events.clear();
+  for (int i = 0; i < 4; ++i) { g.stage_ms[i] = 0; g.stage_launches[i] = 0; }
+  const bool stats = (g.flags & INC_F_STATS) != 0;
+  State::Lane l0 = lane0();
+  g.cur = &l0;
+  for (long long e0 = 0; e0 < n; e0 += (long long)chunk) {
+    const int nc = (int)((n - e0) < (long long)chunk ? (n - e0) : (long long)chunk);
+    inc_residual r = *res;
+    r.A += e0; r.Z += e0; r.Estar += e0; r.px += e0; r.py += e0; r.pz += e0; r.status += e0;
+    const uint8_t *pj = g.projectile ? g.projectile + e0 : nullptr;
+    rc = stats ? launch_chunk<true>(e0, nc, E_in + e0, tid + e0, pj, seed, sec, counts + e0, &r, g.d_offsets + e0)
+               : launch_chunk<false>(e0, nc, E_in + e0, tid + e0, pj, seed, sec, counts + e0, &r, g.d_offsets + e0);
+    if (rc) return rc;
+  }
+  CU_TRY(cudaMemcpyAsync(g.d_offsets + n, &g.d_ctr->total_sec, sizeof(long long), cudaMemcpyDeviceToDevice, g.stream));
+  struct { unsigned long long total; unsigned int err, pad; } tail;
+  CU_TRY(cudaMemcpyAsync(&tail, &g.d_ctr->total_sec, 16, cudaMemcpyDeviceToHost, g.stream));
+  CU_TRY(cudaStreamSynchronize(g.stream));
+  if (int rt = resolve_stage_times()) return rt;
   g.last_n = n; g.last_total = (long long)tail.total;
   g.last_chunks = (int)((n + (long long)chunk - 1) / (long long)chunk);
-  if (tail.err & 32u) return fail(INC_E_STATE, "checked build: an index of the wavefront kernel's queues was out of range (results invalid)");
-  if (tail.err & 16u) return fail(INC_E_STATE, "watchdog: a warp of the wavefront cascade kernel made no progress (results invalid)");
-  if (tail.err & 4u) return kQueueOverflow;
-  if (tail.err) {
-    return fail(INC_E_BADARG, std::string("device-side input check failed:") + ((tail.err & 1u) ? " E_in outside [20,250] MeV" : "") +
-                                  ((tail.err & 2u) ? " target_id not initialised" : "") +
-                                  ((tail.err & 8u) ? " projectile not 0 or 1" : ""));
-  }
+  g.last_offsets_valid = true;
+  if (int64_t er = device_error(tail.err)) return er;
   if ((long long)tail.total > sec->capacity) {
     char buf[160];
     std::snprintf(buf, sizeof buf, "secondary capacity %lld too small, need %llu", (long long)sec->capacity, tail.total);
@@ -734,6 +769,7 @@ extern "C" {
 
 int inc_get_offsets(int64_t *dev_offsets) {
   if (g.last_n < 0) return fail(INC_E_STATE, "no previous inc_simulate");
+  if (!g.last_offsets_valid) return fail(INC_E_STATE, "the last call was a multi-chunk inc_simulate_host: its offsets are per chunk (take the prefix sum of out_counts)");
   if (!dev_offsets) return fail(INC_E_BADARG, "null pointer");
   CU_TRY(cudaMemcpyAsync(dev_offsets, g.d_offsets, (size_t)(g.last_n + 1) * sizeof(long long), cudaMemcpyDeviceToDevice, g.stream));
   CU_TRY(cudaStreamSynchronize(g.stream));
@@ -907,100 +943,164 @@ int inc_philox_blocks(const uint32_t *ctr, uint64_t seed, uint32_t *out, int64_t
 
 int64_t inc_simulate_host(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
                           int32_t *counts, inc_residual *res) {
+  int64_t rc = simulate_host_once(n, E_in, tid, seed, sec, counts, res);
+  if (rc == kQueueOverflow) {        // see inc_simulate
+    const uint32_t f = g.flags;
+    g.flags = (f | INC_F_LANE_STATE_MACHINE) & ~INC_F_TEST_QUEUE_OVF;
+    g.reruns++;
+    rc = simulate_host_once(n, E_in, tid, seed, sec, counts, res);
+    g.flags = f;
+    if (rc == kQueueOverflow) rc = fail(INC_E_STATE, "internal track-queue overflow (results invalid)");
+  }
+  g.projectile = nullptr;
+  return rc;
+}
+
+}  // extern "C"
+
+namespace {
+
+void free_host_ring() {
+  State::HostPath &h = g.hp;
+  for (auto &sl : h.slot) {
+    void **p[] = {(void **)&sl.E, (void **)&sl.tid, (void **)&sl.counts, (void **)&sl.A, (void **)&sl.Z, (void **)&sl.Es,
+                  (void **)&sl.px, (void **)&sl.py, (void **)&sl.pz, (void **)&sl.status, (void **)&sl.sp, (void **)&sl.T,
+                  (void **)&sl.ux, (void **)&sl.uy, (void **)&sl.uz};
+    for (auto q : p) { if (*q) cudaFree(*q); *q = nullptr; }
+    if (sl.computed) { cudaEventDestroy(sl.computed); sl.computed = nullptr; }
+    if (sl.copied) { cudaEventDestroy(sl.copied); sl.copied = nullptr; }
+  }
+  h.chunk_cap = 0;
+}
+
+int ensure_host_ring(size_t chunk) {
+  State::HostPath &h = g.hp;
+  if (!h.copy_stream) CU_TRY(cudaStreamCreateWithFlags(&h.copy_stream, cudaStreamNonBlocking));
+  if (!h.h_tot) CU_TRY(cudaMallocHost((void **)&h.h_tot, State::kRing * sizeof(unsigned long long)));
+  if (!h.h_err) CU_TRY(cudaMallocHost((void **)&h.h_err, sizeof(unsigned int)));
+  if (chunk <= h.chunk_cap) return 0;
+  free_host_ring();
+  const size_t m = chunk, k = chunk * (size_t)kMaxSec;
+  for (auto &sl : h.slot) {
+    CU_TRY(cudaMalloc((void **)&sl.E, m * sizeof(real))); CU_TRY(cudaMalloc((void **)&sl.tid, m * 4));
+    CU_TRY(cudaMalloc((void **)&sl.counts, m * 4)); CU_TRY(cudaMalloc((void **)&sl.A, m * 4)); CU_TRY(cudaMalloc((void **)&sl.Z, m * 4));
+    CU_TRY(cudaMalloc((void **)&sl.Es, m * sizeof(real))); CU_TRY(cudaMalloc((void **)&sl.px, m * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&sl.py, m * sizeof(real))); CU_TRY(cudaMalloc((void **)&sl.pz, m * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&sl.status, m * 4));
+    CU_TRY(cudaMalloc((void **)&sl.sp, k)); CU_TRY(cudaMalloc((void **)&sl.T, k * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&sl.ux, k * sizeof(real))); CU_TRY(cudaMalloc((void **)&sl.uy, k * sizeof(real)));
+    CU_TRY(cudaMalloc((void **)&sl.uz, k * sizeof(real)));
+    CU_TRY(cudaEventCreateWithFlags(&sl.computed, cudaEventDisableTiming));
+    CU_TRY(cudaEventCreateWithFlags(&sl.copied, cudaEventDisableTiming));
+  }
+  h.chunk_cap = chunk;
+  return 0;
+}
+
+// Streaming: the call runs in chunks; chunk c lives in ring slot c % kRing (inputs, per-event
+// outputs, up to kMaxSec secondaries per event, numbered from 0 inside the chunk), is computed on the caller's stream,
+// and its outputs travel to the host on a second stream while the next chunks compute.  Device memory does not depend
+// on n.  The host learns each chunk's number of secondaries (8 bytes, pinned) behind an event: that fixes where its
+// list goes in the caller's arrays.
+int64_t simulate_host_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
+                           int32_t *counts, inc_residual *res) {
   if (!g.tab.captured) return fail(INC_E_STATE, "inc_simulate_host before inc_init");
   if (n < 0 || !sec || !res || (n > 0 && (!E_in || !tid || !counts))) return fail(INC_E_BADARG, "null argument or n < 0");
+  if (n > 0 && (!res->A || !res->Z || !res->Estar || !res->px || !res->py || !res->pz || !res->status))
+    return fail(INC_E_BADARG, "null residual array");
+  if (sec->capacity < 0 || (sec->capacity > 0 && (!sec->species || !sec->T || !sec->ux || !sec->uy || !sec->uz)))
+    return fail(INC_E_BADARG, "null secondary array");
+  // 2^19 events per chunk, 2^20 for long calls (a chunk costs one tail of the cascade kernel, so chunks should not be
+  // smaller than hiding the copies needs); never more than inc_set_chunk_events
+  size_t chunk = (size_t)n > ((size_t)1 << 21) ? 2 * g.host_chunk_events : g.host_chunk_events;
+  if (chunk > g.chunk_events) chunk = g.chunk_events;
+  if ((size_t)n < chunk) chunk = (size_t)(n > 0 ? n : 1);
+  int rc = ensure_ws(chunk, chunk);
+  if (rc) return rc;
+  rc = ensure_host_ring(chunk);
+  if (rc) return rc;
   State::HostPath &h = g.hp;
-  if ((size_t)n > h.n_cap) {
-    void **p[] = {(void **)&h.E, (void **)&h.tid, (void **)&h.counts, (void **)&h.A, (void **)&h.Z, (void **)&h.Es,
-                  (void **)&h.px, (void **)&h.py, (void **)&h.pz, (void **)&h.status};
-    for (auto q : p) { if (*q) cudaFree(*q); *q = nullptr; }
-    const size_t m = (size_t)n;
-    CU_TRY(cudaMalloc((void **)&h.E, m * sizeof(real))); CU_TRY(cudaMalloc((void **)&h.tid, m * 4));
-    CU_TRY(cudaMalloc((void **)&h.counts, m * 4)); CU_TRY(cudaMalloc((void **)&h.A, m * 4)); CU_TRY(cudaMalloc((void **)&h.Z, m * 4));
-    CU_TRY(cudaMalloc((void **)&h.Es, m * sizeof(real))); CU_TRY(cudaMalloc((void **)&h.px, m * sizeof(real)));
-    CU_TRY(cudaMalloc((void **)&h.py, m * sizeof(real))); CU_TRY(cudaMalloc((void **)&h.pz, m * sizeof(real)));
-    CU_TRY(cudaMalloc((void **)&h.status, m * 4));
-    h.n_cap = m;
-  }
-  if ((size_t)sec->capacity > h.sec_cap) {
-    void **p[] = {(void **)&h.sp, (void **)&h.T, (void **)&h.ux, (void **)&h.uy, (void **)&h.uz};
-    for (auto q : p) { if (*q) cudaFree(*q); *q = nullptr; }
-    const size_t m = (size_t)sec->capacity;
-    CU_TRY(cudaMalloc((void **)&h.sp, m)); CU_TRY(cudaMalloc((void **)&h.T, m * sizeof(real)));
-    CU_TRY(cudaMalloc((void **)&h.ux, m * sizeof(real))); CU_TRY(cudaMalloc((void **)&h.uy, m * sizeof(real)));
-    CU_TRY(cudaMalloc((void **)&h.uz, m * sizeof(real)));
-    h.sec_cap = m;
-  }
-  CU_TRY(cudaMemcpyAsync(h.E, E_in, (size_t)n * sizeof(real), cudaMemcpyHostToDevice, g.stream));
-  CU_TRY(cudaMemcpyAsync(h.tid, tid, (size_t)n * 4, cudaMemcpyHostToDevice, g.stream));
-  inc_secondaries ds; ds.species = h.sp; ds.T = h.T; ds.ux = h.ux; ds.uy = h.uy; ds.uz = h.uz; ds.capacity = sec->capacity;
-  inc_residual dr; dr.A = h.A; dr.Z = h.Z; dr.Estar = h.Es; dr.px = h.px; dr.py = h.py; dr.pz = h.pz; dr.status = h.status;
-  // Streaming: the call runs in chunks of <= 2^19 events; while chunk c+1 computes on the
-  // caller's stream, the outputs of chunk c travel to the host on a second stream.  After each chunk its running
-  // total of secondaries is read back (8 bytes, pinned) behind an event: that is the range of its list.
-  constexpr int kMaxHostChunks = 4096;
-  if (!h.copy_stream) CU_TRY(cudaStreamCreateWithFlags(&h.copy_stream, cudaStreamNonBlocking));
-  if (!h.h_tot) CU_TRY(cudaMallocHost((void **)&h.h_tot, kMaxHostChunks * sizeof(unsigned long long)));
-  struct Pending { long long e0; int nc; int c; };
-  std::vector<Pending> pend;
-  auto copy_chunk = [&](const Pending &q) -> int {
-    CU_TRY(cudaEventSynchronize(h.ev[q.c]));
-    const unsigned long long t1 = h.h_tot[q.c], t0 = q.c ? h.h_tot[q.c - 1] : 0ull;
-    const size_t m = (size_t)q.nc, o = (size_t)q.e0;
-    cudaStream_t cs = h.copy_stream;
-    CU_TRY(cudaMemcpyAsync(counts + o, h.counts + o, m * 4, cudaMemcpyDeviceToHost, cs));
-    CU_TRY(cudaMemcpyAsync(res->A + o, h.A + o, m * 4, cudaMemcpyDeviceToHost, cs));
-    CU_TRY(cudaMemcpyAsync(res->Z + o, h.Z + o, m * 4, cudaMemcpyDeviceToHost, cs));
-    CU_TRY(cudaMemcpyAsync(res->Estar + o, h.Es + o, m * sizeof(real), cudaMemcpyDeviceToHost, cs));
-    CU_TRY(cudaMemcpyAsync(res->px + o, h.px + o, m * sizeof(real), cudaMemcpyDeviceToHost, cs));
-    CU_TRY(cudaMemcpyAsync(res->py + o, h.py + o, m * sizeof(real), cudaMemcpyDeviceToHost, cs));
-    CU_TRY(cudaMemcpyAsync(res->pz + o, h.pz + o, m * sizeof(real), cudaMemcpyDeviceToHost, cs));
-    CU_TRY(cudaMemcpyAsync(res->status + o, h.status + o, m * 4, cudaMemcpyDeviceToHost, cs));
-    const unsigned long long cap = (unsigned long long)sec->capacity;
-    const unsigned long long a0 = t0 < cap ? t0 : cap, a1 = t1 < cap ? t1 : cap;     // nothing is written past the capacity
+  const long long n_chunks = (n + (long long)chunk - 1) / (long long)chunk;
+  State::Lane L = lane0();
+  g.cur = &L;
+  CU_TRY(cudaMemsetAsync(g.d_ctr, 0, sizeof(DevCounters), g.stream));
+  if (int rk_rc = set_round_keys(seed)) return rk_rc;
+  for (auto e : g.pending_events) cudaEventDestroy(e);
+  g.pending_events.clear();
+  for (int i = 0; i < 4; ++i) { g.stage_ms[i] = 0; g.stage_launches[i] = 0; }
+  const bool stats = (g.flags & INC_F_STATS) != 0;
+  unsigned long long host_total = 0;                       // secondaries of the chunks copied so far
+  const unsigned long long cap = (unsigned long long)sec->capacity;
+  cudaStream_t cs = h.copy_stream;
+  // outputs of chunk c -> host (its kernels have been enqueued before)
+  auto copy_out = [&](long long c) -> int {
+    State::HostSlot &sl = h.slot[c % State::kRing];
+    const size_t o = (size_t)c * chunk;
+    const size_t m = (size_t)(n - (long long)o) < chunk ? (size_t)(n - (long long)o) : chunk;
+    CU_TRY(cudaEventSynchronize(sl.computed));
+    const unsigned long long t = h.h_tot[c % State::kRing];
+    CU_TRY(cudaMemcpyAsync(counts + o, sl.counts, m * 4, cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->A + o, sl.A, m * 4, cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->Z + o, sl.Z, m * 4, cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->Estar + o, sl.Es, m * sizeof(real), cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->px + o, sl.px, m * sizeof(real), cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->py + o, sl.py, m * sizeof(real), cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->pz + o, sl.pz, m * sizeof(real), cudaMemcpyDeviceToHost, cs));
+    CU_TRY(cudaMemcpyAsync(res->status + o, sl.status, m * 4, cudaMemcpyDeviceToHost, cs));
+    const unsigned long long a0 = host_total < cap ? host_total : cap;                 // nothing is written past the capacity
+    const unsigned long long a1 = host_total + t < cap ? host_total + t : cap;
     if (a1 > a0) {
       const size_t k = (size_t)(a1 - a0), f = (size_t)a0;
-      CU_TRY(cudaMemcpyAsync(sec->species + f, h.sp + f, k, cudaMemcpyDeviceToHost, cs));
-      CU_TRY(cudaMemcpyAsync(sec->T + f, h.T + f, k * sizeof(real), cudaMemcpyDeviceToHost, cs));
-      CU_TRY(cudaMemcpyAsync(sec->ux + f, h.ux + f, k * sizeof(real), cudaMemcpyDeviceToHost, cs));
-      CU_TRY(cudaMemcpyAsync(sec->uy + f, h.uy + f, k * sizeof(real), cudaMemcpyDeviceToHost, cs));
-      CU_TRY(cudaMemcpyAsync(sec->uz + f, h.uz + f, k * sizeof(real), cudaMemcpyDeviceToHost, cs));
+      CU_TRY(cudaMemcpyAsync(sec->species + f, sl.sp, k, cudaMemcpyDeviceToHost, cs));
+      CU_TRY(cudaMemcpyAsync(sec->T + f, sl.T, k * sizeof(real), cudaMemcpyDeviceToHost, cs));
+      CU_TRY(cudaMemcpyAsync(sec->ux + f, sl.ux, k * sizeof(real), cudaMemcpyDeviceToHost, cs));
+      CU_TRY(cudaMemcpyAsync(sec->uy + f, sl.uy, k * sizeof(real), cudaMemcpyDeviceToHost, cs));
+      CU_TRY(cudaMemcpyAsync(sec->uz + f, sl.uz, k * sizeof(real), cudaMemcpyDeviceToHost, cs));
     }
+    host_total += t;
+    CU_TRY(cudaEventRecord(sl.copied, cs));
     return 0;
   };
-  g.chunk_hook = [&](int c, long long e0, int nc) -> int {
-    if (c < 0) {                    // start of a run
-      CU_TRY(cudaStreamSynchronize(h.copy_stream));
-      pend.clear();
-      return 0;
-    }
-    if (c >= kMaxHostChunks) return fail(INC_E_BADARG, "inc_simulate_host: too many chunks (raise the chunk size)");
-    while ((int)h.ev.size() <= c) {
-      cudaEvent_t e;
-      CU_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-      h.ev.push_back(e);
-    }
-    CU_TRY(cudaMemcpyAsync(&h.h_tot[c], &g.d_ctr->total_sec, sizeof(unsigned long long), cudaMemcpyDeviceToHost, g.stream));
-    CU_TRY(cudaEventRecord(h.ev[c], g.stream));
-    if (!pend.empty()) {            // chunk c is enqueued: now wait for chunk c-1 and send its outputs home
-      const Pending q = pend.back();
-      pend.pop_back();
-      if (int rc = copy_chunk(q)) return rc;
-    }
-    pend.push_back(Pending{e0, nc, c});
-    return 0;
-  };
-  const int64_t tot = inc_simulate(n, h.E, h.tid, seed, &ds, h.counts, &dr);
-  g.chunk_hook = nullptr;
-  if (tot < 0 && tot != INC_E_CAPACITY) { cudaStreamSynchronize(h.copy_stream); return tot; }
-  while (!pend.empty()) {
-    const Pending q = pend.back();
-    pend.pop_back();
-    if (int rc = copy_chunk(q)) return rc;
+  for (long long c = 0; c < n_chunks; ++c) {
+    State::HostSlot &sl = h.slot[c % State::kRing];
+    const long long e0 = c * (long long)chunk;
+    const int nc = (int)((n - e0) < (long long)chunk ? (n - e0) : (long long)chunk);
+    // the slot is free once the copies of chunk c - kRing are done (they were enqueued two iterations ago)
+    if (c >= State::kRing) CU_TRY(cudaStreamWaitEvent(L.stream, sl.copied, 0));
+    CU_TRY(cudaMemcpyAsync(sl.E, E_in + e0, (size_t)nc * sizeof(real), cudaMemcpyHostToDevice, L.stream));
+    CU_TRY(cudaMemcpyAsync(sl.tid, tid + e0, (size_t)nc * 4, cudaMemcpyHostToDevice, L.stream));
+    CU_TRY(cudaMemsetAsync(&L.ctr->total_sec, 0, sizeof(unsigned long long), L.stream));     // chunk-local offsets
+    inc_secondaries ds; ds.species = sl.sp; ds.T = sl.T; ds.ux = sl.ux; ds.uy = sl.uy; ds.uz = sl.uz;
+    ds.capacity = (int64_t)chunk * kMaxSec;
+    inc_residual dr; dr.A = sl.A; dr.Z = sl.Z; dr.Estar = sl.Es; dr.px = sl.px; dr.py = sl.py; dr.pz = sl.pz; dr.status = sl.status;
+    const uint8_t *pj = g.projectile ? g.projectile + e0 : nullptr;
+    rc = stats ? launch_chunk<true>(e0, nc, sl.E, sl.tid, pj, seed, &ds, sl.counts, &dr, L.offsets)
+               : launch_chunk<false>(e0, nc, sl.E, sl.tid, pj, seed, &ds, sl.counts, &dr, L.offsets);
+    if (rc) { cudaStreamSynchronize(L.stream); cudaStreamSynchronize(cs); return rc; }
+    CU_TRY(cudaMemcpyAsync(&h.h_tot[c % State::kRing], &L.ctr->total_sec, sizeof(unsigned long long), cudaMemcpyDeviceToHost, L.stream));
+    CU_TRY(cudaEventRecord(sl.computed, L.stream));
+    // chunk c is enqueued: now wait for chunk c - 1 and send its outputs home while c computes
+    if (c >= 1) { rc = copy_out(c - 1); if (rc) return rc; }
   }
-  CU_TRY(cudaStreamSynchronize(h.copy_stream));
-  CU_TRY(cudaStreamSynchronize(g.stream));
-  return tot;
+  if (n_chunks >= 1) { rc = copy_out(n_chunks - 1); if (rc) return rc; }
+  CU_TRY(cudaMemcpyAsync(h.h_err, &L.ctr->error_word, sizeof(unsigned int), cudaMemcpyDeviceToHost, L.stream));
+  CU_TRY(cudaStreamSynchronize(L.stream));
+  CU_TRY(cudaStreamSynchronize(cs));
+  if (int rt = resolve_stage_times()) return rt;
+  g.last_n = n; g.last_total = (long long)host_total;
+  g.last_chunks = (int)n_chunks;
+  g.last_offsets_valid = n_chunks <= 1;
+  if (int64_t er = device_error(n > 0 ? *h.h_err : 0u)) return er;
+  if (host_total > cap) {
+    char buf[160];
+    std::snprintf(buf, sizeof buf, "secondary capacity %lld too small, need %llu", (long long)sec->capacity, host_total);
+    return fail(INC_E_CAPACITY, buf);
+  }
+  return (int64_t)host_total;
 }
+
+}  // namespace
+
+extern "C" {
 
 }  // extern "C"

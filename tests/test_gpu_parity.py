@@ -637,3 +637,54 @@ def test_host_path_streams_in_chunks(gpu, ptables):
     half = ref["total"] // 2
     assert np.array_equal(small["counts"].numpy(), ref["counts"])
     assert np.array_equal(small["T"].numpy()[:half], ref["T"][:half])
+
+
+def test_host_path_memory_is_bounded(gpu, ptables):
+    """inc_simulate_host on 2e7 events (twice config 4): the ring of chunk buffers keeps the library's device memory
+    independent of n (the same workspace as for 3e6 events), every event conserves A and Z, and the first and last
+    1e5 events equal what inc_simulate gives for those global event indices."""
+    import torch
+    import paper_1309_7963_b200.workloads as W
+    n = 20_000_000
+    E1, tid1, targets, seed, _ = W.make_inputs(4, 10_000_000)
+    E = np.concatenate([E1, E1[::-1]]).astype(np.float32)
+    tid = np.concatenate([tid1, tid1[::-1]])
+    lib = gpu.load("f32")
+    lib.inc_shutdown()
+    slots = np.asarray([lib.inc_init(a, z, ptables) for a, z in targets], dtype=np.int32)
+    lib.inc_set_stream(); lib.inc_set_flags(0)
+    Eh = torch.as_tensor(E).pin_memory()
+    th = torch.as_tensor(slots[tid]).pin_memory()
+    out = lib.alloc_outputs(n, n * 7, device="cpu")
+    torch.cuda.synchronize()
+    m = 3_000_000
+    small = {k: (v[:m] if v.shape[0] == n else v) for k, v in out.items()}
+    lib.inc_simulate_host(Eh[:m], th[:m], seed, small)                     # same chunk size as the long call (n > 2^21)
+    free_small = torch.cuda.mem_get_info()[0]
+    tot = lib.inc_simulate_host(Eh, th, seed, out)
+    free_big = torch.cuda.mem_get_info()[0]
+    assert free_small - free_big < (64 << 20), (free_small, free_big)      # no growth with n
+    counts = out["counts"].numpy().astype(np.int64)
+    assert counts.sum() == tot
+    off = np.concatenate([[0], np.cumsum(counts)])
+    At = np.array([a for a, z in targets])[tid]
+    code = out["species"].numpy()[:tot] & 0x7F
+    SA = np.array([1, 1, 2, 3, 3, 4])
+    sumA = np.add.reduceat(SA[code], off[:-1].clip(max=tot - 1)) * (counts > 0)
+    ok = (out["status"].numpy().view(np.uint32) & gpu.ST_FAILED) == 0
+    assert np.all((sumA + out["A"].numpy() == At + 1)[ok])
+    with pytest.raises(gpu.IncError):
+        lib.inc_get_offsets(n)                                             # per-chunk offsets only
+    for lo in (0, n - 100_000):
+        hi = lo + 100_000
+        Ed = torch.as_tensor(E[lo:hi], device="cuda"); td = torch.as_tensor(slots[tid[lo:hi]], device="cuda")
+        dev = lib.alloc_outputs(hi - lo, (hi - lo) * 24)
+        lib.inc_set_event_offset(lo)
+        try:
+            t = lib.inc_simulate(Ed, td, seed, dev)
+        finally:
+            lib.inc_set_event_offset(0)
+        for k in ("counts", "A", "Z", "Estar", "px", "status"):
+            assert np.array_equal(dev[k].cpu().numpy(), out[k].numpy()[lo:hi]), k
+        for k in ("species", "T", "uz"):
+            assert np.array_equal(dev[k][:t].cpu().numpy(), out[k].numpy()[off[lo]:off[hi]]), k
