@@ -43,42 +43,122 @@ def work_per_event(stats: dict) -> dict:
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    """SM clock and throttle reasons DURING the timed region (B200_PROFILING.md).  The timed region of the default run is
+    ~20 ms, so the recipe's `nvidia-smi -lms 200` would see it once at best: this polls NVML from a thread every
+    millisecond instead (same counters), and falls back to nvidia-smi if NVML cannot be loaded."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
-        self.index, self.rows, self.proc = index, [], None
+        self.index, self.rows, self.proc, self.nvml, self.stop_flag = index, [], None, None, False
 
     def start(self):
         try:
+            import pynvml
+            pynvml.nvmlInit()
+            # CUDA_VISIBLE_DEVICES may renumber: take the NVML handle by the PCI bus id of the torch device
+            import torch
+            bus = torch.cuda.get_device_properties(self.index).pci_bus_id if hasattr(torch.cuda.get_device_properties(self.index), "pci_bus_id") else None
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(self.index) if bus is None else pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.nvml = pynvml
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.th = threading.Thread(target=self._poll, daemon=True)
+            self.th.start()
+            return
+        except Exception:
+            self.nvml = None
+        try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+                                          "-lms", "20", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
         except OSError:
             self.proc = None
 
+    def _poll(self):
+        n = self.nvml
+        R = {"hw_slowdown": n.nvmlClocksEventReasonHwSlowdown if hasattr(n, "nvmlClocksEventReasonHwSlowdown") else 0x8,
+             "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
+        get_reasons = getattr(n, "nvmlDeviceGetCurrentClocksEventReasons", None) or getattr(n, "nvmlDeviceGetCurrentClocksThrottleReasons")
+        while not self.stop_flag:
+            try:
+                sm = float(n.nvmlDeviceGetClockInfo(self.h, n.NVML_CLOCK_SM))
+                mask = int(get_reasons(self.h))
+                pw = n.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+                self.rows.append((time.time(), sm, pw, [k for k, bit in R.items() if mask & bit]))
+            except Exception:
+                pass
+            time.sleep(0.001)
+
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+            r = [x.strip() for x in line.split(",")]
+            if len(r) >= 9:
+                names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+                self.rows.append((time.time(), float(r[1]), float(r[3]), [k for k, v in zip(names, r[5:9]) if v.lower().startswith("active")]))
+                self.sm_max = float(r[2])
 
     def stop(self, t0, t1):
-        if not self.proc:
-            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
-        time.sleep(0.15)
-        self.proc.terminate()
-        rows = [r for t, r in self.rows if t0 - 0.05 <= t <= t1 + 0.15 and len(r) >= 9] or [r for _, r in self.rows if len(r) >= 9]
+        self.stop_flag = True
+        if self.nvml is None and not self.proc:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no NVML, no nvidia-smi"])
+        time.sleep(0.03)
+        if self.proc:
+            self.proc.terminate()
+        rows = [r for r in self.rows if t0 <= r[0] <= t1]
+        loaded = [r for r in self.rows if r[0] <= t1]
+        if not rows:
+            rows = loaded[-3:]
         if not rows:
             return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
-        sm = sorted(float(r[1]) for r in rows)
-        reasons = set()
-        for r in rows:
-            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
-                if v.lower().startswith("active"):
-                    reasons.add(name)
-        return dict(sm_mhz=sm[len(sm) // 2], sm_max_mhz=float(rows[0][2]), power_w_max=max(float(r[3]) for r in rows),
-                    samples=len(rows), reasons=sorted(reasons))
+        sm = sorted(r[1] for r in rows)
+        reasons = sorted({k for r in rows for k in r[3]})
+        return dict(sm_mhz=sm[len(sm) // 2], sm_min_mhz=sm[0], sm_max_mhz=getattr(self, "sm_max", None), power_w_max=max(r[2] for r in rows),
+                    samples=len(rows), samples_warmup_and_timed=len(loaded), source="NVML polled every ms" if self.nvml else "nvidia-smi -lms 20",
+                    reasons=reasons)
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def _oracle_shard(job):
+    """One process of the all-core oracle leg: events [a, b) of the config (counter-keyed RNG: shards are exact)."""
+    cfg, n, a, b = job
+    from oracle import oracle as O
+    import paper_1309_7963_b200.workloads as W
+    E, tid, targets, seed, _ = W.make_inputs(cfg, n)
+    t = O.Tables()
+    nuclei = [O.setup_nucleus(A, Z, t) for A, Z in targets]
+    t0 = time.perf_counter()
+    O.simulate(t, nuclei, E[a:b], tid[a:b], seed, e0=a, want_stats=False)
+    return time.perf_counter() - t0
+
+
+def oracle_baseline(cfg, n, one_thread_events, per_core_events):
+    """The oracle as it stands on the host cores: one thread, then one process per core on disjoint event ranges."""
+    import multiprocessing as mp
+    m1 = min(one_thread_events, n)
+    dt1 = _oracle_shard((cfg, n, 0, m1))
+    P = os.cpu_count() or 1
+    per = max(1000, min(per_core_events, n // P))
+    jobs = [(cfg, n, i * per, (i + 1) * per) for i in range(P)]
+    t0 = time.perf_counter()
+    with mp.get_context("spawn").Pool(P) as pool:
+        pool.map(_oracle_shard, jobs[:P])            # (first map also pays the workers' start-up and library load)
+        t1 = time.perf_counter()
+        pool.map(_oracle_shard, jobs)
+        dtP = time.perf_counter() - t1
+    return dict(value=P * per / dtP, unit=UNIT, cores=P, kind="oracle", cpu_model=cpu_model(),
+                single_thread=dict(value=m1 / dt1, events=m1, seconds=round(dt1, 2)),
+                sample=f"config {cfg}: {P} processes x {per} events each in {dtP:.1f} s (aggregate = value); one thread: first {m1} events in "
+                       f"{dt1:.1f} s; oracle/inc_oracle.c as it stands, gcc -O2 -ffp-contract=off")
 
 
 def run_reference(args, rank, world):
@@ -119,8 +199,9 @@ def main():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--events", type=int, default=None, help="override the config's event count")
     ap.add_argument("--ref-events", type=int, default=100000, help="events per step of --impl reference")
-    ap.add_argument("--cpu-events", type=int, default=400000, help="oracle sample of the cpu_baseline leg")
+    ap.add_argument("--cpu-events", type=int, default=400000, help="oracle sample of the cpu_baseline leg: one thread; a quarter of it per core for the all-core leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the one-line-per-config block (configs 1-5, f32 and f64)")
     ap.add_argument("--variant", default="f32", choices=["f32", "f64"])
     ap.add_argument("--flags", type=int, default=0)
     ap.add_argument("--vote", type=int, nargs=2, default=None)
@@ -171,34 +252,29 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- work counters (one untimed pass with INC_F_STATS) and stage timing ----
+    # ---- work counters: one untimed pass with INC_F_STATS ----
     lib.inc_set_flags(args.flags | B.F_STATS)
     total = lib.inc_simulate(E_d, tid_d, seed, out)
     stats = lib.inc_get_stats()
     wpe = work_per_event(stats)
 
-    lib.inc_set_flags(args.flags | B.F_TIMING)
-    for _ in range(args.warmup):
-        lib.inc_simulate(E_d, tid_d, seed, out)
+    # ---- the timed region: K steps in the production configuration (the evaporation kernel overlaps the cascade
+    # kernel's tail, no events between the stages), CUDA events around it on the launching stream ----
+    lib.inc_set_flags(args.flags)
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
-        time.sleep(0.25)
+    for _ in range(args.warmup):
+        lib.inc_simulate(E_d, tid_d, seed, out)
     barrier()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    stage = dict(cascade=0.0, evap=0.0, scan=0.0, compact=0.0)
-    launches = 0
-    t_wall0 = time.time()
     step_ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    t_wall0 = time.time()
     ev0.record()
     step_ev[0].record()
     for k in range(args.steps):
         lib.inc_simulate(E_d, tid_d, seed + k, out)
         step_ev[k + 1].record()
-        ms, nl = lib.inc_get_stage_times()
-        for kk in stage:
-            stage[kk] += ms[kk]
-        launches += sum(nl)
     ev1.record()
     barrier()
     t_wall1 = time.time()
@@ -209,8 +285,27 @@ def main():
     ms_total = float(tmax.item())
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     value = world * n * args.steps / (ms_total * 1e-3)
-
     per_step = sorted(step_ev[k].elapsed_time(step_ev[k + 1]) for k in range(args.steps))
+    chunks = -(-n // (1 << 22))
+    launches = args.steps * chunks * 6          # cascade, evaporation, three scan kernels, compaction per chunk
+
+    # ---- per-kernel durations: the same K steps again with INC_F_TIMING, which puts CUDA events between the stages
+    # and therefore runs them one after the other (the roofline of a kernel needs a duration of its own) ----
+    lib.inc_set_flags(args.flags | B.F_TIMING)
+    lib.inc_simulate(E_d, tid_d, seed, out)
+    stage = dict(cascade=0.0, evap=0.0, scan=0.0, compact=0.0)
+    sv0, sv1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sv0.record()
+    for k in range(args.steps):
+        lib.inc_simulate(E_d, tid_d, seed + k, out)
+        ms, nl = lib.inc_get_stage_times()
+        for kk in stage:
+            stage[kk] += ms[kk]
+    sv1.record()
+    torch.cuda.synchronize()
+    serial_ms = sv0.elapsed_time(sv1) / args.steps
+    timeline = lib.inc_get_drain_timeline()
+
     # ---- extras (outside the timed region) ----
     # divergence-free ceiling: every event draws the random stream of event 0
     lib.inc_set_flags(args.flags | B.F_SAME_STREAM)
@@ -221,10 +316,9 @@ def main():
     pev1.record()
     torch.cuda.synchronize()
     same_stream_ms = pev0.elapsed_time(pev1)
-    lib.inc_set_flags(args.flags | B.F_TIMING)
+    # on-device tallies
+    lib.inc_set_flags(args.flags)
     lib.inc_simulate(E_d, tid_d, seed + args.steps - 1, out)
-    # drain timeline of the last cascade launch, on-device tallies
-    timeline = lib.inc_get_drain_timeline()
     off_d = lib.inc_get_offsets(n)
     tspec, tall = lib.alloc_tallies()
     lib.inc_tally(out, off_d, tspec, tall)
@@ -237,7 +331,6 @@ def main():
     tally_ms = tev0.elapsed_time(tev1) / 5
 
     # ---- end to end through the host-buffer entry point (pinned host memory) ----
-    lib.inc_set_flags(args.flags)
     E_h = torch.as_tensor(E.astype(lib.real)).pin_memory()
     tid_h = torch.as_tensor(slots[tid]).pin_memory()
     out_h = lib.alloc_outputs(n, cap, device="cpu")
@@ -257,6 +350,7 @@ def main():
     rb = E_h.element_size()
     h2d = n * (rb + 4)
     d2h = n * (4 + 4 + 4 + 4 * rb + 4) + tot_h * (1 + 4 * rb)
+    del out_h, E_h, tid_h
 
     if rank != 0:
         if dist is not None:
@@ -274,36 +368,42 @@ def main():
             traffic = json.load(open(tpath)).get("cascade_dram_bytes_per_launch")
         except Exception:
             traffic = None
-    roofline = dict(bound="alu", kernel="cascade_kernel", achieved=achieved / 1e12, peak=peak / 1e12, unit="T lane-instr/s",
+    roofline = dict(bound="alu", kernel="cascade_wavefront_kernel", achieved=achieved / 1e12, peak=peak / 1e12, unit="T lane-instr/s",
                     frac=achieved / peak, traffic=traffic,
                     peak_source=f"measured in this run: {'FFMA' if args.variant == 'f32' else 'DFMA'} chain microbenchmark (inc_measure_issue_peak)",
                     work_lane_instr_per_event=wpe, kernel_ms=dict((k, v / args.steps) for k, v in stage.items()),
+                    kernel_ms_note="stages run one after the other (INC_F_TIMING) over the same K steps; in the timed region the evaporation kernel overlaps the cascade kernel's tail",
+                    serialized_ms_per_step=serial_ms,
                     kernel_share=dict((k, v / max(sum(stage.values()), 1e-9)) for k, v in stage.items()),
+                    evap_frac=wpe["evap"] * n / (stage["evap"] / args.steps * 1e-3) / peak,
                     whole_step_frac=wpe["total"] * n / (ms_total / args.steps * 1e-3) / peak)
+
+    # ---- every config of BASELINE.json, one line each (outside the timed region): production build, events/s of the
+    # whole step, cascade roofline fraction; and the fp64 parity build's events/s ----
+    per_config = None
+    if not args.no_per_config and world == 1 and args.variant == "f32":
+        per_config = {}
+        del out
+        for c in (1, 2, 3, 4, 5):
+            per_config[str(c)] = config_line(c, peak, B, T, W, np, torch)
+        lib.inc_shutdown()
 
     cpu_baseline = None
     if not args.no_cpu_baseline:
-        from oracle import oracle as O
-        m = min(args.cpu_events, n)
-        ot = O.Tables()
-        nuclei = [O.setup_nucleus(a, z, ot) for a, z in targets]
-        t0 = time.perf_counter()
-        O.simulate(ot, nuclei, E[:m], tid[:m], seed, want_stats=False)
-        dtc = time.perf_counter() - t0
-        cpu_baseline = dict(value=m / dtc, unit=UNIT, cores=1, kind="oracle",
-                            sample=f"first {m} events of config {cfg}, single thread, gcc -O2 -ffp-contract=off, {dtc:.1f} s")
+        cpu_baseline = oracle_baseline(cfg, n, args.cpu_events, args.cpu_events // 4)
 
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=ms_total / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype=args.variant, data="synthetic",
                 config=dict(workload=f"config {cfg}: {name}", events_per_step_per_gpu=n, seed=seed,
                             secondaries_per_step=int(total), build=lib.build_info(),
-                            l2="no flush: each step writes and re-reads ~0.3 GB (staging records, post-cascade records, outputs; new seed every step), above the 126 MB L2",
+                            l2="no flush: each step writes and re-reads ~0.3 GB (staging records, nucleus records, outputs; new seed every step), above the 126 MB L2",
                             parallelism=f"dp{world} (independent event ranges, no collective)"),
                 clocks=clocks, e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                                         steps=e2e_steps),
                 gpu_launches=int(launches), roofline=roofline, cpu_baseline=cpu_baseline,
                 per_step_ms=dict(best=per_step[0], median=per_step[len(per_step) // 2]),
+                per_config=per_config,
                 same_stream_probe=dict(ms=same_stream_ms, events_per_s=n / (same_stream_ms * 1e-3),
                                        note="INC_F_SAME_STREAM: all events identical, no divergence (the paper's probe, P:73-75)"),
                 paper_time_split="GTX680, 200 MeV p-16O: INC 72 %, evaporation 23 %, RNG init 3 % (P:142); see roofline.kernel_share",
@@ -317,6 +417,54 @@ def main():
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def config_line(c, peak, B, T, W, np, torch, steps=3):
+    """One BASELINE.json config: events/s of the whole step (production build, device-resident, `steps` steps after two
+    warm-ups), the cascade kernel's roofline fraction (INC_F_TIMING steps), and the fp64 parity build's events/s."""
+    n = W.CONFIGS[c]["n"]
+    E, tid, targets, seed, name = W.make_inputs(c, n)
+    tables = T.default_tables()
+    res = dict(workload=name, events=n)
+    for variant in ("f32", "f64"):
+        lib = B.load(variant)
+        lib.inc_shutdown()
+        slots = np.array([lib.inc_init(a, z, tables) for a, z in targets], dtype=np.int32)
+        lib.inc_set_stream()
+        m = n if variant == "f32" else min(n, 1000000)
+        E_d = torch.as_tensor(E[:m].astype(lib.real), device="cuda")
+        tid_d = torch.as_tensor(slots[tid[:m]], device="cuda")
+        out = lib.alloc_outputs(m, m * 12)
+        if variant == "f32":
+            lib.inc_set_flags(B.F_STATS)
+            lib.inc_simulate(E_d, tid_d, seed, out)
+            wpe = work_per_event(lib.inc_get_stats())
+        lib.inc_set_flags(0)
+        for _ in range(2):
+            lib.inc_simulate(E_d, tid_d, seed, out)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for k in range(steps):
+            lib.inc_simulate(E_d, tid_d, seed + k, out)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        if variant == "f32":
+            lib.inc_set_flags(B.F_TIMING)
+            casc = 0.0
+            for k in range(steps):
+                lib.inc_simulate(E_d, tid_d, seed + k, out)
+                casc += lib.inc_get_stage_times()[0]["cascade"] / steps
+            res.update(events_per_s=m / (ms * 1e-3), ms_per_step=ms, cascade_ms=casc,
+                       roofline_frac=wpe["cascade"] * m / (casc * 1e-3) / peak,
+                       whole_step_frac=wpe["total"] * m / (ms * 1e-3) / peak)
+        else:
+            res.update(f64_events_per_s=m / (ms * 1e-3), f64_events=m)
+        lib.inc_set_flags(0)
+        lib.inc_shutdown()
+        del out, E_d, tid_d
+        torch.cuda.empty_cache()
+    return res
 
 
 if __name__ == "__main__":
