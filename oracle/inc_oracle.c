@@ -213,7 +213,7 @@ double orc_plab(const double p1[3], double m1, const double p2[3], double m2) {
   double s = (E1 + E2_) * (E1 + E2_) - dot3(P, P);
   double Elab = (s - m1 * m1 - m2 * m2) / (2.0 * m2);
   double q = Elab * Elab - m1 * m1;
-  if (q < 0.0) q = 0.0;       /* rounding guard (R-G1) */
+  if (q < 0.0) q = 0.0;       /* rounding guard (R-RG1) */
   return sqrt(q) / 1000.0;
 }
 
@@ -222,7 +222,7 @@ void orc_shell_distances(const double x[3], const double d[3], double r_in, doub
                          int has_inner, double *d_in, double *d_out) {
   double beta = dot3(x, d), r2 = dot3(x, x);
   double disc_out = beta * beta - r2 + r_out * r_out;
-  if (disc_out < 0.0) disc_out = 0.0;   /* rounding guard (R-G2): x sits on/inside r_out */
+  if (disc_out < 0.0) disc_out = 0.0;   /* rounding guard (R-RG2): x sits on/inside r_out */
   *d_out = -beta + sqrt(disc_out);
   *d_in = INFINITY;
   if (has_inner && beta < 0.0) {
@@ -262,7 +262,7 @@ void orc_collide(const double p1[3], double m1, const double p2[3], double m2,
   if (B * (-tmin) < 1e-9) t = u_t * tmin;
   else t = log1p(-u_t * (-expm1(B * tmin))) / B;
   double ct = 1.0 + t / (2.0 * pg2);
-  if (ct < -1.0) ct = -1.0;                      /* rounding guard (R-G3) */
+  if (ct < -1.0) ct = -1.0;                      /* rounding guard (R-RG3) */
   if (ct > 1.0) ct = 1.0;
   if (!same_species && u_back * (1.0 + a_back) < a_back) ct = -ct;
   double st = sqrt(1.0 - ct * ct);
