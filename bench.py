@@ -385,7 +385,7 @@ def main():
         per_config = {}
         del out
         for c in (1, 2, 3, 4, 5):
-            per_config[str(c)] = config_line(c, peak, B, T, W, np, torch)
+            per_config[str(c)] = config_line(c, peak, B, T, W, np, torch, oracle=not args.no_cpu_baseline)
         lib.inc_shutdown()
 
     cpu_baseline = None
@@ -419,7 +419,7 @@ def main():
         dist.destroy_process_group()
 
 
-def config_line(c, peak, B, T, W, np, torch, steps=3):
+def config_line(c, peak, B, T, W, np, torch, steps=3, oracle=True):
     """One BASELINE.json config: events/s of the whole step (production build, device-resident, `steps` steps after two
     warm-ups), the cascade kernel's roofline fraction (INC_F_TIMING steps), and the fp64 parity build's events/s."""
     n = W.CONFIGS[c]["n"]
@@ -438,7 +438,9 @@ def config_line(c, peak, B, T, W, np, torch, steps=3):
         if variant == "f32":
             lib.inc_set_flags(B.F_STATS)
             lib.inc_simulate(E_d, tid_d, seed, out)
-            wpe = work_per_event(lib.inc_get_stats())
+            st = lib.inc_get_stats()
+            wpe = work_per_event(st)
+            res["lanes_per_segment_step"] = st["lane_slots_seg"] / max(st["warp_iters_seg"], 1)
         lib.inc_set_flags(0)
         for _ in range(2):
             lib.inc_simulate(E_d, tid_d, seed, out)
@@ -464,6 +466,10 @@ def config_line(c, peak, B, T, W, np, torch, steps=3):
         lib.inc_shutdown()
         del out, E_d, tid_d
         torch.cuda.empty_cache()
+    if oracle:
+        # the oracle on this config: one thread on 5e4 events, then every core on 2e4 events each
+        ob = oracle_baseline(c, n, min(n, 50000), 20000)
+        res.update(oracle_events_per_s_1thread=ob["single_thread"]["value"], oracle_events_per_s_allcores=ob["value"], oracle_cores=ob["cores"])
     return res
 
 
