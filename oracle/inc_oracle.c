@@ -19,6 +19,13 @@
  *   widths          closed form vs scipy.quad of the Weisskopf-Ewing integrand
  *   sampler         chi^2 vs the normalised pdf; Maxwellian limit
  *   events          exact A,Z conservation; 4-momentum 1e-6; LIFO == FIFO
+ *   decision logic  (tests/test_oracle_decisions.py) zeroed / flat sigma tables with closed forms for the
+ *                   transparent fraction and the partner share, uniform entry disc, blocked fraction of first
+ *                   collisions vs quadrature, cutoff thresholds in the escape spectra, track tree, B / a wiring,
+ *                   retry counters recounted from traces, channel frequencies vs W_j / Sum W, Dostrovsky rows vs
+ *                   numpy.interp; tests/test_pins_bite.py breaks this file 27 ways and each pin must turn red
+ *   GEM             (tests/test_oracle_gem.py) constants and matching, widths vs scipy.quad (2e-10), sampler chi^2
+ *                   and envelope inequality, mode 0 == the Weisskopf-Ewing model
  * PARITY UNPINNED: agreement of the resulting spectra with the paper's Figs. 1-3
  * (figures absent, no numbers printed; cited sub-models [10,12,17,18] not in PAPER.md).
  */
