@@ -1644,50 +1644,91 @@ __device__ __forceinline__ R gem_integral(const LdDev<R> &ld, R X, R beta, R lre
   return gem_range<R>(ld, X, beta, R(0), xs, lref) + gem_range<R>(ld, X, beta, xs, X, lref);
 }
 
-template <typename R, bool STATS, bool GEM>
-__global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const EvapParams<R> P) {
-  const int lane = threadIdx.x & 31;
-  const bool cascade_only = (P.flags & INC_F_CASCADE_ONLY) != 0;
-  const bool same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
-  int ev = -1;
-  unsigned long long pbase = 0;      // the warp's pool of completion-list entries: [pbase + ph, pbase + pn) not handed out yet
-  int pn = 0, ph = 0;
-  uint32_t pent = kNotDone;
-  int A = 0, Z = 0, count = 0;
-  R Es = 0, Px = 0, Py = 0, Pz = 0;
-  uint32_t status = 0, attempt = 0, kblk = 0;
-  RngKey g;
-  g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = 0; g.e1 = 0;
-  bool exhausted = false;
-  unsigned long long n_steps = 0, n_trials = 0, n_emit = 0;
+enum EvapMode : int { kEvapKernel = 0, kEvapHelper = 1, kEvapDrainOnly = 2 };
 
+// The persistent-lane evaporation loop as an object, so that two hosts can run it: the evaporation kernel (one pass after
+// the other until the completion list is exhausted) and the idle warps of the cascade kernel (a pass whenever they have
+// nothing else to do: DESIGN.md section 6).  State = one nucleus per lane + the warp's pool of completion-list entries.
+template <typename R, bool STATS, bool GEM>
+struct EvapLanes {
+  static constexpr int kTrialsPerPass = 2;
+  int lane;
+  bool cascade_only, same_stream;
+  int ev;
+  unsigned long long pbase;      // the warp's pool of completion-list entries: [pbase + ph, pbase + pn) not handed out yet
+  int pn, ph;
+  uint32_t pent;
+  int A, Z, count;
+  R Es, Px, Py, Pz;
+  uint32_t status, attempt, kblk;
+  RngKey g;
+  bool exhausted;
+  unsigned long long n_steps, n_trials, n_emit;
   // state of an emission step whose rejection sampling is not finished yet: at most kTrialsPerPass trials run per
   // pass, a lane that has not accepted by then keeps its step (channel, X, ...) and goes on in the next pass
   // without computing the widths again -- the loop's trip count is the maximum over the warp's lanes (4.7 for a
   // mean of 1.6 trials), and it was 37 % of the kernel's instructions at 6 lanes
-  constexpr int kTrialsPerPass = 2;
-  bool sampling = false;
-  int jsel = -1, ntrial = 0;
-  R Bpar = R(0), X = R(0), a = R(1), beta = R(0), V = R(0), BdBj = R(0), s = R(0), T = R(1), areaA = R(0), areaB = R(0);
-  R u1 = R(0), u2 = R(0);
+  bool sampling;
+  int jsel, ntrial;
+  R Bpar, X, a, beta, V, BdBj, s, T, areaA, areaB;
+  R u1, u2;
   LdDev<R> ldsel;           // GEM mode: level density of the chosen channel's daughter
-  ldsel.a = ldsel.delta = ldsel.Ux = ldsel.Ex = ldsel.T = ldsel.E0 = ldsel.lnT = ldsel.lna4 = R(0);
-  for (;;) {
+
+  __device__ __forceinline__ void init(const EvapParams<R> &P) {
+    lane = threadIdx.x & 31;
+    cascade_only = (P.flags & INC_F_CASCADE_ONLY) != 0;
+    same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
+    ev = -1; pbase = 0; pn = 0; ph = 0; pent = kNotDone;
+    A = 0; Z = 0; count = 0; Es = 0; Px = 0; Py = 0; Pz = 0;
+    status = 0; attempt = 0; kblk = 0;
+    g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = 0; g.e1 = 0;
+    exhausted = false;
+    n_steps = 0; n_trials = 0; n_emit = 0;
+    sampling = false; jsel = -1; ntrial = 0;
+    Bpar = R(0); X = R(0); a = R(1); beta = R(0); V = R(0); BdBj = R(0); s = R(0); T = R(1); areaA = R(0); areaB = R(0);
+    u1 = R(0); u2 = R(0);
+    ldsel.a = ldsel.delta = ldsel.Ux = ldsel.Ex = ldsel.T = ldsel.E0 = ldsel.lnT = ldsel.lna4 = R(0);
+  }
+  __device__ __forceinline__ bool busy() const { return __ballot_sync(kFull, ev >= 0) != 0u; }
+
+  // One pass: refill, one emission step (or up to kTrialsPerPass sampler trials of a pending one) per lane.  Returns
+  // false when there is nothing (more) to do: kernel mode -- the list is exhausted; helper modes -- no lane has an event.
+  __device__ __forceinline__ bool pass(const EvapParams<R> &P, const int mode) {
     __syncwarp();
-    // ---- refill idle lanes from the warp's pool of 32 consecutive entries of the cascade kernel's completion list
-    // (one global atomic and one coalesced load per 32 events; lane i holds entry pbase + i) ----
+    // ---- refill idle lanes from the warp's pool of consecutive entries of the cascade kernel's completion list
+    // (lane i holds entry pbase + i).  Kernel mode: a pool is 32 tickets taken blindly (one global atomic and one
+    // coalesced load per 32 events), entries not published yet are polled.  Helper mode (idle warps of the cascade
+    // kernel): only entries that are published already are taken (compare-and-swap on the ticket counter), so that a
+    // helper never holds a ticket it would have to wait for. ----
     const bool want = ev < 0;
     const unsigned need = __ballot_sync(kFull, want);
-    if (need) {
+    if (need && mode != kEvapDrainOnly) {
       if (ph == pn && !exhausted) {
-        unsigned long long base = 0;
-        if (lane == 0) base = atomicAdd(&P.ctr->next_event_evap, 32ull);
-        base = __shfl_sync(kFull, base, 0);
-        if (base >= (unsigned long long)P.n_chunk) exhausted = true;
-        else {
-          pbase = base; ph = 0; pent = kNotDone;
-          const unsigned long long left = (unsigned long long)P.n_chunk - base;
-          pn = left < 32ull ? (int)left : 32;
+        if (mode == kEvapKernel) {
+          unsigned long long base = 0;
+          if (lane == 0) base = atomicAdd(&P.ctr->next_event_evap, 32ull);
+          base = __shfl_sync(kFull, base, 0);
+          if (base >= (unsigned long long)P.n_chunk) exhausted = true;
+          else {
+            pbase = base; ph = 0; pent = kNotDone;
+            const unsigned long long left = (unsigned long long)P.n_chunk - base;
+            pn = left < 32ull ? (int)left : 32;
+          }
+        } else {
+          unsigned long long cur = 0;
+          if (lane == 0) cur = *(volatile unsigned long long *)&P.ctr->next_event_evap;
+          cur = __shfl_sync(kFull, cur, 0);
+          if (cur >= (unsigned long long)P.n_chunk) exhausted = true;
+          else {
+            const bool in = cur + (unsigned long long)lane < (unsigned long long)P.n_chunk;
+            const uint32_t v = in ? ld_acquire_u32(P.ws.done_list + cur + lane) : kNotDone;
+            const unsigned gap0 = ~__ballot_sync(kFull, v != kNotDone);
+            const int k = gap0 ? __ffs(gap0) - 1 : 32;
+            int ok = 0;
+            if (k > 0 && lane == 0) ok = atomicCAS(&P.ctr->next_event_evap, cur, cur + (unsigned long long)k) == cur;
+            ok = __shfl_sync(kFull, ok, 0);
+            if (ok) { pbase = cur; pn = k; ph = 0; pent = v; }
+          }
         }
       }
       if (ph < pn) {
@@ -1717,9 +1758,10 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
       }
     }
     if (__ballot_sync(kFull, ev >= 0) == 0) {
-      if (exhausted && ph == pn) break;
+      if (mode != kEvapKernel) return false;             // nothing to do right now
+      if (exhausted && ph == pn) return false;
       __nanosleep(200);                     // every lane waits for the cascade kernel
-      continue;
+      return true;
     }
     // The step is written as stages that every lane of the warp walks through, each under its own predicate, with
     // the rejection loop ended by a vote: the warp is converged again before the two-body kinematics.  (With the
@@ -1912,7 +1954,10 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
       P.ws.frec[ev] = r;
       ev = -1;
     }
+    return true;
   }
+
+  __device__ __forceinline__ void flush_stats(const EvapParams<R> &P) {
   if (STATS) {
     unsigned long long v[3] = {n_steps, n_trials, n_emit};
 #pragma unroll
@@ -1922,6 +1967,15 @@ __global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const
       if (lane == 0 && v[i]) atomicAdd(&P.ctr->stats[S_EVSTEPS + i], v[i]);
     }
   }
+  }
+};
+
+template <typename R, bool STATS, bool GEM>
+__global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const EvapParams<R> P) {
+  EvapLanes<R, STATS, GEM> L;
+  L.init(P);
+  while (L.pass(P, kEvapKernel)) { }
+  L.flush_stats(P);
 }
 
 // =================================================================================================
