@@ -11,7 +11,7 @@
 //   coll_step       C3  relativistic two-body scatter, Pauli blocking, cutoff
 //   epilogue_eval   C6  residual nucleus and excitation energy from 4-momentum balance
 // Kernels
-//   cascade_wavefront_kernel  DEFAULT.  Per-warp wavefront: tracks of ~48 events in flight live in
+//   cascade_wavefront_kernel  DEFAULT.  Per-warp wavefront: tracks of ~80 events in flight live in
 //                   per-warp shared-memory queues, sorted by the kind of step they need next
 //                   (segment / collision / epilogue+entry).  Every warp pass pops up to 32 items of
 //                   ONE kind, so lanes execute the same step; queue indices come from warp votes
@@ -20,6 +20,8 @@
 //                   {SEG, COLL, EPI} state machine; the warp votes which phase to run each pass.
 //   evap_kernel     persistent lanes, one Weisskopf-Ewing emission step per pass.
 //   scan_* / compact_kernel   exclusive prefix sum of counts, canonical-order SoA output.
+// Files: inc_common.cuh (model data, records, math, Philox), inc_physics.cuh (the steps), inc_cascade_lane.cuh,
+// inc_cascade_wavefront.cuh, inc_evap.cuh, inc_output.cuh; this header includes them in that order.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -36,2221 +38,10 @@
 #define INC_CHECK(cond) do { } while (0)
 #endif
 
-namespace inc {
 
-constexpr int kMaxShells = 32;
-constexpr int kMaxSeg = 1024;      // R-C2
-constexpr int kMaxAttempt = 256;   // R-C6
-constexpr int kMaxTrial = 64;      // R-E4
-constexpr int kMaxSec = INC_MAX_SEC;
-constexpr int kStackCap = 16;      // lane kernel: pending tracks per event (INC_ST_QUEUE_OVF beyond)
-constexpr int kAmax = 72;          // binding / channel tables cover 0..kAmax-1
-constexpr int kZmax = 66;          // (inc_init accepts Z <= 62; the residual may carry one charge more)
-constexpr unsigned kFull = 0xFFFFFFFFu;
-
-// ---- physical constants (standard values; R-K) -----------------------------------------
-template <typename R> struct K {
-  static constexpr R mp = R(938.27208816);
-  static constexpr R mn = R(939.56542052);
-  static constexpr R imp = R(1.0 / 938.27208816);
-  static constexpr R imn = R(1.0 / 939.56542052);
-};
-
-// ---- device-resident model data ----------------------------------------------------------
-template <typename R> struct ShellDev {   // one constant-density shell; 16 reals
-  R rho_p, rho_n;      // fm^-3
-  R pF_p, pF_n;        // Fermi momenta, MeV/c
-  R pF2_p, pF2_n;      // Pauli threshold on |p'|^2  (T' > E_F  <=>  p'^2 > pF^2)
-  R pc2_p, pc2_n;      // cutoff threshold on |p'|^2 (T' - V <= cut <=> p'^2 <= pc2)
-  R V_p, V_n;          // well depth E_F + E_B, MeV
-  R r_in, r_out;       // shell radii i*dr, (i+1)*dr
-  R ir_in, ir_out;     // reciprocals (ir_in = 0 for the innermost shell)
-  R pad0, pad1;
-};
-
-template <typename R> struct NucDev {
-  int32_t A, Z, ns, live;
-  R Rn, dr, Bt, iRn;                       // radius, shell thickness, target binding energy, 1/R
-  ShellDev<R> sh[kMaxShells + 1];          // [ns] = outside: V = 0
-};
-
-template <typename R> struct __align__(16) EvChan {        // per (A_d, Z_d, channel j): R-E1/E2 constants
-  R V;        // Coulomb barrier of the channel
-  R pref;     // g_j M_j A_d^(2/3) alpha_j   (0 => channel closed: daughter invalid)
-  R beta;     // Dostrovsky beta (neutron) or 0
-  R BdBj;     // B(A_d,Z_d) + B_j, so that X = E* - B(parent) + BdBj - V
-};
-
-// NEXT-2 (GEM level density, R-G2..G4): constants of one daughter nucleus; a = 0 => no level density (channel closed)
-template <typename R> struct __align__(16) LdDev {
-  R a, delta;     // level-density parameter MeV^-1, pairing energy MeV
-  R Ux, Ex;       // matching energy U_x = 150/A_d + 2.5 and E_x = U_x + delta
-  R T, E0;        // constant-temperature branch below E_x: rho = exp((U - E0)/T)/T
-  R lnT, lna4;    // ln T, (1/4) ln a
-};
-template <typename R> struct GaussNodes { R x[16], w[16]; };
-__constant__ GaussNodes<INC_REAL> c_gl;     // 16-point Gauss-Legendre on [-1, 1] (width integral of the GEM mode)
-
-template <typename R> struct ModelDev {
-  const R *tabS;          // [n_xs][4]  {sig_pp, dsig_pp, sig_np, dsig_np} in fm^2 (mb * 0.1)
-  const R *tabC;          // [n_xs][8]  {B_pp, dB_pp, B_np, dB_np, a_np, da_np, 0, 0}
-  const R *bind;          // [kAmax][kZmax] binding energy, MeV; < -1e29 => no such nucleus
-  const EvChan<R> *evch;  // [kAmax][kZmax][6]
-  const LdDev<R> *ld;     // [kAmax][kZmax]  (level_density = 1 only)
-  const NucDev<R> *nuc;   // [INC_MAX_TARGETS]
-  int32_t n_xs;
-  R inv_dp;               // 1 / (grid step in MeV/c)
-  R a_div;                // level density a = A_d / a_div
-};
-
-// One staged secondary.  f32: 32 bytes = one DRAM sector, so an event with n secondaries touches n sectors when it
-// is written (cascade escapes, evaporation emissions) and when the compaction kernel reads it back; the earlier
-// layout (five [chunk][64] arrays) touched 5-10 sectors per event and made the compaction the one HBM-bound kernel.
-template <typename R> struct __align__(16) StageRec {
-  R T, ux, uy, uz;
-  uint32_t code;          // path code | type << 24 ; evaporation: 1 << 31 | species << 24 | sequence number
-  uint32_t pad[3];
-};
-
-// One nucleus record per event: 32 bytes in the f32 build (one DRAM sector), 48 in f64.  Events finish, and are
-// evaporated, in an order unrelated to their index, so a record that is one sector costs one sector of traffic
-// where eight parallel arrays cost eight.  crec: post-cascade nucleus (the paper's "SoA of excited nuclei"),
-// meta = n_casc | attempt << 8 | failed << 16.  frec: final residual, meta = number of secondaries of the event; the
-// compaction kernel, which walks the events in index order, transposes it into the caller's arrays.
-template <typename R> struct __align__(16) NucRec {
-  R E, Px, Py, Pz;
-  int32_t A, Z;
-  uint32_t meta, status;
-};
-
-template <typename R> struct Workspace {   // per-chunk internal buffers (DEVICE)
-  StageRec<R> *st;        // [chunk][kMaxSec] staged secondaries, one record per secondary
-  NucRec<R> *crec;        // [chunk] post-cascade nuclei
-  NucRec<R> *frec;        // [chunk] final residuals
-  // Completion list: the cascade kernel appends the chunk-local index of every event whose post-cascade record is
-  // complete; the evaporation kernel, which may start while the cascade kernel's last CTAs are still draining
-  // (programmatic dependent launch), consumes the entries in order.  kNotDone = not written yet.
-  uint32_t *done_list;    // [chunk]
-};
-constexpr uint32_t kNotDone = 0xFFFFFFFFu;
-
-// release / acquire pair of the completion list (gpu scope)
-__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t *p) {
-  uint32_t v;
-  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-// Warp-collective: publishes the events of the lanes with `pub` set.  Every lane's earlier global writes (post-cascade
-// record; staged escapes, written by lanes of this warp in earlier passes and ordered by the __syncwarp()s since) are
-// made visible before the entry (fence + release store).
-__device__ __forceinline__ void publish_done(bool pub, int ev, unsigned long long *n_done, uint32_t *done_list, int lane) {
-  const unsigned mp = __ballot_sync(kFull, pub);
-  if (mp == 0u) return;
-  const int leader = __ffs(mp) - 1;
-  unsigned long long base = 0;
-  if (lane == leader) base = atomicAdd(n_done, (unsigned long long)__popc(mp));
-  base = __shfl_sync(kFull, base, leader);
-  __threadfence();
-  if (pub) *(volatile uint32_t *)(done_list + base + (unsigned long long)__popc(mp & ((1u << lane) - 1u))) = (uint32_t)ev;
-}
-
-template <typename R>
-__device__ __forceinline__ void stage_write(StageRec<R> *dst, R T, R ux, R uy, R uz, uint32_t code) {
-  StageRec<R> r;
-  r.T = T; r.ux = ux; r.uy = uy; r.uz = uz; r.code = code; r.pad[0] = 0u; r.pad[1] = 0u; r.pad[2] = 0u;
-  *dst = r;               // 16-byte vector stores
-}
-
-struct DevCounters {       // device scalars
-  unsigned long long next_event_casc, next_event_evap;
-  unsigned long long n_done;          // entries of the completion list handed out (cascade -> evaporation)
-  unsigned long long total_sec;
-  unsigned int error_word;   // bit0: E_in out of range, bit1: bad target id
-  unsigned int pad;
-  unsigned long long stats[24];
-  // drain timeline of the wavefront kernel (INC_F_TIMING), %globaltimer ns (low 40 bits): [0] max of ~start
-  // (= ~earliest start), [1] sum over warps of the time the event counter ran out for them, [2] sum of warp
-  // exit times, [3] latest warp exit, [4] number of warps, [5] max of ~exit (= ~earliest exit)
-  unsigned long long tl[6];
-};
-__device__ __forceinline__ unsigned long long global_ns() {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-  return t & 0xFFFFFFFFFFull;     // 40 bits (18 minutes): sums over a few thousand warps stay far below 2^64
-}
-
-enum StatIdx { S_EVENTS = 0, S_FAILED, S_ATTEMPTS, S_SEG, S_BND, S_REFL, S_ESC, S_COLL, S_BLOCKED,
-               S_ALLOWED, S_ABSORBED, S_EVSTEPS, S_EVTRIALS, S_EVEMIT, S_WI_SEG, S_WI_COLL, S_WI_EPI,
-               S_LS_SEG, S_LS_COLL, S_LS_EPI, S_NSTAT };
-
-template <bool ON> struct LaneStats {
-  unsigned long long c[ON ? S_NSTAT : 1];
-  __device__ __forceinline__ void clear() {
-    if (ON) {
-#pragma unroll
-      for (int i = 0; i < S_NSTAT; ++i) c[i] = 0;
-    }
-  }
-  __device__ __forceinline__ void add(int i, unsigned long long v = 1) { if (ON) c[i] += v; }
-  __device__ __forceinline__ void flush(DevCounters *ctr, int lane) {
-    if (ON) {
-#pragma unroll
-      for (int i = 0; i < S_NSTAT; ++i) {
-        unsigned long long v = c[i];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
-        if (lane == 0 && v) atomicAdd(&ctr->stats[i], v);
-      }
-    }
-  }
-};
-
-// ---- math wrappers: exact library calls for double, MUFU-based approximations for float ------
-template <typename R> struct M;
-template <> struct M<double> {
-  static __device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
-  static __device__ __forceinline__ double rsqrt_(double x) { return 1.0 / sqrt(x); }
-  static __device__ __forceinline__ double log_(double x) { return log(x); }
-  static __device__ __forceinline__ double exp_(double x) { return exp(x); }
-  static __device__ __forceinline__ double cbrt_(double x) { return cbrt(x); }
-  static __device__ __forceinline__ double log1p_(double x) { return log1p(x); }
-  static __device__ __forceinline__ double expm1_(double x) { return expm1(x); }
-  static __device__ __forceinline__ void sincos2pi(double u, double *s, double *c) {
-    sincos(6.283185307179586476925286766559 * u, s, c);
-  }
-  static __device__ __forceinline__ double div_(double a, double b) { return a / b; }
-  static __device__ __forceinline__ double rcp_(double a) { return 1.0 / a; }
-  static __device__ __forceinline__ double u01(uint32_t x) {   // R-R3 (fp64): (x + 1/2) 2^-32
-    return ((double)x + 0.5) * (1.0 / 4294967296.0);
-  }
-  // x >= 0 -> integer part k (clamped to kmax) and fraction
-  static __device__ __forceinline__ void split(double x, int kmax, int &k, double &f) {
-    int kk = (int)x;
-    kk = kk > kmax ? kmax : kk;
-    k = kk; f = x - (double)kk;
-  }
-  static constexpr int kSeriesTerms = 24;
-  static __device__ __forceinline__ double series_below() { return 1.0; }
-  // pinned arithmetic: never re-contracted by the compiler, so an inlined function gives the same bits at every
-  // call site.  fp64: product and sum rounded separately, like the oracle (-ffp-contract=off).
-  static __device__ __forceinline__ double mul_(double a, double b) { return __dmul_rn(a, b); }
-  static __device__ __forceinline__ double add_(double a, double b) { return __dadd_rn(a, b); }
-  static __device__ __forceinline__ double sub_(double a, double b) { return __dsub_rn(a, b); }
-  static __device__ __forceinline__ double fma_(double a, double b, double c) { return __dadd_rn(__dmul_rn(a, b), c); }
-};
-template <> struct M<float> {
-  static __device__ __forceinline__ float sqrt_(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-  static __device__ __forceinline__ float rsqrt_(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-  static __device__ __forceinline__ float lg2_(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-  static __device__ __forceinline__ float ex2_(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-  static __device__ __forceinline__ float log_(float x) { return __fmul_rn(0.6931471805599453f, lg2_(x)); }
-  static __device__ __forceinline__ float exp_(float x) { return ex2_(1.4426950408889634f * x); }
-  static __device__ __forceinline__ float cbrt_(float x) { return ex2_(__fmul_rn(0.3333333333f, lg2_(x))); }   // x in (0,1)
-  static __device__ __forceinline__ float log1p_(float x) { return log1pf(x); }
-  static __device__ __forceinline__ float expm1_(float x) { return expm1f(x); }
-  static __device__ __forceinline__ void sincos2pi(float u, float *s, float *c) {
-    // sin.approx / cos.approx scale their argument by 1/(2 pi) before MUFU: feed radians
-    float a = __fmul_rn(6.283185307179586f, u);
-    float ss, cc;
-    asm("sin.approx.ftz.f32 %0, %1;" : "=f"(ss) : "f"(a));
-    asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cc) : "f"(a));
-    *s = ss; *c = cc;
-  }
-  static __device__ __forceinline__ float rcp_(float a) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(a)); return y; }
-  static __device__ __forceinline__ float div_(float a, float b) { return __fmul_rn(a, rcp_(b)); }
-  static __device__ __forceinline__ float u01(uint32_t x) {
-    // R-R3 (fp32): ((x>>9) + 1/2) 2^-23, built from the mantissa bits (no int->float conversion)
-    return __uint_as_float(0x3F800000u | (x >> 9)) - 0.99999994f;
-  }
-  static __device__ __forceinline__ void split(float x, int kmax, int &k, float &f) {
-    // round-to-nearest of (x - 1/2) by the 2^23 trick: stays on the FMA/ALU pipes.  A knot that is
-    // mis-assigned by one ulp gives f just outside [0,1]; the interpolant is continuous there.
-    float y = (x - 0.49999997f) + 8388608.0f;
-    int kk = __float_as_int(y) - 0x4B000000;
-    kk = kk < 0 ? 0 : (kk > kmax ? kmax : kk);
-    k = kk; f = x - (y - 8388608.0f);
-    f = kk == kmax ? x - (float)kmax : f;
-  }
-  static constexpr int kSeriesTerms = 13;
-  // below this s the closed forms of G_1, G_3 are replaced by their series; at 0.25 the closed G_3 still has 3 of
-  // f32's 7 digits (it only weighs channels that are 6 keV from closing), and the 13-iteration series loop, which
-  // a single lane imposes on its whole warp, runs in 5 % instead of 84 % of the passes
-  static __device__ __forceinline__ float series_below() { return 0.25f; }
-  static __device__ __forceinline__ float mul_(float a, float b) { return __fmul_rn(a, b); }
-  static __device__ __forceinline__ float add_(float a, float b) { return __fadd_rn(a, b); }
-  static __device__ __forceinline__ float sub_(float a, float b) { return __fsub_rn(a, b); }
-  static __device__ __forceinline__ float fma_(float a, float b, float c) { return __fmaf_rn(a, b, c); }
-};
-
-// ---- R-R1: Philox4x32-10 ---------------------------------------------------------------------
-// The key is the call's seed for every block, so the ten round keys (key + r * Weyl constants) are the same for
-// the whole call: the host writes them to constant memory once per call and the rounds read them as constant-bank
-// operands, which takes the 20 key additions out of every block (4 % of the issue slots of a segment pass).
-struct RoundKeys { uint32_t k0[10], k1[10]; };
-__constant__ RoundKeys c_rk;
-
-__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3) {
-#pragma unroll
-  for (int r = 0; r < 10; ++r) {
-    const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;   // one IMAD.WIDE each
-    const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
-    const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
-    const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
-    c0 = hi1 ^ c1 ^ c_rk.k0[r];
-    c1 = lo1;
-    c2 = hi0 ^ c3 ^ c_rk.k1[r];
-    c3 = lo0;
-  }
-  return make_uint4(c0, c1, c2, c3);
-}
-
-struct RngKey {
-  uint32_t k0, k1;   // seed (the rounds use its expansion c_rk)
-  uint32_t e0, e1;   // global event index (counter words 2, 3)
-};
-
-// R-R2: block k of stream (attempt, path code pi)
-template <typename R>
-__device__ __forceinline__ void draw4(const RngKey &g, uint32_t attempt, uint32_t pi, uint32_t k, R u[4]) {
-  uint4 o = philox4x32_10(k, (attempt << 24) | pi, g.e0, g.e1);
-  u[0] = M<R>::u01(o.x); u[1] = M<R>::u01(o.y); u[2] = M<R>::u01(o.z); u[3] = M<R>::u01(o.w);
-}
-
-// ---- table lookup (R-N7): y_k + f (y_{k+1} - y_k), clamped to the grid -------------------------
-template <typename R>
-__device__ __forceinline__ void grid_pos(R plab_mev, R inv_dp, int n_xs, int &k, R &f) {
-  R x = M<R>::mul_(plab_mev, inv_dp);
-  const R xmax = R(n_xs - 1);
-  x = x > xmax ? xmax : x;
-  M<R>::split(x, n_xs - 2, k, f);
-}
-
-template <typename R> __device__ __forceinline__ R nucleon_mass(int type) { return type ? K<R>::mp : K<R>::mn; }
-template <typename R> __device__ __forceinline__ R nucleon_imass(int type) { return type ? K<R>::imp : K<R>::imn; }
-
-// Momentum of particle 1 (mass m1, total energy E1) in the rest frame of a partner with momentum q n
-// (mass m2, 1/m2 = im2); pn = p1 . n.  E_lab = (E1 E2 - p1.p2)/m2 is the invariant s expression
-// (s - m1^2 - m2^2)/(2 m2) of R-C2; p_lab = sqrt(T_lab (T_lab + 2 m1)), MeV/c.
-template <typename R>
-__device__ __forceinline__ R plab_of(R m1, R E1, R pn, R q, R m2, R im2) {
-  const R E2 = M<R>::sqrt_(q * q + m2 * m2);
-  const R Tlab = (E1 * E2 - q * pn) * im2 - m1;
-  R a = Tlab * (Tlab + R(2) * m1);
-  a = a > R(0) ? a : R(0);
-  return M<R>::sqrt_(a);
-}
-
-// ---- track state ---------------------------------------------------------------------------------
-template <typename R> struct Track {
-  R x, y, z;          // position, fm
-  R px, py, pz;       // momentum, MeV/c
-  R T;                // kinetic energy, MeV (kept consistent with |p|)
-  uint32_t pi;        // path code (R-R2)
-  uint32_t k;         // next Philox block of this track's stream
-  int nseg;           // segments done (R-C2 cap)
-  int type, shell;    // 1 = proton, 0 = neutron; shell index
-};
-
-template <typename R> struct CollCarry { R f, nx, ny, nz, Sp, Sig; };   // SEG -> COLL hand-over
-template <typename R> struct Escape { R T, ux, uy, uz; };
-
-enum SegOutcome : int { SEG_REFLECT = -1, SEG_CONT = 0, SEG_COLLIDE = 1, SEG_ESCAPE = 2, SEG_CAP = 3 };
-
-// ---------- C0: entry — uniform disc, beam along +z (R-Q15), potential step into the last shell ----------
-template <typename R>
-__device__ __forceinline__ void entry_step(Track<R> &t, const NucDev<R> &nu, R E_in, int ptype, const RngKey &g,
-                                           uint32_t attempt, R &p_in) {
-  R u[4];
-  draw4<R>(g, attempt, 1u, 0u, u);
-  const R b = nu.Rn * M<R>::sqrt_(u[0]);
-  R sb, cb;
-  M<R>::sincos2pi(u[1], &sb, &cb);
-  t.x = b * cb; t.y = b * sb;
-  const R zz = nu.Rn * nu.Rn - b * b;
-  t.z = -M<R>::sqrt_(zz > R(0) ? zz : R(0));
-  // the incident nucleon: proton (ptype 1, the paper's case P:9) or neutron (NEXT-3), with its own mass and potential
-  const R m0 = nucleon_mass<R>(ptype);
-  p_in = M<R>::sqrt_(E_in * (E_in + R(2) * m0));
-  // potential step (cannot reflect: V rises inward)
-  const R ux = t.x * nu.iRn, uy = t.y * nu.iRn, uz = t.z * nu.iRn;
-  const R pr = p_in * uz;
-  const R dV = ptype ? nu.sh[nu.ns - 1].V_p : nu.sh[nu.ns - 1].V_n;
-  const R Tj = E_in + dV;
-  const R prj2 = pr * pr + dV * (E_in + Tj + R(2) * m0);
-  const R prj = -M<R>::sqrt_(prj2 > R(0) ? prj2 : R(0));
-  const R dp = prj - pr;
-  t.px = dp * ux; t.py = dp * uy; t.pz = p_in + dp * uz;
-  t.T = Tj;
-  t.type = ptype; t.shell = nu.ns - 1; t.pi = 1u; t.k = 1u; t.nseg = 0;
-}
-
-// ---------- C2 + C4: one segment (R-Q8 partner first, then the path) ----------
-// Written in pinned arithmetic (M<R>::fma_/mul_/add_/sub_, never re-contracted): the wavefront kernel runs a
-// segment at two call sites (its own segment pass and the drain helpers' look-ahead), and both must give the
-// same bits in the f32 build too.  The f64 operation order is the oracle's.
-template <typename R> struct SegGeom { R dx, dy, dz, d_min; bool inward; };
-
-// R-C2 geometry: distances to the shell spheres along the flight direction
-template <typename R>
-__device__ __forceinline__ void seg_geometry(const Track<R> &t, const ShellDev<R> &sh, SegGeom<R> &gm) {
-  typedef M<R> m;
-  const R p1sq = m::fma_(t.pz, t.pz, m::fma_(t.py, t.py, m::mul_(t.px, t.px)));
-  const R ip = m::rsqrt_(p1sq);
-  gm.dx = m::mul_(t.px, ip); gm.dy = m::mul_(t.py, ip); gm.dz = m::mul_(t.pz, ip);
-  const R beta = m::fma_(t.z, gm.dz, m::fma_(t.y, gm.dy, m::mul_(t.x, gm.dx)));
-  const R r2 = m::fma_(t.z, t.z, m::fma_(t.y, t.y, m::mul_(t.x, t.x)));
-  const R bb = m::sub_(m::mul_(beta, beta), r2);
-  R disc_out = m::fma_(sh.r_out, sh.r_out, bb);
-  disc_out = disc_out > R(0) ? disc_out : R(0);
-  const R d_out = m::sub_(m::sqrt_(disc_out), beta);
-  R d_in = R(1e30);
-  if (t.shell > 0 && beta < R(0)) {
-    const R D = m::fma_(sh.r_in, sh.r_in, bb);
-    if (D > R(0)) d_in = m::sub_(-beta, m::sqrt_(D));
-  }
-  gm.inward = d_in < d_out;
-  gm.d_min = gm.inward ? d_in : d_out;
-}
-
-// R-C4 shell boundary, potential step (P:49 refraction / reflection).  Returns SEG_CONT (refracted into the
-// next shell), SEG_REFLECT (total reflection, shell unchanged) or SEG_ESCAPE (left the nucleus; esc filled).
-// Straight-line code: both outcomes are computed and selected (the lanes of a warp take both anyway), so that the
-// compiler can overlap this chain, which needs no random number, with the cross-section chain of seg_step.
-template <typename R>
-__device__ __forceinline__ int seg_boundary(Track<R> &t, const NucDev<R> &nu, const ShellDev<R> &sh, const SegGeom<R> &gm,
-                                            Escape<R> &esc) {
-  typedef M<R> m;
-  const int j = gm.inward ? t.shell - 1 : t.shell + 1;
-  const R irb = gm.inward ? sh.ir_in : sh.ir_out;
-  const R m1 = nucleon_mass<R>(t.type);
-  R x = m::fma_(gm.d_min, gm.dx, t.x), y = m::fma_(gm.d_min, gm.dy, t.y), z = m::fma_(gm.d_min, gm.dz, t.z);
-  // renormalise onto the sphere: one Newton step of 1/sqrt around |x|^2 = rb^2 (|x| is within rounding of rb)
-  const R rr = m::fma_(z, z, m::fma_(y, y, m::mul_(x, x)));
-  const R corr = m::sub_(R(1.5), m::mul_(m::mul_(m::mul_(R(0.5), rr), irb), irb));
-  x = m::mul_(x, corr); y = m::mul_(y, corr); z = m::mul_(z, corr);
-  t.x = x; t.y = y; t.z = z;
-  const R ux = m::mul_(x, irb), uy = m::mul_(y, irb), uz = m::mul_(z, irb);              // outward normal
-  const R pr = m::fma_(t.pz, uz, m::fma_(t.py, uy, m::mul_(t.px, ux)));
-  const R Vi = t.type ? sh.V_p : sh.V_n;
-  const R Vj = t.type ? nu.sh[j].V_p : nu.sh[j].V_n;
-  const R dV = m::sub_(Vj, Vi);
-  const R Tj = m::add_(t.T, dV);
-  const R prj2 = m::fma_(dV, m::add_(m::add_(t.T, Tj), m::mul_(R(2), m1)), m::mul_(pr, pr));   // p_j^2 - p_t^2
-  const bool refl = (Tj <= R(0) || prj2 <= R(0));
-  // specular reflection: p -= 2 p_r u; refraction: p_r -> sign(p_r) sqrt(p_rj^2)  (one is selected; a reflecting
-  // lane's square root is of a non-positive number and is not used)
-  const R sq = m::sqrt_(prj2);
-  const R dp = refl ? m::mul_(R(-2), pr) : m::sub_(pr >= R(0) ? sq : -sq, pr);
-  t.px = m::fma_(dp, ux, t.px); t.py = m::fma_(dp, uy, t.py); t.pz = m::fma_(dp, uz, t.pz);
-  t.T = refl ? t.T : Tj;
-  t.shell = refl ? t.shell : j;
-  // escape ("exiting particles"): direction of the refracted momentum
-  const R ipj = m::rsqrt_(m::mul_(Tj, m::fma_(R(2), m1, Tj)));
-  esc.T = Tj; esc.ux = m::mul_(t.px, ipj); esc.uy = m::mul_(t.py, ipj); esc.uz = m::mul_(t.pz, ipj);
-  return refl ? SEG_REFLECT : (j == nu.ns ? SEG_ESCAPE : SEG_CONT);
-}
-
-// momentum of the track in the rest frame of a partner with momentum q n (plab_of in pinned arithmetic)
-template <typename R>
-__device__ __forceinline__ R plab_pinned(R m1, R E1, R pn, R q, R m2, R im2) {
-  typedef M<R> m;
-  const R E2 = m::sqrt_(m::fma_(q, q, m::mul_(m2, m2)));
-  const R Tlab = m::fma_(m::fma_(E1, E2, -m::mul_(q, pn)), im2, -m1);
-  R a = m::mul_(Tlab, m::fma_(R(2), m1, Tlab));
-  a = a > R(0) ? a : R(0);
-  return m::sqrt_(a);
-}
-
-template <typename R, bool STATS>
-__device__ __forceinline__ int seg_step(Track<R> &t, const NucDev<R> &nu, const R *s_tabS, int n_xs, R inv_dp,
-                                        const RngKey &g, uint32_t attempt, CollCarry<R> &cc, Escape<R> &esc,
-                                        LaneStats<STATS> &st) {
-  typedef M<R> m;
-  // Straight-line code: the collision point and the boundary step are both computed and one is selected.  The
-  // geometry / boundary chain depends on the track only, the cross-section chain on the random numbers, so they
-  // overlap; with a branch between them the second could not start before the first had ended.
-  const bool cap = t.nseg >= kMaxSeg;                                // R-C2 cap: absorbed (the track is dead then)
-  t.nseg++;
-  if (!cap) st.add(S_SEG);
-  R u[4];
-  draw4<R>(g, attempt, t.pi, t.k++, u);
-  const ShellDev<R> &sh = nu.sh[t.shell];
-  const R m1 = nucleon_mass<R>(t.type);
-  const R E1 = m::add_(t.T, m1);
-  // partner direction and magnitude fraction ("quadratic distribution")
-  const R cth = m::fma_(R(2), u[1], R(-1));
-  R s2 = m::fma_(-cth, cth, R(1));
-  s2 = s2 > R(0) ? s2 : R(0);
-  const R sth = m::sqrt_(s2);
-  R sph, cph;
-  m::sincos2pi(u[2], &sph, &cph);
-  const R nx = m::mul_(sth, cph), ny = m::mul_(sth, sph), nz = cth;
-  const R f = m::cbrt_(u[0]);
-  const R pn = m::fma_(t.pz, nz, m::fma_(t.py, ny, m::mul_(t.px, nx)));
-  // cross sections against a proton and a neutron partner (same n, f: R-C2)
-  const R plab_p = plab_pinned<R>(m1, E1, pn, m::mul_(sh.pF_p, f), K<R>::mp, K<R>::imp);
-  const R plab_n = plab_pinned<R>(m1, E1, pn, m::mul_(sh.pF_n, f), K<R>::mn, K<R>::imn);
-  int kp, kn; R fp, fn;
-  grid_pos<R>(plab_p, inv_dp, n_xs, kp, fp);
-  grid_pos<R>(plab_n, inv_dp, n_xs, kn, fn);
-  // tabS row {sig_pp, d, sig_np, d}: vs a proton pp if the track is a proton else np; vs a neutron the opposite
-  const R *rp = s_tabS + 4 * kp + (t.type ? 0 : 2);
-  const R *rn = s_tabS + 4 * kn + (t.type ? 2 : 0);
-  const R Sp = m::mul_(sh.rho_p, m::fma_(fp, rp[1], rp[0]));
-  const R Sn = m::mul_(sh.rho_n, m::fma_(fn, rn[1], rn[0]));
-  const R Sig = m::add_(Sp, Sn);
-  const R nlu = -m::log_(u[3]);                  // d_coll = nlu / Sig
-  SegGeom<R> gm;
-  seg_geometry<R>(t, sh, gm);
-  // ---------- C4: shell boundary, potential step (on a copy) ----------
-  Track<R> tb = t;
-  const int rb = seg_boundary<R>(tb, nu, sh, gm, esc);
-  // ---------- collision point reached first (d_coll < d_min)?  Then hand over to the collision step ----------
-  const bool coll = nlu < m::mul_(Sig, gm.d_min);
-  const R d_coll = m::div_(nlu, Sig);
-  cc.f = f; cc.nx = nx; cc.ny = ny; cc.nz = nz; cc.Sp = Sp; cc.Sig = Sig;
-  t.x = coll ? m::fma_(d_coll, gm.dx, t.x) : tb.x;
-  t.y = coll ? m::fma_(d_coll, gm.dy, t.y) : tb.y;
-  t.z = coll ? m::fma_(d_coll, gm.dz, t.z) : tb.z;
-  t.px = coll ? t.px : tb.px; t.py = coll ? t.py : tb.py; t.pz = coll ? t.pz : tb.pz;
-  t.T = coll ? t.T : tb.T;
-  t.shell = coll ? t.shell : tb.shell;
-  if (STATS) {
-    if (cap) st.add(S_ABSORBED);
-    else if (!coll) { st.add(S_BND); if (rb == SEG_REFLECT) st.add(S_REFL); if (rb == SEG_ESCAPE) st.add(S_ESC); }
-  }
-  return cap ? SEG_CAP : (coll ? SEG_COLLIDE : (rb == SEG_ESCAPE ? SEG_ESCAPE : SEG_CONT));
-}
-
-// ---------- C3: collision.  Returns false if Pauli-blocked (track t continues, k advanced) ----------
-template <typename R, bool STATS>
-__device__ __forceinline__ bool coll_step(Track<R> &t, const CollCarry<R> &cc, const NucDev<R> &nu, const R *tabC,
-                                          int n_xs, R inv_dp, const RngKey &g, uint32_t attempt,
-                                          Track<R> &c2, bool &keep1, bool &keep2, uint32_t &status, LaneStats<STATS> &st) {
-  st.add(S_COLL);
-  const ShellDev<R> &sh = nu.sh[t.shell];
-  R u[4];
-  draw4<R>(g, attempt, t.pi, t.k++, u);
-  const int t2 = (u[0] * cc.Sig < cc.Sp) ? 1 : 0;
-  const R m1 = nucleon_mass<R>(t.type), m2 = nucleon_mass<R>(t2);
-  const R q = (t2 ? sh.pF_p : sh.pF_n) * cc.f;
-  const R p2x = q * cc.nx, p2y = q * cc.ny, p2z = q * cc.nz;
-  const R E1 = t.T + m1;
-  const R E2 = M<R>::sqrt_(q * q + m2 * m2);
-  const R pn = t.px * cc.nx + t.py * cc.ny + t.pz * cc.nz;
-  const R Tlab = (E1 * E2 - q * pn) * nucleon_imass<R>(t2) - m1;
-  R pl2 = Tlab * (Tlab + R(2) * m1);
-  const R plab = M<R>::sqrt_(pl2 > R(0) ? pl2 : R(0));
-  int kk; R ff;
-  grid_pos<R>(plab, inv_dp, n_xs, kk, ff);
-  const bool same = (t2 == t.type);
-  const R *row = tabC + 8 * kk;
-  const R B = same ? (__ldg(row + 0) + ff * __ldg(row + 1)) : (__ldg(row + 2) + ff * __ldg(row + 3));
-  const R ab = same ? R(0) : (__ldg(row + 4) + ff * __ldg(row + 5));
-  // boost to the CM frame
-  const R Px = t.px + p2x, Py = t.py + p2y, Pz = t.pz + p2z;
-  const R E = E1 + E2;
-  const R s = E * E - (Px * Px + Py * Py + Pz * Pz);
-  const R iE = M<R>::rcp_(E);
-  const R bx = Px * iE, by = Py * iE, bz = Pz * iE;
-  const R gam = E * M<R>::rsqrt_(s);
-  const R gfac = M<R>::div_(gam * gam, gam + R(1));      // (gamma - 1) / beta^2
-  const R pb = t.px * bx + t.py * by + t.pz * bz;
-  const R fb = gfac * pb - gam * E1;
-  const R qx = t.px + fb * bx, qy = t.py + fb * by, qz = t.pz + fb * bz;   // p1 in the CM frame
-  const R pcm2 = qx * qx + qy * qy + qz * qz;
-  const R ipcm = M<R>::rsqrt_(pcm2);
-  const R pcm = pcm2 * ipcm;
-  // scattering angle: dsigma/dt ~ exp(B t), t in (GeV/c)^2 (R-Q10)
-  const R pg2 = pcm2 * R(1e-6);
-  const R tmin = R(-4) * pg2;
-  R tt;
-  if (B * (-tmin) < R(1e-9)) tt = u[1] * tmin;
-  else tt = M<R>::div_(M<R>::log1p_(-u[1] * (-M<R>::expm1_(B * tmin))), B);
-  R ct = R(1) + M<R>::div_(tt, R(2) * pg2);
-  ct = ct < R(-1) ? R(-1) : (ct > R(1) ? R(1) : ct);
-  if (!same && u[2] * (R(1) + ab) < ab) ct = -ct;       // np backward term
-  const R st2 = R(1) - ct * ct;
-  const R stt = M<R>::sqrt_(st2 > R(0) ? st2 : R(0));
-  R sphi, cphi;
-  M<R>::sincos2pi(u[3], &sphi, &cphi);
-  // rotation frame around n = q/|q|
-  const R n0 = qx * ipcm, n1 = qy * ipcm, n2 = qz * ipcm;
-  const R q2 = n0 * n0 + n1 * n1;
-  R e1x, e1y, e1z, e2x, e2y;
-  if (q2 > R(1e-24)) {
-    const R iq = M<R>::rsqrt_(q2);
-    e1x = n0 * n2 * iq; e1y = n1 * n2 * iq; e1z = -q2 * iq;
-    e2x = -n1 * iq; e2y = n0 * iq;
-  } else {
-    e1x = R(1); e1y = R(0); e1z = R(0);
-    e2x = R(0); e2y = n2 >= R(0) ? R(1) : R(-1);
-  }
-  const R a1 = stt * cphi, a2 = stt * sphi;
-  const R w1x = pcm * (a1 * e1x + a2 * e2x + ct * n0);
-  const R w1y = pcm * (a1 * e1y + a2 * e2y + ct * n1);
-  const R w1z = pcm * (a1 * e1z + ct * n2);
-  // boost back; partner by momentum conservation
-  const R E1cm = M<R>::sqrt_(pcm2 + m1 * m1);
-  const R wb = w1x * bx + w1y * by + w1z * bz;
-  const R fo = gfac * wb + gam * E1cm;
-  const R o1x = w1x + fo * bx, o1y = w1y + fo * by, o1z = w1z + fo * bz;
-  const R o2x = Px - o1x, o2y = Py - o1y, o2z = Pz - o1z;
-  const R o1sq = o1x * o1x + o1y * o1y + o1z * o1z;
-  const R o2sq = o2x * o2x + o2y * o2y + o2z * o2z;
-  // Pauli blocking: both products above their Fermi energies (strict, R-Q12)
-  const R pF2_1 = t.type ? sh.pF2_p : sh.pF2_n;
-  const R pF2_2 = t2 ? sh.pF2_p : sh.pF2_n;
-  if (!(o1sq > pF2_1 && o2sq > pF2_2)) {
-    st.add(S_BLOCKED);
-    return false;                                     // projectile continues unchanged (R-Q13)
-  }
-  st.add(S_ALLOWED);
-  keep1 = false; keep2 = false;
-  if (2u * t.pi + 1u >= (1u << 24)) {                 // depth cap (R-C3)
-    status |= INC_ST_DEPTH_CAP;
-    st.add(S_ABSORBED, 2);
-  } else {
-    // cutoff: E_F + E_B (n), E_F + E_B + E_C (p)
-    keep1 = o1sq > (t.type ? sh.pc2_p : sh.pc2_n);
-    keep2 = o2sq > (t2 ? sh.pc2_p : sh.pc2_n);
-    st.add(S_ABSORBED, (keep1 ? 0 : 1) + (keep2 ? 0 : 1));
-  }
-  // children: scattered projectile keeps the lane's track slot (pi' = 2 pi), recoil is c2 (pi' = 2 pi + 1)
-  c2.x = t.x; c2.y = t.y; c2.z = t.z; c2.px = o2x; c2.py = o2y; c2.pz = o2z;
-  c2.T = M<R>::div_(o2sq, M<R>::sqrt_(o2sq + m2 * m2) + m2);
-  c2.pi = 2u * t.pi + 1u; c2.k = 0u; c2.nseg = 0; c2.type = t2; c2.shell = t.shell;
-  t.px = o1x; t.py = o1y; t.pz = o1z;
-  t.T = M<R>::div_(o1sq, M<R>::sqrt_(o1sq + m1 * m1) + m1);
-  t.pi = 2u * t.pi; t.k = 0u; t.nseg = 0;
-  return true;
-}
-
-// ---------- C6: epilogue ("excitation energy ... through energy conservation") ----------
-// Eavail = E_in - sum T_k, (Prx,Pry,Prz) = p_in - sum p_k.  Returns true if the attempt is accepted.
-template <typename R>
-__device__ __forceinline__ bool epilogue_eval(const NucDev<R> &nu, const R *bind, int ptype, int n_esc, int n_p, int n_real,
-                                              R Eavail, R Prx, R Pry, R Prz, bool keep_transparent,
-                                              int &A_res, int &Z_res, R &Estar) {
-  A_res = nu.A + 1 - n_esc; Z_res = nu.Z + ptype - n_p;   // (the nucleon masses cancel for either projectile)
-  Estar = R(0);
-  if (!((n_real > 0) || keep_transparent)) return false;       // transparent: not a non-elastic event
-  R Bres = R(-1e30);
-  if (A_res >= 1 && A_res < kAmax && Z_res >= 0 && Z_res < kZmax) Bres = __ldg(bind + A_res * kZmax + Z_res);
-  if (Bres < R(-1e29)) return false;                            // no such nucleus
-  // E_res - M_res = X with the nucleon masses cancelled analytically; E* = M* - M_res in rationalised form
-  const R X = Eavail + Bres - nu.Bt;
-  const R Mres = R(Z_res) * K<R>::mp + R(A_res - Z_res) * K<R>::mn - Bres;
-  const R P2 = Prx * Prx + Pry * Pry + Prz * Prz;
-  const R Er = Mres + X;
-  const R M2 = Er * Er - P2;
-  const R Mstar = M2 > R(0) ? M<R>::sqrt_(M2) : R(0);
-  Estar = (R(2) * Mres * X + X * X - P2) / (Mstar + Mres);
-  if (Estar < R(0) && !(keep_transparent && n_real == 0)) return false;
-  return true;
-}
-
-// ---- kernel parameters ------------------------------------------------------------------------------
-template <typename R> struct CascadeParams {
-  ModelDev<R> model;
-  Workspace<R> ws;
-  DevCounters *ctr;
-  const R *E_in;            // chunk base
-  const int32_t *target_id; // chunk base
-  const uint8_t *projectile; // chunk base; 0 = neutron, 1 = proton; nullptr = all protons
-  long long e_base;         // global index of the chunk's first event
-  int n_chunk;
-  uint32_t seed_lo, seed_hi;
-  uint32_t flags;
-  int vote_coll, vote_epi;  // lane kernel: phase-vote thresholds
-  int long_seg;             // wavefront kernel: tracks with this many segments behind them may go to a drain helper
-  int seg_per_pass;         // wavefront kernel: segment steps per segment pass (1..8)
-  int n_stage;              // nuclei slots staged into shared memory (target_id must be < n_stage)
-  uint32_t *wtrace;         // INC_F_TIMING: kWTrace words per warp of the wavefront kernel (inc_get_warp_trace), or nullptr
-};
-constexpr int kWTrace = 8;  // [0] ns (low 32 bits) when the event counter ran out for the warp, [1] ns at exit of its own work,
-                            // [2] passes of the drain phase, [3] segment passes among them, [4] lanes summed over those,
-                            // [5] highest attempt number started in the drain, [6] tracks handed to helpers, [7] ns at kernel entry
-
-// shared-memory staging of the model: [NucDev x n_stage] [tabS n_xs*4]   (n_stage = highest live slot + 1)
-template <typename R> __host__ __device__ inline size_t model_smem_bytes(int n_xs, int n_stage) {
-  return sizeof(NucDev<R>) * (size_t)n_stage + sizeof(R) * 4 * (size_t)n_xs;
-}
-
-template <typename R>
-__device__ __forceinline__ void stage_model(const ModelDev<R> &model, int n_stage, NucDev<R> *s_nuc, R *s_tabS) {
-  const int nw = (int)(sizeof(NucDev<R>) / 4);
-  for (int t = 0; t < n_stage; ++t) {
-    if (!model.nuc[t].live) { if (threadIdx.x == 0) s_nuc[t].live = 0; continue; }
-    const uint32_t *src = reinterpret_cast<const uint32_t *>(&model.nuc[t]);
-    uint32_t *dst = reinterpret_cast<uint32_t *>(&s_nuc[t]);
-    for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
-  }
-  const int nt = model.n_xs * 4;
-  for (int i = threadIdx.x; i < nt; i += blockDim.x) s_tabS[i] = model.tabS[i];
-  __syncthreads();
-}
-
-// validate an event's inputs; on failure write neutral outputs and raise the device error word
-template <typename R>
-__device__ __forceinline__ bool check_inputs(const CascadeParams<R> &P, const NucDev<R> *s_nuc, int ev, R E_in, int tgt, int ptype) {
-  unsigned err = 0;
-  if (ptype != 0 && ptype != 1) err |= 8u;
-  if (!(E_in >= R(INC_E_MIN) && E_in <= R(INC_E_MAX))) err |= 1u;
-  if (tgt < 0 || tgt >= P.n_stage) err |= 2u;
-  else if (!s_nuc[tgt].live) err |= 2u;
-  if (!err) return true;
-  atomicOr(&P.ctr->error_word, err);
-  NucRec<R> r;
-  r.E = R(0); r.Px = R(0); r.Py = R(0); r.Pz = R(0); r.A = 0; r.Z = 0; r.meta = (1u << 16); r.status = INC_ST_FAILED;
-  P.ws.crec[ev] = r;
-  return false;
-}
-
-template <typename R>
-__device__ __forceinline__ void write_cascade_result(const Workspace<R> &ws, int ev, int A, int Z, R Es, R Px, R Py, R Pz,
-                                                     uint32_t meta, uint32_t status) {
-  NucRec<R> r;
-  r.E = Es; r.Px = Px; r.Py = Py; r.Pz = Pz; r.A = A; r.Z = Z; r.meta = meta; r.status = status;
-  ws.crec[ev] = r;          // 16-byte vector stores
-}
-
-// Order-independent sums (escaped energy and momentum): fixed point, so that any processing order of
-// an event's tracks gives bit-identical residuals.  double: int64, unit 2^-40 MeV; float: int32, unit
-// 2^-20 MeV (|values| < 2048 MeV, resolution below the fp32 rounding of the addends).
-template <typename R> struct Fx;
-template <> struct Fx<double> {
-  typedef long long T; typedef unsigned long long U;
-  static __device__ __forceinline__ T to(double v) { return __double2ll_rn(v * 1099511627776.0); }
-  static __device__ __forceinline__ double from(T v) { return (double)v * (1.0 / 1099511627776.0); }
-};
-template <> struct Fx<float> {
-  typedef int T; typedef unsigned int U;
-  static __device__ __forceinline__ T to(float v) { return __float2int_rn(v * 1048576.0f); }
-  static __device__ __forceinline__ float from(T v) { return (float)v * (1.0f / 1048576.0f); }
-};
-
-// =================================================================================================
-// Cascade kernel A: lane-per-event state machine with warp-voted phases
-// =================================================================================================
-enum LaneState : int { ST_SEG = 0, ST_COLL = 1, ST_EPI = 2, ST_DONE = 3 };
-
-template <typename R> struct TrackRec {   // pending track (local-memory stack)
-  R x, y, z, px, py, pz, T;
-  uint32_t pi;
-  uint32_t meta;   // type | shell << 1
-};
-
-template <typename R, bool STATS>
-__global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParams<R> P) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  NucDev<R> *s_nuc = reinterpret_cast<NucDev<R> *>(smem_raw);
-  R *s_tabS = reinterpret_cast<R *>(smem_raw + sizeof(NucDev<R>) * P.n_stage);
-  stage_model<R>(P.model, P.n_stage, s_nuc, s_tabS);
-  // programmatic dependent launch: the evaporation kernel may be scheduled as soon as every CTA of this grid is
-  // resident; it takes its events from the completion list, never from stream order
-  asm volatile("griddepcontrol.launch_dependents;");
-
-  const int lane = threadIdx.x & 31;
-  const int n_xs = P.model.n_xs;
-  const R inv_dp = P.model.inv_dp;
-  const bool keep_transparent = (P.flags & INC_F_KEEP_TRANSPARENT) != 0;
-  const bool same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
-
-  int state = ST_EPI;
-  int ev = -1, tgt = 0, ptype = 1;
-  uint32_t attempt = 0;
-  R E_in = R(0);
-  RngKey g;
-  g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = 0; g.e1 = 0;
-  Track<R> t;
-  t.x = t.y = t.z = t.px = t.py = t.pz = t.T = R(0); t.pi = 0; t.k = 0; t.nseg = 0; t.type = 0; t.shell = 0;
-  typename Fx<R>::T fxE = 0, fxX = 0, fxY = 0, fxZ = 0;   // fixed-point E_in - sum T, p_in - sum p
-  int n_esc = 0, n_p = 0, n_real = 0;
-  uint32_t st_try = 0;
-  TrackRec<R> stack[kStackCap];
-  int sp = 0;
-  CollCarry<R> cc;
-  cc.f = cc.nx = cc.ny = cc.nz = cc.Sp = cc.Sig = R(0);
-  LaneStats<STATS> st;
-  st.clear();
-
-  auto pop_or_finish = [&]() {
-    if (sp > 0) {
-      const TrackRec<R> &r = stack[--sp];
-      t.x = r.x; t.y = r.y; t.z = r.z; t.px = r.px; t.py = r.py; t.pz = r.pz; t.T = r.T;
-      t.pi = r.pi; t.type = r.meta & 1; t.shell = (int)(r.meta >> 1);
-      t.k = 0; t.nseg = 0;
-      state = ST_SEG;
-    } else {
-      state = ST_EPI;
-    }
-  };
-
-  for (;;) {
-    __syncwarp();
-    const unsigned mS = __ballot_sync(kFull, state == ST_SEG);
-    const unsigned mC = __ballot_sync(kFull, state == ST_COLL);
-    const unsigned mE = __ballot_sync(kFull, state == ST_EPI);
-    const int nS = __popc(mS), nC = __popc(mC), nE = __popc(mE);
-    if ((nS | nC | nE) == 0) break;
-    int phase;
-    if (nC >= P.vote_coll || (nS == 0 && nC > 0 && nC >= nE)) phase = ST_COLL;
-    else if (nE >= P.vote_epi || (nS == 0 && nE > 0)) phase = ST_EPI;
-    else phase = ST_SEG;
-
-    if (phase == ST_SEG) {
-      if (lane == 0) { st.add(S_WI_SEG); st.add(S_LS_SEG, nS); }
-      if (state == ST_SEG) {
-        Escape<R> esc;
-        const int out = seg_step<R, STATS>(t, s_nuc[tgt], s_tabS, n_xs, inv_dp, g, attempt, cc, esc, st);
-        if (out == SEG_COLLIDE) state = ST_COLL;
-        else if (out == SEG_ESCAPE) {
-          if (n_esc < kMaxSec) {
-            const size_t o = (size_t)ev * kMaxSec + n_esc;
-            stage_write<R>(P.ws.st + o, esc.T, esc.ux, esc.uy, esc.uz, t.pi | ((uint32_t)t.type << 24));
-            n_esc++; n_p += t.type;
-            fxE -= Fx<R>::to(esc.T); fxX -= Fx<R>::to(t.px); fxY -= Fx<R>::to(t.py); fxZ -= Fx<R>::to(t.pz);
-          } else {
-            st_try |= INC_ST_SEC_TRUNC;
-          }
-          pop_or_finish();
-        } else if (out == SEG_CAP) {
-          st_try |= INC_ST_SEG_CAP;
-          pop_or_finish();
-        }
-      }
-    } else if (phase == ST_COLL) {
-      if (lane == 0) { st.add(S_WI_COLL); st.add(S_LS_COLL, nC); }
-      if (state == ST_COLL) {
-        Track<R> c2;
-        bool keep1 = false, keep2 = false;
-        const bool allowed = coll_step<R, STATS>(t, cc, s_nuc[tgt], P.model.tabC, n_xs, inv_dp, g, attempt, c2, keep1, keep2, st_try, st);
-        if (!allowed) state = ST_SEG;
-        else {
-          n_real++;
-          if (keep1 && keep2) {
-            if (sp < kStackCap) {
-              TrackRec<R> &r = stack[sp++];
-              r.x = c2.x; r.y = c2.y; r.z = c2.z; r.px = c2.px; r.py = c2.py; r.pz = c2.pz; r.T = c2.T;
-              r.pi = c2.pi; r.meta = (uint32_t)c2.type | ((uint32_t)c2.shell << 1);
-            } else {
-              st_try |= INC_ST_QUEUE_OVF;
-            }
-            state = ST_SEG;
-          } else if (keep1) state = ST_SEG;
-          else if (keep2) { t = c2; state = ST_SEG; }
-          else pop_or_finish();
-        }
-      }
-    } else {  // EPI phase: epilogue of the finished attempt, then entry of the next attempt / event
-      if (lane == 0) { st.add(S_WI_EPI); st.add(S_LS_EPI, nE); }
-      bool want_event = false;
-      bool done_now = false;
-      int ev_done = ev;
-      if (state == ST_EPI) {
-        if (ev >= 0) {
-          const NucDev<R> &nu = s_nuc[tgt];
-          int A_res, Z_res;
-          R Estar;
-          const R Eavail = Fx<R>::from(fxE), Prx = Fx<R>::from(fxX), Pry = Fx<R>::from(fxY), Prz = Fx<R>::from(fxZ);
-          const bool ok = epilogue_eval<R>(nu, P.model.bind, ptype, n_esc, n_p, n_real, Eavail, Prx, Pry, Prz, keep_transparent, A_res, Z_res, Estar);
-          if (ok) {
-            const uint32_t used = attempt + 1u > 255u ? 255u : attempt + 1u;
-            write_cascade_result<R>(P.ws, ev, A_res, Z_res, Estar, Prx, Pry, Prz, (uint32_t)n_esc | (attempt << 8), st_try | used);
-            ev = -1;
-            done_now = true;
-          } else {
-            attempt++;
-            if (attempt >= (uint32_t)kMaxAttempt) {          // FAILED: count 0, target at rest
-              write_cascade_result<R>(P.ws, ev, nu.A, nu.Z, R(0), R(0), R(0), R(0), (1u << 16), INC_ST_FAILED | 0xFFu);
-              st.add(S_FAILED);
-              ev = -1;
-              done_now = true;
-            }
-          }
-        }
-        want_event = (ev < 0);
-      }
-      publish_done(done_now, ev_done, &P.ctr->n_done, P.ws.done_list, lane);
-      const unsigned need = __ballot_sync(kFull, want_event);
-      if (need) {
-        bool rejected = false;
-        int ev_rej = 0;
-        const int leader = __ffs(need) - 1;
-        unsigned long long base = 0;
-        if (lane == leader) base = atomicAdd(&P.ctr->next_event_casc, (unsigned long long)__popc(need));
-        base = __shfl_sync(kFull, base, leader);
-        if (want_event) {
-          const unsigned long long mine = base + (unsigned long long)__popc(need & ((1u << lane) - 1u));
-          if (mine < (unsigned long long)P.n_chunk) {
-            ev = (int)mine;
-            attempt = 0;
-            E_in = P.E_in[ev];
-            tgt = P.target_id[ev];
-            ptype = P.projectile ? (int)P.projectile[ev] : 1;
-            if (!check_inputs<R>(P, s_nuc, ev, E_in, tgt, ptype)) { rejected = true; ev_rej = ev; ev = -1; tgt = 0; }
-            else {
-              const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
-              g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
-              st.add(S_EVENTS);
-            }
-          } else {
-            state = ST_DONE;
-          }
-        }
-        publish_done(rejected, ev_rej, &P.ctr->n_done, P.ws.done_list, lane);   // (neutral outputs are complete results too)
-      }
-      if (state == ST_EPI && ev >= 0) {
-        st.add(S_ATTEMPTS);
-        R p_in;
-        entry_step<R>(t, s_nuc[tgt], E_in, ptype, g, attempt, p_in);
-        fxE = Fx<R>::to(E_in); fxX = 0; fxY = 0; fxZ = Fx<R>::to(p_in);
-        n_esc = 0; n_p = 0; n_real = 0; st_try = 0; sp = 0;
-        state = ST_SEG;
-      }
-    }
-  }
-  st.flush(P.ctr, lane);
-}
-
-// =================================================================================================
-// Cascade kernel B (default): per-warp wavefront with shared-memory queues
-// =================================================================================================
-
-// ---- drain helpers ---------------------------------------------------------------------------------
-// A track that orbits in the outer shells (nearly tangential, reflected at every surface hit, short chords,
-// hardly any collision) runs up to kMaxSeg = 1024 segments, one per pass of its warp; the last such tracks of a
-// launch kept single lanes busy for ~0.5 ms while the rest of the GPU idled.  Between collisions the path is
-// deterministic, so a warp that has finished its own events (a "helper") takes such a track over: every lane
-// walks the collision-free path (seg_geometry + seg_boundary only) and lane j keeps the state at the start of
-// segment j; then the 32 lanes run seg_step on their segments in parallel.  If all 32 simply continue, the track
-// has advanced 32 segments in one pass; otherwise the state at the start of the first segment that does not
-// continue (collision, escape, cap) goes back to the owner, which runs that segment in the ordinary way.  The
-// owner's bookkeeping is never touched by a helper.  seg_step is written in pinned arithmetic, so the helper's
-// path is bit-identical to the owner's: results do not depend on whether, or when, a track was helped.
-constexpr int kCtaLongQ = 32;      // hand-over queue owners -> helpers (per CTA)
-constexpr int kRetQ = 8;           // returns helpers -> owner (per warp) = max tracks an owner has out at a time
-constexpr int kLongSegDefault = 48;
-
-template <typename R> struct CtaLong {
-  int credits;              // free entries of q (producers reserve with atomicSub, consumers give back)
-  int avail;                // published, not yet taken entries
-  uint32_t tail, head;      // producer / consumer tickets
-  uint32_t n_helpers;       // warps that have finished their own events
-  uint32_t lock;            // consumers take entries one at a time, in ticket order: the ring frees in order, so a
-                            // producer that holds a credit always finds the entry of its ticket free
-  int idle;                 // helpers waiting for an entry: owners hand a track over only to a helper that is free
-  uint32_t pad;
-  uint32_t valid[kCtaLongQ];
-  R q[7][kCtaLongQ];        // x y z px py pz T
-  uint32_t qi[5][kCtaLongQ];   // pi, k | nseg << 16, meta (type | shell << 1 | slot << 8), event, attempt | tgt << 8 | owner << 16
-};
-
-template <typename R, int NS, int QS, int QC> struct WarpMem {
-  // event slots (32 B each in the f32 build)
-  int32_t ev[NS];
-  uint32_t info[NS];        // n_esc | n_p << 8 | attempt << 16 | tgt << 24 (7 bits) | projectile type << 31
-  uint32_t cnt[NS];         // pending tracks of the attempt (low 16) | real collisions (high 16)
-  uint32_t status[NS];
-  typename Fx<R>::T acc[4][NS];   // fixed-point E_in - sum T, p_in - sum p (x, y, z)
-  // segment queue (structure of arrays: lane-consecutive addresses)
-  R qx[QS], qy[QS], qz[QS], qpx[QS], qpy[QS], qpz[QS], qT[QS];
-  uint32_t qpi[QS], qkn[QS], qmeta[QS];   // qkn = k | nseg << 16 ; qmeta = type | shell << 1 | slot << 8
-  // collision queue
-  R cx[QC], cy[QC], cz[QC], cpx[QC], cpy[QC], cpz[QC], cT[QC];
-  uint32_t cpi[QC], ckn[QC], cmeta[QC];
-  R cf[QC], cnx[QC], cny[QC], cnz[QC], cSp[QC], cSig[QC];
-  // slot lists
-  uint8_t epi_q[NS], free_q[NS];
-  // finished events waiting to be published in the completion list (a batch costs one fence and one global atomic)
-  uint32_t pub_q[96];
-  // tracks coming back from the drain helpers
-  uint32_t r_tail;
-  uint32_t r_valid[kRetQ];
-  R rq[7][kRetQ];
-  uint32_t rqi[3][kRetQ];
-};
-
-// Defaults per build; -DINC_WNS= -DINC_WQS= -DINC_WQC= -DINC_WWARPS= (all four) override them for the build's real type:
-// tuning experiments and the small-queue test build, which exercises the capacity guards.  Needs QS >= 64, QC >= 33.
-#ifdef INC_WNS
-static_assert(INC_WQS >= 64 && INC_WQC >= 33 && INC_WNS <= 128 && INC_WNS >= 32, "wavefront queue sizes");
-template <typename R> struct WaveCfg { static constexpr int NS = INC_WNS, QS = INC_WQS, QC = INC_WQC, WARPS = INC_WWARPS; };
-#else
-template <typename R> struct WaveCfg;
-template <> struct WaveCfg<float> { static constexpr int NS = 80, QS = 128, QC = 64, WARPS = 16; };
-template <> struct WaveCfg<double> { static constexpr int NS = 64, QS = 128, QC = 64, WARPS = 8; };
-#endif
-
-template <typename R> __host__ __device__ inline size_t wave_smem_bytes(int n_xs, int n_stage) {
-  typedef WaveCfg<R> C;
-  return model_smem_bytes<R>(n_xs, n_stage) + 32 + sizeof(CtaLong<R>) + sizeof(WarpMem<R, C::NS, C::QS, C::QC>) * C::WARPS;
-}
-
-// One warp, done with its own events, serves the CTA's hand-over queue until every warp of the CTA is done.
-template <typename R, typename WM>
-__device__ __forceinline__ void help_long_tracks(const CascadeParams<R> &P, const NucDev<R> *s_nuc, const R *s_tabS, WM *wm,
-                                              CtaLong<R> &cq, int n_warps) {
-  const int lane = threadIdx.x & 31;
-  const bool same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
-  LaneStats<false> st;      // the STATS build never hands tracks over (its counters would see the speculative lanes)
-  bool idle = false;
-  for (;;) {
-    // ---- take an entry (under the CTA's consumer lock) ----
-    int h = -1;
-    if (lane == 0) {
-      if (atomicSub(&cq.avail, 1) > 0) {
-        while (atomicCAS(&cq.lock, 0u, 1u) != 0u) { }
-        h = (int)(*(volatile uint32_t *)&cq.head & (kCtaLongQ - 1));
-        while (((volatile uint32_t *)cq.valid)[h] == 0u) { }      // its producer is just publishing it
-      } else {
-        atomicAdd(&cq.avail, 1);
-      }
-    }
-    h = __shfl_sync(kFull, h, 0);
-    if (h < 0) {
-      if (*(volatile uint32_t *)&cq.n_helpers == (uint32_t)n_warps) break;     // nobody has a track out any more
-      if (!idle) { idle = true; if (lane == 0) atomicAdd(&cq.idle, 1); }
-      __nanosleep(64);
-      continue;
-    }
-    if (idle) { idle = false; if (lane == 0) atomicSub(&cq.idle, 1); }
-    __threadfence_block();
-    Track<R> cur;
-    cur.x = cq.q[0][h]; cur.y = cq.q[1][h]; cur.z = cq.q[2][h]; cur.px = cq.q[3][h]; cur.py = cq.q[4][h]; cur.pz = cq.q[5][h];
-    cur.T = cq.q[6][h]; cur.pi = cq.qi[0][h];
-    const uint32_t kn = cq.qi[1][h], mt = cq.qi[2][h], ev = cq.qi[3][h], ao = cq.qi[4][h];
-    cur.k = kn & 0xFFFFu; cur.nseg = (int)(kn >> 16);
-    cur.type = mt & 1u; cur.shell = (int)((mt >> 1) & 0x7Fu);
-    __syncwarp();
-    if (lane == 0) {
-      ((volatile uint32_t *)cq.valid)[h] = 0u;
-      *(volatile uint32_t *)&cq.head = *(volatile uint32_t *)&cq.head + 1u;
-      __threadfence_block();
-      atomicAdd(&cq.credits, 1);
-      atomicExch(&cq.lock, 0u);
-    }
-    const uint32_t attempt = ao & 0xFFu;
-    const NucDev<R> &nu = s_nuc[(ao >> 8) & 0xFFu];
-    RngKey g;
-    const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + (long long)ev);
-    g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
-    // ---- advance it up to 32 segments per pass while every segment just continues (8 in the first pass: a
-    // track that has only just become long often collides within a few segments) ----
-    int depth = 8;
-    for (;;) {
-      Track<R> mine = cur;
-      int n_look = depth;
-#pragma unroll 1
-      for (int j = 0; j < depth; ++j) {
-        if (j == lane) mine = cur;
-        if (cur.nseg >= kMaxSeg) { n_look = j + 1; break; }       // segment j ends at the cap
-        cur.nseg++; cur.k++;
-        const ShellDev<R> &sh = nu.sh[cur.shell];
-        SegGeom<R> gm;
-        Escape<R> e;
-        seg_geometry<R>(cur, sh, gm);
-        if (seg_boundary<R>(cur, nu, sh, gm, e) == SEG_ESCAPE) { n_look = j + 1; break; }   // segment j ends outside
-      }
-      int out = -1;
-      if (lane < n_look) {
-        Track<R> post = mine;
-        CollCarry<R> cc;
-        Escape<R> esc;
-        out = seg_step<R, false>(post, nu, s_tabS, P.model.n_xs, P.model.inv_dp, g, attempt, cc, esc, st);
-      }
-      const unsigned ended = __ballot_sync(kFull, out > SEG_CONT);
-      if (ended == 0u && n_look == depth) { depth = 32; continue; }     // cur = the state after `depth` continuing segments
-      // the start of the first segment that does not continue goes back to the owner (were the walk and seg_step
-      // ever to disagree about an escape or the cap, the start of the last walked segment does)
-      const int f = ended ? __ffs(ended) - 1 : n_look - 1;
-      if (lane == f) {
-        WM &o = wm[ao >> 16];
-        const int i = (int)(atomicAdd(&o.r_tail, 1u) & (kRetQ - 1));
-        o.rq[0][i] = mine.x; o.rq[1][i] = mine.y; o.rq[2][i] = mine.z; o.rq[3][i] = mine.px; o.rq[4][i] = mine.py; o.rq[5][i] = mine.pz;
-        o.rq[6][i] = mine.T; o.rqi[0][i] = mine.pi; o.rqi[1][i] = mine.k | ((uint32_t)mine.nseg << 16);
-        o.rqi[2][i] = (uint32_t)mine.type | ((uint32_t)mine.shell << 1) | (mt & 0xFFFFFF00u);
-        __threadfence_block();
-        ((volatile uint32_t *)o.r_valid)[i] = 1u;
-      }
-      break;
-    }
-  }
-}
-
-template <typename R, bool STATS>
-__global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_kernel(const CascadeParams<R> P) {
-  typedef WaveCfg<R> C;
-  typedef WarpMem<R, C::NS, C::QS, C::QC> WM;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  NucDev<R> *s_nuc = reinterpret_cast<NucDev<R> *>(smem_raw);
-  R *s_tabS = reinterpret_cast<R *>(smem_raw + sizeof(NucDev<R>) * P.n_stage);
-  const size_t off = (model_smem_bytes<R>(P.model.n_xs, P.n_stage) + 15) & ~(size_t)15;
-  CtaLong<R> &cq = *reinterpret_cast<CtaLong<R> *>(smem_raw + off);
-  WM *wm = reinterpret_cast<WM *>(smem_raw + off + ((sizeof(CtaLong<R>) + 15) & ~(size_t)15));
-  WM &w = wm[threadIdx.x >> 5];
-  const int lane = threadIdx.x & 31;
-  if (lane < kRetQ) w.r_valid[lane] = 0u;
-  if (lane == 0) w.r_tail = 0u;
-  if (threadIdx.x < kCtaLongQ) cq.valid[threadIdx.x] = 0u;
-  if ((P.flags & INC_F_TEST_QUEUE_OVF) && blockIdx.x == 0 && threadIdx.x == 0) atomicOr(&P.ctr->error_word, 4u);
-  if (threadIdx.x == 0) { cq.credits = kCtaLongQ; cq.avail = 0; cq.tail = 0u; cq.head = 0u; cq.n_helpers = 0u; cq.lock = 0u; cq.idle = 0; }
-  stage_model<R>(P.model, P.n_stage, s_nuc, s_tabS);      // ends with __syncthreads()
-  // programmatic dependent launch: the evaporation kernel may be scheduled as soon as every CTA of this grid is
-  // resident (it then fills the SMs whose CTA has finished); it takes its events from the completion list
-  asm volatile("griddepcontrol.launch_dependents;");
-
-  const unsigned lt = (1u << lane) - 1u;
-  const int n_xs = P.model.n_xs;
-  const R inv_dp = P.model.inv_dp;
-  const bool keep_transparent = (P.flags & INC_F_KEEP_TRANSPARENT) != 0;
-  const bool same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
-  const int spp = P.seg_per_pass;
-  LaneStats<STATS> st;
-  st.clear();
-
-  // warp-uniform queue sizes (every queue operation is warp-collective, so all lanes agree)
-  int nSeg = 0, nColl = 0, nEpi = 0, nFree = C::NS;
-  bool exhausted = false;
-  // drain helpers: a track with long_seg segments behind it is handed to a warp that has finished its own events
-  // (if there is one).  The STATS build keeps every track (a helper's speculative lanes would be counted).
-  const bool helpers_on = !STATS && (P.flags & INC_F_NO_DRAIN_HELPERS) == 0;
-  const int long_seg = helpers_on ? P.long_seg : (1 << 30);
-  int n_out = 0;              // tracks of ours that are with helpers
-  uint32_t r_head = 0u;       // returns consumed
-  for (int i = lane; i < C::NS; i += 32) { w.free_q[i] = (uint8_t)i; w.ev[i] = -1; }
-  __syncwarp();
-  const bool timeline = (P.flags & INC_F_TIMING) != 0;
-  if (timeline && lane == 0) { atomicMax(&P.ctr->tl[0], ~global_ns()); atomicAdd(&P.ctr->tl[4], 1ull); }
-  // per-warp drain trace (diagnostic, INC_F_TIMING only)
-  uint32_t *wt = (timeline && P.wtrace) ? P.wtrace + (size_t)kWTrace * (blockIdx.x * C::WARPS + (threadIdx.x >> 5)) : nullptr;
-  uint32_t tr_pass = 0, tr_seg = 0, tr_lanes = 0, tr_att = 0, tr_out = 0, tr_wait = 0;
-  if (wt && lane == 0) wt[7] = (uint32_t)global_ns();
-
-  auto load_key = [&](int slot, RngKey &g, uint32_t &attempt, int &tgt, int &ev) {
-    ev = w.ev[slot];
-    const uint32_t m = w.info[slot];
-    attempt = (m >> 16) & 0xFFu; tgt = (int)((m >> 24) & 0x7Fu);
-    const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
-    g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
-  };
-  auto push_seg = [&](bool pred, const Track<R> &t, int slot) {
-    const unsigned m = __ballot_sync(kFull, pred);
-    if (pred) {
-      const int i = nSeg + __popc(m & lt);
-      INC_CHECK(i >= 0 && i < C::QS && slot >= 0 && slot < C::NS);
-      w.qx[i] = t.x; w.qy[i] = t.y; w.qz[i] = t.z; w.qpx[i] = t.px; w.qpy[i] = t.py; w.qpz[i] = t.pz; w.qT[i] = t.T;
-      w.qpi[i] = t.pi; w.qkn[i] = t.k | ((uint32_t)t.nseg << 16);
-      w.qmeta[i] = (uint32_t)t.type | ((uint32_t)t.shell << 1) | ((uint32_t)slot << 8);
-    }
-    nSeg += __popc(m);
-  };
-  // Completion list: finished events are collected per warp and published in batches.
-  int nPub = 0;
-  auto push_pub = [&](bool pred, int ev) {
-    const unsigned m = __ballot_sync(kFull, pred);
-    INC_CHECK(!pred || (nPub + __popc(m & lt) < 96 && ev >= 0 && ev < P.n_chunk));
-    if (pred) w.pub_q[nPub + __popc(m & lt)] = (uint32_t)ev;
-    nPub += __popc(m);
-  };
-  auto flush_pub = [&]() {
-    if (nPub == 0) return;
-    unsigned long long base = 0;
-    if (lane == 0) base = atomicAdd(&P.ctr->n_done, (unsigned long long)nPub);
-    base = __shfl_sync(kFull, base, 0);
-    __syncwarp();
-    __threadfence();          // every lane: its records (and, through the __syncwarp()s since, the warp's) before the entries
-    for (int i = lane; i < nPub; i += 32) *(volatile uint32_t *)(P.ws.done_list + base + i) = w.pub_q[i];
-    nPub = 0;
-  };
-  auto push_epi = [&](bool pred, int slot) {
-    const unsigned m = __ballot_sync(kFull, pred);
-    INC_CHECK(!pred || (nEpi + __popc(m & lt) < C::NS && slot >= 0 && slot < C::NS));
-    if (pred) w.epi_q[nEpi + __popc(m & lt)] = (uint8_t)slot;
-    nEpi += __popc(m);
-  };
-
-  // lane-resident segment track: stays in registers across consecutive segment passes; only lanes whose
-  // track left the segment state (collision, escape, cap) touch the queues
-  Track<R> rt;
-  rt.x = rt.y = rt.z = rt.px = rt.py = rt.pz = rt.T = R(0); rt.pi = 0; rt.k = 0; rt.nseg = 0; rt.type = 0; rt.shell = 0;
-  int rslot = 0, rev = 0, rtgt = 0;
-  uint32_t rattempt = 0, rge0 = 0, rge1 = 0;
-  bool rhas = false;
-  int nRes = 0;   // warp-uniform count of resident tracks
-
-  // One pass of the warp (returns true when the warp has nothing left to do).  Two instances: the steady state,
-  // and the drain phase (after the event counter has run out for this warp), which alone carries the hand-over
-  // of long tracks to drain helpers -- so that code costs the steady-state loop nothing (registers, uniform
-  // registers, instructions).
-  auto pass = [&](auto drain_tag) -> bool {
-    constexpr bool DRAIN = decltype(drain_tag)::value;
-    __syncwarp();
-    if (DRAIN && n_out > 0) {
-      // ---- a track back from a helper: it continues here, at the segment that ends its collision-free run ----
-      const int i = (int)(r_head & (kRetQ - 1));
-      // (votes make the loaded flags warp-uniform for the compiler as well)
-      const bool back = __ballot_sync(kFull, ((volatile uint32_t *)w.r_valid)[i] != 0u) == kFull;
-      if (back && nSeg + nRes < C::QS) {
-        __threadfence_block();
-        Track<R> t;
-        t.x = w.rq[0][i]; t.y = w.rq[1][i]; t.z = w.rq[2][i]; t.px = w.rq[3][i]; t.py = w.rq[4][i]; t.pz = w.rq[5][i];
-        t.T = w.rq[6][i]; t.pi = w.rqi[0][i];
-        const uint32_t kn = w.rqi[1][i], mt = w.rqi[2][i];
-        t.k = kn & 0xFFFFu; t.nseg = (int)(kn >> 16);
-        t.type = mt & 1u; t.shell = (int)((mt >> 1) & 0x7Fu);
-        __syncwarp();
-        if (lane == 0) ((volatile uint32_t *)w.r_valid)[i] = 0u;
-        push_seg(lane == 0, t, (int)(mt >> 8));
-        r_head++; n_out--;
-      }
-    }
-    // ---- choose the kind of step of this pass (warp-uniform) ----
-    // Queue invariants: a segment pass adds at most one collision item per running lane, a collision pass at most two
-    // segment tracks per item, an entry pass one per item.  kCollTrig: from this many waiting collisions on a full
-    // segment pass might not fit into the collision queue, so a collision pass runs first.
-    constexpr int kCollTrig = C::QC - 31 < 32 ? C::QC - 31 : 32;
-    constexpr int kAdmit = (C::QS + C::QC) / 3;       // admission control: no new attempts while more tracks wait
-    const int nSegT = nSeg + nRes;
-    const int availE = nEpi + (exhausted ? 0 : nFree);
-    int phase = ST_SEG;
-    int lim = 32;                                 // tracks the refill of a segment pass may take
-    if (!(nColl < kCollTrig && nSegT >= 32)) {        // (the common case needs none of what follows)
-      if (nColl >= kCollTrig) phase = ST_COLL;
-      else if (availE >= 32) phase = ST_EPI;
-      else {
-        // nothing fills a whole pass: take the fullest queue (ties: entry first, it creates work)
-        if (availE > 0 && availE >= nSegT && availE >= nColl) phase = ST_EPI;
-        else if (nColl > 0 && nColl >= nSegT) phase = ST_COLL;
-        else if (nSegT > 0) phase = ST_SEG;
-        else if (DRAIN && n_out > 0) { __nanosleep(100); tr_wait++; return false; }      // our last tracks are with helpers
-        else return true;
-      }
-      if (phase == ST_EPI && nSegT + nColl > kAdmit) phase = nSegT > 0 ? ST_SEG : ST_COLL;   // admission control
-      // While a full collision pass does not fit into the segment queue, segment passes make room first (nSegT > 0
-      // then, because QS >= 64); as long as the collision queue can take a full segment pass they are ordinary ones,
-      // beyond that a partial collision pass runs if it can (m >= 1), else a segment pass of at most QC - nColl lanes:
-      // the resident tracks go back to the queue and the refill takes no more than that.  So some pass can always run
-      // unless both queues are full (error bit 4: inc_simulate reruns the call with the lane kernel).
-      if (phase == ST_COLL && nSegT + 2 * (nColl < 32 ? nColl : 32) > C::QS) {
-        if (nColl <= C::QC - 32) phase = ST_SEG;
-        else if (C::QS - nSegT < 2 && nColl < C::QC) {
-          push_seg(rhas, rt, rslot);
-          rhas = false; nRes = 0;
-          phase = ST_SEG; lim = C::QC - nColl;
-        }
-      }
-    }
-
-    if (phase == ST_SEG) {
-      // refill lanes without a resident track from the top of the segment queue
-      {
-        const bool need = !rhas;
-        const unsigned mk = __ballot_sync(kFull, need);
-        int take = __popc(mk);
-        take = take < nSeg ? take : nSeg;
-        take = take < lim ? take : lim;
-        const int r = __popc(mk & lt);
-        if (need && r < take) {
-          const int i = nSeg - 1 - r;
-          INC_CHECK(i >= 0 && i < C::QS);
-          rt.x = w.qx[i]; rt.y = w.qy[i]; rt.z = w.qz[i]; rt.px = w.qpx[i]; rt.py = w.qpy[i]; rt.pz = w.qpz[i]; rt.T = w.qT[i];
-          rt.pi = w.qpi[i];
-          const uint32_t kn = w.qkn[i], mt = w.qmeta[i];
-          rt.k = kn & 0xFFFFu; rt.nseg = (int)(kn >> 16);
-          rt.type = mt & 1u; rt.shell = (int)((mt >> 1) & 0x7Fu); rslot = (int)(mt >> 8);
-          rev = w.ev[rslot];
-          {
-            const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + rev);
-            rge0 = (uint32_t)ge; rge1 = (uint32_t)(ge >> 32);       // counter words 2, 3 of this track's event
-          }
-          const uint32_t inf = w.info[rslot];
-          rattempt = (inf >> 16) & 0xFFu; rtgt = (int)((inf >> 24) & 0x7Fu);
-          rhas = true;
-        }
-        nSeg -= take; nRes += take;
-      }
-      if (lane == 0) { st.add(S_WI_SEG); st.add(S_LS_SEG, nRes); }
-      if (DRAIN && wt) { tr_seg++; tr_lanes += (uint32_t)nRes; }
-      int out = -1;
-      CollCarry<R> cc;
-      Escape<R> esc;
-      // Several segment steps per pass (P.seg_per_pass): a track continues in ~87 % of its segments (16O; 76 % in
-      // 48Ti), so a second and third step still run at most of the lanes, and the refill, the hand-over of the tracks
-      // that leave and the scheduling are paid once per pass instead of once per step.  (Config 2, cascade kernel:
-      // 1 step 1.78 ms, 2 steps 1.63, 3 steps 1.57; 48Ti: 1.88, 1.74, 1.77.)
-      {
-        RngKey g;
-        g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = rge0; g.e1 = rge1;
-        bool act = rhas;
-#pragma unroll 1
-        for (int it = 0; it < spp; ++it) {
-          if (STATS && it > 0) {
-            const int na = __popc(__ballot_sync(kFull, act));
-            if (lane == 0) { st.add(S_WI_SEG); st.add(S_LS_SEG, na); }
-          }
-          if (act) out = seg_step<R, STATS>(rt, s_nuc[rtgt], s_tabS, n_xs, inv_dp, g, rattempt, cc, esc, st);
-          act = act && out == SEG_CONT;
-        }
-      }
-      {
-        // long tracks go to a helper, if there is one and its queue and our return queue have room
-        // ... and only tracks that have hardly collided so far (k - nseg = collisions <= nseg / 16): those are the
-        // orbits whose collision-free runs are long enough for a helper to pay off
-        const bool wl = DRAIN && rhas && out == SEG_CONT && rt.nseg >= long_seg && ((int)rt.k - rt.nseg) * 16 <= rt.nseg;
-        const unsigned ml = __ballot_sync(kFull, wl);
-        if (ml) {
-          bool moved = false;
-          // only to helpers that are free right now: a track never waits in the queue behind another one
-          const int free_helpers = *(volatile int *)&cq.idle - *(volatile int *)&cq.avail;
-          const int room = free_helpers < kRetQ - n_out ? free_helpers : kRetQ - n_out;
-          if (wl && __popc(ml & lt) < room) {
-            if (atomicSub(&cq.credits, 1) > 0) {
-              const int i = (int)(atomicAdd(&cq.tail, 1u) & (kCtaLongQ - 1));
-              cq.q[0][i] = rt.x; cq.q[1][i] = rt.y; cq.q[2][i] = rt.z; cq.q[3][i] = rt.px; cq.q[4][i] = rt.py; cq.q[5][i] = rt.pz;
-              cq.q[6][i] = rt.T; cq.qi[0][i] = rt.pi; cq.qi[1][i] = rt.k | ((uint32_t)rt.nseg << 16);
-              cq.qi[2][i] = (uint32_t)rt.type | ((uint32_t)rt.shell << 1) | ((uint32_t)rslot << 8);
-              cq.qi[3][i] = (uint32_t)rev;
-              cq.qi[4][i] = rattempt | ((uint32_t)rtgt << 8) | ((uint32_t)(threadIdx.x >> 5) << 16);
-              __threadfence_block();
-              ((volatile uint32_t *)cq.valid)[i] = 1u;
-              atomicAdd(&cq.avail, 1);
-              moved = true;
-            } else {
-              atomicAdd(&cq.credits, 1);
-            }
-          }
-          const unsigned mm = __ballot_sync(kFull, moved);
-          if (moved) rhas = false;
-          nRes -= __popc(mm); n_out += __popc(mm);
-          if (wt) tr_out += (uint32_t)__popc(mm);
-        }
-      }
-      const unsigned left = __ballot_sync(kFull, out > SEG_CONT);     // tracks that leave the segment state
-      if (left) {
-        {   // collisions -> collision queue
-          const bool pc = out == SEG_COLLIDE;
-          const unsigned mk = __ballot_sync(kFull, pc);
-          if (pc) {
-            const int i = nColl + __popc(mk & lt);
-            INC_CHECK(i >= 0 && i < C::QC && rslot >= 0 && rslot < C::NS);
-            w.cx[i] = rt.x; w.cy[i] = rt.y; w.cz[i] = rt.z; w.cpx[i] = rt.px; w.cpy[i] = rt.py; w.cpz[i] = rt.pz; w.cT[i] = rt.T;
-            w.cpi[i] = rt.pi; w.ckn[i] = rt.k | ((uint32_t)rt.nseg << 16);
-            w.cmeta[i] = (uint32_t)rt.type | ((uint32_t)rt.shell << 1) | ((uint32_t)rslot << 8);
-            w.cf[i] = cc.f; w.cnx[i] = cc.nx; w.cny[i] = cc.ny; w.cnz[i] = cc.nz; w.cSp[i] = cc.Sp; w.cSig[i] = cc.Sig;
-          }
-          nColl += __popc(mk);
-        }
-        bool finished = false;
-        if (out == SEG_ESCAPE || out == SEG_CAP) {
-          if (out == SEG_ESCAPE) {
-            const uint32_t old = atomicAdd(&w.info[rslot], 1u + ((uint32_t)rt.type << 8));
-            const int idx = (int)(old & 0xFFu);
-            if (idx < kMaxSec) {
-              const size_t o = (size_t)rev * kMaxSec + idx;
-              INC_CHECK(rev >= 0 && rev < P.n_chunk && rslot >= 0 && rslot < C::NS && w.ev[rslot] == rev);
-              stage_write<R>(P.ws.st + o, esc.T, esc.ux, esc.uy, esc.uz, rt.pi | ((uint32_t)rt.type << 24));
-              typedef typename Fx<R>::U FU;
-              atomicAdd((FU *)&w.acc[0][rslot], (FU)(-Fx<R>::to(esc.T)));
-              atomicAdd((FU *)&w.acc[1][rslot], (FU)(-Fx<R>::to(rt.px)));
-              atomicAdd((FU *)&w.acc[2][rslot], (FU)(-Fx<R>::to(rt.py)));
-              atomicAdd((FU *)&w.acc[3][rslot], (FU)(-Fx<R>::to(rt.pz)));
-            } else {
-              atomicSub(&w.info[rslot], 1u + ((uint32_t)rt.type << 8));
-              atomicOr(&w.status[rslot], INC_ST_SEC_TRUNC);
-            }
-          } else {
-            atomicOr(&w.status[rslot], INC_ST_SEG_CAP);
-          }
-          finished = (atomicSub(&w.cnt[rslot], 1u) & 0xFFFFu) == 1u;
-        }
-        push_epi(finished, rslot);
-        if (out > SEG_CONT) rhas = false;
-        nRes -= __popc(left);
-      }
-      return false;
-    }
-
-    // any other pass: park the resident tracks in the segment queue first
-    if (nRes > 0) {
-      push_seg(rhas, rt, rslot);
-      rhas = false; nRes = 0;
-    }
-
-    if (phase == ST_COLL) {
-      int m = nColl < 32 ? nColl : 32;
-      if (2 * m > C::QS - nSeg) m = (C::QS - nSeg) / 2;
-      if (m <= 0) {   // both queues full: implementation limit exceeded -> fail loudly, never hang
-        if (lane == 0) atomicOr(&P.ctr->error_word, 4u);
-        return true;
-      }
-      if (lane == 0) { st.add(S_WI_COLL); st.add(S_LS_COLL, m); }
-      const bool has = lane < m;
-      Track<R> t, c2;
-      CollCarry<R> cc;
-      int slot = 0;
-      if (has) {
-        const int i = nColl - 1 - lane;
-        INC_CHECK(i >= 0 && i < C::QC);
-        t.x = w.cx[i]; t.y = w.cy[i]; t.z = w.cz[i]; t.px = w.cpx[i]; t.py = w.cpy[i]; t.pz = w.cpz[i]; t.T = w.cT[i];
-        t.pi = w.cpi[i];
-        const uint32_t kn = w.ckn[i], mt = w.cmeta[i];
-        t.k = kn & 0xFFFFu; t.nseg = (int)(kn >> 16);
-        t.type = mt & 1u; t.shell = (int)((mt >> 1) & 0x7Fu); slot = (int)(mt >> 8);
-        cc.f = w.cf[i]; cc.nx = w.cnx[i]; cc.ny = w.cny[i]; cc.nz = w.cnz[i]; cc.Sp = w.cSp[i]; cc.Sig = w.cSig[i];
-      }
-      nColl -= m;
-      __syncwarp();
-      bool keep1 = false, keep2 = false, allowed = false, finished = false;
-      if (has) {
-        RngKey g;
-        uint32_t attempt;
-        int tgt, ev;
-        load_key(slot, g, attempt, tgt, ev);
-        uint32_t stbits = 0;
-        allowed = coll_step<R, STATS>(t, cc, s_nuc[tgt], P.model.tabC, n_xs, inv_dp, g, attempt, c2, keep1, keep2, stbits, st);
-        if (stbits) atomicOr(&w.status[slot], stbits);
-        if (allowed) {
-          // one real collision (high half) and the change of the pending count (low half) in one atomic
-          const uint32_t delta = (1u << 16) + (keep1 ? 1u : 0u) + (keep2 ? 1u : 0u) - 1u;
-          finished = ((atomicAdd(&w.cnt[slot], delta) + delta) & 0xFFFFu) == 0u;
-        } else {
-          keep1 = true;   // blocked: the projectile continues from the collision point
-        }
-      }
-      push_seg(has && keep1, t, slot);
-      push_seg(has && allowed && keep2, c2, slot);
-      push_epi(finished, slot);
-      return false;
-    }
-
-    // ---------- EPI pass: epilogue of finished attempts, event fetch, entry ----------
-    {
-      int m = availE < 32 ? availE : 32;
-      if (m > C::QS - nSeg) m = C::QS - nSeg;
-      const int mE = nEpi < m ? nEpi : m;          // finished slots first, then free slots
-      const int mF = m - mE;
-      if (lane == 0) { st.add(S_WI_EPI); st.add(S_LS_EPI, m); }
-      const bool has = lane < m;
-      int slot = 0;
-      INC_CHECK(!has || (lane < mE ? (nEpi - 1 - lane >= 0 && nEpi - 1 - lane < C::NS) : (nFree - 1 - (lane - mE) >= 0 && nFree - 1 - (lane - mE) < C::NS)));
-      if (has) slot = lane < mE ? w.epi_q[nEpi - 1 - lane] : w.free_q[nFree - 1 - (lane - mE)];
-      INC_CHECK(slot >= 0 && slot < C::NS);
-      nEpi -= mE; nFree -= mF;
-      __syncwarp();
-      bool want_event = has && lane >= mE;
-      bool do_entry = false;
-      bool done_now = false;
-      int ev_done = 0;
-      int ev = -1, tgt = 0, ptype = 1;
-      uint32_t attempt = 0;
-      R E_in = R(0);
-      if (has && lane < mE) {
-        ev = w.ev[slot];
-        const uint32_t ne = w.info[slot];
-        attempt = (ne >> 16) & 0xFFu; tgt = (int)((ne >> 24) & 0x7Fu); ptype = (int)(ne >> 31);
-        E_in = P.E_in[ev];
-        const NucDev<R> &nu = s_nuc[tgt];
-        const int n_esc = (int)(ne & 0xFFu), n_p = (int)((ne >> 8) & 0xFFu);
-        const R Eavail = Fx<R>::from(w.acc[0][slot]);
-        const R Prx = Fx<R>::from(w.acc[1][slot]), Pry = Fx<R>::from(w.acc[2][slot]), Prz = Fx<R>::from(w.acc[3][slot]);
-        int A_res, Z_res;
-        R Estar;
-        const bool ok = epilogue_eval<R>(nu, P.model.bind, ptype, n_esc, n_p, (int)(w.cnt[slot] >> 16), Eavail, Prx, Pry, Prz, keep_transparent, A_res, Z_res, Estar);
-        if (ok) {
-          const uint32_t used = attempt + 1u > 255u ? 255u : attempt + 1u;
-          write_cascade_result<R>(P.ws, ev, A_res, Z_res, Estar, Prx, Pry, Prz, (uint32_t)n_esc | (attempt << 8), w.status[slot] | used);
-          want_event = true; done_now = true; ev_done = ev;
-        } else if (attempt + 1u >= (uint32_t)kMaxAttempt) {    // FAILED: count 0, target at rest
-          write_cascade_result<R>(P.ws, ev, nu.A, nu.Z, R(0), R(0), R(0), R(0), (1u << 16), INC_ST_FAILED | 0xFFu);
-          st.add(S_FAILED);
-          want_event = true; done_now = true; ev_done = ev;
-        } else {
-          attempt++;
-          do_entry = true;
-        }
-      }
-      push_pub(done_now, ev_done);                 // finished events -> evaporation kernel
-      // ---- warp-aggregated event fetch ----
-      const unsigned need = __ballot_sync(kFull, want_event && !exhausted);
-      bool got_none = false;
-      if (need) {
-        bool rejected = false;
-        int ev_rej = 0;
-        const int leader = __ffs(need) - 1;
-        unsigned long long base = 0;
-        if (lane == leader) base = atomicAdd(&P.ctr->next_event_casc, (unsigned long long)__popc(need));
-        base = __shfl_sync(kFull, base, leader);
-        if (want_event) {
-          const unsigned long long mine = base + (unsigned long long)__popc(need & lt);
-          if (mine < (unsigned long long)P.n_chunk) {
-            ev = (int)mine;
-            attempt = 0;
-            E_in = P.E_in[ev];
-            tgt = P.target_id[ev];
-            ptype = P.projectile ? (int)P.projectile[ev] : 1;
-            if (check_inputs<R>(P, s_nuc, ev, E_in, tgt, ptype)) { do_entry = true; st.add(S_EVENTS); }
-            else { rejected = true; ev_rej = ev; }
-          } else {
-            got_none = true;
-          }
-        }
-        push_pub(rejected, ev_rej);               // (neutral outputs are complete results too)
-      }
-      // a batch is more than a pass's worth (one fence + one global atomic round trip each); the rest goes out when
-      // the warp has finished its own events
-      if (nPub > 32) flush_pub();
-      const bool ran_out = __ballot_sync(kFull, got_none) != 0u;
-      if (timeline && ran_out && !exhausted && lane == 0) { atomicAdd(&P.ctr->tl[1], global_ns()); if (wt) wt[0] = (uint32_t)global_ns(); }
-      if (DRAIN && wt) { const uint32_t am = __reduce_max_sync(kFull, do_entry ? attempt : 0u); tr_att = am > tr_att ? am : tr_att; }
-      if (ran_out) exhausted = true;
-      // slots that did not get work go back to the free list
-      {
-        const bool fr = has && !do_entry;
-        const unsigned mk = __ballot_sync(kFull, fr);
-        INC_CHECK(!fr || nFree + __popc(mk & lt) < C::NS);
-        if (fr) { w.free_q[nFree + __popc(mk & lt)] = (uint8_t)slot; w.ev[slot] = -1; }
-        nFree += __popc(mk);
-      }
-      Track<R> t;
-      if (do_entry) {
-        st.add(S_ATTEMPTS);
-        RngKey g;
-        const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
-        g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
-        R p_in;
-        entry_step<R>(t, s_nuc[tgt], E_in, ptype, g, attempt, p_in);
-        w.ev[slot] = ev; w.info[slot] = (attempt << 16) | ((uint32_t)tgt << 24) | ((uint32_t)ptype << 31);
-        w.cnt[slot] = 1u; w.status[slot] = 0;
-        w.acc[0][slot] = Fx<R>::to(E_in); w.acc[1][slot] = 0; w.acc[2][slot] = 0; w.acc[3][slot] = Fx<R>::to(p_in);
-      }
-      push_seg(do_entry, t, slot);
-    }
-    return false;
-  };
-  bool done = false;
-  while (!exhausted && !done) done = pass(std::false_type());
-  // watchdog: a drain phase is a few hundred passes (thousands with waits for helpers); 2^24 means a scheduling bug:
-  // fail loudly (error bit 16 -> INC_E_STATE) instead of hanging the device
-  while (!done) {
-    done = pass(std::true_type());
-    if (++tr_pass > (1u << 24)) {
-      if (wt) {   // (debug dump of the stuck state)
-        const unsigned mh = __ballot_sync(kFull, rhas);
-        const int fl = mh ? __ffs(mh) - 1 : 0;
-        const uint32_t ns = (uint32_t)__shfl_sync(kFull, rt.nseg, fl), sl = (uint32_t)__shfl_sync(kFull, rslot, fl), kk = __shfl_sync(kFull, rt.k, fl), pp = __shfl_sync(kFull, rt.pi, fl);
-        if (lane == 0) { wt[0] = mh; wt[1] = ns | (kk << 16); wt[6] = w.status[sl]; wt[7] = tr_seg; wt[3] = (uint32_t)nSeg | ((uint32_t)nRes << 16); }
-      }
-      if (lane == 0) {
-        atomicOr(&P.ctr->error_word, 16u);
-        if (wt) { wt[2] = tr_pass; wt[4] = (uint32_t)nColl | ((uint32_t)nEpi << 16); wt[5] = (uint32_t)nFree | ((uint32_t)n_out << 16); }
-      }
-      break;
-    }
-  }
-  if (wt && lane == 0 && tr_pass <= (1u << 24)) { wt[1] = (uint32_t)global_ns(); wt[2] = tr_pass; wt[3] = tr_seg; wt[4] = tr_lanes; wt[5] = tr_att | (tr_wait << 8); wt[6] = tr_out; }
-  if (timeline && lane == 0) {
-    const unsigned long long t = global_ns();
-    atomicAdd(&P.ctr->tl[2], t); atomicMax(&P.ctr->tl[3], t); atomicMax(&P.ctr->tl[5], ~t);
-  }
-  INC_CHECK(nSeg == 0 && nColl == 0 && nEpi == 0 && nRes == 0 && n_out == 0 && nFree == C::NS);   // every slot came back
-  flush_pub();
-  st.flush(P.ctr, lane);
-  if (helpers_on) {
-    if (lane == 0) { __threadfence_block(); atomicAdd(&cq.n_helpers, 1u); }
-    help_long_tracks<R, WM>(P, s_nuc, s_tabS, wm, cq, C::WARPS);
-  }
-}
-
-// =================================================================================================
-// Evaporation: Weisskopf-Ewing emission of n, p, d, t, 3He, 4He until no channel is
-// open.  One lane = one nucleus at a time; one emission step per warp pass; lanes refill.
-// =================================================================================================
-__constant__ int c_evA[6] = {1, 1, 2, 3, 3, 4};
-__constant__ int c_evZ[6] = {0, 1, 1, 1, 2, 2};
-
-template <typename R> struct EvapParams {
-  ModelDev<R> model;
-  Workspace<R> ws;
-  DevCounters *ctr;
-  long long e_base;
-  int n_chunk;
-  uint32_t seed_lo, seed_hi;
-  uint32_t flags;
-  int32_t *out_counts;      // caller array, chunk base (the residual goes to ws.frec, see compact_kernel)
-};
-
-// G_n(s) e^{-s_ref} with G_n(s) = int_0^s t^n e^t dt, n = 1 or 3 (closed forms of R-E2)
-template <typename R>
-__device__ __forceinline__ void G13_scaled(R s, R s_ref, R &g1, R &g3) {
-  if (s < M<R>::series_below()) {
-    // series sum_k s^(n+1+k) / (k! (n+1+k)); the closed forms cancel catastrophically here
-    R term = s * s;   // s^(2+k)/k!
-    R a1 = R(0), a3 = R(0);
-#pragma unroll 1
-    for (int k = 0; k < M<R>::kSeriesTerms; ++k) {
-      a1 += M<R>::div_(term, R(k + 2));
-      a3 += M<R>::div_(term * s * s, R(k + 4));
-      term *= M<R>::div_(s, R(k + 1));
-    }
-    const R e = M<R>::exp_(-s_ref);
-    g1 = a1 * e; g3 = a3 * e;
-  } else {
-    const R e1 = M<R>::exp_(s - s_ref), e0 = M<R>::exp_(-s_ref);
-    g1 = (s - R(1)) * e1 + e0;
-    g3 = (((s - R(3)) * s + R(6)) * s - R(6)) * e1 + R(6) * e0;
-  }
-}
-
-// ---- NEXT-2: GEM level density (DESIGN.md R-G1..G6) ----
-// ln rho(U): Fermi gas with the pre-exponential factor above E_x, constant temperature below (R-G1, R-G5)
-template <typename R>
-__device__ __forceinline__ R gem_lnrho(const LdDev<R> &ld, R U) {
-  if (U >= ld.Ex) {
-    const R u = U - ld.delta;
-    return R(2) * M<R>::sqrt_(ld.a * u) - ld.lna4 - R(1.25) * M<R>::log_(u);
-  }
-  return M<R>::div_(U - ld.E0, ld.T) - ld.lnT;
-}
-
-// int_x0^x1 (x + beta) rho(X - x) e^(-lref) dx: panels of at most 8 MeV, 16 Gauss-Legendre nodes each (R-G5: the
-// definition, evaluated by quadrature)
-template <typename R>
-__device__ __forceinline__ R gem_range(const LdDev<R> &ld, R X, R beta, R x0, R x1, R lref) {
-  if (!(x1 > x0)) return R(0);
-  int np = (int)ceil((double)((x1 - x0) * R(0.125)));
-  np = np < 1 ? 1 : np;
-  const R h = M<R>::div_(x1 - x0, R(np));
-  R sum = R(0);
-#pragma unroll 1
-  for (int p = 0; p < np; ++p) {
-    const R a0 = x0 + h * R(p);
-#pragma unroll 1
-    for (int q = 0; q < 16; ++q) {
-      const R x = a0 + R(0.5) * h * (c_gl.x[q] + R(1));
-      R U = X - x;
-      U = U < R(0) ? R(0) : U;
-      sum += R(0.5) * h * c_gl.w[q] * (x + beta) * M<R>::exp_(gem_lnrho<R>(ld, U) - lref);
-    }
-  }
-  return sum;
-}
-
-template <typename R>
-__device__ __forceinline__ R gem_integral(const LdDev<R> &ld, R X, R beta, R lref) {
-  const R xs = X - ld.Ex;                         // x below xs: daughter above E_x (Fermi gas)
-  if (xs <= R(0)) return gem_range<R>(ld, X, beta, R(0), X, lref);
-  return gem_range<R>(ld, X, beta, R(0), xs, lref) + gem_range<R>(ld, X, beta, xs, X, lref);
-}
-
-enum EvapMode : int { kEvapKernel = 0, kEvapHelper = 1, kEvapDrainOnly = 2 };
-
-// The persistent-lane evaporation loop as an object, so that two hosts can run it: the evaporation kernel (one pass after
-// the other until the completion list is exhausted) and the idle warps of the cascade kernel (a pass whenever they have
-// nothing else to do: DESIGN.md section 6).  State = one nucleus per lane + the warp's pool of completion-list entries.
-template <typename R, bool STATS, bool GEM>
-struct EvapLanes {
-  static constexpr int kTrialsPerPass = 2;
-  int lane;
-  bool cascade_only, same_stream;
-  int ev;
-  unsigned long long pbase;      // the warp's pool of completion-list entries: [pbase + ph, pbase + pn) not handed out yet
-  int pn, ph;
-  uint32_t pent;
-  int A, Z, count;
-  R Es, Px, Py, Pz;
-  uint32_t status, attempt, kblk;
-  RngKey g;
-  bool exhausted;
-  unsigned long long n_steps, n_trials, n_emit;
-  // state of an emission step whose rejection sampling is not finished yet: at most kTrialsPerPass trials run per
-  // pass, a lane that has not accepted by then keeps its step (channel, X, ...) and goes on in the next pass
-  // without computing the widths again -- the loop's trip count is the maximum over the warp's lanes (4.7 for a
-  // mean of 1.6 trials), and it was 37 % of the kernel's instructions at 6 lanes
-  bool sampling;
-  int jsel, ntrial;
-  R Bpar, X, a, beta, V, BdBj, s, T, areaA, areaB;
-  R u1, u2;
-  LdDev<R> ldsel;           // GEM mode: level density of the chosen channel's daughter
-
-  __device__ __forceinline__ void init(const EvapParams<R> &P) {
-    lane = threadIdx.x & 31;
-    cascade_only = (P.flags & INC_F_CASCADE_ONLY) != 0;
-    same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
-    ev = -1; pbase = 0; pn = 0; ph = 0; pent = kNotDone;
-    A = 0; Z = 0; count = 0; Es = 0; Px = 0; Py = 0; Pz = 0;
-    status = 0; attempt = 0; kblk = 0;
-    g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = 0; g.e1 = 0;
-    exhausted = false;
-    n_steps = 0; n_trials = 0; n_emit = 0;
-    sampling = false; jsel = -1; ntrial = 0;
-    Bpar = R(0); X = R(0); a = R(1); beta = R(0); V = R(0); BdBj = R(0); s = R(0); T = R(1); areaA = R(0); areaB = R(0);
-    u1 = R(0); u2 = R(0);
-    ldsel.a = ldsel.delta = ldsel.Ux = ldsel.Ex = ldsel.T = ldsel.E0 = ldsel.lnT = ldsel.lna4 = R(0);
-  }
-  __device__ __forceinline__ bool busy() const { return __ballot_sync(kFull, ev >= 0) != 0u; }
-
-  // One pass: refill, one emission step (or up to kTrialsPerPass sampler trials of a pending one) per lane.  Returns
-  // false when there is nothing (more) to do: kernel mode -- the list is exhausted; helper modes -- no lane has an event.
-  __device__ __forceinline__ bool pass(const EvapParams<R> &P, const int mode) {
-    __syncwarp();
-    // ---- refill idle lanes from the warp's pool of consecutive entries of the cascade kernel's completion list
-    // (lane i holds entry pbase + i).  Kernel mode: a pool is 32 tickets taken blindly (one global atomic and one
-    // coalesced load per 32 events), entries not published yet are polled.  Helper mode (idle warps of the cascade
-    // kernel): only entries that are published already are taken (compare-and-swap on the ticket counter), so that a
-    // helper never holds a ticket it would have to wait for. ----
-    const bool want = ev < 0;
-    const unsigned need = __ballot_sync(kFull, want);
-    if (need && mode != kEvapDrainOnly) {
-      if (ph == pn && !exhausted) {
-        if (mode == kEvapKernel) {
-          unsigned long long base = 0;
-          if (lane == 0) base = atomicAdd(&P.ctr->next_event_evap, 32ull);
-          base = __shfl_sync(kFull, base, 0);
-          if (base >= (unsigned long long)P.n_chunk) exhausted = true;
-          else {
-            pbase = base; ph = 0; pent = kNotDone;
-            const unsigned long long left = (unsigned long long)P.n_chunk - base;
-            pn = left < 32ull ? (int)left : 32;
-          }
-        } else {
-          unsigned long long cur = 0;
-          if (lane == 0) cur = *(volatile unsigned long long *)&P.ctr->next_event_evap;
-          cur = __shfl_sync(kFull, cur, 0);
-          if (cur >= (unsigned long long)P.n_chunk) exhausted = true;
-          else {
-            const bool in = cur + (unsigned long long)lane < (unsigned long long)P.n_chunk;
-            const uint32_t v = in ? ld_acquire_u32(P.ws.done_list + cur + lane) : kNotDone;
-            const unsigned gap0 = ~__ballot_sync(kFull, v != kNotDone);
-            const int k = gap0 ? __ffs(gap0) - 1 : 32;
-            int ok = 0;
-            if (k > 0 && lane == 0) ok = atomicCAS(&P.ctr->next_event_evap, cur, cur + (unsigned long long)k) == cur;
-            ok = __shfl_sync(kFull, ok, 0);
-            if (ok) { pbase = cur; pn = k; ph = 0; pent = v; }
-          }
-        }
-      }
-      if (ph < pn) {
-        // (the cascade kernel may still be running: poll the entries not seen yet; acquire = their events' records)
-        const bool mine = lane >= ph && lane < pn;
-        if (mine && pent == kNotDone) pent = ld_acquire_u32(P.ws.done_list + pbase + lane);
-        const unsigned rdy = __ballot_sync(kFull, mine && pent != kNotDone);
-        const unsigned gap = ~rdy & (kFull << ph);                    // first entry from ph on that is not there yet
-        const int nready = (gap ? __ffs(gap) - 1 : 32) - ph;
-        const int r = __popc(need & ((1u << lane) - 1u));
-        int give = __popc(need);
-        give = give < nready ? give : nready;
-        const uint32_t d = __shfl_sync(kFull, pent, (ph + r) & 31);
-        if (want && r < give) {
-          ev = (int)d;
-          const NucRec<R> rec = P.ws.crec[ev];
-          A = rec.A; Z = rec.Z; Es = rec.E; Px = rec.Px; Py = rec.Py; Pz = rec.Pz;
-          const uint32_t meta = rec.meta;
-          count = (int)(meta & 0xFFu); attempt = (meta >> 8) & 0xFFu;
-          status = rec.status;
-          kblk = 0;
-          const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
-          g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
-          if ((meta >> 16) & 1u) count = 0;   // FAILED or rejected input
-        }
-        ph += give;
-      }
-    }
-    if (__ballot_sync(kFull, ev >= 0) == 0) {
-      if (mode != kEvapKernel) return false;             // nothing to do right now
-      if (exhausted && ph == pn) return false;
-      __nanosleep(200);                     // every lane waits for the cascade kernel
-      return true;
-    }
-    // The step is written as stages that every lane of the warp walks through, each under its own predicate, with
-    // the rejection loop ended by a vote: the warp is converged again before the two-body kinematics.  (With the
-    // loop left by `break`, the compiler ran everything behind it once per group of lanes that left the loop
-    // together: 2.9 executions per pass at 6 lanes instead of one at 20.)
-    const bool have = ev >= 0;
-    const bool carry = sampling;      // a step from the previous pass is still being sampled
-    bool finish = have && !carry && (cascade_only || !(Es > R(0)) || (status & INC_ST_FAILED));
-    if (have && !finish && !carry) {
-      jsel = -1;
-      // ---------- E1/E2: channel widths ----------
-      Bpar = __ldg(P.model.bind + A * kZmax + Z);
-      R Xj[6], sj[6], aj[6];
-      EvChan<R> ch[6];
-      R s_ref = R(0);
-      bool any = false;
-#pragma unroll
-      for (int j = 0; j < 6; ++j) {
-        const int Ad = A - c_evA[j], Zd = Z - c_evZ[j];
-        Xj[j] = R(-1); sj[j] = R(0); aj[j] = R(1);
-        ch[j].pref = R(0); ch[j].V = R(0); ch[j].beta = R(0); ch[j].BdBj = R(0);
-        if (Ad >= 1 && Zd >= 0 && Zd <= Ad) {
-          const EvChan<R> c = P.model.evch[(Ad * kZmax + Zd) * 6 + j];
-          if (c.pref > R(0)) {
-            const R Xc = Es - Bpar + c.BdBj - c.V;
-            if (GEM) {
-              // (GEM mode: sj = ln rho(X) of the daughter, the largest value of the integrand's density; s_ref, their
-              // maximum, scales the f32 integrals like e^{-s_max} does in the Weisskopf-Ewing mode)
-              if (Xc > R(0)) {
-                const LdDev<R> ld = P.model.ld[Ad * kZmax + Zd];
-                if (ld.a > R(0)) {
-                  ch[j] = c;
-                  Xj[j] = Xc;
-                  sj[j] = gem_lnrho<R>(ld, Xc);
-                  s_ref = (!any || sj[j] > s_ref) ? sj[j] : s_ref;
-                  any = true;
-                }
-              }
-            } else if (Xc > R(0)) {
-              ch[j] = c;
-              Xj[j] = Xc;
-              aj[j] = M<R>::div_(R(Ad), P.model.a_div);
-              sj[j] = R(2) * M<R>::sqrt_(aj[j] * Xc);
-              s_ref = sj[j] > s_ref ? sj[j] : s_ref;
-              any = true;
-            }
-          }
-        }
-      }
-      if (!any) finish = true;
-      else if (count >= kMaxSec) { status |= INC_ST_SEC_TRUNC; finish = true; }
-      else {
-        if (STATS) n_steps++;
-        R W[6];
-        R Wsum = R(0);
-#pragma unroll
-        for (int j = 0; j < 6; ++j) {
-          W[j] = R(0);
-          if (GEM) {
-            if (Xj[j] > R(0)) {
-              // R-G5: W_j = g_j M_j A_d^(2/3) alpha_j int_0^X (x + beta) rho(X - x) dx by quadrature (the f64 build
-              // leaves the integrand unscaled, like the oracle)
-              const LdDev<R> ld = P.model.ld[((A - c_evA[j]) * kZmax + (Z - c_evZ[j]))];
-              const R w = ch[j].pref * gem_integral<R>(ld, Xj[j], ch[j].beta, sizeof(R) == 4 ? s_ref : R(0));
-              W[j] = w > R(0) ? w : R(0);
-              Wsum += W[j];
-            }
-          } else if (Xj[j] > R(0)) {
-            R g1, g3;
-            G13_scaled<R>(sj[j], s_ref, g1, g3);
-            const R I0 = M<R>::div_(g1, R(2) * aj[j]);
-            const R I1 = Xj[j] * I0 - M<R>::div_(g3, R(8) * aj[j] * aj[j]);
-            R w = ch[j].pref * (I1 + ch[j].beta * I0);
-            W[j] = w > R(0) ? w : R(0);
-            Wsum += W[j];
-          }
-        }
-        if (!(Wsum > R(0))) finish = true;
-        else {
-          // ---------- E3: choose the channel ----------
-          R u[4];
-          draw4<R>(g, attempt, 0u, kblk++, u);
-          u1 = u[1]; u2 = u[2];
-          R cum = R(0);
-          const R thr = u[0] * Wsum;
-          bool done = false;
-#pragma unroll
-          for (int j = 0; j < 6; ++j) {
-            if (!done && W[j] > R(0)) { cum += W[j]; jsel = j; if (thr < cum) done = true; }
-          }
-#pragma unroll
-          for (int j = 0; j < 6; ++j) if (j == jsel) { X = Xj[j]; a = aj[j]; beta = ch[j].beta; V = ch[j].V; BdBj = ch[j].BdBj; }
-          if (GEM) {
-            // R-G6: envelope slope = the smallest slope of ln rho on [0, X]: 1/T of the constant-temperature branch,
-            // or the Fermi-gas slope at X if that is smaller; s holds ln rho(X)
-            ldsel = P.model.ld[((A - c_evA[jsel]) * kZmax + (Z - c_evZ[jsel]))];
-            R mm = M<R>::div_(R(1), ldsel.T);
-            if (X > ldsel.Ex) {
-              const R uu = X - ldsel.delta;
-              const R sfg = M<R>::sqrt_(M<R>::div_(ldsel.a, uu)) - M<R>::div_(R(1.25), uu);
-              mm = sfg < mm ? sfg : mm;
-            }
-            T = M<R>::div_(R(1), mm);
-            s = gem_lnrho<R>(ldsel, X);
-          } else {
-            s = R(2) * M<R>::sqrt_(a * X);
-            T = M<R>::sqrt_(M<R>::div_(X, a));
-          }
-          areaA = T * (T + beta); areaB = R(0.5) * X * X + beta * X;
-          sampling = true; ntrial = 0;
-        }
-      }
-    }
-    // ---------- E4: rejection sampling of x (two envelopes, R-E4); warp-uniform loop ----------
-    R xs = R(-1);
-    bool pending = sampling;
-#pragma unroll 1
-    for (int n = 0; n < kTrialsPerPass; ++n) {
-      if (__ballot_sync(kFull, pending) == 0u) break;
-      if (pending && ntrial >= kMaxTrial) pending = false;      // trial cap (R-E4): xs stays < 0
-      if (pending) {
-        R v[4];
-        draw4<R>(g, attempt, 0u, kblk++, v);
-        ntrial++;
-        if (STATS) n_trials++;
-        R xx;
-        if (areaB < areaA) {
-          xx = -beta + M<R>::sqrt_(beta * beta + v[1] * (X * X + R(2) * beta * X));
-          R rem = X - xx;
-          rem = rem > R(0) ? rem : R(0);
-          const R lr = GEM ? gem_lnrho<R>(ldsel, rem) : R(2) * M<R>::sqrt_(a * rem);
-          if (M<R>::log_(v[3]) < lr - s) { xs = xx < X ? xx : X; pending = false; }
-        } else {
-          if (v[0] * (T + beta) < T) xx = -T * M<R>::log_(v[1] * v[2]);
-          else xx = -T * M<R>::log_(v[1]);
-          if (xx < X) {
-            const R lr = GEM ? gem_lnrho<R>(ldsel, X - xx) : R(2) * M<R>::sqrt_(a * (X - xx));
-            if (M<R>::log_(v[3]) < lr - s + M<R>::div_(xx, T)) { xs = xx; pending = false; }
-          }
-        }
-      }
-    }
-    __syncwarp();
-    if (sampling && !(pending && ntrial < kMaxTrial)) {      // accepted, or the cap was reached
-      sampling = false;
-      if (xs < R(0)) { status |= INC_ST_TRIAL_CAP; finish = true; }
-      else {
-        // ---------- E5: two-body decay in the parent rest frame, isotropic, boost to lab ----------
-        const int Aj = c_evA[jsel], Zj = c_evZ[jsel];
-        const int Ad = A - Aj, Zd = Z - Zj;
-        const R Bj = __ldg(P.model.bind + Aj * kZmax + Zj);
-        const R Mj = R(Zj) * K<R>::mp + R(Aj - Zj) * K<R>::mn - Bj;
-        const R Bd = BdBj - Bj;
-        const R Esd = X - xs;
-        const R Mds = R(Zd) * K<R>::mp + R(Ad - Zd) * K<R>::mn - Bd + Esd;
-        const R Mpar = R(Z) * K<R>::mp + R(A - Z) * K<R>::mn - Bpar + Es;
-        const R eps = V + xs;   // total kinetic energy released in the parent frame
-        const R p2 = M<R>::div_(eps * (R(2) * Mpar - eps) * (R(2) * Mds + eps) * (R(2) * Mj + eps), R(4) * Mpar * Mpar);
-        const R pm = M<R>::sqrt_(p2 > R(0) ? p2 : R(0));
-        const R Ej = M<R>::sqrt_(p2 + Mj * Mj);
-        const R cth = R(2) * u1 - R(1);
-        R s2 = R(1) - cth * cth;
-        const R sth = M<R>::sqrt_(s2 > R(0) ? s2 : R(0));
-        R sph, cph;
-        M<R>::sincos2pi(u2, &sph, &cph);
-        const R qx = pm * sth * cph, qy = pm * sth * sph, qz = pm * cth;
-        const R Epar = M<R>::sqrt_(Mpar * Mpar + Px * Px + Py * Py + Pz * Pz);
-        const R iEp = M<R>::rcp_(Epar);
-        const R bx = Px * iEp, by = Py * iEp, bz = Pz * iEp;
-        const R gam = M<R>::div_(Epar, Mpar);
-        const R gfac = M<R>::div_(gam * gam, gam + R(1));
-        const R fo = gfac * (qx * bx + qy * by + qz * bz) + gam * Ej;
-        const R lx = qx + fo * bx, ly = qy + fo * by, lz = qz + fo * bz;
-        const R l2 = lx * lx + ly * ly + lz * lz;
-        const R El = M<R>::sqrt_(l2 + Mj * Mj);
-        const R Tl = M<R>::div_(l2, El + Mj);
-        const R il = M<R>::rsqrt_(l2);
-        const size_t o = (size_t)ev * kMaxSec + count;
-        stage_write<R>(P.ws.st + o, Tl, lx * il, ly * il, lz * il, 0x80000000u | ((uint32_t)jsel << 24) | (uint32_t)count);
-        count++;
-        if (STATS) n_emit++;
-        A = Ad; Z = Zd; Es = Esd;
-        Px -= lx; Py -= ly; Pz -= lz;
-      }
-    }
-    if (finish) {
-      P.out_counts[ev] = count;
-      NucRec<R> r;
-      r.E = Es; r.Px = Px; r.Py = Py; r.Pz = Pz; r.A = A; r.Z = Z; r.meta = (uint32_t)count; r.status = status;
-      P.ws.frec[ev] = r;
-      ev = -1;
-    }
-    return true;
-  }
-
-  __device__ __forceinline__ void flush_stats(const EvapParams<R> &P) {
-  if (STATS) {
-    unsigned long long v[3] = {n_steps, n_trials, n_emit};
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(kFull, v[i], o);
-      if (lane == 0 && v[i]) atomicAdd(&P.ctr->stats[S_EVSTEPS + i], v[i]);
-    }
-  }
-  }
-};
-
-template <typename R, bool STATS, bool GEM>
-__global__ void __launch_bounds__(256, sizeof(R) == 4 ? 3 : 2) evap_kernel(const EvapParams<R> P) {
-  EvapLanes<R, STATS, GEM> L;
-  L.init(P);
-  while (L.pass(P, kEvapKernel)) { }
-  L.flush_stats(P);
-}
-
-// =================================================================================================
-// Output: exclusive prefix sum of the per-event counts, then canonical-order SoA compaction
-// (BASELINE.json north_star "prefix-sum compaction of variable-length secondary lists into
-// coalesced SoA buffers").
-// =================================================================================================
-constexpr int kScanBlock = 256;
-constexpr int kScanItems = 8;                       // per thread
-constexpr int kScanTile = kScanBlock * kScanItems;  // 2048 events per block
-
-__device__ __forceinline__ long long block_exclusive_scan(long long v, long long *s_warp, long long &block_total) {
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  long long incl = v;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    long long t = __shfl_up_sync(kFull, incl, o);
-    if (lane >= o) incl += t;
-  }
-  if (lane == 31) s_warp[wid] = incl;
-  __syncthreads();
-  if (wid == 0) {
-    long long w = lane < (kScanBlock / 32) ? s_warp[lane] : 0;
-    long long wi = w;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      long long t = __shfl_up_sync(kFull, wi, o);
-      if (lane >= o) wi += t;
-    }
-    if (lane < (kScanBlock / 32)) s_warp[lane] = wi - w;
-    if (lane == (kScanBlock / 32) - 1) s_warp[kScanBlock / 32] = wi;
-  }
-  __syncthreads();
-  block_total = s_warp[kScanBlock / 32];
-  return incl - v + s_warp[wid];
-}
-
-// pass 1: per-tile sums
-__global__ void __launch_bounds__(kScanBlock) scan_tile_sums(const int32_t *counts, int n, long long *tile_sums) {
-  __shared__ long long s_warp[kScanBlock / 32 + 1];
-  const int base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
-  long long v = 0;
-#pragma unroll
-  for (int i = 0; i < kScanItems; ++i) if (base + i < n) v += counts[base + i];
-  long long total;
-  block_exclusive_scan(v, s_warp, total);
-  if (threadIdx.x == 0) tile_sums[blockIdx.x] = total;
-}
-
-// pass 2: one block scans the tile sums (n_tiles <= 2^20/2048 * ... loop) and adds the running base
-__global__ void __launch_bounds__(kScanBlock) scan_tiles(long long *tile_sums, int n_tiles, unsigned long long *running_total) {
-  __shared__ long long s_warp[kScanBlock / 32 + 1];
-  __shared__ long long s_carry;
-  if (threadIdx.x == 0) s_carry = (long long)*running_total;
-  __syncthreads();
-  for (int b = 0; b < n_tiles; b += kScanBlock) {
-    const int i = b + threadIdx.x;
-    const long long v = i < n_tiles ? tile_sums[i] : 0;
-    long long total;
-    const long long ex = block_exclusive_scan(v, s_warp, total);
-    const long long carry = s_carry;
-    if (i < n_tiles) tile_sums[i] = carry + ex;
-    __syncthreads();
-    if (threadIdx.x == 0) s_carry = carry + total;
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) *running_total = (unsigned long long)s_carry;
-}
-
-// pass 3: offsets[e] = tile base + exclusive scan inside the tile
-__global__ void __launch_bounds__(kScanBlock) scan_write_offsets(const int32_t *counts, int n, const long long *tile_sums,
-                                                                 long long *offsets) {
-  __shared__ long long s_warp[kScanBlock / 32 + 1];
-  const int base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
-  int c[kScanItems];
-  long long v = 0;
-#pragma unroll
-  for (int i = 0; i < kScanItems; ++i) { c[i] = base + i < n ? counts[base + i] : 0; v += c[i]; }
-  long long total;
-  long long ex = block_exclusive_scan(v, s_warp, total) + tile_sums[blockIdx.x];
-#pragma unroll
-  for (int i = 0; i < kScanItems; ++i) {
-    if (base + i < n) offsets[base + i] = ex;
-    ex += c[i];
-  }
-}
-
-template <typename R> struct CompactParams {
-  Workspace<R> ws;
-  const long long *offsets;   // chunk-local array of global output offsets
-  const int32_t *counts;
-  int n_chunk;
-  uint8_t *species;
-  R *T, *ux, *uy, *uz;
-  long long capacity;
-  // residual of the caller (chunk base): transposed from ws.frec
-  int32_t *rA, *rZ;
-  R *rE, *rPx, *rPy, *rPz;
-  uint32_t *rstatus;
-};
-
-// One warp per group of 32 events; lanes sweep the records of each event so that the stores of a
-// warp cover one contiguous span of the output arrays.  Cascade records are placed by the rank of
-// their path code (canonical order), evaporation records keep their emission order.
-template <typename R>
-__global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) {
-  const int lane = threadIdx.x & 31;
-  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int e0 = warp * 32;
-  if (e0 >= P.n_chunk) return;
-  const int e = e0 + lane;
-  long long off = 0;
-  int cnt = 0;
-  if (e < P.n_chunk) {
-    off = P.offsets[e]; cnt = P.counts[e];
-    const NucRec<R> r = P.ws.frec[e];
-    P.rA[e] = r.A; P.rZ[e] = r.Z; P.rE[e] = r.E; P.rPx[e] = r.Px; P.rPy[e] = r.Py; P.rPz[e] = r.Pz; P.rstatus[e] = r.status;
-  }
-  // flatten (event, record) pairs of the 32 events over the lanes
-  int incl = cnt;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    int t = __shfl_up_sync(kFull, incl, o);
-    if (lane >= o) incl += t;
-  }
-  const int total = __shfl_sync(kFull, incl, 31);
-  const int excl = incl - cnt;
-  for (int i0 = 0; i0 < total; i0 += 32) {
-    const int i = i0 + lane;
-    // find the event: largest l with excl_l <= i  (binary search over the 32 lanes' excl via shuffles)
-    int lo = 0;
-#pragma unroll
-    for (int step = 16; step > 0; step >>= 1) {
-      const int cand = lo + step;
-      const int ex_c = __shfl_sync(kFull, excl, cand & 31);
-      if (cand < 32 && ex_c <= i) lo = cand;
-    }
-    const int ex_l = __shfl_sync(kFull, excl, lo);
-    const long long off_l = __shfl_sync(kFull, off, lo);
-    if (i < total) {
-      const int el = e0 + lo;
-      const int j = i - ex_l;
-      const size_t sbase = (size_t)el * kMaxSec;
-      const StageRec<R> *row = P.ws.st + sbase;
-      const StageRec<R> rec = row[j];
-      const uint32_t code = rec.code;
-      int rank = j;
-      uint8_t sp;
-      if (code & 0x80000000u) {
-        sp = (uint8_t)(0x80u | ((code >> 24) & 0x7u));
-      } else {
-        sp = (uint8_t)((code >> 24) & 1u);
-        const uint32_t key = code & 0xFFFFFFu;
-        const int n_casc = (int)(P.ws.crec[el].meta & 0xFFu);
-        rank = 0;
-        for (int l = 0; l < n_casc; ++l) rank += ((row[l].code & 0xFFFFFFu) < key) ? 1 : 0;
-      }
-      const long long dst = off_l + rank;
-      if (dst < P.capacity) {
-        P.species[dst] = sp;
-        P.T[dst] = rec.T; P.ux[dst] = rec.ux; P.uy[dst] = rec.uy; P.uz[dst] = rec.uz;
-      }
-    }
-  }
-}
-
-// =================================================================================================
-// On-device tallies (inc_tally): double-differential spectra per
-// class, multiplicities, residual nuclide chart, yields.  One thread per event (grid-stride); each block
-// histograms into 32-bit shared-memory bins and adds its non-zero bins to the caller's 64-bit tallies at the end
-// (smem = 0: straight to the global tallies, for bin counts that do not fit in shared memory).
-// =================================================================================================
-template <typename R> struct TallyParams {
-  const uint8_t *species; const R *T, *uz;
-  const int32_t *counts; const long long *offsets;
-  const int32_t *rA, *rZ;
-  long long n_events;
-  int n_T, n_cos, mult_max, A_max, Z_max;
-  R T_scale, cos_scale;          // n_T / T_max and n_cos / 2, rounded once to R
-  unsigned long long *dd, *mult, *nuclide, *yield;
-  int smem;                      // 1 = shared-memory bins
-};
-
-template <typename R>
-__global__ void __launch_bounds__(256) tally_kernel(const TallyParams<R> P) {
-  extern __shared__ unsigned int s_bins[];
-  const int n_dd = 3 * P.n_cos * (P.n_T + 1), n_mult = 4 * (P.mult_max + 1), n_nuc = (P.A_max + 1) * (P.Z_max + 1);
-  const int o_mult = n_dd, o_nuc = n_dd + n_mult, o_y = o_nuc + n_nuc, n_all = o_y + 12;
-  if (P.smem) {
-    for (int i = threadIdx.x; i < n_all; i += blockDim.x) s_bins[i] = 0u;
-    __syncthreads();
-  }
-  auto bump = [&](int bin) {
-    if (P.smem) atomicAdd(&s_bins[bin], 1u);
-    else {
-      unsigned long long *g = bin < o_mult ? P.dd + bin : bin < o_nuc ? P.mult + (bin - o_mult)
-                            : bin < o_y ? P.nuclide + (bin - o_nuc) : P.yield + (bin - o_y);
-      atomicAdd(g, 1ull);
-    }
-  };
-  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < P.n_events; e += (long long)gridDim.x * blockDim.x) {
-    const long long b = P.offsets[e];
-    const int n = P.counts[e];
-    int m[3] = {0, 0, 0};
-    for (int k = 0; k < n; ++k) {
-      const unsigned sp = P.species[b + k];
-      const int code = (int)(sp & 0x7u);
-      const int c = code < 2 ? code : 2;
-      m[c]++;
-      int a = (int)((P.uz[b + k] + R(1)) * P.cos_scale);
-      a = a < 0 ? 0 : (a > P.n_cos - 1 ? P.n_cos - 1 : a);
-      const R tt = P.T[b + k] * P.T_scale;
-      int t = tt >= R(P.n_T) ? P.n_T : (int)tt;
-      t = t < 0 ? 0 : t;
-      bump((c * P.n_cos + a) * (P.n_T + 1) + t);
-      if (code < 6) bump(o_y + code * 2 + (int)(sp >> 7));
-    }
-    const int mm = P.mult_max;
-    bump(o_mult + 0 * (mm + 1) + (m[0] < mm ? m[0] : mm));
-    bump(o_mult + 1 * (mm + 1) + (m[1] < mm ? m[1] : mm));
-    bump(o_mult + 2 * (mm + 1) + (m[2] < mm ? m[2] : mm));
-    bump(o_mult + 3 * (mm + 1) + (n < mm ? n : mm));
-    const int A = P.rA[e], Z = P.rZ[e];
-    if (A >= 0 && A <= P.A_max && Z >= 0 && Z <= P.Z_max) bump(o_nuc + A * (P.Z_max + 1) + Z);
-  }
-  if (P.smem) {
-    __syncthreads();
-    for (int i = threadIdx.x; i < n_all; i += blockDim.x) {
-      const unsigned int v = s_bins[i];
-      if (v) {
-        unsigned long long *g = i < o_mult ? P.dd + i : i < o_nuc ? P.mult + (i - o_mult)
-                              : i < o_y ? P.nuclide + (i - o_nuc) : P.yield + (i - o_y);
-        atomicAdd(g, (unsigned long long)v);
-      }
-    }
-  }
-}
-
-// post-cascade records -> parallel arrays (inc_get_cascade_stage); any pointer may be null
-template <typename R>
-__global__ void unpack_cascade_kernel(const NucRec<R> *rec, long long n, int32_t *A, int32_t *Z, R *E, R *px, R *py, R *pz, int32_t *ncs) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const NucRec<R> r = rec[i];
-  if (A) A[i] = r.A;
-  if (Z) Z[i] = r.Z;
-  if (E) E[i] = r.E;
-  if (px) px[i] = r.Px;
-  if (py) py[i] = r.Py;
-  if (pz) pz[i] = r.Pz;
-  if (ncs) ncs[i] = (int32_t)(r.meta & 0xFFu);
-}
-
-// ---- issue-peak microbenchmark: 8 independent FMA chains per thread ------------------------------
-template <typename R>
-__global__ void __launch_bounds__(256) fma_peak_kernel(R *out, int iters, R a, R b) {
-  R v0 = R(threadIdx.x) * R(1e-3), v1 = v0 + R(1), v2 = v0 + R(2), v3 = v0 + R(3);
-  R v4 = v0 + R(4), v5 = v0 + R(5), v6 = v0 + R(6), v7 = v0 + R(7);
-#pragma unroll 1
-  for (int i = 0; i < iters; ++i) {
-#pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      v0 = fma(v0, a, b); v1 = fma(v1, a, b); v2 = fma(v2, a, b); v3 = fma(v3, a, b);
-      v4 = fma(v4, a, b); v5 = fma(v5, a, b); v6 = fma(v6, a, b); v7 = fma(v7, a, b);
-    }
-  }
-  R s = v0 + v1 + v2 + v3 + v4 + v5 + v6 + v7;
-  if (s == R(123456.789)) out[0] = s;
-}
-
-__global__ void philox_blocks_kernel(const uint32_t *ctr, uint32_t *out, long long n) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const uint4 o = philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3]);
-  out[4 * i] = o.x; out[4 * i + 1] = o.y; out[4 * i + 2] = o.z; out[4 * i + 3] = o.w;
-}
-
-}  // namespace inc
+#include "inc_common.cuh"
+#include "inc_physics.cuh"
+#include "inc_cascade_lane.cuh"
+#include "inc_cascade_wavefront.cuh"
+#include "inc_evap.cuh"
+#include "inc_output.cuh"
