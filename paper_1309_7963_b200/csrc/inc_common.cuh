@@ -81,7 +81,7 @@ template <typename R> struct __align__(16) StageRec {
 // One nucleus record per event: 32 bytes in the f32 build (one DRAM sector), 48 in f64.  Events finish, and are
 // evaporated, in an order unrelated to their index, so a record that is one sector costs one sector of traffic
 // where eight parallel arrays cost eight.  crec: post-cascade nucleus (the paper's "SoA of excited nuclei"),
-// meta = n_casc | attempt << 8 | failed << 16.  frec: final residual, meta = number of secondaries of the event; the
+// meta = n_casc | attempt << 8 | failed << 16.  frec: final residual, meta = number of secondaries | n_casc << 8; the
 // compaction kernel, which walks the events in index order, transposes it into the caller's arrays.
 template <typename R> struct __align__(16) NucRec {
   R E, Px, Py, Pz;

@@ -99,7 +99,7 @@ struct EvapLanes {
   unsigned long long pbase;      // the warp's pool of completion-list entries: [pbase + ph, pbase + pn) not handed out yet
   int pn, ph;
   uint32_t pent;
-  int A, Z, count;
+  int A, Z, count, n_casc;     // n_casc: cascade secondaries of the event (passed on to the compaction kernel)
   R Es, Px, Py, Pz;
   uint32_t status, attempt, kblk;
   RngKey g;
@@ -120,7 +120,7 @@ struct EvapLanes {
     cascade_only = (P.flags & INC_F_CASCADE_ONLY) != 0;
     same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
     ev = -1; pbase = 0; pn = 0; ph = 0; pent = kNotDone;
-    A = 0; Z = 0; count = 0; Es = 0; Px = 0; Py = 0; Pz = 0;
+    A = 0; Z = 0; count = 0; n_casc = 0; Es = 0; Px = 0; Py = 0; Pz = 0;
     status = 0; attempt = 0; kblk = 0;
     g.k0 = P.seed_lo; g.k1 = P.seed_hi; g.e0 = 0; g.e1 = 0;
     exhausted = false;
@@ -194,6 +194,7 @@ struct EvapLanes {
           const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
           g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);
           if ((meta >> 16) & 1u) count = 0;   // FAILED or rejected input
+          n_casc = count;
         }
         ph += give;
       }
@@ -391,7 +392,7 @@ struct EvapLanes {
     if (finish) {
       P.out_counts[ev] = count;
       NucRec<R> r;
-      r.E = Es; r.Px = Px; r.Py = Py; r.Pz = Pz; r.A = A; r.Z = Z; r.meta = (uint32_t)count; r.status = status;
+      r.E = Es; r.Px = Px; r.Py = Py; r.Pz = Pz; r.A = A; r.Z = Z; r.meta = (uint32_t)count | ((uint32_t)n_casc << 8); r.status = status;
       P.ws.frec[ev] = r;
       ev = -1;
     }

@@ -114,10 +114,11 @@ __global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) 
   if (e0 >= P.n_chunk) return;
   const int e = e0 + lane;
   long long off = 0;
-  int cnt = 0;
+  int cnt = 0, ncs = 0;
   if (e < P.n_chunk) {
     off = P.offsets[e]; cnt = P.counts[e];
     const NucRec<R> r = P.ws.frec[e];
+    ncs = (int)((r.meta >> 8) & 0xFFu);             // cascade secondaries of event e (frec.meta = count | n_casc << 8)
     P.rA[e] = r.A; P.rZ[e] = r.Z; P.rE[e] = r.E; P.rPx[e] = r.Px; P.rPy[e] = r.Py; P.rPz[e] = r.Pz; P.rstatus[e] = r.status;
   }
   // flatten (event, record) pairs of the 32 events over the lanes
@@ -141,6 +142,7 @@ __global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) 
     }
     const int ex_l = __shfl_sync(kFull, excl, lo);
     const long long off_l = __shfl_sync(kFull, off, lo);
+    const int n_casc = __shfl_sync(kFull, ncs, lo);
     if (i < total) {
       const int el = e0 + lo;
       const int j = i - ex_l;
@@ -155,7 +157,6 @@ __global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) 
       } else {
         sp = (uint8_t)((code >> 24) & 1u);
         const uint32_t key = code & 0xFFFFFFu;
-        const int n_casc = (int)(P.ws.crec[el].meta & 0xFFu);
         rank = 0;
         for (int l = 0; l < n_casc; ++l) rank += ((row[l].code & 0xFFFFFFu) < key) ? 1 : 0;
       }
