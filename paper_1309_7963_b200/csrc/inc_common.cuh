@@ -61,7 +61,8 @@ template <typename R> struct ModelDev {
   const R *tabS;          // [n_xs][4]  {sig_pp, dsig_pp, sig_np, dsig_np} in fm^2 (mb * 0.1)
   const R *tabC;          // [n_xs][8]  {B_pp, dB_pp, B_np, dB_np, a_np, da_np, 0, 0}
   const R *bind;          // [kAmax][kZmax] binding energy, MeV; < -1e29 => no such nucleus
-  const EvChan<R> *evch;  // [kAmax][kZmax][6]
+  const EvChan<R> *evp;   // [kAmax][kZmax][8] by PARENT (A, Z): entries 0-5 the channels' constants (of the daughters
+                          // (A - A_j, Z - Z_j); pref = 0: channel closed), entry 6: V = B(A, Z), entry 7 unused
   const LdDev<R> *ld;     // [kAmax][kZmax]  (level_density = 1 only)
   const NucDev<R> *nuc;   // [INC_MAX_TARGETS]
   int32_t n_xs;

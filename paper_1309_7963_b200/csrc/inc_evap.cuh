@@ -215,7 +215,10 @@ struct EvapLanes {
     if (have && !finish && !carry) {
       jsel = -1;
       // ---------- E1/E2: channel widths ----------
-      Bpar = __ldg(P.model.bind + A * kZmax + Z);
+      // one 128-byte row per PARENT nucleus: the six channels' constants and the parent's binding energy (a step then
+      // touches one cache line instead of seven scattered ones; the loads were 10 % of the kernel's stall samples)
+      const EvChan<R> *prow = P.model.evp + ((size_t)(A * kZmax + Z) << 3);
+      Bpar = prow[6].V;
       R Xj[6], sj[6], aj[6];
       EvChan<R> ch[6];
       R s_ref = R(0);
@@ -226,7 +229,7 @@ struct EvapLanes {
         Xj[j] = R(-1); sj[j] = R(0); aj[j] = R(1);
         ch[j].pref = R(0); ch[j].V = R(0); ch[j].beta = R(0); ch[j].BdBj = R(0);
         if (Ad >= 1 && Zd >= 0 && Zd <= Ad) {
-          const EvChan<R> c = P.model.evch[(Ad * kZmax + Zd) * 6 + j];
+          const EvChan<R> c = prow[j];
           if (c.pref > R(0)) {
             const R Xc = Es - Bpar + c.BdBj - c.V;
             if (GEM) {

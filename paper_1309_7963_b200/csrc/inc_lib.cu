@@ -392,7 +392,19 @@ int upload_model() {
   CU_TRY(up((void **)&g.d_tabS, S.data(), S.size() * sizeof(real)));
   CU_TRY(up((void **)&g.d_tabC, Cc.data(), Cc.size() * sizeof(real)));
   CU_TRY(up((void **)&g.d_bind, bind.data(), bind.size() * sizeof(real)));
-  CU_TRY(up((void **)&g.d_evch, ev.data(), ev.size() * sizeof(EvChan<real>)));
+  // the channel constants re-indexed by parent nucleus, eight entries (128 bytes in f32) per parent
+  std::vector<EvChan<real>> evp((size_t)kAmax * kZmax * 8);
+  std::memset(evp.data(), 0, evp.size() * sizeof(EvChan<real>));
+  for (int A = 1; A < kAmax; ++A)
+    for (int Z = 0; Z < kZmax && Z <= A; ++Z) {
+      EvChan<real> *row = &evp[((size_t)A * kZmax + Z) * 8];
+      for (int j = 0; j < 6; ++j) {
+        const int Ad = A - kEvA[j], Zd = Z - kEvZ[j];
+        if (Ad >= 1 && Zd >= 0 && Zd <= Ad && Zd < kZmax) row[j] = ev[((size_t)Ad * kZmax + Zd) * 6 + j];
+      }
+      row[6].V = bind[(size_t)A * kZmax + Z];
+    }
+  CU_TRY(up((void **)&g.d_evch, evp.data(), evp.size() * sizeof(EvChan<real>)));
   CU_TRY(up((void **)&g.d_ld, ldv.data(), ldv.size() * sizeof(LdDev<real>)));
   if (!g.d_nuc) {
     CU_TRY(cudaMalloc((void **)&g.d_nuc, sizeof(NucDev<real>) * INC_MAX_TARGETS));
@@ -407,7 +419,7 @@ int upload_model() {
 
 ModelDev<real> model_dev() {
   ModelDev<real> m;
-  m.tabS = g.d_tabS; m.tabC = g.d_tabC; m.bind = g.d_bind; m.evch = g.d_evch; m.nuc = g.d_nuc; m.ld = g.d_ld;
+  m.tabS = g.d_tabS; m.tabC = g.d_tabC; m.bind = g.d_bind; m.evp = g.d_evch; m.nuc = g.d_nuc; m.ld = g.d_ld;
   m.n_xs = g.tab.n_xs;
   m.inv_dp = (real)(1.0 / (g.tab.plab_max / (g.tab.n_xs - 1) * 1000.0));
   m.a_div = (real)g.tab.evap_a_div;
