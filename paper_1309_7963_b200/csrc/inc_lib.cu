@@ -568,7 +568,13 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = (timing || (g.flags & INC_F_NO_OVERLAP)) ? 0 : 1;
-    CU_TRY(cudaLaunchKernelEx(&cfg, ekern, ep));
+    cudaError_t le = cudaLaunchKernelEx(&cfg, ekern, ep);
+    if (le != cudaSuccess && cfg.numAttrs) {      // (a driver without programmatic dependent launch: plain stream order)
+      (void)cudaGetLastError();
+      cfg.numAttrs = 0;
+      le = cudaLaunchKernelEx(&cfg, ekern, ep);
+    }
+    CU_TRY(le);
   }
   CU_TRY(cudaGetLastError());
   if (mark(timing)) return INC_E_CUDA;
