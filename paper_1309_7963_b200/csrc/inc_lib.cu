@@ -108,7 +108,7 @@ struct State {
   int seg_per_pass = 0;             // 0 = chosen from the targets
   size_t chunk_events = (size_t)1 << 22;
   const uint8_t *projectile = nullptr;   // DEVICE, caller-owned; nullptr = protons
-  int sm_count = 0;
+  int sm_count = 0, smem_max = 0;
   std::string err;
 };
 
@@ -414,6 +414,7 @@ int upload_model() {
   int dev = 0;
   CU_TRY(cudaGetDevice(&dev));
   CU_TRY(cudaDeviceGetAttribute(&g.sm_count, cudaDevAttrMultiProcessorCount, dev));
+  CU_TRY(cudaDeviceGetAttribute(&g.smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
   return 0;
 }
 
@@ -465,6 +466,25 @@ State::Lane lane0() {
   return l;
 }
 
+// Launch shapes are queried once per (kernel, block size, dynamic shared memory): the attribute and occupancy calls cost
+// microseconds each, and they sit between two steps of a caller's loop, when the GPU has nothing to do.
+struct LaunchShape { const void *kern; int threads; size_t smem; int occ; };
+std::vector<LaunchShape> g_shapes;
+
+int launch_shape(const void *kern, int threads, size_t smem, int *occ) {
+  for (const auto &sh : g_shapes)
+    if (sh.kern == kern && sh.threads == threads && sh.smem == smem) { *occ = sh.occ; return 0; }
+  // the dynamic shared-memory limit is per kernel: it only ever grows (a launch needs limit >= its size)
+  size_t limit = 0;
+  for (const auto &sh : g_shapes) if (sh.kern == kern && sh.smem > limit) limit = sh.smem;
+  if (smem > limit) CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int o = 0;
+  CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kern, threads, smem));
+  g_shapes.push_back(LaunchShape{kern, threads, smem, o});
+  *occ = o;
+  return 0;
+}
+
 int mark(bool timing) {
   if (!timing) return 0;
   cudaEvent_t e;
@@ -508,9 +528,7 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   cp.n_stage = n_stage;
   const bool timing = (g.flags & INC_F_TIMING) != 0;
   const int need = (n_chunk + 255) / 256;
-  int dev = 0, smem_max = 0;
-  CU_TRY(cudaGetDevice(&dev));
-  CU_TRY(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  const int smem_max = g.smem_max;
   const size_t wsmem = wave_smem_bytes<real>(model.n_xs, n_stage);
   const bool lane_kernel = naive || (g.flags & INC_F_LANE_STATE_MACHINE) != 0 || wsmem > (size_t)smem_max;
   CU_TRY(cudaMemsetAsync(&L.ctr->next_event_casc, 0, 3 * sizeof(unsigned long long), L.stream));   // + next_event_evap, n_done
@@ -519,9 +537,8 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   if (lane_kernel) {
     const size_t smem = model_smem_bytes<real>(model.n_xs, n_stage);
     auto kern = cascade_lane_kernel<real, STATS>;
-    CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
-    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, smem));
+    if (int lr = launch_shape((const void *)kern, 256, smem, &occ)) return lr;
     if (occ < 1) return fail(INC_E_CUDA, "cascade kernel does not fit on an SM");
     int blocks = occ * g.sm_count;
     if (blocks > need) blocks = need;
@@ -530,9 +547,8 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
     // one persistent CTA per SM; each warp keeps WaveCfg::NS events in flight in its shared-memory queues
     auto kern = cascade_wavefront_kernel<real, STATS>;
     const int threads = WaveCfg<real>::WARPS * 32;
-    CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wsmem));
     int occ = 0;
-    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, wsmem));
+    if (int lr = launch_shape((const void *)kern, threads, wsmem, &occ)) return lr;
     if (occ < 1) return fail(INC_E_CUDA, "wavefront cascade kernel does not fit on an SM");
     int blocks = occ * g.sm_count;
     const int wneed = (n_chunk + threads - 1) / threads;
@@ -554,7 +570,7 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   ep.out_counts = counts;
   auto ekern = g.tab.level_density == 1 ? evap_kernel<real, STATS, true> : evap_kernel<real, STATS, false>;
   int eocc = 0;
-  CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&eocc, ekern, 256, 0));
+  if (int lr = launch_shape((const void *)ekern, 256, 0, &eocc)) return lr;
   if (eocc < 1) return fail(INC_E_CUDA, "evaporation kernel does not fit on an SM");
   int eblocks = eocc * g.sm_count;
   if (eblocks > need) eblocks = need;
