@@ -184,7 +184,6 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   if (lane < kRetQ) w.r_valid[lane] = 0u;
   if (lane == 0) w.r_tail = 0u;
   if (threadIdx.x < kCtaLongQ) cq.valid[threadIdx.x] = 0u;
-  if ((P.flags & INC_F_TEST_QUEUE_OVF) && blockIdx.x == 0 && threadIdx.x == 0) atomicOr(&P.ctr->error_word, 4u);
   if (threadIdx.x == 0) { cq.credits = kCtaLongQ; cq.avail = 0; cq.tail = 0u; cq.head = 0u; cq.n_helpers = 0u; cq.lock = 0u; cq.idle = 0; }
   stage_model<R>(P.model, P.n_stage, s_nuc, s_tabS);      // ends with __syncthreads()
   // programmatic dependent launch: the evaporation kernel may be scheduled as soon as every CTA of this grid is
@@ -620,6 +619,13 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
     return false;
   };
   bool done = false;
+  if ((P.flags & INC_F_TEST_QUEUE_OVF) && blockIdx.x == 0 && (threadIdx.x >> 5) == 0) {
+    // test hook: this warp fetches its first events, reports a queue overflow and abandons them, as a real overflow
+    // would: the evaporation kernel must not wait for them, and inc_simulate must run the call again
+    pass(std::false_type());
+    if (lane == 0) atomicOr(&P.ctr->error_word, 4u);
+    done = true; exhausted = true;
+  }
   while (!exhausted && !done) done = pass(std::false_type());
   // watchdog: a drain phase is a few hundred passes (thousands with waits for helpers); 2^24 means a scheduling bug:
   // fail loudly (error bit 16 -> INC_E_STATE) instead of hanging the device

@@ -202,7 +202,12 @@ struct EvapLanes {
     if (__ballot_sync(kFull, ev >= 0) == 0) {
       if (mode != kEvapKernel) return false;             // nothing to do right now
       if (exhausted && ph == pn) return false;
-      __nanosleep(200);                     // every lane waits for the cascade kernel
+      // every lane waits for the cascade kernel -- unless that has given up (queue overflow, watchdog, failed index
+      // check): its unfinished events never reach the list, and the call fails or is run again anyway
+      unsigned int err = 0;
+      if (lane == 0) err = *(volatile unsigned int *)&P.ctr->error_word;
+      if (__shfl_sync(kFull, err, 0) & (4u | 16u | 32u)) return false;
+      __nanosleep(200);
       return true;
     }
     // The step is written as stages that every lane of the warp walks through, each under its own predicate, with
