@@ -85,8 +85,9 @@ extern "C" {
 
 #define INC_F_NO_OVERLAP 512u       /* scheduling variant: the evaporation kernel starts only after the cascade kernel
                                       has finished (no programmatic dependent launch).  Results never depend on it. */
-#define INC_F_TEST_QUEUE_OVF 1024u  /* test hook: the wavefront kernel reports a track-queue overflow although there is
-                                      none, which exercises the library's rerun of the call with the lane kernel     */
+#define INC_F_TEST_QUEUE_OVF 1024u  /* test hook: one warp of the wavefront kernel reports a track-queue overflow and
+                                      abandons its events, as a real overflow would; exercises the library's rerun of
+                                      the call with the lane kernel                                                  */
 #define INC_F_NO_DRAIN_HELPERS 256u /* scheduling variant: every track stays with the warp that owns its
                                       event (no drain helpers).  Results never depend on it.   */
 
