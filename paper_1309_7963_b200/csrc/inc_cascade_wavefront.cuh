@@ -91,9 +91,15 @@ __device__ __forceinline__ void help_long_tracks(const CascadeParams<R> &P, cons
     int h = -1;
     if (lane == 0) {
       if (atomicSub(&cq.avail, 1) > 0) {
-        while (atomicCAS(&cq.lock, 0u, 1u) != 0u) { }
+        // (both waits are a few instructions of another warp long; the bound turns a protocol bug into error bit 16 --
+        // INC_E_STATE -- instead of a hung device)
+        unsigned spins = 0;
+        while (atomicCAS(&cq.lock, 0u, 1u) != 0u) { if (++spins > (1u << 26)) { atomicOr(&P.ctr->error_word, 16u); break; } }
         h = (int)(*(volatile uint32_t *)&cq.head & (kCtaLongQ - 1));
-        while (((volatile uint32_t *)cq.valid)[h] == 0u) { }      // its producer is just publishing it
+        spins = 0;
+        while (((volatile uint32_t *)cq.valid)[h] == 0u) {         // its producer is just publishing it
+          if (++spins > (1u << 26)) { atomicOr(&P.ctr->error_word, 16u); break; }
+        }
       } else {
         atomicAdd(&cq.avail, 1);
       }
