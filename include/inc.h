@@ -144,10 +144,16 @@ int inc_set_vote_thresholds(int coll, int epi);
  * value is an input error (INC_E_BADARG, found on the device like E_in out of range). */
 int inc_set_projectiles(const uint8_t *projectile /*DEVICE [n] or NULL*/);
 /* A call is processed in chunks of at most `n` events (default 2^22; 0 restores it; 1024 .. 2^24): the
- * library's staging workspace is sized for one chunk (64 records of 32 bytes per event in the f32
- * build: 8.6 GB at the default) and every chunk is one launch of each kernel, so large chunks mean
- * few drain phases of the persistent cascade kernel.  Results never depend on it (R-R4). */
+ * library's staging workspace is sized for one chunk (16 records of 32 bytes per event in the f32
+ * build plus an overflow pool and two 32-byte nucleus records: 2.4 GB at the default) and every chunk is one
+ * launch of each kernel, so large chunks mean few tails of the persistent cascade kernel.  Results never
+ * depend on it (R-R4). */
 int inc_set_chunk_events(int64_t n);
+/* Staging overflow pool: an event's first 16 secondaries are staged in its own row, an event with more (up to
+ * INC_MAX_SEC) takes one row of a pool that has, by default, a row for one event in 64.  A batch that needs more makes
+ * inc_simulate run the call again with a row for every event (inc_get_rerun_count counts it) and keeps that size.
+ * `rows` > 0 fixes the pool size (tests use 1 to force that path); 0 restores the default.  Results never depend on it. */
+int inc_set_stage_overflow_rows(int64_t rows);
 /* Scheduling knob of the default (wavefront) cascade kernel: a track that has run `n_segments`
  * segments may be handed to a warp that has finished its own events, which evaluates 32 consecutive
  * segments of the one track per pass along its collision-free path (drain helpers, DESIGN.md
@@ -244,9 +250,10 @@ int inc_get_drain_timeline(double ms[4] /*HOST*/);
  * [7] ns at kernel entry.  Returns the number of warps written (<= max_warps), 0 if none was recorded.  Diagnostic. */
 int inc_get_warp_trace(uint32_t *out /*HOST [8 * max_warps]*/, int32_t max_warps);
 
-/* How many inc_simulate calls so far were run a second time with the lane-per-event cascade kernel because the
- * wavefront kernel's per-warp track queues overflowed (an implementation limit of the default kernel, never a
- * property of the result: both kernels give the same events).  Diagnostic; expected to stay 0. */
+/* How many inc_simulate calls so far were run a second time: with the lane-per-event cascade kernel because the
+ * wavefront kernel's per-warp track queues overflowed, or with a larger staging overflow pool (implementation limits
+ * of the default configuration, never a property of the result: the events are the same).  Diagnostic; expected to
+ * stay 0. */
 int64_t inc_get_rerun_count(void);
 
 /* Nuclear-setup record of a target, for tests of inc_init (all HOST, fp64, length n_shells

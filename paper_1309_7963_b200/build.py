@@ -28,8 +28,9 @@ VARIANTS = {
     "f64": ["-DINC_REAL_IS_DOUBLE", "-fmad=false"],
     # test build: the f64 library with very small per-warp queues, so that the capacity guards of the wavefront
     # scheduler (partial collision passes, lane-capped segment passes, admission control) run all the time
-    # ... and with every queue / ring / slot index checked (INC_CHECKED: error bit 32 -> INC_E_STATE)
-    "f64q": ["-DINC_REAL_IS_DOUBLE", "-fmad=false", "-DINC_WNS=40", "-DINC_WQS=64", "-DINC_WQC=33", "-DINC_WWARPS=8", "-DINC_CHECKED"],
+    # ... with every queue / ring / slot index checked (INC_CHECKED: error bit 32 -> INC_E_STATE), and with 4 instead of
+    # 16 staged records in an event's own row, so that the staging overflow pool is in constant use
+    "f64q": ["-DINC_REAL_IS_DOUBLE", "-fmad=false", "-DINC_WNS=40", "-DINC_WQS=64", "-DINC_WQC=33", "-DINC_WWARPS=8", "-DINC_CHECKED", "-DINC_STAGE_MAIN=4"],
 }
 
 

@@ -81,8 +81,8 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
         if (out == SEG_COLLIDE) state = ST_COLL;
         else if (out == SEG_ESCAPE) {
           if (n_esc < kMaxSec) {
-            const size_t o = (size_t)ev * kMaxSec + n_esc;
-            stage_write<R>(P.ws.st + o, esc.T, esc.ux, esc.uy, esc.uz, t.pi | ((uint32_t)t.type << 24));
+            StageRec<R> *dst = stage_slot<R>(P.ws, P.ctr, ev, n_esc);
+            if (dst) stage_write<R>(dst, esc.T, esc.ux, esc.uy, esc.uz, t.pi | ((uint32_t)t.type << 24));
             n_esc++; n_p += t.type;
             fxE -= Fx<R>::to(esc.T); fxX -= Fx<R>::to(t.px); fxY -= Fx<R>::to(t.py); fxZ -= Fx<R>::to(t.pz);
           } else {

@@ -442,11 +442,20 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
           if (out == SEG_ESCAPE) {
             const uint32_t old = atomicAdd(&w.info[rslot], 1u + ((uint32_t)rt.type << 8));
             const int idx = (int)(old & 0xFFu);
-            if (idx < kMaxSec) {
-              const size_t o = (size_t)rev * kMaxSec + idx;
+            typedef typename Fx<R>::U FU;
+            if (idx < kStageMain) {
               INC_CHECK(rev >= 0 && rev < P.n_chunk && rslot >= 0 && rslot < C::NS && w.ev[rslot] == rev);
+              const size_t o = (size_t)rev * kStageMain + idx;
               stage_write<R>(P.ws.st + o, esc.T, esc.ux, esc.uy, esc.uz, rt.pi | ((uint32_t)rt.type << 24));
-              typedef typename Fx<R>::U FU;
+              atomicAdd((FU *)&w.acc[0][rslot], (FU)(-Fx<R>::to(esc.T)));
+              atomicAdd((FU *)&w.acc[1][rslot], (FU)(-Fx<R>::to(rt.px)));
+              atomicAdd((FU *)&w.acc[2][rslot], (FU)(-Fx<R>::to(rt.py)));
+              atomicAdd((FU *)&w.acc[3][rslot], (FU)(-Fx<R>::to(rt.pz)));
+            } else if (idx < kMaxSec) {
+              // (rare: the record goes to the event's overflow row; kept apart so that the common branch is the code
+              // it was before there were overflow rows)
+              StageRec<R> *dst = stage_slot_overflow<R>(P.ws.ovf, P.ws.ovf_id, P.ws.ovf_rows, P.ctr, rev, idx);
+              if (dst) stage_write<R>(dst, esc.T, esc.ux, esc.uy, esc.uz, rt.pi | ((uint32_t)rt.type << 24));
               atomicAdd((FU *)&w.acc[0][rslot], (FU)(-Fx<R>::to(esc.T)));
               atomicAdd((FU *)&w.acc[1][rslot], (FU)(-Fx<R>::to(rt.px)));
               atomicAdd((FU *)&w.acc[2][rslot], (FU)(-Fx<R>::to(rt.py)));

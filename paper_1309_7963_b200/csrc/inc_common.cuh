@@ -90,8 +90,21 @@ template <typename R> struct __align__(16) NucRec {
   uint32_t meta, status;
 };
 
+// Staged secondaries: an event's first kStageMain records sit in its own row; an event that has more (R-C5 allows 64, the
+// mean is 4-6) gets one row of the overflow pool for records kStageMain..63, its number kept in ovf_id[event].  The rows
+// are then a quarter of what 64 records per event would take (2.1 GB instead of 8.6 GB at 2^22 events per chunk).
+// (Of 6e4 250 MeV p-48Ti events none has more than 16 secondaries; the checked test build uses 4 per row.)
+#ifndef INC_STAGE_MAIN
+#define INC_STAGE_MAIN 16      // (the checked test build uses 4, so that the overflow rows are in constant use)
+#endif
+constexpr int kStageMain = INC_STAGE_MAIN;
+constexpr int kStageOvf = kMaxSec - kStageMain;
+
 template <typename R> struct Workspace {   // per-chunk internal buffers (DEVICE)
-  StageRec<R> *st;        // [chunk][kMaxSec] staged secondaries, one record per secondary
+  StageRec<R> *st;        // [chunk][kStageMain] staged secondaries, one record per secondary
+  StageRec<R> *ovf;       // [ovf_rows][kStageOvf] overflow pool
+  int32_t *ovf_id;        // [chunk] overflow row of the event, -1 = none (-2 = being allocated)
+  int32_t ovf_rows;
   NucRec<R> *crec;        // [chunk] post-cascade nuclei
   NucRec<R> *frec;        // [chunk] final residuals
   // Completion list: the cascade kernel appends the chunk-local index of every event whose post-cascade record is
@@ -131,6 +144,7 @@ __device__ __forceinline__ void stage_write(StageRec<R> *dst, R T, R ux, R uy, R
 struct DevCounters {       // device scalars
   unsigned long long next_event_casc, next_event_evap;
   unsigned long long n_done;          // entries of the completion list handed out (cascade -> evaporation)
+  unsigned long long ovf_next;        // rows of the staging overflow pool handed out
   unsigned long long total_sec;
   unsigned int error_word;   // bit0: E_in out of range, bit1: bad target id
   unsigned int pad;
@@ -140,6 +154,49 @@ struct DevCounters {       // device scalars
   // exit times, [3] latest warp exit, [4] number of warps, [5] max of ~exit (= ~earliest exit)
   unsigned long long tl[6];
 };
+
+// Where record `idx` of event `ev` is staged.  Records beyond the event's own row go to its overflow row, allocated by
+// whoever needs it first.  The cascade escapes of one event are written by lanes of ONE warp, possibly in the same pass:
+// one claims the row (compare-and-swap -1 -> -2), the others wait for its number (independent thread scheduling lets
+// lanes of a warp wait for each other; the wait is bounded all the same).  Returns nullptr if the pool is exhausted
+// (error bit 64: the library runs the call again with a pool that has a row for every event).
+// (the overflow part is a real function call: as inline code in the cascade kernel's escape block it cost the steady
+// state 1.2 % without ever running)
+template <typename R>
+__device__ __noinline__ StageRec<R> *stage_slot_overflow(StageRec<R> *ovf, int32_t *ovf_id, int32_t ovf_rows, DevCounters *ctr, int ev, int idx) {
+  Workspace<R> ws;
+  ws.ovf = ovf; ws.ovf_id = ovf_id; ws.ovf_rows = ovf_rows;
+  volatile int32_t *pid = ws.ovf_id + ev;
+  int id = *pid;
+  if (id < 0) {
+    const int prev = atomicCAS(ws.ovf_id + ev, -1, -2);
+    if (prev == -1) {
+      const unsigned long long r = atomicAdd(&ctr->ovf_next, 1ull);
+      id = r < (unsigned long long)ws.ovf_rows ? (int)r : 0x7FFFFFFF;
+      if (id == 0x7FFFFFFF) atomicOr(&ctr->error_word, 64u);
+      __threadfence();
+      *pid = id;
+    } else if (prev >= 0) {
+      id = prev;
+    } else {
+      unsigned spins = 0;
+      while ((id = *pid) < 0) { if (++spins > (1u << 26)) { atomicOr(&ctr->error_word, 16u); return nullptr; } }
+    }
+  }
+  if (id == 0x7FFFFFFF) return nullptr;
+  return ws.ovf + (size_t)id * kStageOvf + (idx - kStageMain);
+}
+template <typename R>
+__device__ __forceinline__ StageRec<R> *stage_slot(const Workspace<R> &ws, DevCounters *ctr, int ev, int idx) {
+  if (idx < kStageMain) return ws.st + (size_t)ev * kStageMain + idx;
+  return stage_slot_overflow<R>(ws.ovf, ws.ovf_id, ws.ovf_rows, ctr, ev, idx);
+}
+// the same for a reader: the row exists
+template <typename R>
+__device__ __forceinline__ const StageRec<R> *stage_at(const Workspace<R> &ws, int ev, int idx, int ovf_row) {
+  return idx < kStageMain ? ws.st + (size_t)ev * kStageMain + idx : ws.ovf + (size_t)ovf_row * kStageOvf + (idx - kStageMain);
+}
+
 __device__ __forceinline__ unsigned long long global_ns() {
   unsigned long long t;
   asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));

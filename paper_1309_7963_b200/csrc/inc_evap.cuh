@@ -389,8 +389,8 @@ struct EvapLanes {
         const R El = M<R>::sqrt_(l2 + Mj * Mj);
         const R Tl = M<R>::div_(l2, El + Mj);
         const R il = M<R>::rsqrt_(l2);
-        const size_t o = (size_t)ev * kMaxSec + count;
-        stage_write<R>(P.ws.st + o, Tl, lx * il, ly * il, lz * il, 0x80000000u | ((uint32_t)jsel << 24) | (uint32_t)count);
+        StageRec<R> *dst = stage_slot<R>(P.ws, P.ctr, ev, count);
+        if (dst) stage_write<R>(dst, Tl, lx * il, ly * il, lz * il, 0x80000000u | ((uint32_t)jsel << 24) | (uint32_t)count);
         count++;
         if (STATS) n_emit++;
         A = Ad; Z = Zd; Es = Esd;

@@ -95,7 +95,9 @@ struct State {
   long long last_n = -1;
   int last_chunks = 0;
   bool last_offsets_valid = false;  // inc_get_offsets: the last call left the offsets of the whole call on the device
-  long long reruns = 0;             // calls run again with the lane kernel after a queue overflow of the wavefront kernel              // chunks of the last inc_simulate (the cascade stage survives single-chunk calls only)
+  long long reruns = 0;
+  bool ovf_all = false;             // a call has exhausted the staging overflow pool: from then on a row for every event
+  long long ovf_rows_user = 0;      // inc_set_stage_overflow_rows (0 = automatic)             // calls run again with the lane kernel after a queue overflow of the wavefront kernel              // chunks of the last inc_simulate (the cascade stage survives single-chunk calls only)
   long long last_total = 0;
   long long event_offset = 0;
   // stage timing (INC_F_TIMING)
@@ -428,16 +430,32 @@ ModelDev<real> model_dev() {
 }
 
 void free_ws() {
-  void **p[] = {(void **)&g.ws.st, (void **)&g.ws.crec, (void **)&g.ws.frec, (void **)&g.ws.done_list};
+  void **p[] = {(void **)&g.ws.st, (void **)&g.ws.ovf, (void **)&g.ws.ovf_id, (void **)&g.ws.crec, (void **)&g.ws.frec, (void **)&g.ws.done_list};
+  g.ws.ovf_rows = 0;
   for (auto q : p) { if (*q) cudaFree(*q); *q = nullptr; }
   g.ws_chunk = 0;
 }
 
 int ensure_ws(size_t chunk, size_t n_total) {
-  if (chunk > g.ws_chunk) {
+  // overflow pool of the staging rows: a row for one event in 64 (at least 4096 rows; none of 6e4 250 MeV p-48Ti events
+  // has more than 16 secondaries); for every event once a call has
+  // exhausted the pool (g.ovf_all), or what the caller says (inc_set_stage_overflow_rows)
+  auto rows_for = [&](size_t c) -> size_t {
+    size_t r = g.ovf_rows_user > 0 ? (size_t)g.ovf_rows_user : (g.ovf_all ? c : (c / 64 > 4096 ? c / 64 : 4096));
+    if (r > c) r = c;
+    return r < 1 ? 1 : r;
+  };
+  const size_t ws_c = chunk > g.ws_chunk ? chunk : g.ws_chunk;
+  const bool rows_bad = g.ovf_rows_user > 0 ? (size_t)g.ws.ovf_rows != rows_for(ws_c) : (size_t)g.ws.ovf_rows < rows_for(chunk);
+  if (chunk > g.ws_chunk || rows_bad) {
     free_ws();
-    const size_t ns = chunk * kMaxSec;
+    chunk = ws_c;
+    const size_t want_rows = rows_for(chunk);
+    const size_t ns = chunk * kStageMain;
     CU_TRY(cudaMalloc((void **)&g.ws.st, ns * sizeof(StageRec<real>)));
+    CU_TRY(cudaMalloc((void **)&g.ws.ovf, want_rows * kStageOvf * sizeof(StageRec<real>)));
+    CU_TRY(cudaMalloc((void **)&g.ws.ovf_id, chunk * sizeof(int32_t)));
+    g.ws.ovf_rows = (int32_t)want_rows;
     CU_TRY(cudaMalloc((void **)&g.ws.crec, chunk * sizeof(NucRec<real>)));
     CU_TRY(cudaMalloc((void **)&g.ws.frec, chunk * sizeof(NucRec<real>)));
     CU_TRY(cudaMalloc((void **)&g.ws.done_list, chunk * sizeof(uint32_t)));
@@ -531,7 +549,8 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   const int smem_max = g.smem_max;
   const size_t wsmem = wave_smem_bytes<real>(model.n_xs, n_stage);
   const bool lane_kernel = naive || (g.flags & INC_F_LANE_STATE_MACHINE) != 0 || wsmem > (size_t)smem_max;
-  CU_TRY(cudaMemsetAsync(&L.ctr->next_event_casc, 0, 3 * sizeof(unsigned long long), L.stream));   // + next_event_evap, n_done
+  CU_TRY(cudaMemsetAsync(&L.ctr->next_event_casc, 0, 4 * sizeof(unsigned long long), L.stream));   // + next_event_evap, n_done, ovf_next
+  CU_TRY(cudaMemsetAsync(L.ws.ovf_id, 0xFF, (size_t)n_chunk * sizeof(int32_t), L.stream));         // -1: no overflow row
   CU_TRY(cudaMemsetAsync(L.ws.done_list, 0xFF, (size_t)n_chunk * sizeof(uint32_t), L.stream));      // kNotDone
   if (mark(timing)) return INC_E_CUDA;
   if (lane_kernel) {
@@ -683,12 +702,14 @@ void inc_shutdown(void) {
   g.tab.captured = false;
   g.last_n = -1;
   g.event_offset = 0;
+  g.ovf_all = false;
 }
 
 }  // extern "C"
 
 namespace {
 constexpr int64_t kQueueOverflow = -1000;   // internal: the wavefront kernel's track queues overflowed
+constexpr int64_t kPoolOverflow = -1001;    // internal: more events than overflow rows had over kStageMain secondaries
 
 int64_t simulate_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
                       int32_t *counts, inc_residual *res);
@@ -703,6 +724,13 @@ extern "C" {
 int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
                      int32_t *counts, inc_residual *res) {
   int64_t rc = simulate_once(n, E_in, tid, seed, sec, counts, res);
+  if (rc == kPoolOverflow) {
+    // The staging overflow pool (one row per 16 events) was too small for this batch: from now on every event has a row.
+    g.ovf_all = true; g.ovf_rows_user = 0;
+    g.reruns++;
+    rc = simulate_once(n, E_in, tid, seed, sec, counts, res);
+    if (rc == kPoolOverflow) rc = fail(INC_E_STATE, "staging overflow pool exhausted (results invalid)");
+  }
   if (rc == kQueueOverflow) {
     // The default cascade kernel keeps its tracks in fixed per-warp queues; a batch that overflows them (never seen:
     // it takes ~190 simultaneous tracks in one warp's ~80 events) is run again with the lane-per-event kernel, which
@@ -744,6 +772,7 @@ int64_t device_error(unsigned int err) {
   if (err & 32u) return fail(INC_E_STATE, "checked build: an index of the wavefront kernel's queues was out of range (results invalid)");
   if (err & 16u) return fail(INC_E_STATE, "watchdog: a warp of the wavefront cascade kernel made no progress (results invalid)");
   if (err & 4u) return kQueueOverflow;
+  if (err & 64u) return kPoolOverflow;
   if (err) {
     return fail(INC_E_BADARG, std::string("device-side input check failed:") + ((err & 1u) ? " E_in outside [20,250] MeV" : "") +
                                   ((err & 2u) ? " target_id not initialised" : "") + ((err & 8u) ? " projectile not 0 or 1" : ""));
@@ -902,6 +931,12 @@ int inc_set_segments_per_pass(int n) {
   return 0;
 }
 
+int inc_set_stage_overflow_rows(int64_t rows) {
+  if (rows < 0) return fail(INC_E_BADARG, "rows must be >= 0");
+  g.ovf_rows_user = rows;
+  return 0;
+}
+
 int inc_set_long_track_threshold(int n_segments) {
   if (n_segments < 0) return fail(INC_E_BADARG, "threshold must be >= 0");
   g.long_seg = n_segments == 0 ? kLongSegDefault : n_segments;
@@ -978,6 +1013,12 @@ int inc_philox_blocks(const uint32_t *ctr, uint64_t seed, uint32_t *out, int64_t
 int64_t inc_simulate_host(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
                           int32_t *counts, inc_residual *res) {
   int64_t rc = simulate_host_once(n, E_in, tid, seed, sec, counts, res);
+  if (rc == kPoolOverflow) {         // see inc_simulate
+    g.ovf_all = true; g.ovf_rows_user = 0;
+    g.reruns++;
+    rc = simulate_host_once(n, E_in, tid, seed, sec, counts, res);
+    if (rc == kPoolOverflow) rc = fail(INC_E_STATE, "staging overflow pool exhausted (results invalid)");
+  }
   if (rc == kQueueOverflow) {        // see inc_simulate
     const uint32_t f = g.flags;
     g.flags = (f | INC_F_LANE_STATE_MACHINE) & ~INC_F_TEST_QUEUE_OVF;

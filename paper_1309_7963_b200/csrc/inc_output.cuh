@@ -114,9 +114,10 @@ __global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) 
   if (e0 >= P.n_chunk) return;
   const int e = e0 + lane;
   long long off = 0;
-  int cnt = 0, ncs = 0;
+  int cnt = 0, ncs = 0, oid = -1;
   if (e < P.n_chunk) {
     off = P.offsets[e]; cnt = P.counts[e];
+    if (cnt > kStageMain) oid = P.ws.ovf_id[e];     // records beyond the event's own row sit in its overflow row
     const NucRec<R> r = P.ws.frec[e];
     ncs = (int)((r.meta >> 8) & 0xFFu);             // cascade secondaries of event e (frec.meta = count | n_casc << 8)
     P.rA[e] = r.A; P.rZ[e] = r.Z; P.rE[e] = r.E; P.rPx[e] = r.Px; P.rPy[e] = r.Py; P.rPz[e] = r.Pz; P.rstatus[e] = r.status;
@@ -143,12 +144,13 @@ __global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) 
     const int ex_l = __shfl_sync(kFull, excl, lo);
     const long long off_l = __shfl_sync(kFull, off, lo);
     const int n_casc = __shfl_sync(kFull, ncs, lo);
+    int oid_l = __shfl_sync(kFull, oid, lo);
+    // (a missing overflow row -- pool exhausted, error bit 64, the call is run again -- reads row 0: nothing faults)
+    oid_l = (oid_l >= 0 && oid_l < P.ws.ovf_rows) ? oid_l : 0;
     if (i < total) {
       const int el = e0 + lo;
       const int j = i - ex_l;
-      const size_t sbase = (size_t)el * kMaxSec;
-      const StageRec<R> *row = P.ws.st + sbase;
-      const StageRec<R> rec = row[j];
+      const StageRec<R> rec = *stage_at<R>(P.ws, el, j, oid_l);
       const uint32_t code = rec.code;
       int rank = j;
       uint8_t sp;
@@ -158,7 +160,7 @@ __global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) 
         sp = (uint8_t)((code >> 24) & 1u);
         const uint32_t key = code & 0xFFFFFFu;
         rank = 0;
-        for (int l = 0; l < n_casc; ++l) rank += ((row[l].code & 0xFFFFFFu) < key) ? 1 : 0;
+        for (int l = 0; l < n_casc; ++l) rank += ((stage_at<R>(P.ws, el, l, oid_l)->code & 0xFFFFFFu) < key) ? 1 : 0;
       }
       const long long dst = off_l + rank;
       if (dst < P.capacity) {

@@ -258,13 +258,43 @@ def test_small_queue_build_and_overflow_rerun(gpu, ptables, cfg, n):
         small.inc_set_long_track_threshold(0)
     for k in keys:
         assert np.array_equal(ref[k], got[k]), k
-    print(f"[small queues] config {cfg}: reruns with the lane kernel: {small.inc_get_rerun_count() - r0}")
+    print(f"[small queues] config {cfg}: reruns (lane kernel or larger staging pool): {small.inc_get_rerun_count() - r0}")
     lib = gpu.load("f64")
     r1 = lib.inc_get_rerun_count()
     forced = gpu.simulate(lib, targets, E, tid, seed, ptables, flags=gpu.F_TEST_QUEUE_OVF)
     assert lib.inc_get_rerun_count() == r1 + 1
     for k in keys:
         assert np.array_equal(ref[k], forced[k]), k
+
+
+def test_staging_overflow_rows(gpu, ptables):
+    """Staging: the first records of an event in its own row (16; 4 in the f64q test build), the rest (up to 64) in a row of
+    the overflow pool.  With 4 per row a third of the 48Ti events need an overflow row; with a pool of ONE row the batch
+    exhausts it, inc_simulate runs the call again with a row per event, and every result is the normal f64 build's, bit
+    for bit."""
+    E, tid, targets, seed, _ = _inputs(5, 60000)
+    keys = ("species", "T", "ux", "uy", "uz", "counts", "A", "Z", "Estar", "px", "py", "pz", "status", "offsets")
+    ref = gpu.simulate(gpu.load("f64"), targets, E, tid, seed, ptables)
+    lib = gpu.load("f64q")
+    big = int((ref["counts"] > 4).sum())
+    print(f"[staging overflow] {big} of {len(E)} events have more than 4 secondaries, {int((ref['counts'] > 16).sum())} more than 16, max {ref['counts'].max()}")
+    assert big > 1000
+    r0 = lib.inc_get_rerun_count()
+    got = gpu.simulate(lib, targets, E, tid, seed, ptables)             # default pool: a row for 1 event in 16 is too few here
+    for k in keys:
+        assert np.array_equal(ref[k], got[k]), k
+    assert lib.inc_get_rerun_count() == r0 + 1                           # ... so the call ran twice, and the pool grew
+    lib.inc_set_stage_overflow_rows(1)
+    try:
+        got = gpu.simulate(lib, targets, E, tid, seed, ptables)
+    finally:
+        lib.inc_set_stage_overflow_rows(0)
+    assert lib.inc_get_rerun_count() == r0 + 2
+    for k in keys:
+        assert np.array_equal(ref[k], got[k]), k
+    again = gpu.simulate(lib, targets, E, tid, seed, ptables)
+    for k in keys:
+        assert np.array_equal(ref[k], again[k]), k
 
 
 def test_fp64_transparent_and_failed(gpu, orc, ptables):
