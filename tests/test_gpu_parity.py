@@ -718,3 +718,25 @@ def test_host_path_memory_is_bounded(gpu, ptables):
             assert np.array_equal(dev[k].cpu().numpy(), out[k].numpy()[lo:hi]), k
         for k in ("species", "T", "uz"):
             assert np.array_equal(dev[k][:t].cpu().numpy(), out[k].numpy()[off[lo]:off[hi]]), k
+
+
+def test_fp64_edge_targets_and_energies(gpu, orc, otables, ptables):
+    """The corners of the supported domain (include/inc.h: 6 <= A <= 64, 2 <= Z <= A - 2, 20 <= E_in <= 250 MeV; P:9):
+    lightest and heaviest targets, both energy limits, protons and neutrons, in one mixed batch: the fp64 build equals the
+    oracle event by event and conserves A, Z and 4-momentum."""
+    targets = [(6, 3), (7, 2), (64, 28), (64, 30), (63, 40)]
+    n = 6000
+    rng = np.random.default_rng(11)
+    tid = rng.integers(0, len(targets), n).astype(np.int32)
+    E = rng.choice(np.array([20.0, 20.000001, 135.0, 249.999999, 250.0]), n)
+    proj = (rng.random(n) < 0.7).astype(np.uint8)
+    seed = 77
+    g = gpu.simulate(gpu.load("f64"), targets, E, tid, seed, ptables, projectile=proj)
+    o = orc.simulate(otables, targets, E, tid, seed, projectile=proj)
+    frac, max_err, ident = H.event_identity(g, o, rel=REL_F64)
+    print(f"[edges] identical {frac:.5f}, max rel err {max_err:.2e}, failed events {int(((g['status'] & gpu.ST_FAILED) != 0).sum())}")
+    assert frac >= FRAC_IDENTICAL and max_err <= REL_F64
+    assert np.array_equal(g["status"][ident], o["status"][ident])
+    _assert_conservation(g, targets, tid, E, orc, otables, 1e-12, 1e-9, projectile=proj)
+    g32 = gpu.simulate(gpu.load("f32"), targets, E, tid, seed, ptables, projectile=proj)
+    _assert_conservation(g32, targets, tid, E, orc, otables, 2e-6, 2e-4, projectile=proj)
