@@ -125,7 +125,11 @@ typedef struct inc_tables {   /* HOST memory, caller-owned, copied during inc_in
  * shells, Fermi momenta/energies, V = E_F + E_B, Coulomb barrier) done in fp64 on the host,
  * uploaded once.  The first call also captures the NN / evaporation tables.
  * Supported: 6 <= A <= 64, 2 <= Z <= A-2 (the separation energies need valid A-1 nuclei; the library's binding-energy
- * and evaporation-channel tables cover every nucleus a cascade on such a target can leave).  Returns target_id >= 0 (slot, < INC_MAX_TARGETS). */
+ * and evaporation-channel tables cover every nucleus a cascade on such a target can leave).  Returns target_id >= 0 (slot, < INC_MAX_TARGETS).
+ * Performance note: the default (wavefront) cascade kernel stages the records of all live target slots in shared memory
+ * beside its track queues, which leaves room for slots 0..9 in the f32 build with tables of at most 15 shells (0..4 with
+ * more shells); while a higher slot is live the library uses the lane-per-event cascade kernel instead (same results,
+ * about half the throughput).  Free unused targets. */
 int inc_init(int A, int Z, const inc_tables *tables /*HOST*/);
 int inc_free_target(int target_id);
 void inc_shutdown(void);       /* frees every target, the tables and the workspace          */

@@ -18,9 +18,10 @@ template <typename R> struct TrackRec {   // pending track (local-memory stack)
 template <typename R, bool STATS>
 __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParams<R> P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  NucDev<R> *s_nuc = reinterpret_cast<NucDev<R> *>(smem_raw);
-  R *s_tabS = reinterpret_cast<R *>(smem_raw + sizeof(NucDev<R>) * P.n_stage);
-  stage_model<R>(P.model, P.n_stage, s_nuc, s_tabS);
+  NucTab<R, 0> s_nuc;
+  s_nuc.base = smem_raw; s_nuc.stride = P.nuc_stride;
+  R *s_tabS = reinterpret_cast<R *>(smem_raw + (size_t)P.nuc_stride * P.n_stage);
+  stage_model<R>(P.model, P.n_stage, P.nuc_stride, smem_raw, s_tabS);
   // programmatic dependent launch: the evaporation kernel may be scheduled as soon as every CTA of this grid is
   // resident; it takes its events from the completion list, never from stream order
   asm volatile("griddepcontrol.launch_dependents;");
@@ -163,7 +164,7 @@ __global__ void __launch_bounds__(256, 2) cascade_lane_kernel(const CascadeParam
             E_in = P.E_in[ev];
             tgt = P.target_id[ev];
             ptype = P.projectile ? (int)P.projectile[ev] : 1;
-            if (!check_inputs<R>(P, s_nuc, ev, E_in, tgt, ptype)) { rejected = true; ev_rej = ev; ev = -1; tgt = 0; }
+            if (!check_inputs<R, NucTab<R, 0>>(P, s_nuc, ev, E_in, tgt, ptype)) { rejected = true; ev_rej = ev; ev = -1; tgt = 0; }
             else {
               const unsigned long long ge = same_stream ? 0ull : (unsigned long long)(P.e_base + ev);
               g.e0 = (uint32_t)ge; g.e1 = (uint32_t)(ge >> 32);

@@ -73,14 +73,14 @@ template <> struct WaveCfg<float> { static constexpr int NS = 80, QS = 128, QC =
 template <> struct WaveCfg<double> { static constexpr int NS = 64, QS = 128, QC = 64, WARPS = 8; };
 #endif
 
-template <typename R> __host__ __device__ inline size_t wave_smem_bytes(int n_xs, int n_stage) {
+template <typename R> __host__ __device__ inline size_t wave_smem_bytes(int n_xs, int n_stage, int n_shells) {
   typedef WaveCfg<R> C;
-  return model_smem_bytes<R>(n_xs, n_stage) + 32 + sizeof(CtaLong<R>) + sizeof(WarpMem<R, C::NS, C::QS, C::QC>) * C::WARPS;
+  return model_smem_bytes<R>(n_xs, n_stage, n_shells) + 32 + sizeof(CtaLong<R>) + sizeof(WarpMem<R, C::NS, C::QS, C::QC>) * C::WARPS;
 }
 
 // One warp, done with its own events, serves the CTA's hand-over queue until every warp of the CTA is done.
-template <typename R, typename WM>
-__device__ __forceinline__ void help_long_tracks(const CascadeParams<R> &P, const NucDev<R> *s_nuc, const R *s_tabS, WM *wm,
+template <typename R, typename WM, typename TAB>
+__device__ __forceinline__ void help_long_tracks(const CascadeParams<R> &P, const TAB &s_nuc, const R *s_tabS, WM *wm,
                                               CtaLong<R> &cq, int n_warps) {
   const int lane = threadIdx.x & 31;
   const bool same_stream = (P.flags & INC_F_SAME_STREAM) != 0;
@@ -175,14 +175,16 @@ __device__ __forceinline__ void help_long_tracks(const CascadeParams<R> &P, cons
   }
 }
 
-template <typename R, bool STATS>
+// NSH: shells per staged nucleus record (15: the paper's value and the default tables'; 32: any other table)
+template <typename R, bool STATS, int NSH>
 __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_kernel(const CascadeParams<R> P) {
   typedef WaveCfg<R> C;
   typedef WarpMem<R, C::NS, C::QS, C::QC> WM;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  NucDev<R> *s_nuc = reinterpret_cast<NucDev<R> *>(smem_raw);
-  R *s_tabS = reinterpret_cast<R *>(smem_raw + sizeof(NucDev<R>) * P.n_stage);
-  const size_t off = (model_smem_bytes<R>(P.model.n_xs, P.n_stage) + 15) & ~(size_t)15;
+  NucTab<R, NSH> s_nuc;
+  s_nuc.base = smem_raw; s_nuc.stride = P.nuc_stride;
+  R *s_tabS = reinterpret_cast<R *>(smem_raw + (size_t)P.nuc_stride * P.n_stage);
+  const size_t off = ((size_t)P.nuc_stride * P.n_stage + sizeof(R) * 4 * (size_t)P.model.n_xs + 15) & ~(size_t)15;
   CtaLong<R> &cq = *reinterpret_cast<CtaLong<R> *>(smem_raw + off);
   WM *wm = reinterpret_cast<WM *>(smem_raw + off + ((sizeof(CtaLong<R>) + 15) & ~(size_t)15));
   WM &w = wm[threadIdx.x >> 5];
@@ -191,7 +193,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   if (lane == 0) w.r_tail = 0u;
   if (threadIdx.x < kCtaLongQ) cq.valid[threadIdx.x] = 0u;
   if (threadIdx.x == 0) { cq.credits = kCtaLongQ; cq.avail = 0; cq.tail = 0u; cq.head = 0u; cq.n_helpers = 0u; cq.lock = 0u; cq.idle = 0; }
-  stage_model<R>(P.model, P.n_stage, s_nuc, s_tabS);      // ends with __syncthreads()
+  stage_model<R>(P.model, P.n_stage, P.nuc_stride, smem_raw, s_tabS);      // ends with __syncthreads()
   // programmatic dependent launch: the evaporation kernel may be scheduled as soon as every CTA of this grid is
   // resident (it then fills the SMs whose CTA has finished); it takes its events from the completion list
   asm volatile("griddepcontrol.launch_dependents;");
@@ -594,7 +596,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
             E_in = P.E_in[ev];
             tgt = P.target_id[ev];
             ptype = P.projectile ? (int)P.projectile[ev] : 1;
-            if (check_inputs<R>(P, s_nuc, ev, E_in, tgt, ptype)) { do_entry = true; st.add(S_EVENTS); }
+            if (check_inputs<R, NucTab<R, NSH>>(P, s_nuc, ev, E_in, tgt, ptype)) { do_entry = true; st.add(S_EVENTS); }
             else { rejected = true; ev_rej = ev; }
           } else {
             got_none = true;
@@ -670,7 +672,7 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
   st.flush(P.ctr, lane);
   if (helpers_on) {
     if (lane == 0) { __threadfence_block(); atomicAdd(&cq.n_helpers, 1u); }
-    help_long_tracks<R, WM>(P, s_nuc, s_tabS, wm, cq, C::WARPS);
+    help_long_tracks<R, WM, NucTab<R, NSH>>(P, s_nuc, s_tabS, wm, cq, C::WARPS);
   }
 }
 

@@ -544,17 +544,20 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   int n_stage = 0;
   for (int i = 0; i < INC_MAX_TARGETS; ++i) if (g.nuc[i].live) n_stage = i + 1;
   cp.n_stage = n_stage;
+  // staged nucleus records: 15 shells (+ the outside) when the tables have at most 15, as the paper's have; else all 32
+  const bool wide = g.tab.n_shells > 15;
+  cp.nuc_stride = nuc_stride_bytes<real>(wide ? kMaxShells : 15);
   const bool timing = (g.flags & INC_F_TIMING) != 0;
   const int need = (n_chunk + 255) / 256;
   const int smem_max = g.smem_max;
-  const size_t wsmem = wave_smem_bytes<real>(model.n_xs, n_stage);
+  const size_t wsmem = wave_smem_bytes<real>(model.n_xs, n_stage, wide ? kMaxShells : 15);
   const bool lane_kernel = naive || (g.flags & INC_F_LANE_STATE_MACHINE) != 0 || wsmem > (size_t)smem_max;
   CU_TRY(cudaMemsetAsync(&L.ctr->next_event_casc, 0, 4 * sizeof(unsigned long long), L.stream));   // + next_event_evap, n_done, ovf_next
   CU_TRY(cudaMemsetAsync(L.ws.ovf_id, 0xFF, (size_t)n_chunk * sizeof(int32_t), L.stream));         // -1: no overflow row
   CU_TRY(cudaMemsetAsync(L.ws.done_list, 0xFF, (size_t)n_chunk * sizeof(uint32_t), L.stream));      // kNotDone
   if (mark(timing)) return INC_E_CUDA;
   if (lane_kernel) {
-    const size_t smem = model_smem_bytes<real>(model.n_xs, n_stage);
+    const size_t smem = model_smem_bytes<real>(model.n_xs, n_stage, wide ? kMaxShells : 15);
     auto kern = cascade_lane_kernel<real, STATS>;
     int occ = 0;
     if (int lr = launch_shape((const void *)kern, 256, smem, &occ)) return lr;
@@ -564,7 +567,7 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
     kern<<<blocks, 256, smem, L.stream>>>(cp);
   } else {
     // one persistent CTA per SM; each warp keeps WaveCfg::NS events in flight in its shared-memory queues
-    auto kern = cascade_wavefront_kernel<real, STATS>;
+    auto kern = wide ? cascade_wavefront_kernel<real, STATS, kMaxShells> : cascade_wavefront_kernel<real, STATS, 15>;
     const int threads = WaveCfg<real>::WARPS * 32;
     int occ = 0;
     if (int lr = launch_shape((const void *)kern, threads, wsmem, &occ)) return lr;

@@ -314,6 +314,7 @@ template <typename R> struct CascadeParams {
   int long_seg;             // wavefront kernel: tracks with this many segments behind them may go to a drain helper
   int seg_per_pass;         // wavefront kernel: segment steps per segment pass (1..8)
   int n_stage;              // nuclei slots staged into shared memory (target_id must be < n_stage)
+  int nuc_stride;           // bytes of one staged nucleus (nuc_stride_bytes)
   uint32_t *wtrace;         // INC_F_TIMING: kWTrace words per warp of the wavefront kernel (inc_get_warp_trace), or nullptr
 };
 constexpr int kWTrace = 8;  // [0] ns (low 32 bits) when the event counter ran out for the warp, [1] ns at exit of its own work,
@@ -321,17 +322,33 @@ constexpr int kWTrace = 8;  // [0] ns (low 32 bits) when the event counter ran o
                             // [5] highest attempt number started in the drain, [6] tracks handed to helpers, [7] ns at kernel entry
 
 // shared-memory staging of the model: [NucDev x n_stage] [tabS n_xs*4]   (n_stage = highest live slot + 1)
-template <typename R> __host__ __device__ inline size_t model_smem_bytes(int n_xs, int n_stage) {
-  return sizeof(NucDev<R>) * (size_t)n_stage + sizeof(R) * 4 * (size_t)n_xs;
+// The staged copy of a nucleus is truncated after its last shell (header + ns + 1 shells of the 33 a NucDev has room
+// for): 1056 instead of 2144 bytes in the f32 build at 15 shells, so that ten live targets fit beside the queues of the
+// wavefront kernel instead of five.  All targets of a library state have the same number of shells.
+template <typename R> __host__ __device__ inline int nuc_stride_bytes(int n_shells) {
+  return (int)(sizeof(NucDev<R>) - sizeof(ShellDev<R>) * (size_t)(kMaxShells - n_shells));
+}
+// NSH > 0: the stride is that of NSH shells, known at compile time (the wavefront kernel's hot path: a run-time stride
+// cost its steady state 2.5 %); NSH = 0: the run-time stride.
+template <typename R, int NSH> struct NucTab {
+  const unsigned char *base;
+  int stride;
+  __device__ __forceinline__ const NucDev<R> &operator[](int t) const {
+    const size_t s = NSH > 0 ? sizeof(NucDev<R>) - sizeof(ShellDev<R>) * (size_t)(kMaxShells - NSH) : (size_t)stride;
+    return *reinterpret_cast<const NucDev<R> *>(base + (size_t)t * s);
+  }
+};
+template <typename R> __host__ __device__ inline size_t model_smem_bytes(int n_xs, int n_stage, int n_shells) {
+  return (size_t)nuc_stride_bytes<R>(n_shells) * (size_t)n_stage + sizeof(R) * 4 * (size_t)n_xs;
 }
 
 template <typename R>
-__device__ __forceinline__ void stage_model(const ModelDev<R> &model, int n_stage, NucDev<R> *s_nuc, R *s_tabS) {
-  const int nw = (int)(sizeof(NucDev<R>) / 4);
+__device__ __forceinline__ void stage_model(const ModelDev<R> &model, int n_stage, int stride, unsigned char *s_nuc, R *s_tabS) {
+  const int nw = stride / 4;
   for (int t = 0; t < n_stage; ++t) {
-    if (!model.nuc[t].live) { if (threadIdx.x == 0) s_nuc[t].live = 0; continue; }
+    uint32_t *dst = reinterpret_cast<uint32_t *>(s_nuc + (size_t)t * (size_t)stride);
+    if (!model.nuc[t].live) { if (threadIdx.x == 0) reinterpret_cast<NucDev<R> *>(dst)->live = 0; continue; }
     const uint32_t *src = reinterpret_cast<const uint32_t *>(&model.nuc[t]);
-    uint32_t *dst = reinterpret_cast<uint32_t *>(&s_nuc[t]);
     for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
   }
   const int nt = model.n_xs * 4;
@@ -340,8 +357,8 @@ __device__ __forceinline__ void stage_model(const ModelDev<R> &model, int n_stag
 }
 
 // validate an event's inputs; on failure write neutral outputs and raise the device error word
-template <typename R>
-__device__ __forceinline__ bool check_inputs(const CascadeParams<R> &P, const NucDev<R> *s_nuc, int ev, R E_in, int tgt, int ptype) {
+template <typename R, typename TAB>
+__device__ __forceinline__ bool check_inputs(const CascadeParams<R> &P, const TAB &s_nuc, int ev, R E_in, int tgt, int ptype) {
   unsigned err = 0;
   if (ptype != 0 && ptype != 1) err |= 8u;
   if (!(E_in >= R(INC_E_MIN) && E_in <= R(INC_E_MAX))) err |= 1u;

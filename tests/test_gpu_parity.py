@@ -740,3 +740,23 @@ def test_fp64_edge_targets_and_energies(gpu, orc, otables, ptables):
     _assert_conservation(g, targets, tid, E, orc, otables, 1e-12, 1e-9, projectile=proj)
     g32 = gpu.simulate(gpu.load("f32"), targets, E, tid, seed, ptables, projectile=proj)
     _assert_conservation(g32, targets, tid, E, orc, otables, 2e-6, 2e-4, projectile=proj)
+
+
+def test_ten_live_targets(gpu, orc, otables, ptables):
+    """Ten live target slots (a tissue mix: C, N, O, Na, Mg, P, S, K, Ca, Fe-like): the staged nucleus records are
+    truncated after their last shell, so ten of them fit beside the wavefront kernel's queues; the fp64 build equals the
+    oracle event by event, and the result does not depend on the cascade kernel variant."""
+    targets = [(12, 6), (14, 7), (16, 8), (23, 11), (24, 12), (31, 15), (32, 16), (39, 19), (40, 20), (56, 26)]
+    n = 12000
+    rng = np.random.default_rng(5)
+    tid = rng.integers(0, len(targets), n).astype(np.int32)
+    E = rng.uniform(70.0, 250.0, n)
+    lib = gpu.load("f64")
+    g = gpu.simulate(lib, targets, E, tid, 9, ptables)
+    o = orc.simulate(otables, targets, E, tid, 9)
+    frac, max_err, ident = H.event_identity(g, o, rel=REL_F64)
+    assert frac >= FRAC_IDENTICAL and max_err <= REL_F64
+    _assert_conservation(g, targets, tid, E, orc, otables, 1e-12, 1e-9)
+    alt = gpu.simulate(lib, targets, E, tid, 9, ptables, flags=gpu.F_LANE_STATE_MACHINE)
+    for k in ("species", "T", "counts", "A", "Z", "Estar", "status"):
+        assert np.array_equal(g[k], alt[k]), k
