@@ -55,6 +55,9 @@ template <typename R> struct __align__(16) LdDev {
   R lnT, lna4;    // ln T, (1/4) ln a
 };
 template <typename R> struct GaussNodes { R x[16], w[16]; };
+template <typename R> struct __align__(16) GemNode { R l0, d0, l1, d1; };
+constexpr int kGemPoints = 1281;        // table points per daughter nucleus: X = E_x .. E_x + 320 MeV
+#define INC_GEM_STEP 0.25               // MeV
 __constant__ GaussNodes<INC_REAL> c_gl;     // 16-point Gauss-Legendre on [-1, 1] (width integral of the GEM mode)
 
 template <typename R> struct ModelDev {
@@ -64,6 +67,11 @@ template <typename R> struct ModelDev {
   const EvChan<R> *evp;   // [kAmax][kZmax][8] by PARENT (A, Z): entries 0-5 the channels' constants (of the daughters
                           // (A - A_j, Z - Z_j); pref = 0: channel closed), entry 6: V = B(A, Z), entry 7 unused
   const LdDev<R> *ld;     // [kAmax][kZmax]  (level_density = 1 only)
+  // GEM width integrals (R-G5) as tables built at inc_init: for daughter row r = ldrow[A_d * kZmax + Z_d] (-1: none) and
+  // X_k = E_x + k * kGemStep, gtab[r * kGemPoints + k] = {ln J0, d ln J0 / dX, ln J1, d ln J1 / dX} with
+  // J0(X) = int_0^X rho(U) dU and J1(X) = int_0^X (X - U) rho(U) dU, so that int_0^X (x + beta) rho(X - x) dx = J1 + beta J0
+  const int32_t *ldrow;
+  const GemNode<R> *gtab;
   const NucDev<R> *nuc;   // [INC_MAX_TARGETS]
   int32_t n_xs;
   R inv_dp;               // 1 / (grid step in MeV/c)

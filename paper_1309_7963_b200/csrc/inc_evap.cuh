@@ -90,6 +90,38 @@ enum EvapMode : int { kEvapKernel = 0, kEvapHelper = 1, kEvapDrainOnly = 2 };
 // The persistent-lane evaporation loop as an object, so that two hosts can run it: the evaporation kernel (one pass after
 // the other until the completion list is exhausted) and the idle warps of the cascade kernel (a pass whenever they have
 // nothing else to do: DESIGN.md section 6).  State = one nucleus per lane + the warp's pool of completion-list entries.
+// ln J0(X), ln J1(X) of a daughter nucleus (R-G5; ModelDev::gtab): elementary below E_x (constant temperature), cubic
+// Hermite interpolation of the tables built at inc_init above.  Returns false if X lies beyond the table (the caller then
+// integrates directly).  The interpolation error (~1e-8 in the logarithm at a 0.25 MeV step) only enters the channel
+// choice; emission energies come from the sampler, which uses ln rho itself.
+template <typename R>
+__device__ __forceinline__ bool gem_lnJ(const ModelDev<R> &md, const LdDev<R> &ld, int row, R X, R &l0, R &l1) {
+  const R Xs = ld.Ex > R(0) ? ld.Ex : R(0);
+  if (X <= Xs) {
+    const R z = M<R>::div_(X, ld.T);
+    const R em = M<R>::expm1_(z);                      // e^z - 1
+    R em2 = em - z;                                    // e^z - 1 - z (series where the difference cancels)
+    if (z < R(0.5)) em2 = R(0.5) * z * z * (R(1) + z * R(1.0 / 3.0) * (R(1) + z * R(0.25) * (R(1) + z * R(0.2) * (R(1) + z * R(1.0 / 6.0) *
+                          (R(1) + z * R(1.0 / 7.0) * (R(1) + z * R(0.125) * (R(1) + z * R(1.0 / 9.0) * (R(1) + z * R(0.1)))))))));
+    const R base = -M<R>::div_(ld.E0, ld.T);
+    l0 = base + M<R>::log_(em);
+    l1 = base + ld.lnT + M<R>::log_(em2);
+    return true;
+  }
+  if (row < 0) return false;
+  const R t = (X - Xs) * R(1.0 / INC_GEM_STEP);
+  const int k = (int)t;
+  if (k >= kGemPoints - 1) return false;
+  const R f = t - R(k);
+  const GemNode<R> n0 = md.gtab[(size_t)row * kGemPoints + k], n1 = md.gtab[(size_t)row * kGemPoints + k + 1];
+  const R f2 = f * f, f3 = f2 * f;
+  const R h00 = R(2) * f3 - R(3) * f2 + R(1), h10 = (f3 - R(2) * f2 + f) * R(INC_GEM_STEP);
+  const R h01 = R(3) * f2 - R(2) * f3, h11 = (f3 - f2) * R(INC_GEM_STEP);
+  l0 = h00 * n0.l0 + h10 * n0.d0 + h01 * n1.l0 + h11 * n1.d0;
+  l1 = h00 * n0.l1 + h10 * n0.d1 + h01 * n1.l1 + h11 * n1.d1;
+  return true;
+}
+
 template <typename R, bool STATS, bool GEM>
 struct EvapLanes {
   static constexpr int kTrialsPerPass = 2;
@@ -228,6 +260,7 @@ struct EvapLanes {
       EvChan<R> ch[6];
       R s_ref = R(0);
       bool any = false;
+      bool direct = false;          // GEM mode: some channel's X lies beyond its table
 #pragma unroll
       for (int j = 0; j < 6; ++j) {
         const int Ad = A - c_evA[j], Zd = Z - c_evZ[j];
@@ -245,8 +278,12 @@ struct EvapLanes {
                 if (ld.a > R(0)) {
                   ch[j] = c;
                   Xj[j] = Xc;
-                  sj[j] = gem_lnrho<R>(ld, Xc);
-                  s_ref = (!any || sj[j] > s_ref) ? sj[j] : s_ref;
+                  // sj, aj = ln J0, ln J1 from the tables; a channel beyond its table makes the step integrate directly
+                  R l0, l1;
+                  if (!gem_lnJ<R>(P.model, ld, P.model.ldrow[Ad * kZmax + Zd], Xc, l0, l1)) { direct = true; l0 = l1 = R(0); }
+                  sj[j] = l0; aj[j] = l1;
+                  const R lm = l0 > l1 ? l0 : l1;
+                  s_ref = (!any || lm > s_ref) ? lm : s_ref;
                   any = true;
                 }
               }
@@ -267,15 +304,33 @@ struct EvapLanes {
         if (STATS) n_steps++;
         R W[6];
         R Wsum = R(0);
+        R dref = R(0);              // direct GEM quadrature in f32: common scale = the largest ln rho_j(X_j)
+        if (GEM && direct && sizeof(R) == 4) {
+          bool first = true;
+#pragma unroll
+          for (int j = 0; j < 6; ++j) {
+            if (Xj[j] > R(0)) {
+              const R l = gem_lnrho<R>(P.model.ld[((A - c_evA[j]) * kZmax + (Z - c_evZ[j]))], Xj[j]);
+              dref = (first || l > dref) ? l : dref;
+              first = false;
+            }
+          }
+        }
 #pragma unroll
         for (int j = 0; j < 6; ++j) {
           W[j] = R(0);
           if (GEM) {
             if (Xj[j] > R(0)) {
-              // R-G5: W_j = g_j M_j A_d^(2/3) alpha_j int_0^X (x + beta) rho(X - x) dx by quadrature (the f64 build
-              // leaves the integrand unscaled, like the oracle)
-              const LdDev<R> ld = P.model.ld[((A - c_evA[j]) * kZmax + (Z - c_evZ[j]))];
-              const R w = ch[j].pref * gem_integral<R>(ld, Xj[j], ch[j].beta, sizeof(R) == 4 ? s_ref : R(0));
+              // R-G5: W_j = g_j M_j A_d^(2/3) alpha_j int_0^X (x + beta) rho(X - x) dx = ... (J1 + beta J0), from the
+              // tables (scaled by the largest ln J of the step); by direct quadrature if a channel is beyond its table
+              R w;
+              if (direct) {
+                const LdDev<R> ld = P.model.ld[((A - c_evA[j]) * kZmax + (Z - c_evZ[j]))];
+                w = ch[j].pref * gem_integral<R>(ld, Xj[j], ch[j].beta, sizeof(R) == 4 ? gem_lnrho<R>(ld, Xj[j]) : R(0));
+                if (sizeof(R) == 4) w *= M<R>::exp_(gem_lnrho<R>(ld, Xj[j]) - dref);
+              } else {
+                w = ch[j].pref * (M<R>::exp_(aj[j] - s_ref) + ch[j].beta * M<R>::exp_(sj[j] - s_ref));
+              }
               W[j] = w > R(0) ? w : R(0);
               Wsum += W[j];
             }

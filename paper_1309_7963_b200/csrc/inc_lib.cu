@@ -55,6 +55,8 @@ struct State {
   real *d_tabS = nullptr, *d_tabC = nullptr, *d_bind = nullptr;
   EvChan<real> *d_evch = nullptr;
   LdDev<real> *d_ld = nullptr;
+  int32_t *d_ldrow = nullptr;       // GEM width tables (level_density = 1)
+  GemNode<real> *d_gtab = nullptr;
   NucDev<real> *d_nuc = nullptr;
   DevCounters *d_ctr = nullptr;
   uint32_t *d_wtrace = nullptr; int wtrace_warps = 0;   // inc_get_warp_trace (INC_F_TIMING)
@@ -380,6 +382,75 @@ int upload_model() {
       }
     std::vector<double> gx, gw;
     gauss_legendre(16, gx, gw);
+    // R-G5 tables: J0(X) = int_0^X rho, J1(X) = int_0^X (X - U) rho(U) dU per daughter nucleus, X = E_x + k h.  Below E_x the
+    // density is the constant-temperature form and both are elementary (the kernel evaluates them directly); from E_x on
+    // they are accumulated interval by interval with the 16-point rule on the Fermi-gas density:
+    //   J0(X + h) = J0(X) + int_X^{X+h} rho,   J1(X + h) = J1(X) + h J0(X) + int_X^{X+h} (X + h - U) rho(U) dU.
+    // The kernel interpolates ln J0 and ln J1 (cubic Hermite with the exact derivatives rho / J0 and J0 / J1).
+    {
+      std::vector<int32_t> ldrow((size_t)kAmax * kZmax, -1);
+      int rows = 0;
+      for (size_t i = 0; i < ldv.size(); ++i) if (ldv[i].a > (real)0) ldrow[i] = rows++;
+      std::vector<GemNode<real>> gt((size_t)(rows > 0 ? rows : 1) * kGemPoints);
+      const double h = INC_GEM_STEP;
+      auto tab = [](const std::vector<double> &y, int i) { return (i >= 0 && i < (int)y.size()) ? y[i] : 0.0; };
+      for (int Ad = 1; Ad < kAmax; ++Ad)
+        for (int Zd = 0; Zd < kZmax && Zd <= Ad; ++Zd) {
+          const int r = ldrow[(size_t)Ad * kZmax + Zd];
+          if (r < 0) continue;
+          // (the constants again in double: the table must not inherit the f32 rounding of LdDev)
+          const double S = tab(t.shell_Z, Zd) + tab(t.shell_N, Ad - Zd);
+          const double a = (double)Ad * (t.gc_a0 + t.gc_a1 * S), delta = tab(t.pair_Z, Zd) + tab(t.pair_N, Ad - Zd);
+          const double Ux = 150.0 / (double)Ad + 2.5, Ex = Ux + delta;
+          const double T = 1.0 / (std::sqrt(a / Ux) - 1.5 / Ux);
+          const double E0 = Ex - T * (std::log(T) - 0.25 * std::log(a) - 1.25 * std::log(Ux) + 2.0 * std::sqrt(a * Ux));
+          auto lnrho_fg = [&](double U) { const double u = U - delta; return 2.0 * std::sqrt(a * u) - 0.25 * std::log(a) - 1.25 * std::log(u); };
+          // at E_x from the constant-temperature forms (E_x <= 0 can happen with negative pairing inputs: start from 0)
+          double X = Ex, J0, J1;
+          if (Ex > 0.0) {
+            const double z = Ex / T, c = std::exp(-E0 / T);
+            J0 = c * std::expm1(z);
+            J1 = c * T * (std::expm1(z) - z);
+          } else { X = 0.0; J0 = 0.0; J1 = 0.0; }
+          // scaled by e^{-ref} to stay in range whatever the inputs: ref follows the running maximum of ln rho
+          GemNode<real> *row = &gt[(size_t)r * kGemPoints];
+          double ref = 0.0;                       // J0, J1 hold the true values times e^{-ref}
+          for (int k = 0; k < kGemPoints; ++k) {
+            const double Xk = X + k * h;
+            if (k > 0) {
+              const double Xa = Xk - h;
+              double A0 = 0, A1 = 0;
+              const double lr = lnrho_fg(Xk > delta + 1e-9 ? Xk : delta + 1e-9);
+              const double nref = lr > ref ? lr : ref;
+              const double sc = std::exp(ref - nref);
+              J0 *= sc; J1 *= sc; ref = nref;
+              for (int q = 0; q < 16; ++q) {
+                const double U = Xa + 0.5 * h * (gx[q] + 1.0);
+                const double u = U - delta;
+                const double rho = u > 0.0 ? std::exp(lnrho_fg(U) - ref) : 0.0;
+                A0 += 0.5 * h * gw[q] * rho;
+                A1 += 0.5 * h * gw[q] * (Xk - U) * rho;
+              }
+              J1 += h * J0 + A1;
+              J0 += A0;
+            }
+            const double rhoX = Xk >= Ex ? ((Xk - delta) > 0.0 ? std::exp(lnrho_fg(Xk) - ref) : 0.0) : std::exp((Xk - E0) / T - std::log(T) - ref);
+            const bool ok = J0 > 0.0 && J1 > 0.0;
+            row[k].l0 = (real)(ok ? std::log(J0) + ref : -1e30);
+            row[k].l1 = (real)(ok ? std::log(J1) + ref : -1e30);
+            row[k].d0 = (real)(ok ? rhoX / J0 : 0.0);
+            row[k].d1 = (real)(ok ? J0 / J1 : 0.0);
+          }
+        }
+      auto up2 = [&](void **dst, const void *src, size_t bytes) -> cudaError_t {
+        if (*dst) cudaFree(*dst);
+        cudaError_t e = cudaMalloc(dst, bytes);
+        if (e != cudaSuccess) return e;
+        return cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice);
+      };
+      CU_TRY(up2((void **)&g.d_ldrow, ldrow.data(), ldrow.size() * sizeof(int32_t)));
+      CU_TRY(up2((void **)&g.d_gtab, gt.data(), gt.size() * sizeof(GemNode<real>)));
+    }
     // (nodes in the order of the Newton start values cos(pi (i + 3/4) / 16.5), i = 0..15, so that a panel sum runs in one fixed order)
     GaussNodes<real> gn;
     for (int i = 0; i < 16; ++i) { gn.x[i] = (real)gx[i]; gn.w[i] = (real)gw[i]; }
@@ -422,7 +493,7 @@ int upload_model() {
 
 ModelDev<real> model_dev() {
   ModelDev<real> m;
-  m.tabS = g.d_tabS; m.tabC = g.d_tabC; m.bind = g.d_bind; m.evp = g.d_evch; m.nuc = g.d_nuc; m.ld = g.d_ld;
+  m.tabS = g.d_tabS; m.tabC = g.d_tabC; m.bind = g.d_bind; m.evp = g.d_evch; m.nuc = g.d_nuc; m.ld = g.d_ld; m.ldrow = g.d_ldrow; m.gtab = g.d_gtab;
   m.n_xs = g.tab.n_xs;
   m.inv_dp = (real)(1.0 / (g.tab.plab_max / (g.tab.n_xs - 1) * 1000.0));
   m.a_div = (real)g.tab.evap_a_div;
@@ -693,7 +764,7 @@ int inc_free_target(int id) {
 
 void inc_shutdown(void) {
   free_ws();
-  void **p[] = {(void **)&g.d_tabS, (void **)&g.d_tabC, (void **)&g.d_bind, (void **)&g.d_evch, (void **)&g.d_ld, (void **)&g.d_nuc,
+  void **p[] = {(void **)&g.d_tabS, (void **)&g.d_tabC, (void **)&g.d_bind, (void **)&g.d_evch, (void **)&g.d_ld, (void **)&g.d_ldrow, (void **)&g.d_gtab, (void **)&g.d_nuc,
                 (void **)&g.d_ctr, (void **)&g.d_wtrace, (void **)&g.d_offsets, (void **)&g.d_tiles};
   for (auto q : p) { if (*q) cudaFree(*q); *q = nullptr; }
   g.offsets_cap = g.tiles_cap = 0;
