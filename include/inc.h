@@ -114,7 +114,7 @@ typedef struct inc_tables {   /* HOST memory, caller-owned, copied during inc_in
    * (the paper prints none): delta = pair_Z[Z_d] + pair_N[N_d]; a = A_d (gc_a0 + gc_a1 (shell_Z[Z_d] + shell_N[N_d]));
    * indices beyond the arrays count as 0; a <= 0 closes the channel.  It changes the emission widths (E2) and the
    * energy sampler (E4) only.  inc_init then also builds per-nucleus tables of the width integrals (about a second of
-   * host time and 30 MB (f32) / 60 MB (f64) of device memory). */
+   * host time and 55 MB (f32) / 110 MB (f64) of device memory). */
   int32_t level_density;
   int32_t n_ldZ, n_ldN;              /* lengths of the arrays below (may be 0 with NULL pointers)            */
   const double *pair_Z, *pair_N;     /* [n_ldZ], [n_ldN] pairing energies, MeV                               */
