@@ -386,6 +386,8 @@ def main():
         del out
         for c in (1, 2, 3, 4, 5):
             per_config[str(c)] = config_line(c, peak, B, T, W, np, torch, oracle=not args.no_cpu_baseline)
+        # the same headline workload with the GEM level density (NEXT-2; no pairing / shell arrays: the uncorrected a = A/8)
+        per_config["2_gem"] = config_line(2, peak, B, T, W, np, torch, oracle=False, tables_kw=dict(level_density=1))
         lib.inc_shutdown()
 
     cpu_baseline = None
@@ -419,13 +421,13 @@ def main():
         dist.destroy_process_group()
 
 
-def config_line(c, peak, B, T, W, np, torch, steps=3, oracle=True):
+def config_line(c, peak, B, T, W, np, torch, steps=3, oracle=True, tables_kw=None):
     """One BASELINE.json config: events/s of the whole step (production build, device-resident, `steps` steps after two
     warm-ups), the cascade kernel's roofline fraction (INC_F_TIMING steps), and the fp64 parity build's events/s."""
     n = W.CONFIGS[c]["n"]
     E, tid, targets, seed, name = W.make_inputs(c, n)
-    tables = T.default_tables()
-    res = dict(workload=name, events=n)
+    tables = T.default_tables(**(tables_kw or {}))
+    res = dict(workload=name + (" [GEM level density]" if tables_kw else ""), events=n)
     for variant in ("f32", "f64"):
         lib = B.load(variant)
         lib.inc_shutdown()
