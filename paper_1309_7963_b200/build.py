@@ -29,8 +29,9 @@ VARIANTS = {
     # test build: the f64 library with very small per-warp queues, so that the capacity guards of the wavefront
     # scheduler (partial collision passes, lane-capped segment passes, admission control) run all the time
     # ... with every queue / ring / slot index checked (INC_CHECKED: error bit 32 -> INC_E_STATE), and with 4 instead of
-    # 16 staged records in an event's own row, so that the staging overflow pool is in constant use
-    "f64q": ["-DINC_REAL_IS_DOUBLE", "-fmad=false", "-DINC_WNS=40", "-DINC_WQS=64", "-DINC_WQC=33", "-DINC_WWARPS=8", "-DINC_CHECKED", "-DINC_STAGE_MAIN=4"],
+    # 16 staged records in an event's own row, so that the staging overflow pool is in constant use, and with GEM width
+    # tables that end 30 MeV above E_x, so that the direct-quadrature fallback of the GEM mode runs
+    "f64q": ["-DINC_REAL_IS_DOUBLE", "-fmad=false", "-DINC_WNS=40", "-DINC_WQS=64", "-DINC_WQC=33", "-DINC_WWARPS=8", "-DINC_CHECKED", "-DINC_STAGE_MAIN=4", "-DINC_GEM_POINTS=121"],
 }
 
 

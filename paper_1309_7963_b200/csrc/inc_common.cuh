@@ -56,7 +56,10 @@ template <typename R> struct __align__(16) LdDev {
 };
 template <typename R> struct GaussNodes { R x[16], w[16]; };
 template <typename R> struct __align__(16) GemNode { R l0, d0, l1, d1; };
-constexpr int kGemPoints = 1281;        // table points per daughter nucleus: X = E_x .. E_x + 320 MeV
+#ifndef INC_GEM_POINTS
+#define INC_GEM_POINTS 1281             // (the checked test build uses 121, so that most steps take the direct-quadrature fallback)
+#endif
+constexpr int kGemPoints = INC_GEM_POINTS;   // table points per daughter nucleus: X = E_x .. E_x + 320 MeV
 #define INC_GEM_STEP 0.25               // MeV
 __constant__ GaussNodes<INC_REAL> c_gl;     // 16-point Gauss-Legendre on [-1, 1] (width integral of the GEM mode)
 

@@ -558,6 +558,20 @@ def test_gem_fp64_identity(gpu, orc, ptables, cfg, n):
         assert np.array_equal(base[k], old[k]), k
 
 
+def test_gem_direct_quadrature_fallback(gpu, orc):
+    """GEM widths beyond the end of a table are integrated directly (16-point rule of R-G5).  The f64q test build's tables
+    end 30 MeV above E_x, so most emission steps of 250 MeV p-48Ti take that path: still the oracle's events."""
+    import paper_1309_7963_b200.tables as T
+    E, tid, targets, seed, _ = _inputs(5, 3000)
+    kw = H.gem_inputs()
+    g = gpu.simulate(gpu.load("f64q"), targets, E, tid, seed, T.default_tables(**kw))
+    o = orc.simulate(orc.Tables(**kw), targets, E, tid, seed)
+    frac, max_err, ident = H.event_identity(g, o, rel=REL_F64)
+    assert frac >= FRAC_IDENTICAL and max_err <= REL_F64, (frac, max_err)
+    ref = gpu.simulate(gpu.load("f64"), targets, E, tid, seed, T.default_tables(**kw))
+    assert (ref["counts"] == g["counts"]).mean() > 0.999          # tables vs direct: the same channel choices
+
+
 @pytest.mark.parametrize("cfg", [2, 5])
 def test_gem_fp32_histograms(gpu, orc, cfg):
     """GEM mode, production build, full-size batch against a 2e5-event oracle sample (criterion (3)), plus exact
