@@ -220,6 +220,27 @@ int64_t inc_simulate_host(int64_t n_events, const INC_REAL *E_in /*HOST*/,
  * the first secondary of event e, dev_offsets[n_events] the total. */
 int inc_get_offsets(int64_t *dev_offsets /*DEVICE [n_events+1]*/);
 
+/* inc_scan_counts_static — the same exclusive prefix sum (the "prefix-sum" step of the compaction, BASELINE.json
+ * north_star) as an entry point that allocates nothing, for callers who cannot let this library call
+ * cudaMalloc.  Those are: a host program that has handed all of the device's memory to an arena of its own (a transport
+ * Monte Carlo with a fixed budget, or a framework allocator holding the whole GPU), where a cudaMalloc from a library
+ * fails or steals from that budget; and a caller inside a latency-critical loop, because cudaMalloc and cudaFree
+ * synchronise the whole device and stall every other stream.  (inc_simulate sizes its workspace with cudaMalloc when it
+ * first sees a batch size; this call never does, and calls no cudaFree or other allocating routine either.)
+ *   counts  DEVICE [n]      per-event numbers of secondaries (e.g. out_counts of inc_simulate), caller-owned, read only
+ *   offsets DEVICE [n + 1]  caller-owned; offsets[e] = counts[0] + ... + counts[e-1], offsets[n] = the total
+ * The scan's scratch (one partial sum per 2048 events and the running total) is a fixed array inside the library,
+ * 64.25 KB of device memory that every GPU which loads the library holds until the process exits.  Hence the limit:
+ * n <= INC_SCAN_STATIC_MAX_EVENTS; a larger n is refused with INC_E_BADARG and a message, nothing is written.
+ * The first call on a device looks up the array's device address (once per device, with the device that is current at
+ * the call): make that first call before any stream capture begins.  All calls share the one array and it keeps the
+ * previous call's contents (the call clears the one word that must start at zero), so two calls whose kernels
+ * overlap on the GPU (issued from two host threads, say) race on it and both results are garbage: serialise them.
+ * Work is enqueued on the inc_set_stream stream and the call returns when it has finished.  Needs no
+ * inc_init.  Returns 0, INC_E_BADARG or INC_E_CUDA. */
+#define INC_SCAN_STATIC_MAX_EVENTS (1 << 24)
+int inc_scan_counts_static(int64_t n, const int32_t *counts /*DEVICE [n]*/, int64_t *offsets /*DEVICE [n+1]*/);
+
 /* Post-cascade nuclei of the last inc_simulate (the paper's "SoA of excited nuclei", P:69,
  * P:83), for stage-level tests: any pointer may be NULL; n_cascade_secondaries[e] is the number of
  * cascade nucleons of event e.  Only after a call that ran as ONE chunk (n_events <= the chunk size):

@@ -20,6 +20,7 @@ F_NO_DRAIN_HELPERS = 256
 F_NO_OVERLAP = 512
 F_TEST_QUEUE_OVF = 1024
 MAX_SEC = 64
+SCAN_STATIC_MAX_EVENTS = 1 << 24
 
 _DP = C.POINTER(C.c_double)
 
@@ -96,7 +97,7 @@ def make_tables_struct(t: dict):
 EXPORTS = ["inc_init", "inc_free_target", "inc_shutdown", "inc_set_stream", "inc_set_flags", "inc_set_event_offset",
            "inc_get_stage_times", "inc_get_drain_timeline", "inc_get_warp_trace", "inc_get_rerun_count", "inc_set_vote_thresholds", "inc_set_long_track_threshold", "inc_set_segments_per_pass", "inc_set_stage_overflow_rows", "inc_set_chunk_events", "inc_set_projectiles", "inc_simulate",
            "inc_simulate_host", "inc_get_offsets", "inc_get_cascade_stage", "inc_get_stats", "inc_get_nucleus",
-           "inc_measure_issue_peak", "inc_philox_blocks", "inc_tally", "inc_last_error", "inc_build_info"]
+           "inc_measure_issue_peak", "inc_philox_blocks", "inc_tally", "inc_scan_counts_static", "inc_last_error", "inc_build_info"]
 
 
 class IncTallySpec(C.Structure):
@@ -136,6 +137,7 @@ class IncLibrary:
             f.argtypes = [C.c_int64, vp, vp, C.c_uint64, C.POINTER(IncSecondaries), vp, C.POINTER(IncResidual)]
             f.restype = C.c_int64
         L.inc_get_offsets.argtypes = [vp]
+        L.inc_scan_counts_static.argtypes = [C.c_int64, vp, vp]
         L.inc_get_cascade_stage.argtypes = [vp] * 7
         L.inc_get_stats.argtypes = [C.POINTER(IncStats)]
         L.inc_get_nucleus.argtypes = [C.c_int] + [vp] * 16
@@ -286,6 +288,14 @@ class IncLibrary:
         off = torch.empty(n + 1, dtype=torch.int64, device="cuda")
         self._check(self.lib.inc_get_offsets(C.c_void_p(off.data_ptr())))
         return off
+
+    def inc_scan_counts_static(self, counts, offsets, n=None, check: bool = True):
+        """Exclusive prefix sum of `counts` (CUDA int32 tensor) into `offsets` (CUDA int64 tensor, n + 1 long, the
+        caller's) through the library's allocation-free entry point: for callers that cannot let the library call
+        cudaMalloc (include/inc.h says who and why).  At most SCAN_STATIC_MAX_EVENTS events per call."""
+        n = counts.numel() if n is None else int(n)
+        rc = self.lib.inc_scan_counts_static(C.c_int64(n), C.c_void_p(counts.data_ptr()), C.c_void_p(offsets.data_ptr()))
+        return self._check(rc) if check else rc
 
     def inc_get_cascade_stage(self, n: int):
         import torch

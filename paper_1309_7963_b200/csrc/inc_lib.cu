@@ -1250,6 +1250,67 @@ int64_t simulate_host_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, 
 
 }  // namespace
 
+// =================================================================================================
+// inc_scan_counts_static: the prefix sum of the per-event counts for callers that must not allocate (include/inc.h).
+// The scan's scratch -- one partial sum per tile of kScanTile events, then the running total -- lives in the array
+// below instead of a cudaMalloc'ed buffer.  It is part of the library image: every GPU that loads the library carries
+// these 64.25 KB from the load until the process ends, whether or not the entry point is ever called.
+// =================================================================================================
+constexpr int kStaticScanTiles = INC_SCAN_STATIC_MAX_EVENTS / kScanTile;        // 8192 tiles of 2048 events
+static_assert(kStaticScanTiles * kScanTile == INC_SCAN_STATIC_MAX_EVENTS, "the maximum is a whole number of tiles");
+// [0, kStaticScanTiles): tile sums, each rewritten by every call that uses the tile; [kStaticScanTiles]: the running
+// total, which a call must find at zero and therefore clears itself (the array keeps what the previous call left)
+static __device__ __align__(256) long long s_scan_scratch[kStaticScanTiles + 32];
+
+namespace {
+
+// In host code `s_scan_scratch` names a host-side shadow of the array, NOT device memory: handing it to a kernel would
+// fault (or, on a system whose GPU can read host memory, quietly scan into the wrong place).  The device address comes
+// from cudaGetSymbolAddress, asked once per device with that device current, and is kept here by device ordinal.
+constexpr int kMaxDevices = 64;
+long long *g_scan_scratch_dev[kMaxDevices] = {};
+
+int static_scan_scratch(long long **out) {
+  int dev = -1;
+  CU_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return fail(INC_E_CUDA, "inc_scan_counts_static: device ordinal beyond 63");
+  if (!g_scan_scratch_dev[dev]) {
+    void *p = nullptr;
+    CU_TRY(cudaGetSymbolAddress(&p, s_scan_scratch));
+    if (!p) return fail(INC_E_CUDA, "inc_scan_counts_static: cudaGetSymbolAddress gave no address");
+    g_scan_scratch_dev[dev] = static_cast<long long *>(p);
+  }
+  *out = g_scan_scratch_dev[dev];
+  return 0;
+}
+
+}  // namespace
+
 extern "C" {
+
+int inc_scan_counts_static(int64_t n, const int32_t *counts, int64_t *offsets) {
+  if (n < 0 || !offsets || (n > 0 && !counts)) return fail(INC_E_BADARG, "inc_scan_counts_static: null pointer or n < 0");
+  if (n > (int64_t)INC_SCAN_STATIC_MAX_EVENTS) {
+    char buf[200];
+    std::snprintf(buf, sizeof buf, "inc_scan_counts_static: n = %lld is beyond the %d events its fixed scratch array holds "
+                  "(split the call, or use inc_get_offsets)", (long long)n, (int)INC_SCAN_STATIC_MAX_EVENTS);
+    return fail(INC_E_BADARG, buf);
+  }
+  long long *scratch = nullptr;
+  if (int rc = static_scan_scratch(&scratch)) return rc;
+  long long *total = scratch + kStaticScanTiles;
+  long long *off = reinterpret_cast<long long *>(offsets);
+  CU_TRY(cudaMemsetAsync(total, 0, sizeof(long long), g.stream));                 // the previous call's total is still there
+  if (n > 0) {
+    const int tiles = (int)((n + kScanTile - 1) / kScanTile);
+    scan_tile_sums<<<tiles, kScanBlock, 0, g.stream>>>(counts, (int)n, scratch);
+    scan_tiles<<<1, kScanBlock, 0, g.stream>>>(scratch, tiles, reinterpret_cast<unsigned long long *>(total));
+    scan_write_offsets<<<tiles, kScanBlock, 0, g.stream>>>(counts, (int)n, scratch, off);
+    CU_TRY(cudaGetLastError());
+  }
+  CU_TRY(cudaMemcpyAsync(off + n, total, sizeof(long long), cudaMemcpyDeviceToDevice, g.stream));
+  CU_TRY(cudaStreamSynchronize(g.stream));
+  return 0;
+}
 
 }  // extern "C"
