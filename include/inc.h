@@ -227,7 +227,8 @@ int inc_get_offsets(int64_t *dev_offsets /*DEVICE [n_events+1]*/);
  * fails or steals from that budget; and a caller inside a latency-critical loop, because cudaMalloc and cudaFree
  * synchronise the whole device and stall every other stream.  (inc_simulate sizes its workspace with cudaMalloc when it
  * first sees a batch size; this call never does, and calls no cudaFree or other allocating routine either.)
- *   counts  DEVICE [n]      per-event numbers of secondaries (e.g. out_counts of inc_simulate), caller-owned, read only
+ *   counts  DEVICE [n]      per-event numbers of secondaries (e.g. out_counts of inc_simulate), caller-owned, read only;
+ *                           a value outside [0, INC_MAX_SEC] is read as the nearer end of that range, as everywhere in the library
  *   offsets DEVICE [n + 1]  caller-owned; offsets[e] = counts[0] + ... + counts[e-1], offsets[n] = the total
  * The scan's scratch (one partial sum per 2048 events and the running total) is a fixed array inside the library,
  * 64.25 KB of device memory that every GPU which loads the library holds until the process exits.  Hence the limit:

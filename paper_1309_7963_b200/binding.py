@@ -350,7 +350,7 @@ def load(variant: str = "f32") -> IncLibrary:
 
 
 def simulate(lib: IncLibrary, targets, E_in_np, target_idx_np, seed, tables: dict, flags: int = 0, capacity_per_event: int = 24,
-             chunk_events: int = 1 << 22, projectile=None, event_offset: int = 0):
+             chunk_events: int = 1 << 22, projectile=None, event_offset: int = 0, prefill_counts=None):
     """Convenience used by tests/bench: init targets, run on the GPU, return numpy arrays.
     targets: list of (A,Z); target_idx_np indexes that list."""
     import torch
@@ -366,6 +366,8 @@ def simulate(lib: IncLibrary, targets, E_in_np, target_idx_np, seed, tables: dic
     lib.inc_set_projectiles(None if projectile is None else torch.as_tensor(np.asarray(projectile, dtype=np.uint8), device="cuda"))
     cap = max(64, n * capacity_per_event)
     out = lib.alloc_outputs(n, cap)
+    if prefill_counts is not None:          # tests: every byte of the caller's counts buffer holds this value at the call
+        out["counts"].view(torch.uint8).fill_(int(prefill_counts))
     try:
         total = lib.inc_simulate(E, tid, seed, out)
     finally:

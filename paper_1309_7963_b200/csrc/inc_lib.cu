@@ -95,11 +95,11 @@ struct State {
   size_t host_chunk_events = (size_t)1 << 19;
   // last call
   long long last_n = -1;
-  int last_chunks = 0;
+  int last_chunks = 0;              // chunks of the last inc_simulate (the cascade stage survives single-chunk calls only)
   bool last_offsets_valid = false;  // inc_get_offsets: the last call left the offsets of the whole call on the device
-  long long reruns = 0;
+  long long reruns = 0;             // calls run again: lane kernel after a queue overflow of the wavefront kernel, or a larger pool
   bool ovf_all = false;             // a call has exhausted the staging overflow pool: from then on a row for every event
-  long long ovf_rows_user = 0;      // inc_set_stage_overflow_rows (0 = automatic)             // calls run again with the lane kernel after a queue overflow of the wavefront kernel              // chunks of the last inc_simulate (the cascade stage survives single-chunk calls only)
+  long long ovf_rows_user = 0;      // inc_set_stage_overflow_rows (0 = automatic)
   long long last_total = 0;
   long long event_offset = 0;
   // stage timing (INC_F_TIMING)
@@ -140,7 +140,7 @@ bool valid_nucleus(int A, int Z) {
 
 double binding(int A, int Z, const TablesHost &t) {
   static const double light[5][3] = {{0, 0, 0}, {0, 0, 0}, {0, 2.224566, 0}, {0, 8.481798, 7.718043}, {0, 0, 28.29566}};
-  if (A <= 4) return light[A][Z];
+  if (A <= 4) return (A >= 0 && Z >= 0 && Z <= 2) ? light[A][Z] : 0.0;
   const double a = A, z = Z, a13 = std::cbrt(a);
   double B = t.semf[0] * a - t.semf[1] * a13 * a13 - t.semf[2] * z * (z - 1.0) / a13 -
              t.semf[3] * (a - 2.0 * z) * (a - 2.0 * z) / a;
@@ -626,6 +626,10 @@ int launch_chunk(long long e_base, int n_chunk, const real *E_in, const int32_t 
   CU_TRY(cudaMemsetAsync(&L.ctr->next_event_casc, 0, 4 * sizeof(unsigned long long), L.stream));   // + next_event_evap, n_done, ovf_next
   CU_TRY(cudaMemsetAsync(L.ws.ovf_id, 0xFF, (size_t)n_chunk * sizeof(int32_t), L.stream));         // -1: no overflow row
   CU_TRY(cudaMemsetAsync(L.ws.done_list, 0xFF, (size_t)n_chunk * sizeof(uint32_t), L.stream));      // kNotDone
+  // the evaporation kernel writes the count of every event it finishes; if the cascade kernel gives up (queue overflow,
+  // watchdog, failed index check) the events it abandoned are never finished, and the scan and the compaction, which are
+  // enqueued all the same, must find zeros there rather than whatever the caller's buffer held
+  CU_TRY(cudaMemsetAsync(counts, 0, (size_t)n_chunk * sizeof(int32_t), L.stream));
   if (mark(timing)) return INC_E_CUDA;
   if (lane_kernel) {
     const size_t smem = model_smem_bytes<real>(model.n_xs, n_stage, wide ? kMaxShells : 15);
@@ -791,33 +795,37 @@ int64_t simulate_host_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, 
                            int32_t *counts, inc_residual *res);
 int resolve_stage_times();
 int64_t device_error(unsigned int err);
+
+// A call that hits one of the two implementation limits of the default configuration is run again, and the rerun can
+// hit the other one (the abandoned first run allocates fewer overflow rows than a complete one needs), so the two
+// recoveries loop: at most three reruns, and an internal code never reaches the caller.
+//  - kPoolOverflow: the staging overflow pool (a row for one event in 64) was too small for this batch: from now on
+//    every event has a row.
+//  - kQueueOverflow: the default cascade kernel keeps its tracks in fixed per-warp queues; a batch that overflows them
+//    (never seen: it takes ~190 simultaneous tracks in one warp's ~80 events) is run with the lane-per-event kernel,
+//    which has no such limit and gives the same events (R-R4: a track's fate depends only on its own draws).
+template <typename F> int64_t run_with_recovery(F once) {
+  const uint32_t f0 = g.flags;
+  int64_t rc = once();
+  for (int rerun = 0; rerun < 3 && (rc == kPoolOverflow || rc == kQueueOverflow); ++rerun) {
+    if (rc == kPoolOverflow) { g.ovf_all = true; g.ovf_rows_user = 0; }
+    else g.flags = (g.flags | INC_F_LANE_STATE_MACHINE) & ~INC_F_TEST_QUEUE_OVF;
+    g.reruns++;
+    rc = once();
+  }
+  g.flags = f0;
+  if (rc == kPoolOverflow) rc = fail(INC_E_STATE, "staging overflow pool exhausted (results invalid)");
+  if (rc == kQueueOverflow) rc = fail(INC_E_STATE, "internal track-queue overflow (results invalid)");
+  g.projectile = nullptr;       // inc_set_projectiles applies to one call
+  return rc;
+}
 }  // namespace
 
 extern "C" {
 
 int64_t inc_simulate(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
                      int32_t *counts, inc_residual *res) {
-  int64_t rc = simulate_once(n, E_in, tid, seed, sec, counts, res);
-  if (rc == kPoolOverflow) {
-    // The staging overflow pool (one row per 16 events) was too small for this batch: from now on every event has a row.
-    g.ovf_all = true; g.ovf_rows_user = 0;
-    g.reruns++;
-    rc = simulate_once(n, E_in, tid, seed, sec, counts, res);
-    if (rc == kPoolOverflow) rc = fail(INC_E_STATE, "staging overflow pool exhausted (results invalid)");
-  }
-  if (rc == kQueueOverflow) {
-    // The default cascade kernel keeps its tracks in fixed per-warp queues; a batch that overflows them (never seen:
-    // it takes ~190 simultaneous tracks in one warp's ~80 events) is run again with the lane-per-event kernel, which
-    // has no such limit and gives the same events (R-R4: a track's fate depends only on its own draws).
-    const uint32_t f = g.flags;
-    g.flags = (f | INC_F_LANE_STATE_MACHINE) & ~INC_F_TEST_QUEUE_OVF;
-    g.reruns++;
-    rc = simulate_once(n, E_in, tid, seed, sec, counts, res);
-    g.flags = f;
-    if (rc == kQueueOverflow) rc = fail(INC_E_STATE, "internal track-queue overflow (results invalid)");
-  }
-  g.projectile = nullptr;       // inc_set_projectiles applies to one call
-  return rc;
+  return run_with_recovery([&]() { return simulate_once(n, E_in, tid, seed, sec, counts, res); });
 }
 
 int64_t inc_get_rerun_count(void) { return g.reruns; }
@@ -843,9 +851,9 @@ int resolve_stage_times() {
 
 // the device error word of a finished call -> 0, kQueueOverflow, or a negative INC_E_* code with its message
 int64_t device_error(unsigned int err) {
-  if (err & 32u) return fail(INC_E_STATE, "checked build: an index of the wavefront kernel's queues was out of range (results invalid)");
   if (err & 16u) return fail(INC_E_STATE, "watchdog: a warp of the wavefront cascade kernel made no progress (results invalid)");
-  if (err & 4u) return kQueueOverflow;
+  if (err & 4u) return kQueueOverflow;       // (before bit 32: the launch was given up, the call is run again with the lane kernel)
+  if (err & 32u) return fail(INC_E_STATE, "checked build: an index of the wavefront kernel's queues was out of range (results invalid)");
   if (err & 64u) return kPoolOverflow;
   if (err) {
     return fail(INC_E_BADARG, std::string("device-side input check failed:") + ((err & 1u) ? " E_in outside [20,250] MeV" : "") +
@@ -1086,23 +1094,7 @@ int inc_philox_blocks(const uint32_t *ctr, uint64_t seed, uint32_t *out, int64_t
 
 int64_t inc_simulate_host(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
                           int32_t *counts, inc_residual *res) {
-  int64_t rc = simulate_host_once(n, E_in, tid, seed, sec, counts, res);
-  if (rc == kPoolOverflow) {         // see inc_simulate
-    g.ovf_all = true; g.ovf_rows_user = 0;
-    g.reruns++;
-    rc = simulate_host_once(n, E_in, tid, seed, sec, counts, res);
-    if (rc == kPoolOverflow) rc = fail(INC_E_STATE, "staging overflow pool exhausted (results invalid)");
-  }
-  if (rc == kQueueOverflow) {        // see inc_simulate
-    const uint32_t f = g.flags;
-    g.flags = (f | INC_F_LANE_STATE_MACHINE) & ~INC_F_TEST_QUEUE_OVF;
-    g.reruns++;
-    rc = simulate_host_once(n, E_in, tid, seed, sec, counts, res);
-    g.flags = f;
-    if (rc == kQueueOverflow) rc = fail(INC_E_STATE, "internal track-queue overflow (results invalid)");
-  }
-  g.projectile = nullptr;
-  return rc;
+  return run_with_recovery([&]() { return simulate_host_once(n, E_in, tid, seed, sec, counts, res); });
 }
 
 }  // extern "C"
@@ -1151,8 +1143,25 @@ int ensure_host_ring(size_t chunk) {
 // and its outputs travel to the host on a second stream while the next chunks compute.  Device memory does not depend
 // on n.  The host learns each chunk's number of secondaries (8 bytes, pinned) behind an event: that fixes where its
 // list goes in the caller's arrays.
+int64_t simulate_host_chunks(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
+                             int32_t *counts, inc_residual *res);
+
+// Every exit, the error exits included, waits for both streams: asynchronous copies into the caller's host buffers and
+// kernels on the ring slots must not be in flight when the caller gets control back and may free or reuse its buffers.
 int64_t simulate_host_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
                            int32_t *counts, inc_residual *res) {
+  const int64_t rc = simulate_host_chunks(n, E_in, tid, seed, sec, counts, res);
+  if (rc < 0) {
+    const std::string msg = g.err;           // (keep the first failure's message)
+    cudaStreamSynchronize(g.stream);
+    if (g.hp.copy_stream) cudaStreamSynchronize(g.hp.copy_stream);
+    g.err = msg;
+  }
+  return rc;
+}
+
+int64_t simulate_host_chunks(int64_t n, const INC_REAL *E_in, const int32_t *tid, uint64_t seed, inc_secondaries *sec,
+                             int32_t *counts, inc_residual *res) {
   if (!g.tab.captured) return fail(INC_E_STATE, "inc_simulate_host before inc_init");
   if (n < 0 || !sec || !res || (n > 0 && (!E_in || !tid || !counts))) return fail(INC_E_BADARG, "null argument or n < 0");
   if (n > 0 && (!res->A || !res->Z || !res->Estar || !res->px || !res->py || !res->pz || !res->status))
@@ -1225,7 +1234,7 @@ int64_t simulate_host_once(int64_t n, const INC_REAL *E_in, const int32_t *tid, 
     const uint8_t *pj = g.projectile ? g.projectile + e0 : nullptr;
     rc = stats ? launch_chunk<true>(e0, nc, sl.E, sl.tid, pj, seed, &ds, sl.counts, &dr, L.offsets)
                : launch_chunk<false>(e0, nc, sl.E, sl.tid, pj, seed, &ds, sl.counts, &dr, L.offsets);
-    if (rc) { cudaStreamSynchronize(L.stream); cudaStreamSynchronize(cs); return rc; }
+    if (rc) return rc;
     CU_TRY(cudaMemcpyAsync(&h.h_tot[c % State::kRing], &L.ctr->total_sec, sizeof(unsigned long long), cudaMemcpyDeviceToHost, L.stream));
     CU_TRY(cudaEventRecord(sl.computed, L.stream));
     // chunk c is enqueued: now wait for chunk c - 1 and send its outputs home while c computes

@@ -13,6 +13,12 @@ constexpr int kScanBlock = 256;
 constexpr int kScanItems = 8;                       // per thread
 constexpr int kScanTile = kScanBlock * kScanItems;  // 2048 events per block
 
+// A per-event count as the scan and the compaction read it: the counts array is caller memory, and a value outside
+// [0, kMaxSec] (an event the evaporation kernel never reached after an abandoned cascade launch, a caller's stale
+// buffer) must not turn into a huge or negative offset: those would send the compaction outside the staging workspace
+// or in front of the caller's arrays.
+__device__ __forceinline__ int clamp_count(int c) { return c < 0 ? 0 : (c > kMaxSec ? kMaxSec : c); }
+
 __device__ __forceinline__ long long block_exclusive_scan(long long v, long long *s_warp, long long &block_total) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   long long incl = v;
@@ -45,7 +51,7 @@ __global__ void __launch_bounds__(kScanBlock) scan_tile_sums(const int32_t *coun
   const int base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
   long long v = 0;
 #pragma unroll
-  for (int i = 0; i < kScanItems; ++i) if (base + i < n) v += counts[base + i];
+  for (int i = 0; i < kScanItems; ++i) if (base + i < n) v += clamp_count(counts[base + i]);
   long long total;
   block_exclusive_scan(v, s_warp, total);
   if (threadIdx.x == 0) tile_sums[blockIdx.x] = total;
@@ -79,7 +85,7 @@ __global__ void __launch_bounds__(kScanBlock) scan_write_offsets(const int32_t *
   int c[kScanItems];
   long long v = 0;
 #pragma unroll
-  for (int i = 0; i < kScanItems; ++i) { c[i] = base + i < n ? counts[base + i] : 0; v += c[i]; }
+  for (int i = 0; i < kScanItems; ++i) { c[i] = base + i < n ? clamp_count(counts[base + i]) : 0; v += c[i]; }
   long long total;
   long long ex = block_exclusive_scan(v, s_warp, total) + tile_sums[blockIdx.x];
 #pragma unroll
@@ -116,7 +122,7 @@ __global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) 
   long long off = 0;
   int cnt = 0, ncs = 0, oid = -1;
   if (e < P.n_chunk) {
-    off = P.offsets[e]; cnt = P.counts[e];
+    off = P.offsets[e]; cnt = clamp_count(P.counts[e]);
     if (cnt > kStageMain) oid = P.ws.ovf_id[e];     // records beyond the event's own row sit in its overflow row
     const NucRec<R> r = P.ws.frec[e];
     ncs = (int)((r.meta >> 8) & 0xFFu);             // cascade secondaries of event e (frec.meta = count | n_casc << 8)
@@ -163,7 +169,7 @@ __global__ void __launch_bounds__(256) compact_kernel(const CompactParams<R> P) 
         for (int l = 0; l < n_casc; ++l) rank += ((stage_at<R>(P.ws, el, l, oid_l)->code & 0xFFFFFFu) < key) ? 1 : 0;
       }
       const long long dst = off_l + rank;
-      if (dst < P.capacity) {
+      if (dst >= 0 && dst < P.capacity) {
         P.species[dst] = sp;
         P.T[dst] = rec.T; P.ux[dst] = rec.ux; P.uy[dst] = rec.uy; P.uz[dst] = rec.uz;
       }

@@ -265,6 +265,19 @@ def test_small_queue_build_and_overflow_rerun(gpu, ptables, cfg, n):
     assert lib.inc_get_rerun_count() == r1 + 1
     for k in keys:
         assert np.array_equal(ref[k], forced[k]), k
+    # The abandoned first run still enqueues the scan and the compaction over the caller's counts buffer, and the
+    # evaporation kernel never writes the counts of the events the cascade kernel gave up: with every byte
+    # of that buffer at 0x7F (huge positive counts) or 0xBF (negative ones) nothing may fault or be written out of
+    # bounds, and the rerun must still give the same events.
+    for fill in (0x7F, 0xBF):
+        r2 = lib.inc_get_rerun_count()
+        forced = gpu.simulate(lib, targets, E, tid, seed, ptables, flags=gpu.F_TEST_QUEUE_OVF, prefill_counts=fill)
+        assert lib.inc_get_rerun_count() == r2 + 1
+        for k in keys:
+            assert np.array_equal(ref[k], forced[k]), (k, fill)
+    again = gpu.simulate(lib, targets, E, tid, seed, ptables, prefill_counts=0xBF)      # and the device is still healthy
+    for k in keys:
+        assert np.array_equal(ref[k], again[k]), k
 
 
 def test_staging_overflow_rows(gpu, ptables):
