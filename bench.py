@@ -190,6 +190,30 @@ def run_reference(args, rank, world):
     print(json.dumps(line))
 
 
+def check_world(gpus: int, world_env, visible=None) -> bool:
+    """--gpus N against the launch: returns True if this process must start N ranks itself (N > 1 and no torchrun
+    environment), False if it is a rank (or N = 1) and the numbers agree.  Anything else stops the run: a line that says
+    n_gpus: 1 for a run asked to use N GPUs, or N ranks sharing fewer than N devices, is never printed."""
+    if world_env is None:
+        if gpus <= 1:
+            return False
+        if visible is None:
+            import torch
+            visible = torch.cuda.device_count()
+        if visible < gpus:
+            raise SystemExit(f"bench.py --gpus {gpus}: only {visible} CUDA device(s) visible; not reporting a {gpus}-GPU number from fewer")
+        return True
+    if int(world_env) != gpus:
+        raise SystemExit(f"bench.py --gpus {gpus} launched with WORLD_SIZE={world_env}: the two must agree")
+    return False
+
+
+def rank_share(rank: int, world: int, n: int, ms_by_rank) -> dict:
+    """The multi-GPU arithmetic of the bench (events are independent): rank r owns global events
+    [r n, (r + 1) n) -- no collective on the data path -- and the job's time is the slowest rank's."""
+    return dict(event_offset=rank * n, ms=max(ms_by_rank), events=world * n)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -211,6 +235,17 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "ours":
+        relaunch = check_world(args.gpus, os.environ.get("WORLD_SIZE"))
+        if relaunch:
+            # started as plain `python bench.py --gpus N`: start the N ranks ourselves (one process per GPU)
+            import socket
+            with socket.socket() as sk:
+                sk.bind(("127.0.0.1", 0))
+                port = sk.getsockname()[1]
+            cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+                   "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+            os.execv(sys.executable, cmd)
 
     if args.impl == "reference":
         run_reference(args, rank, world)
@@ -245,7 +280,7 @@ def main():
     tid_d = torch.as_tensor(slots[tid], device="cuda")
     cap = n * 16
     out = lib.alloc_outputs(n, cap)
-    lib.inc_set_event_offset(rank * n)      # weak scaling: rank r owns global events [r n, (r+1) n)
+    lib.inc_set_event_offset(rank_share(rank, world, n, [0.0])["event_offset"])      # weak scaling: rank r owns global events [r n, (r+1) n)
 
     def barrier():
         if dist is not None:
@@ -347,6 +382,18 @@ def main():
     if dist is not None:
         dist.all_reduce(tm, op=dist.ReduceOp.MAX)
     e2e_value = world * n * e2e_steps / float(tm.item())
+    # the host link itself: one 256 MB device-to-host copy into pinned memory, timed (the floor of the e2e number)
+    lk_d = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    lk_h = torch.empty(256 << 20, dtype=torch.uint8).pin_memory()
+    lk_h.copy_(lk_d, non_blocking=True)
+    torch.cuda.synchronize()
+    l0, l1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0.record()
+    lk_h.copy_(lk_d, non_blocking=True)
+    l1.record()
+    torch.cuda.synchronize()
+    d2h_GBps = (256 << 20) / (l0.elapsed_time(l1) * 1e-3) / 1e9
+    del lk_d, lk_h
     rb = E_h.element_size()
     h2d = n * (rb + 4)
     d2h = n * (4 + 4 + 4 + 4 * rb + 4) + tot_h * (1 + 4 * rb)
@@ -402,7 +449,9 @@ def main():
                             l2="no flush: each step writes and re-reads ~0.3 GB (staging records, nucleus records, outputs; new seed every step), above the 126 MB L2",
                             parallelism=f"dp{world} (independent event ranges, no collective)"),
                 clocks=clocks, e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
-                                        steps=e2e_steps),
+                                        steps=e2e_steps, d2h_link_GBps=d2h_GBps,
+                                        link_floor_events_per_s=n / (d2h / (d2h_GBps * 1e9)),
+                                        note="link: one 256 MB device-to-pinned-host copy timed in this run; floor = the step's D2H bytes at that rate"),
                 gpu_launches=int(launches), roofline=roofline, cpu_baseline=cpu_baseline,
                 per_step_ms=dict(best=per_step[0], median=per_step[len(per_step) // 2]),
                 per_config=per_config,
@@ -463,7 +512,11 @@ def config_line(c, peak, B, T, W, np, torch, steps=3, oracle=True, tables_kw=Non
                        roofline_frac=wpe["cascade"] * m / (casc * 1e-3) / peak,
                        whole_step_frac=wpe["total"] * m / (ms * 1e-3) / peak)
         else:
-            res.update(f64_events_per_s=m / (ms * 1e-3), f64_events=m)
+            # the parity build against ITS roofline: the same algorithmic lane-instructions, the DFMA issue peak measured
+            # with this library's own chain microbenchmark
+            peak64, _ = lib.inc_measure_issue_peak()
+            res.update(f64_events_per_s=m / (ms * 1e-3), f64_events=m, f64_ms_per_step=ms, f64_dfma_peak_T_lane_instr_per_s=peak64 / 1e12,
+                       f64_roofline_frac=wpe["total"] * m / (ms * 1e-3) / peak64)
         lib.inc_set_flags(0)
         lib.inc_shutdown()
         del out, E_d, tid_d

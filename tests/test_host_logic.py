@@ -168,3 +168,26 @@ def test_statistics_helpers():
     assert h["T_n"].sum() == 2 and h["T_p"].sum() == 1 and h["T_over_p"] == 1 and h["T_comp"].sum() == 1
     assert h["mult_all"][3] == 1 and h["mult_all"][2] == 1 and h["A_res"][14] == 1
     assert not H.compare_histograms(h, h)
+
+
+def test_bench_gpus_flag_never_underreports():
+    """bench.py --gpus N: without a torchrun environment it starts N ranks itself, and it refuses to run when
+    fewer than N devices are visible or when WORLD_SIZE disagrees -- it can never print n_gpus: 1 for a run asked for N."""
+    import bench
+    assert bench.check_world(1, None) is False
+    assert bench.check_world(2, None, visible=2) is True          # plain `python bench.py --gpus 2` on a 2-GPU node
+    assert bench.check_world(2, "2") is False                     # a rank under torchrun
+    with pytest.raises(SystemExit, match="only 1 CUDA device"):
+        bench.check_world(2, None, visible=1)
+    with pytest.raises(SystemExit, match="must agree"):
+        bench.check_world(8, "2")
+    # the rank arithmetic: disjoint event ranges, the slowest rank's time, the whole job's events
+    sh = [bench.rank_share(r, 4, 1000, [1.0, 3.5, 2.0, 1.5]) for r in range(4)]
+    assert [x["event_offset"] for x in sh] == [0, 1000, 2000, 3000]
+    assert all(x["ms"] == 3.5 and x["events"] == 4000 for x in sh)
+    # and as the driver would start it here (no GPU): a loud failure, not a line
+    env = dict(os.environ, CUDA_VISIBLE_DEVICES="")
+    env.pop("WORLD_SIZE", None)
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1"], env=env,
+                       capture_output=True, text=True, timeout=300)
+    assert r.returncode != 0 and "n_gpus" not in r.stdout and "CUDA device" in r.stderr
