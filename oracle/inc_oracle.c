@@ -414,6 +414,7 @@ int orc_gem_ld(int A_d, int Z_d, const orc_tables *t, orc_ld *ld) {
   ld->Ex = ld->Ux + ld->delta;
   if (!(ld->a > 0.0)) return -1;
   double invT = sqrt(ld->a / ld->Ux) - 1.5 / ld->Ux;
+  if (!(invT > 0.0)) return -1;                    /* R-G7: no constant-temperature branch exists: channel closed */
   ld->T = 1.0 / invT;
   ld->E0 = ld->Ex - ld->T * (log(ld->T) - 0.25 * log(ld->a) - 1.25 * log(ld->Ux) + 2.0 * sqrt(ld->a * ld->Ux));
   return 0;
@@ -465,7 +466,7 @@ double orc_gem_integral(const orc_ld *ld, double X, double beta) {
   double gx[16], gw[16];
   gl16(gx, gw);
   double xs = X - ld->Ex;                          /* x below xs: daughter above E_x (Fermi gas) */
-  if (xs <= 0.0) return gem_range(ld, X, beta, 0.0, X, gx, gw);
+  if (xs <= 0.0 || xs >= X) return gem_range(ld, X, beta, 0.0, X, gx, gw);   /* one branch on all of [0, X] (R-G7: E_x <= 0) */
   return gem_range(ld, X, beta, 0.0, xs, gx, gw) + gem_range(ld, X, beta, xs, X, gx, gw);
 }
 

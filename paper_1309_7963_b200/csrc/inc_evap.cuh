@@ -81,7 +81,7 @@ __device__ __forceinline__ R gem_range(const LdDev<R> &ld, R X, R beta, R x0, R 
 template <typename R>
 __device__ __forceinline__ R gem_integral(const LdDev<R> &ld, R X, R beta, R lref) {
   const R xs = X - ld.Ex;                         // x below xs: daughter above E_x (Fermi gas)
-  if (xs <= R(0)) return gem_range<R>(ld, X, beta, R(0), X, lref);
+  if (xs <= R(0) || xs >= X) return gem_range<R>(ld, X, beta, R(0), X, lref);      // one branch on all of [0, X] (R-G7: E_x <= 0)
   return gem_range<R>(ld, X, beta, R(0), xs, lref) + gem_range<R>(ld, X, beta, xs, X, lref);
 }
 
@@ -112,6 +112,9 @@ __device__ __forceinline__ bool gem_lnJ(const ModelDev<R> &md, const LdDev<R> &l
   const R t = (X - Xs) * R(1.0 / INC_GEM_STEP);
   const int k = (int)t;
   if (k >= kGemPoints - 1) return false;
+  // R-G7: a table of a nucleus with E_x <= 0 starts at X = 0, where J0 = J1 = 0 have no logarithm: its first interval is
+  // integrated directly
+  if (k == 0 && !(ld.Ex > R(0))) return false;
   const R f = t - R(k);
   const GemNode<R> n0 = md.gtab[(size_t)row * kGemPoints + k], n1 = md.gtab[(size_t)row * kGemPoints + k + 1];
   const R f2 = f * f, f3 = f2 * f;

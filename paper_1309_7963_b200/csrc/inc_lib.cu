@@ -375,6 +375,7 @@ int upload_model() {
         if (!(a > 0.0)) continue;                                                   // a = 0 in the table: channel closed
         const double Ex = Ux + delta;
         const double invT = std::sqrt(a / Ux) - 1.5 / Ux;
+        if (!(invT > 0.0)) continue;                                                // R-G7: no constant-temperature branch: closed as well
         const double T = 1.0 / invT;
         const double E0 = Ex - T * (std::log(T) - 0.25 * std::log(a) - 1.25 * std::log(Ux) + 2.0 * std::sqrt(a * Ux));
         d.a = (real)a; d.delta = (real)delta; d.Ux = (real)Ux; d.Ex = (real)Ex; d.T = (real)T; d.E0 = (real)E0;

@@ -191,3 +191,27 @@ def test_gem_events_conserve_and_differ(orc, otables, A, Z, E, corr):
     L = orc.lib()
     for e in range(0, n, 97):
         assert _widths(orc, t, int(g["A"][e]), int(g["Z"][e]), float(g["Estar"][e]))[0] == 0.0
+
+
+def test_gem_degenerate_inputs(orc):
+    """DESIGN.md R-G7: caller inputs that leave no constant-temperature branch (1/T <= 0 with a > 0) close the channel;
+    a pairing input below -U_x (E_x <= 0) puts the daughter on the Fermi-gas branch everywhere, and the width integral is
+    int_0^X (x + beta) rho_FG(X - x) dx over [0, X] only -- checked against scipy.integrate.quad of that integrand."""
+    L = orc.lib()
+    sz = np.zeros(40); sz[6] = -13.0                       # a = A_d (0.125 - 0.1192) > 0, sqrt(a/U_x) < 1.5/U_x
+    t = orc.Tables(level_density=1, shell_Z=sz)
+    ld = orc.OrcLd()
+    assert L.orc_gem_ld(12, 6, C.byref(t.c), C.byref(ld)) == -1
+    a, Ux = 12 * (0.125 + 0.00917 * -13.0), 150.0 / 12 + 2.5
+    assert a > 0 and np.sqrt(a / Ux) - 1.5 / Ux < 0
+    assert L.orc_gem_ld(12, 5, C.byref(t.c), C.byref(ld)) == 0          # the neighbours are untouched
+    tot, W, X = _widths(orc, t, 13, 6, 40.0)[:3]
+    assert W[0] == 0.0 and X[0] < 0 and W[1] > 0.0                      # n (daughter 12,6) closed, p (daughter 12,5) open
+    pz = np.zeros(40); pz[7] = -20.0                       # E_x = U_x - 20 < 0 for Z_d = 7
+    t2 = orc.Tables(level_density=1, pair_Z=pz)
+    ld = _ld(orc, t2, 15, 7)
+    assert ld.Ex < 0
+    for Xv, beta in ((0.1, 0.0), (3.0, 1.5), (25.0, -0.8), (60.0, 2.0)):
+        f = lambda x: (x + beta) * np.exp(2 * np.sqrt(ld.a * (Xv - x - ld.delta)) - 0.25 * np.log(ld.a) - 1.25 * np.log(Xv - x - ld.delta))
+        want = integrate.quad(f, 0.0, Xv, epsabs=0, epsrel=1e-12, limit=200)[0]
+        assert L.orc_gem_integral(C.byref(ld), Xv, beta) == pytest.approx(want, rel=1e-9)
