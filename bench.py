@@ -229,6 +229,7 @@ def main():
     ap.add_argument("--variant", default="f32", choices=["f32", "f64"])
     ap.add_argument("--flags", type=int, default=0)
     ap.add_argument("--vote", type=int, nargs=2, default=None)
+    ap.add_argument("--taper", type=int, default=None, help="inc_set_event_taper (scheduling experiment)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -275,6 +276,8 @@ def main():
     lib.inc_set_stream()
     if args.vote:
         lib.inc_set_vote_thresholds(*args.vote)
+    if args.taper is not None:
+        lib.inc_set_event_taper(args.taper)
     real_t = lib.torch_real()
     E_d = torch.as_tensor(E.astype(lib.real), device="cuda")
     tid_d = torch.as_tensor(slots[tid], device="cuda")

@@ -169,6 +169,13 @@ int inc_set_long_track_threshold(int n_segments);
  * refilled.  0 (the default) lets the library choose: 3 while every live target has A <= 20 (a track then continues
  * in ~87 % of its segments), otherwise 2.  Results never depend on it. */
 int inc_set_segments_per_pass(int n);
+/* Scheduling knob of the default (wavefront) cascade kernel: with `min_events_per_warp` > 0 a warp holds at most its
+ * share of the events of the chunk that have not been handed out yet (at least that minimum, at most its slot count), so
+ * the last events of a chunk are spread over all warps instead of queueing in the warps that asked first, and a batch
+ * smaller than the GPU's slot count (~1.9e5 events) is spread over all SMs from the start.  0 switches it off (every warp
+ * fills all its slots while events remain); -1 (the default) lets the library choose: 8 for chunks below 1e5 events (1e4
+ * events: 0.51 -> 0.44 ms), off above, where it was measured to change nothing.  Results never depend on it (R-R4). */
+int inc_set_event_taper(int min_events_per_warp);
 /* Global index of the first event of the following inc_simulate calls (default 0): event i of a
  * call uses the random stream of global event e = offset + i.  This is how a job is sharded over
  * several GPUs or calls with bit-identical per-event results (R-R4). */

@@ -95,7 +95,7 @@ def make_tables_struct(t: dict):
 
 
 EXPORTS = ["inc_init", "inc_free_target", "inc_shutdown", "inc_set_stream", "inc_set_flags", "inc_set_event_offset",
-           "inc_get_stage_times", "inc_get_drain_timeline", "inc_get_warp_trace", "inc_get_rerun_count", "inc_set_vote_thresholds", "inc_set_long_track_threshold", "inc_set_segments_per_pass", "inc_set_stage_overflow_rows", "inc_set_chunk_events", "inc_set_projectiles", "inc_simulate",
+           "inc_get_stage_times", "inc_get_drain_timeline", "inc_get_warp_trace", "inc_get_rerun_count", "inc_set_vote_thresholds", "inc_set_long_track_threshold", "inc_set_event_taper", "inc_set_segments_per_pass", "inc_set_stage_overflow_rows", "inc_set_chunk_events", "inc_set_projectiles", "inc_simulate",
            "inc_simulate_host", "inc_get_offsets", "inc_get_cascade_stage", "inc_get_stats", "inc_get_nucleus",
            "inc_measure_issue_peak", "inc_philox_blocks", "inc_tally", "inc_scan_counts_static", "inc_last_error", "inc_build_info"]
 
@@ -202,6 +202,9 @@ class IncLibrary:
 
     def inc_set_segments_per_pass(self, n: int):
         self._check(self.lib.inc_set_segments_per_pass(int(n)))
+
+    def inc_set_event_taper(self, min_events_per_warp: int):
+        self._check(self.lib.inc_set_event_taper(int(min_events_per_warp)))
 
     def inc_set_long_track_threshold(self, n_segments: int):
         self._check(self.lib.inc_set_long_track_threshold(int(n_segments)))

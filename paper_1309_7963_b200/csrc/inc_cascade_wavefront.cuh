@@ -220,6 +220,16 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
 
   // warp-uniform queue sizes (every queue operation is warp-collective, so all lanes agree)
   int nSeg = 0, nColl = 0, nEpi = 0, nFree = C::NS;
+  // Taper (P.taper_min > 0): a warp holds at most `quota` events, its share of the events not handed out yet (never
+  // fewer than taper_min).  While the chunk has more than NS events per warp left that is NS and changes nothing; then
+  // the last events are spread over all warps instead of sitting 80 deep in the warps that asked first, and a small
+  // batch is spread over the whole grid from the start.  Scheduling only: results never depend on it (R-R4).
+  const float inv_warps = 1.0f / (float)(gridDim.x * C::WARPS);
+  int quota = C::NS;
+  if (P.taper_min > 0) {
+    const int q = __float2int_ru((float)P.n_chunk * inv_warps);
+    quota = q < P.taper_min ? P.taper_min : (q > C::NS ? C::NS : q);
+  }
   bool exhausted = false;
   // drain helpers: a track with long_seg segments behind it is handed to a warp that has finished its own events
   // (if there is one).  The STATS build keeps every track (a helper's speculative lanes would be counted).
@@ -321,7 +331,9 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
     constexpr int kCollTrig = C::QC - 31 < 32 ? C::QC - 31 : 32;
     constexpr int kAdmit = (C::QS + C::QC) / 3;       // admission control: no new attempts while more tracks wait
     const int nSegT = nSeg + nRes;
-    const int availE = nEpi + (exhausted ? 0 : nFree);
+    int freeU = quota - (C::NS - nFree);           // free slots the taper lets this warp fill (all of them while quota = NS)
+    freeU = freeU < 0 ? 0 : freeU;
+    const int availE = nEpi + (exhausted ? 0 : freeU);
     int phase = ST_SEG;
     int lim = 32;                                 // tracks the refill of a segment pass may take
     if (!(nColl < kCollTrig && nSegT >= 32)) {        // (the common case needs none of what follows)
@@ -599,6 +611,11 @@ __global__ void __launch_bounds__(WaveCfg<R>::WARPS * 32, 1) cascade_wavefront_k
         unsigned long long base = 0;
         if (lane == leader) base = atomicAdd(&P.ctr->next_event_casc, (unsigned long long)__popc(need));
         base = __shfl_sync(kFull, base, leader);
+        if (P.taper_min > 0) {
+          const int left = P.n_chunk - (int)(base < (unsigned long long)P.n_chunk ? base : (unsigned long long)P.n_chunk);
+          const int q = __float2int_ru((float)left * inv_warps);
+          quota = q < P.taper_min ? P.taper_min : (q > C::NS ? C::NS : q);
+        }
         if (want_event) {
           const unsigned long long mine = base + (unsigned long long)__popc(need & lt);
           if (mine < (unsigned long long)P.n_chunk) {

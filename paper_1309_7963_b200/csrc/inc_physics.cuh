@@ -312,6 +312,7 @@ template <typename R> struct CascadeParams {
   uint32_t flags;
   int vote_coll, vote_epi;  // lane kernel: phase-vote thresholds
   int long_seg;             // wavefront kernel: tracks with this many segments behind them may go to a drain helper
+  int taper_min;            // wavefront kernel: 0 = off; else a warp holds at most max(taper_min, events left / warps) events
   int seg_per_pass;         // wavefront kernel: segment steps per segment pass (1..8)
   int n_stage;              // nuclei slots staged into shared memory (target_id must be < n_stage)
   int nuc_stride;           // bytes of one staged nucleus (nuc_stride_bytes)

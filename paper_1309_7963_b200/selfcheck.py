@@ -4,10 +4,14 @@ conservation laws that hold for every event (BASELINE.json criterion (1)) -- no 
     python -m paper_1309_7963_b200.selfcheck [--config C] [--events N] [--variant f32|f64]
                                              [--long-seg S] [--chunk M] [--host]
 
-It is also the target of the sanitizer runs kept under profiles/ (SURVEY section 5):
+It was written as the target of compute-sanitizer runs:
 
     compute-sanitizer --tool memcheck  python -m paper_1309_7963_b200.selfcheck --config 1 --long-seg 2
     compute-sanitizer --tool racecheck python -m paper_1309_7963_b200.selfcheck --config 1 --long-seg 2
+
+No such run exists under profiles/: the GPU pool this was developed on refuses the tool.  The substitute that does run
+is the checked small-queue build (libinc_f64q.so, -DINC_CHECKED: every queue, ring and slot index verified on the
+device), exercised by tests/test_gpu_parity.py::test_small_queue_build_and_overflow_rerun.
 
 (--long-seg 2 makes almost every drain-phase track go through the drain helpers' shared-memory rings.)
 """

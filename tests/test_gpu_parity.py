@@ -20,6 +20,7 @@ pytestmark = pytest.mark.gpu
 
 REL_F64 = 1e-9          # north_star criterion (2)
 FRAC_IDENTICAL = 0.999  # north_star criterion (2)
+TAPER_DEFAULT = -1      # the library's default of inc_set_event_taper (automatic)
 
 
 @pytest.fixture(scope="module")
@@ -223,9 +224,14 @@ def test_drain_helpers_change_nothing(gpu, orc, otables, ptables, variant, cfg, 
         for spp in (1, 2, 5):           # segment steps per pass of the wavefront kernel
             lib.inc_set_segments_per_pass(spp)
             runs.append(gpu.simulate(lib, targets, E, tid, seed, ptables))
+        lib.inc_set_segments_per_pass(0)
+        for tp in (0, 1, 4, 16, -1):    # event taper of the wavefront kernel (share of the remaining events per warp)
+            lib.inc_set_event_taper(tp)
+            runs.append(gpu.simulate(lib, targets, E, tid, seed, ptables))
     finally:
         lib.inc_set_long_track_threshold(0)
         lib.inc_set_segments_per_pass(0)
+        lib.inc_set_event_taper(TAPER_DEFAULT)
     for other in runs[1:]:
         for k in ("species", "T", "ux", "uy", "uz", "counts", "A", "Z", "Estar", "px", "py", "pz", "status", "offsets"):
             assert np.array_equal(runs[0][k], other[k]), k
@@ -612,7 +618,7 @@ def test_gem_direct_quadrature_fallback(gpu, orc):
 
 @pytest.mark.parametrize("cfg", [2, 5])
 def test_gem_fp32_histograms(gpu, orc, cfg):
-    """GEM mode, production build, full-size batch against a 2e5-event oracle sample (criterion (3)), plus exact
+    """GEM mode, production build, full-size batch against a 1e6-event oracle sample (criterion (3)), plus exact
     conservation of A and Z and 4-momentum to fp32 accuracy."""
     import torch
     import paper_1309_7963_b200.tables as T
@@ -623,7 +629,7 @@ def test_gem_fp32_histograms(gpu, orc, cfg):
     g = gpu.simulate(gpu.load("f32"), targets, E, tid, seed, T.default_tables(**kw), capacity_per_event=12)
     assert not np.any(g["status"] & (gpu.ST_FAILED | gpu.ST_QUEUE_OVF))
     hg = H.histograms(g["species"], g["T"].astype(np.float64), g["uz"].astype(np.float64), g["counts"], g["A"])
-    ho, _ = H.oracle_histograms(cfg, 200000, tables_kw=kw)
+    ho, _ = H.oracle_histograms(cfg, 1000000, tables_kw=kw)
     fails = H.compare_histograms(hg, ho)
     assert not fails, fails
     m = 100000
